@@ -1,0 +1,156 @@
+/* ddf.h - C ABI of libddf: batched Directed Distance Field queries on one B200 (sm_100a).
+ *
+ * The operation: PAPER.md:58-62 (Sec. III-A, Eq. 1)  f(x, d) = (t, xi): for a ray with origin
+ * x and unit direction d, t is the distance to the first surface along d and xi the predicted
+ * probability that the ray hits at all; "Every query is one forward pass" (PAPER.md:80,
+ * Sec. III-C).  The network family is the paper's "sinusoidal encoding with a wide MLP"
+ * (Sec. IV-C) in the shapes BASELINE.json's configs fix:
+ *
+ *   gamma(v) = [v, sin(2^0 pi v), cos(2^0 pi v), ..., sin(2^(L-1) pi v), cos(2^(L-1) pi v)]
+ *              (3 sines then 3 cosines per band), gamma = [gamma_Lo(origin) ; gamma_Ld(dir)]
+ *   h_0 = gamma;  h_{l+1} = ReLU(W_l in_l + b_l),  in_l = [h_l ; gamma] if l == skip_layer else h_l
+ *   z = W_out h_last + b_out;  t = softplus(z_0);  xi = sigmoid(z_1)          (n_out == 2)
+ *   s = z_0                                                                   (n_out == 1, SDF)
+ *
+ * Arithmetic: weights and activations are bf16 operands (fp32 blobs are rounded to bf16 RNE at
+ * create), products accumulate in fp32, bias + ReLU in fp32, gamma and every hidden activation
+ * but the last are rounded to bf16 RNE; the head reads the last activation un-rounded.
+ *
+ * General rules
+ *  - Every function returns 0 (DDF_OK) or a negative ddf_status; none throws, aborts or prints.
+ *  - Pointers marked [device] are CUDA device pointers on the current device, caller-owned,
+ *    contiguous, 4-byte aligned (16-byte alignment enables the vectorised path); [host] are
+ *    host pointers.  Inputs and outputs must not alias.
+ *  - All work is enqueued on `stream` (a cudaStream_t passed as void*; NULL = default stream);
+ *    no call synchronises the stream except ddf_create / ddf_destroy / *_host variants.
+ *    Results are valid once the stream reaches the point after the call.
+ *  - n == 0 is DDF_OK and a no-op; n < 0 or a NULL pointer with n > 0 is DDF_E_INVALID_ARG.
+ *  - Results are a pure function of (weights, ray): independent of n and of the ray's position
+ *    in the batch, bit-reproducible run to run.  Directions must be unit length (not checked).
+ *  - There is no CPU fallback: without a CUDA device of compute capability 10.x the calls
+ *    return DDF_E_UNSUPPORTED / DDF_E_CUDA.
+ */
+#ifndef DDF_H
+#define DDF_H
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum ddf_status {
+  DDF_OK = 0,
+  DDF_E_INVALID_ARG = -1,   /* NULL pointer, negative count, bad enum value                 */
+  DDF_E_BAD_LAYOUT  = -2,   /* ddf_layout fields inconsistent or struct_size/version wrong  */
+  DDF_E_UNSUPPORTED = -3,   /* shape or device not supported by any kernel                  */
+  DDF_E_CUDA        = -4,   /* a CUDA call failed; see ddf_last_cuda_error()                */
+  DDF_E_NOMEM       = -5    /* host or device allocation failed                             */
+} ddf_status;
+
+#define DDF_LAYOUT_VERSION 1u
+
+/* POD, caller-owned, copied by ddf_create. */
+typedef struct ddf_layout {
+  uint32_t struct_size;        /* sizeof(ddf_layout)                                        */
+  uint32_t version;            /* DDF_LAYOUT_VERSION                                        */
+  uint32_t input_kind;         /* 0 = ray (origin + direction), 1 = point (SDF networks)    */
+  uint32_t n_freq_origin;      /* L_o >= 0 (identity always included)                       */
+  uint32_t n_freq_dir;         /* L_d >= 0; ignored for input_kind 1                        */
+  uint32_t n_hidden;           /* number of Linear+ReLU layers, >= 1                        */
+  uint32_t width;              /* output width of every hidden layer                        */
+  int32_t  skip_layer;         /* 0-based layer whose input is [h ; gamma]; -1 none; else 1..n_hidden-1 */
+  uint32_t n_out;              /* 2 = (distance logit, visibility logit); 1 = linear value  */
+  uint32_t weight_dtype;       /* 0 = fp32, 1 = bf16 (raw uint16)                           */
+  uint32_t weights_on_device;  /* 0 = `weights` is a host pointer, 1 = device pointer       */
+} ddf_layout;
+
+/* Weight blob: layers 0..n_hidden-1 then the head; each layer is W[out][in] row-major followed
+ * by b[out], all in `weight_dtype`.  in(layer 0) = E = (3+6 L_o) + (3+6 L_d) (ray) or 3+6 L_o
+ * (point); in(skip layer) = width + E ordered [h ; gamma]; head rows are (distance, visibility). */
+
+typedef struct ddf_model ddf_model;            /* opaque; owns a pre-tiled device copy of the weights */
+
+typedef struct ddf_camera { float pos[3]; float look_at[3]; float fov_deg; } ddf_camera;
+typedef struct ddf_scene  { float sphere_c[3]; float sphere_r; float box_min[3]; float box_max[3]; } ddf_scene;
+
+/* ---------------------------------------------------------------- model life cycle
+ * ddf_create copies `weights` (host or device per layout->weights_on_device), rounds fp32 to
+ * bf16, builds the tiled device copy and the per-model workspace; the caller may free `weights`
+ * on return.  Synchronises the device.  *out is NULL on failure. */
+int  ddf_create(const void* weights, const ddf_layout* layout, ddf_model** out);
+int  ddf_destroy(ddf_model* model);                       /* NULL is DDF_OK */
+const char* ddf_status_string(int status);
+int  ddf_last_cuda_error(void);                           /* cudaError_t of the last DDF_E_CUDA on this thread */
+/* kernel selection: 0 = automatic (tcgen05 path when the layout allows, else the SIMT path),
+ * 1 = force the SIMT path, 2 = force the tcgen05 path (DDF_E_UNSUPPORTED if it cannot run). */
+int  ddf_set_path(ddf_model* model, int path);
+/* which = 0: 1 if the tcgen05 path serves this model, else 0; 1: kernels launched by the
+ * last query call on this model; 2: E (encoded input width); 3: rays per tile of the path. */
+int64_t ddf_get_info(const ddf_model* model, int which);
+
+/* ---------------------------------------------------------------- the query
+ * origins, dirs: [device] float[n][3].  out_dist, out_vis: [device] float[n]
+ * (out_vis may be NULL; for n_out == 1 models out_dist receives the linear value z_0). */
+int  ddf_query(ddf_model* model, const float* origins, const float* dirs, int64_t n,
+               float* out_dist, float* out_vis, void* stream);
+/* Same through [host] buffers (pinned for full speed): H2D copies, query, D2H copies, and a
+ * stream synchronise, all inside the call.  The end-to-end entry point bench.py times. */
+int  ddf_query_host(ddf_model* model, const float* origins, const float* dirs, int64_t n,
+                    float* out_dist, float* out_vis, void* stream);
+/* Debug/parity aid: raw logits z[n][n_out] instead of the head nonlinearities. */
+int  ddf_query_logits(ddf_model* model, const float* origins, const float* dirs, int64_t n,
+                      float* out_z, void* stream);
+
+/* ---------------------------------------------------------------- ray generators
+ * All pointers [device]; rays are float[.][3]. */
+/* Host helper (A13): camera at `radius` on the sphere, position drawn from the counter
+ * generator (seed, stream, indices 0,1), looking at the origin, 50 degree field of view. */
+int  ddf_camera_from_seed(uint64_t seed, uint64_t stream, float radius, ddf_camera* out);
+/* Pinhole primary rays, row-major, all origins = cam->pos ("evaluate f at the camera"). */
+int  ddf_gen_camera(const ddf_camera* cam, int width, int height, float* o, float* d, void* stream);
+/* n points uniform on the sphere |p| = radius with outward normals (counters 2i, 2i+1). */
+int  ddf_gen_sphere_points(uint64_t seed, uint64_t rng_stream, int64_t n, float radius,
+                           float* p, float* nrm, void* stream);
+/* Shadow rays: o = p + eps n, d = normalise(light - o), tmax = |light - o| (tmax may be NULL). */
+int  ddf_gen_shadow(const float* p, const float* nrm, int64_t n, const float light[3], float eps,
+                    float* o, float* d, float* tmax, void* stream);
+/* G-buffer: first hit of every camera ray against a sphere inside an axis-aligned room seen
+ * from inside (inward wall normals).  t_hit may be NULL. */
+int  ddf_gen_gbuffer(const ddf_camera* cam, const ddf_scene* scene, int width, int height,
+                     float* p, float* nrm, float* t_hit, void* stream);
+/* AO rays: spp cosine-weighted hemisphere directions per point, pixel-major; o = p + eps n. */
+int  ddf_gen_ao(const float* p, const float* nrm, int64_t n_pts, int spp, uint64_t seed,
+                uint64_t rng_stream, float eps, float* o, float* d, void* stream);
+/* ao[i] = 1 - mean_s( vis > 0.5 and dist < ao_radius ) ("average the hit flag"). */
+int  ddf_ao_reduce(const float* vis, const float* dist, int64_t n_pts, int spp, float ao_radius,
+                   float* ao, void* stream);
+/* Query + reduce in one call; the per-ray results never reach global memory when the tile size
+ * is a multiple of spp (else a workspace of 8 bytes per ray owned by the model is used). */
+int  ddf_query_ao(ddf_model* model, const float* o, const float* d, int64_t n_pts, int spp,
+                  float ao_radius, float* ao, void* stream);
+/* shadow[i] = 1 if vis > 0.5 and dist < tmax ("occluded within the distance to the light"). */
+int  ddf_shadow_test(const float* vis, const float* dist, const float* tmax, int64_t n,
+                     uint8_t* shadow, void* stream);
+
+/* ---------------------------------------------------------------- sphere-tracing comparison
+ * (BASELINE.json configs[4]).  `model` must have input_kind 1, n_out 1.
+ * Traces s(p) = (|p| - base_radius) + alpha * MLP(p):
+ *   t = 0; for step < max_steps: p = o + t d; s = s(p); if |s| < eps: hit, stop;
+ *          t += s; if t > t_max or t < 0: miss, stop.   Unconverged: miss.
+ * early_exit 0: every ray is evaluated max_steps times (finished rays keep their state);
+ * early_exit 1: finished rays are compacted away between steps.
+ * out_t [n], out_hit [n] (0/1), out_steps [n] (SDF evaluations that counted for the ray).
+ * trace_p / trace_s (may be NULL): [n][max_steps][3] / [n][max_steps] visited points and values
+ * (unvisited entries are NaN).  total_evals [device] int64 (may be NULL): MLP evaluations made. */
+typedef struct sdf_trace_params {
+  int32_t max_steps; float eps; float t_max; float base_radius; float alpha; int32_t early_exit;
+} sdf_trace_params;
+int  sdf_sphere_trace(ddf_model* model, const float* o, const float* d, int64_t n,
+                      const sdf_trace_params* params, float* out_t, uint8_t* out_hit,
+                      int32_t* out_steps, float* trace_p, float* trace_s, int64_t* total_evals,
+                      void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

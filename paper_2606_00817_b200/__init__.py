@@ -1,0 +1,14 @@
+"""paper_2606_00817_b200 - B200-native batched Directed Distance Field queries.
+
+Thin Python binding (argument marshalling only) over the C ABI in include/ddf.h; every step of
+the path runs in the CUDA kernels of csrc/.  torch is used for device memory and streams only.
+There is no CPU fallback: importing works anywhere, calling needs libddf.so and a B200.
+"""
+from .binding import (  # noqa: F401
+    DdfError, DdfLayout, DdfCamera, DdfScene, SdfTraceParams, Model, lib, lib_path,
+    ddf_create, ddf_destroy, ddf_query, ddf_query_host, ddf_query_logits, ddf_query_ao, ddf_set_path,
+    ddf_get_info, ddf_camera_from_seed, ddf_gen_camera, ddf_gen_sphere_points, ddf_gen_shadow,
+    ddf_gen_gbuffer, ddf_gen_ao, ddf_ao_reduce, ddf_shadow_test, sdf_sphere_trace, ddf_status_string,
+    EXPORTED_SYMBOLS,
+)
+from .build import build  # noqa: F401

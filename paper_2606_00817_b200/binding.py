@@ -1,0 +1,223 @@
+"""ctypes binding of libddf.so - same names as include/ddf.h, argument marshalling only.
+
+Tensors are torch CUDA tensors (float32, contiguous); the stream defaults to torch's current
+stream.  Nothing here computes: a missing library or device raises DdfError.
+"""
+import ctypes as C
+import os
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libddf.so")
+
+EXPORTED_SYMBOLS = [
+    "ddf_create", "ddf_destroy", "ddf_status_string", "ddf_last_cuda_error", "ddf_set_path",
+    "ddf_get_info", "ddf_query", "ddf_query_host", "ddf_query_logits", "ddf_camera_from_seed",
+    "ddf_gen_camera", "ddf_gen_sphere_points", "ddf_gen_shadow", "ddf_gen_gbuffer", "ddf_gen_ao",
+    "ddf_ao_reduce", "ddf_query_ao", "ddf_shadow_test", "sdf_sphere_trace",
+]
+
+
+class DdfError(RuntimeError):
+    pass
+
+
+class DdfLayout(C.Structure):
+    _fields_ = [("struct_size", C.c_uint32), ("version", C.c_uint32), ("input_kind", C.c_uint32),
+                ("n_freq_origin", C.c_uint32), ("n_freq_dir", C.c_uint32), ("n_hidden", C.c_uint32),
+                ("width", C.c_uint32), ("skip_layer", C.c_int32), ("n_out", C.c_uint32),
+                ("weight_dtype", C.c_uint32), ("weights_on_device", C.c_uint32)]
+
+
+class DdfCamera(C.Structure):
+    _fields_ = [("pos", C.c_float * 3), ("look_at", C.c_float * 3), ("fov_deg", C.c_float)]
+
+
+class DdfScene(C.Structure):
+    _fields_ = [("sphere_c", C.c_float * 3), ("sphere_r", C.c_float),
+                ("box_min", C.c_float * 3), ("box_max", C.c_float * 3)]
+
+
+class SdfTraceParams(C.Structure):
+    _fields_ = [("max_steps", C.c_int32), ("eps", C.c_float), ("t_max", C.c_float),
+                ("base_radius", C.c_float), ("alpha", C.c_float), ("early_exit", C.c_int32)]
+
+
+_lib = None
+
+
+def lib_path():
+    return _LIB_PATH
+
+
+def lib():
+    """Loads libddf.so (built in-tree by paper_2606_00817_b200.build.build()); fails loudly."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_LIB_PATH):
+            raise DdfError("libddf.so is not built: run `python -m paper_2606_00817_b200.build` "
+                           "(there is no CPU or PyTorch fallback)")
+        _lib = C.CDLL(_LIB_PATH)
+        _lib.ddf_status_string.restype = C.c_char_p
+        _lib.ddf_get_info.restype = C.c_int64
+    return _lib
+
+
+def ddf_status_string(rc):
+    return lib().ddf_status_string(C.c_int(rc)).decode()
+
+
+def _check(rc, what):
+    if rc != 0:
+        extra = ""
+        if rc == -4:
+            extra = " (cudaError %d)" % lib().ddf_last_cuda_error()
+        raise DdfError("%s failed: %s%s" % (what, ddf_status_string(rc), extra))
+
+
+def _stream(stream):
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return C.c_void_p(stream.cuda_stream if hasattr(stream, "cuda_stream") else int(stream))
+
+
+def _dev(t, dtype=torch.float32):
+    if t is None:
+        return C.c_void_p(0)
+    if not (t.is_cuda and t.is_contiguous() and t.dtype == dtype):
+        raise DdfError("expected a contiguous CUDA tensor of %s" % dtype)
+    return C.c_void_p(t.data_ptr())
+
+
+def _host(t, dtype=torch.float32):
+    if t is None:
+        return C.c_void_p(0)
+    if t.is_cuda or not t.is_contiguous() or t.dtype != dtype:
+        raise DdfError("expected a contiguous host tensor of %s" % dtype)
+    return C.c_void_p(t.data_ptr())
+
+
+class Model:
+    """Owns a ddf_model*; see ddf_create."""
+
+    def __init__(self, handle, layout):
+        self.handle = handle
+        self.layout = layout
+
+    def close(self):
+        if self.handle:
+            ddf_destroy(self)
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def make_layout(lay, weights_on_device=0):
+    """lay: any object with the ddf_layout field names (e.g. ddf_inputs.Layout)."""
+    return DdfLayout(C.sizeof(DdfLayout), 1, lay.input_kind, lay.n_freq_origin, lay.n_freq_dir, lay.n_hidden,
+                     lay.width, lay.skip_layer, lay.n_out, lay.weight_dtype, weights_on_device)
+
+
+def ddf_create(weights, lay):
+    """weights: numpy array (float32 / uint16 bf16 bits) or a CUDA tensor of the blob."""
+    import numpy as np
+    if isinstance(weights, torch.Tensor):
+        L = make_layout(lay, 1 if weights.is_cuda else 0)
+        ptr = C.c_void_p(weights.data_ptr())
+    else:
+        weights = np.ascontiguousarray(weights)
+        L = make_layout(lay, 0)
+        ptr = weights.ctypes.data_as(C.c_void_p)
+    h = C.c_void_p(0)
+    _check(lib().ddf_create(ptr, C.byref(L), C.byref(h)), "ddf_create")
+    return Model(h, lay)
+
+
+def ddf_destroy(model):
+    if model.handle:
+        rc = lib().ddf_destroy(model.handle)
+        model.handle = None
+        _check(rc, "ddf_destroy")
+
+
+def ddf_set_path(model, path):
+    _check(lib().ddf_set_path(model.handle, C.c_int(path)), "ddf_set_path")
+
+
+def ddf_get_info(model, which):
+    return int(lib().ddf_get_info(model.handle, C.c_int(which)))
+
+
+def ddf_query(model, origins, dirs, n, out_dist, out_vis, stream=None):
+    _check(lib().ddf_query(model.handle, _dev(origins), _dev(dirs), C.c_int64(n), _dev(out_dist), _dev(out_vis),
+                           _stream(stream)), "ddf_query")
+
+
+def ddf_query_host(model, origins, dirs, n, out_dist, out_vis, stream=None):
+    _check(lib().ddf_query_host(model.handle, _host(origins), _host(dirs), C.c_int64(n), _host(out_dist),
+                                _host(out_vis), _stream(stream)), "ddf_query_host")
+
+
+def ddf_query_logits(model, origins, dirs, n, out_z, stream=None):
+    _check(lib().ddf_query_logits(model.handle, _dev(origins), _dev(dirs), C.c_int64(n), _dev(out_z),
+                                  _stream(stream)), "ddf_query_logits")
+
+
+def ddf_query_ao(model, o, d, n_pts, spp, ao_radius, ao, stream=None):
+    _check(lib().ddf_query_ao(model.handle, _dev(o), _dev(d), C.c_int64(n_pts), C.c_int(spp), C.c_float(ao_radius),
+                              _dev(ao), _stream(stream)), "ddf_query_ao")
+
+
+def ddf_camera_from_seed(seed, rng_stream, radius=2.5):
+    cam = DdfCamera()
+    _check(lib().ddf_camera_from_seed(C.c_uint64(seed), C.c_uint64(rng_stream), C.c_float(radius), C.byref(cam)),
+           "ddf_camera_from_seed")
+    return cam
+
+
+def ddf_gen_camera(cam, width, height, o, d, stream=None):
+    _check(lib().ddf_gen_camera(C.byref(cam), C.c_int(width), C.c_int(height), _dev(o), _dev(d), _stream(stream)),
+           "ddf_gen_camera")
+
+
+def ddf_gen_sphere_points(seed, rng_stream, n, radius, p, nrm, stream=None):
+    _check(lib().ddf_gen_sphere_points(C.c_uint64(seed), C.c_uint64(rng_stream), C.c_int64(n), C.c_float(radius),
+                                       _dev(p), _dev(nrm), _stream(stream)), "ddf_gen_sphere_points")
+
+
+def ddf_gen_shadow(p, nrm, n, light, eps, o, d, tmax, stream=None):
+    li = (C.c_float * 3)(*[float(x) for x in light])
+    _check(lib().ddf_gen_shadow(_dev(p), _dev(nrm), C.c_int64(n), li, C.c_float(eps), _dev(o), _dev(d), _dev(tmax),
+                                _stream(stream)), "ddf_gen_shadow")
+
+
+def ddf_gen_gbuffer(cam, scene, width, height, p, nrm, t_hit, stream=None):
+    _check(lib().ddf_gen_gbuffer(C.byref(cam), C.byref(scene), C.c_int(width), C.c_int(height), _dev(p), _dev(nrm),
+                                 _dev(t_hit), _stream(stream)), "ddf_gen_gbuffer")
+
+
+def ddf_gen_ao(p, nrm, n_pts, spp, seed, rng_stream, eps, o, d, stream=None):
+    _check(lib().ddf_gen_ao(_dev(p), _dev(nrm), C.c_int64(n_pts), C.c_int(spp), C.c_uint64(seed),
+                            C.c_uint64(rng_stream), C.c_float(eps), _dev(o), _dev(d), _stream(stream)), "ddf_gen_ao")
+
+
+def ddf_ao_reduce(vis, dist, n_pts, spp, ao_radius, ao, stream=None):
+    _check(lib().ddf_ao_reduce(_dev(vis), _dev(dist), C.c_int64(n_pts), C.c_int(spp), C.c_float(ao_radius), _dev(ao),
+                               _stream(stream)), "ddf_ao_reduce")
+
+
+def ddf_shadow_test(vis, dist, tmax, n, shadow, stream=None):
+    _check(lib().ddf_shadow_test(_dev(vis), _dev(dist), _dev(tmax), C.c_int64(n), _dev(shadow, torch.uint8),
+                                 _stream(stream)), "ddf_shadow_test")
+
+
+def sdf_sphere_trace(model, o, d, n, params, out_t, out_hit, out_steps, trace_p=None, trace_s=None,
+                     total_evals=None, stream=None):
+    _check(lib().sdf_sphere_trace(model.handle, _dev(o), _dev(d), C.c_int64(n), C.byref(params), _dev(out_t),
+                                  _dev(out_hit, torch.uint8), _dev(out_steps, torch.int32), _dev(trace_p),
+                                  _dev(trace_s), _dev(total_evals, torch.int64), _stream(stream)),
+           "sdf_sphere_trace")

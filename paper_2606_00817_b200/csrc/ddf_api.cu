@@ -1,0 +1,247 @@
+// ddf_api.cu - C ABI entry points of libddf (include/ddf.h): model life cycle and query dispatch.
+#include "ddf_common.cuh"
+#include <stdlib.h>
+#include <string.h>
+#include <new>
+#include <vector>
+
+namespace ddf {
+
+thread_local int g_last_cuda_error = 0;
+
+static inline uint16_t f32_to_bf16_rne(float f) {
+  uint32_t b; memcpy(&b, &f, 4);
+  if ((b & 0x7F800000u) == 0x7F800000u) return (uint16_t)(b >> 16);
+  return (uint16_t)((b + 0x7FFFu + ((b >> 16) & 1u)) >> 16);
+}
+static inline float bf16_to_f32(uint16_t h) { uint32_t b = (uint32_t)h << 16; float f; memcpy(&f, &b, 4); return f; }
+
+static int check_layout(const ddf_layout* L) {
+  if (L->struct_size != sizeof(ddf_layout) || L->version != DDF_LAYOUT_VERSION) return DDF_E_BAD_LAYOUT;
+  if (L->input_kind > 1 || L->weight_dtype > 1 || L->weights_on_device > 1) return DDF_E_BAD_LAYOUT;
+  if (L->n_hidden < 1 || L->n_hidden >= (uint32_t)kMaxLayers || L->width < 1) return DDF_E_BAD_LAYOUT;
+  if (L->n_out < 1 || L->n_out > 2) return DDF_E_BAD_LAYOUT;
+  if (L->skip_layer != -1 && (L->skip_layer < 1 || L->skip_layer >= (int32_t)L->n_hidden)) return DDF_E_BAD_LAYOUT;
+  if (L->n_freq_origin > 16 || L->n_freq_dir > 16) return DDF_E_UNSUPPORTED;
+  if (L->width > 16384) return DDF_E_UNSUPPORTED;
+  return DDF_OK;
+}
+
+static void free_model(Model* m) {
+  if (!m) return;
+  tc_plan_destroy(m);
+  cudaFree(m->d_w); cudaFree(m->d_b); cudaFree(m->d_head_w);
+  cudaFree(m->ws_gamma); cudaFree(m->ws_act0); cudaFree(m->ws_act1); cudaFree(m->ws_last);
+  cudaFree(m->ws_dist); cudaFree(m->ws_vis);
+  cudaFree(m->h2d_o); cudaFree(m->h2d_d); cudaFree(m->d2h_dist); cudaFree(m->d2h_vis);
+  cudaFree(m->trace_ws);
+  (void)cudaGetLastError();
+  delete m;
+}
+
+}  // namespace ddf
+
+using namespace ddf;
+
+extern "C" const char* ddf_status_string(int s) {
+  switch (s) {
+    case DDF_OK: return "ok";
+    case DDF_E_INVALID_ARG: return "invalid argument";
+    case DDF_E_BAD_LAYOUT: return "bad layout";
+    case DDF_E_UNSUPPORTED: return "unsupported layout or device";
+    case DDF_E_CUDA: return "CUDA error";
+    case DDF_E_NOMEM: return "out of memory";
+    default: return "unknown status";
+  }
+}
+
+extern "C" int ddf_last_cuda_error(void) { return g_last_cuda_error; }
+
+extern "C" int ddf_create(const void* weights, const ddf_layout* layout, ddf_model** out) {
+  if (out) *out = nullptr;
+  if (!weights || !layout || !out) return DDF_E_INVALID_ARG;
+  int rc = check_layout(layout);
+  if (rc != DDF_OK) return rc;
+  int dev = 0; cudaDeviceProp prop;
+  DDF_CUDA_TRY(cudaGetDevice(&dev));
+  DDF_CUDA_TRY(cudaGetDeviceProperties(&prop, dev));
+  if (prop.major != 10) return DDF_E_UNSUPPORTED;            // sm_100a code only
+
+  Model* m = new (std::nothrow) Model();
+  if (!m) return DDF_E_NOMEM;
+  memset(m, 0, sizeof(Model));
+  m->lay = *layout;
+  m->sm_count = prop.multiProcessorCount;
+  const ddf_layout& L = m->lay;
+  m->E = 3 + 6 * (int)L.n_freq_origin + (L.input_kind == 0 ? 3 + 6 * (int)L.n_freq_dir : 0);
+  m->E_pad = round_up(m->E, kKBlock);
+  m->width_pad = round_up((int)L.width, kKBlock);
+  m->n_layers = (int)L.n_hidden + 1;
+
+  // walk the blob, lay out the padded device copy
+  size_t blob_elems = 0, w_elems = 0, b_elems = 0;
+  std::vector<size_t> src_w(m->n_layers), src_b(m->n_layers);
+  std::vector<int> fan_in(m->n_layers);
+  for (int l = 0; l < m->n_layers; ++l) {
+    LayerDesc& d = m->layers[l];
+    const bool head = (l == m->n_layers - 1);
+    d.n_out = head ? (int)L.n_out : (int)L.width;
+    d.k0 = (l == 0) ? m->E : (int)L.width;
+    d.k0_pad = (l == 0) ? m->E_pad : m->width_pad;
+    d.k1 = (l == L.skip_layer) ? m->E : 0;
+    d.k1_pad = d.k1 ? m->E_pad : 0;
+    d.k_pad = d.k0_pad + d.k1_pad;
+    fan_in[l] = d.k0 + d.k1;
+    src_w[l] = blob_elems; blob_elems += (size_t)d.n_out * fan_in[l];
+    src_b[l] = blob_elems; blob_elems += (size_t)d.n_out;
+    d.w_off = w_elems; w_elems += (size_t)round_up(d.n_out, 128) * d.k_pad;
+    d.b_off = b_elems; b_elems += (size_t)round_up(d.n_out, 128);
+  }
+  m->w_elems = w_elems; m->b_elems = b_elems;
+
+  const size_t esz = L.weight_dtype == 1 ? 2 : 4;
+  std::vector<uint8_t> host_copy;
+  const uint8_t* src = (const uint8_t*)weights;
+  if (L.weights_on_device) {
+    host_copy.resize(blob_elems * esz);
+    cudaError_t e = cudaMemcpy(host_copy.data(), weights, blob_elems * esz, cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) { g_last_cuda_error = (int)e; (void)cudaGetLastError(); free_model(m); return DDF_E_CUDA; }
+    src = host_copy.data();
+  }
+  auto src_bf16 = [&](size_t i) -> uint16_t {
+    return L.weight_dtype == 1 ? ((const uint16_t*)src)[i] : f32_to_bf16_rne(((const float*)src)[i]);
+  };
+  auto src_f32 = [&](size_t i) -> float {
+    return L.weight_dtype == 1 ? bf16_to_f32(((const uint16_t*)src)[i]) : ((const float*)src)[i];
+  };
+  std::vector<uint16_t> hw(w_elems, 0);
+  std::vector<float> hb(b_elems, 0.0f);
+  std::vector<float> hhead((size_t)L.n_out * L.width);
+  for (int l = 0; l < m->n_layers; ++l) {
+    const LayerDesc& d = m->layers[l];
+    for (int j = 0; j < d.n_out; ++j) {
+      const size_t srow = src_w[l] + (size_t)j * fan_in[l];
+      uint16_t* drow = hw.data() + d.w_off + (size_t)j * d.k_pad;
+      for (int k = 0; k < d.k0; ++k) drow[k] = src_bf16(srow + k);
+      for (int k = 0; k < d.k1; ++k) drow[d.k0_pad + k] = src_bf16(srow + d.k0 + k);
+      hb[d.b_off + j] = src_f32(src_b[l] + j);                 // biases stay fp32
+      if (l == m->n_layers - 1)
+        for (int k = 0; k < d.k0; ++k) hhead[(size_t)j * L.width + k] = bf16_to_f32(src_bf16(srow + k));
+    }
+  }
+  cudaError_t e;
+  if ((e = cudaMalloc(&m->d_w, w_elems * 2)) != cudaSuccess ||
+      (e = cudaMalloc(&m->d_b, b_elems * 4)) != cudaSuccess ||
+      (e = cudaMalloc(&m->d_head_w, hhead.size() * 4)) != cudaSuccess ||
+      (e = cudaMemcpy(m->d_w, hw.data(), w_elems * 2, cudaMemcpyHostToDevice)) != cudaSuccess ||
+      (e = cudaMemcpy(m->d_b, hb.data(), b_elems * 4, cudaMemcpyHostToDevice)) != cudaSuccess ||
+      (e = cudaMemcpy(m->d_head_w, hhead.data(), hhead.size() * 4, cudaMemcpyHostToDevice)) != cudaSuccess) {
+    g_last_cuda_error = (int)e; (void)cudaGetLastError(); free_model(m);
+    return e == cudaErrorMemoryAllocation ? DDF_E_NOMEM : DDF_E_CUDA;
+  }
+  rc = tc_plan_create(m);
+  if (rc != DDF_OK) { free_model(m); return rc; }
+  DDF_CUDA_TRY(cudaDeviceSynchronize());
+  *out = reinterpret_cast<ddf_model*>(m);
+  return DDF_OK;
+}
+
+extern "C" int ddf_destroy(ddf_model* model) {
+  if (!model) return DDF_OK;
+  cudaDeviceSynchronize();
+  free_model(reinterpret_cast<Model*>(model));
+  return DDF_OK;
+}
+
+extern "C" int ddf_set_path(ddf_model* model, int path) {
+  if (!model || path < 0 || path > 2) return DDF_E_INVALID_ARG;
+  Model* m = reinterpret_cast<Model*>(model);
+  if (path == 2 && !m->tc) return DDF_E_UNSUPPORTED;
+  m->path = path;
+  return DDF_OK;
+}
+
+extern "C" int64_t ddf_get_info(const ddf_model* model, int which) {
+  if (!model) return DDF_E_INVALID_ARG;
+  const Model* m = reinterpret_cast<const Model*>(model);
+  switch (which) {
+    case 0: return (m->tc && m->path != 1) ? 1 : 0;
+    case 1: return m->last_launches;
+    case 2: return m->E;
+    case 3: return (m->tc && m->path != 1) ? 256 : 64;
+    default: return DDF_E_INVALID_ARG;
+  }
+}
+
+static int run_query(Model* m, const float* o, const float* d, int64_t n, int mode_out,
+                     float* out0, float* out1, void* stream) {
+  if (n < 0) return DDF_E_INVALID_ARG;
+  if (n == 0) { m->last_launches = 0; return DDF_OK; }
+  if (!o || !out0 || (m->lay.input_kind == 0 && !d)) return DDF_E_INVALID_ARG;
+  cudaStream_t st = (cudaStream_t)stream;
+  if (m->tc && m->path != 1) return tc_forward(m, o, d, n, nullptr, mode_out, out0, out1, 0, 0.0f, st);
+  return simt_forward(m, o, d, n, mode_out, out0, out1, st);
+}
+
+extern "C" int ddf_query(ddf_model* model, const float* origins, const float* dirs, int64_t n,
+                         float* out_dist, float* out_vis, void* stream) {
+  if (!model) return DDF_E_INVALID_ARG;
+  return run_query(reinterpret_cast<Model*>(model), origins, dirs, n, 0, out_dist, out_vis, stream);
+}
+
+extern "C" int ddf_query_logits(ddf_model* model, const float* origins, const float* dirs, int64_t n,
+                                float* out_z, void* stream) {
+  if (!model) return DDF_E_INVALID_ARG;
+  return run_query(reinterpret_cast<Model*>(model), origins, dirs, n, 1, out_z, nullptr, stream);
+}
+
+extern "C" int ddf_query_host(ddf_model* model, const float* origins, const float* dirs, int64_t n,
+                              float* out_dist, float* out_vis, void* stream) {
+  if (!model || n < 0) return DDF_E_INVALID_ARG;
+  if (n == 0) return DDF_OK;
+  Model* m = reinterpret_cast<Model*>(model);
+  const bool ray = m->lay.input_kind == 0, two = m->lay.n_out == 2;
+  if (!origins || !out_dist || (ray && !dirs)) return DDF_E_INVALID_ARG;
+  if (n > m->host_rows) {
+    cudaFree(m->h2d_o); cudaFree(m->h2d_d); cudaFree(m->d2h_dist); cudaFree(m->d2h_vis);
+    m->h2d_o = m->h2d_d = m->d2h_dist = m->d2h_vis = nullptr; m->host_rows = 0;
+    DDF_CUDA_TRY(cudaMalloc(&m->h2d_o, (size_t)n * 12));
+    DDF_CUDA_TRY(cudaMalloc(&m->h2d_d, (size_t)n * 12));
+    DDF_CUDA_TRY(cudaMalloc(&m->d2h_dist, (size_t)n * 4));
+    DDF_CUDA_TRY(cudaMalloc(&m->d2h_vis, (size_t)n * 4));
+    m->host_rows = n;
+  }
+  cudaStream_t st = (cudaStream_t)stream;
+  DDF_CUDA_TRY(cudaMemcpyAsync(m->h2d_o, origins, (size_t)n * 12, cudaMemcpyHostToDevice, st));
+  if (ray) DDF_CUDA_TRY(cudaMemcpyAsync(m->h2d_d, dirs, (size_t)n * 12, cudaMemcpyHostToDevice, st));
+  int rc = run_query(m, m->h2d_o, ray ? m->h2d_d : nullptr, n, 0, m->d2h_dist, two ? m->d2h_vis : nullptr, stream);
+  if (rc != DDF_OK) return rc;
+  DDF_CUDA_TRY(cudaMemcpyAsync(out_dist, m->d2h_dist, (size_t)n * 4, cudaMemcpyDeviceToHost, st));
+  if (two && out_vis) DDF_CUDA_TRY(cudaMemcpyAsync(out_vis, m->d2h_vis, (size_t)n * 4, cudaMemcpyDeviceToHost, st));
+  DDF_CUDA_TRY(cudaStreamSynchronize(st));
+  return DDF_OK;
+}
+
+extern "C" int ddf_query_ao(ddf_model* model, const float* o, const float* d, int64_t n_pts, int spp,
+                            float ao_radius, float* ao, void* stream) {
+  if (!model || n_pts < 0 || spp <= 0) return DDF_E_INVALID_ARG;
+  if (n_pts == 0) return DDF_OK;
+  Model* m = reinterpret_cast<Model*>(model);
+  if (!o || !d || !ao || m->lay.n_out != 2 || m->lay.input_kind != 0) return DDF_E_INVALID_ARG;
+  const int64_t n = n_pts * spp;
+  cudaStream_t st = (cudaStream_t)stream;
+  if (m->tc && m->path != 1 && 256 % spp == 0)
+    return tc_forward(m, o, d, n, nullptr, 2, ao, nullptr, spp, ao_radius, st);
+  if (n > m->ws_out_rows) {
+    cudaFree(m->ws_dist); cudaFree(m->ws_vis); m->ws_dist = m->ws_vis = nullptr; m->ws_out_rows = 0;
+    DDF_CUDA_TRY(cudaMalloc(&m->ws_dist, (size_t)n * 4));
+    DDF_CUDA_TRY(cudaMalloc(&m->ws_vis, (size_t)n * 4));
+    m->ws_out_rows = n;
+  }
+  int rc = run_query(m, o, d, n, 0, m->ws_dist, m->ws_vis, stream);
+  if (rc != DDF_OK) return rc;
+  int launches = m->last_launches;
+  rc = ddf_ao_reduce(m->ws_vis, m->ws_dist, n_pts, spp, ao_radius, ao, stream);
+  m->last_launches = launches + 1;
+  return rc;
+}

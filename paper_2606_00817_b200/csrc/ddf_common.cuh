@@ -1,0 +1,116 @@
+// ddf_common.cuh - shared declarations of libddf (model object, error plumbing, device helpers).
+// Product code: shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <cuda_bf16.h>
+#include <stdint.h>
+#include "../../include/ddf.h"
+
+namespace ddf {
+
+extern thread_local int g_last_cuda_error;
+
+#define DDF_CUDA_TRY(expr)                                   \
+  do {                                                       \
+    cudaError_t _e = (expr);                                 \
+    if (_e != cudaSuccess) {                                 \
+      ddf::g_last_cuda_error = (int)_e;                      \
+      (void)cudaGetLastError();                              \
+      return DDF_E_CUDA;                                     \
+    }                                                        \
+  } while (0)
+
+constexpr int kMaxLayers = 32;
+constexpr int kKBlock = 64;          // K granularity of the tiled weight copy (bf16 elements)
+
+inline int round_up(int x, int m) { return (x + m - 1) / m * m; }
+
+// One Linear layer of the device weight copy.  W is bf16 [n_out_pad][k_pad] row-major with
+// k_pad = k0_pad + k1_pad: segment 0 multiplies h (or gamma for layer 0), segment 1 multiplies
+// gamma at the skip layer.  Pad rows / columns are zero.
+struct LayerDesc {
+  int n_out;            // true output count
+  int k0, k0_pad;       // first input segment (true, padded to kKBlock)
+  int k1, k1_pad;       // second input segment (skip: gamma), 0 if none
+  int k_pad;            // row stride of W in elements
+  size_t w_off;         // element offset of W in the bf16 weight arena
+  size_t b_off;         // element offset of the bias in the fp32 bias arena
+};
+
+struct TcPlan;          // tcgen05 path state (ddf_tc.cu)
+
+struct Model {
+  ddf_layout lay;
+  int E, E_pad;                    // encoded width, padded to kKBlock
+  int width_pad;                   // width padded to kKBlock
+  int n_layers;                    // n_hidden + 1 (head last)
+  LayerDesc layers[kMaxLayers];
+  __nv_bfloat16* d_w;              // weight arena (hidden layers, padded; head stored too)
+  float* d_b;                      // bias arena (fp32)
+  float* d_head_w;                 // head weights as fp32 [n_out][width] (bf16-rounded values)
+  size_t w_elems, b_elems;
+  // workspace for the SIMT path and the sphere tracer (grown on demand, never in the hot loop
+  // once sized): two bf16 activation buffers + one fp32 buffer for the last hidden layer
+  int64_t ws_rows;
+  __nv_bfloat16 *ws_gamma, *ws_act0, *ws_act1;
+  float* ws_last;
+  float *ws_dist, *ws_vis;         // ddf_query_ao fallback
+  int64_t ws_out_rows;
+  // staging for ddf_query_host
+  float *h2d_o, *h2d_d, *d2h_dist, *d2h_vis;
+  int64_t host_rows;
+  // sphere tracer state
+  void* trace_ws; size_t trace_ws_bytes;
+  int path;                        // 0 auto, 1 SIMT, 2 tcgen05
+  TcPlan* tc;                      // non-null when the tcgen05 path can serve the layout
+  int sm_count;
+  int last_launches;
+};
+
+// ---- SIMT path (ddf_simt.cu)
+int simt_forward(Model* m, const float* o, const float* d, int64_t n, int mode_out,
+                 float* out0, float* out1, cudaStream_t st);
+int ensure_workspace(Model* m, int64_t rows);
+
+// ---- tcgen05 path (ddf_tc.cu)
+int tc_plan_create(Model* m);                 // sets m->tc or leaves it null (unsupported shape)
+void tc_plan_destroy(Model* m);
+// mode_out: 0 = heads (dist, vis), 1 = raw logits into out0 [n][n_out], 2 = AO reduce into out0
+int tc_forward(Model* m, const float* o, const float* d, int64_t n, const int64_t* n_dev,
+               int mode_out, float* out0, float* out1, int spp, float ao_radius, cudaStream_t st);
+
+// ---- device helpers -------------------------------------------------------------------------
+#ifdef __CUDACC__
+__device__ __forceinline__ uint64_t dev_mix64(uint64_t z) {
+  z += 0x9E3779B97F4A7C15ull;
+  z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+  z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+  return z ^ (z >> 31);
+}
+// key = mix64(mix64(seed) ^ stream) is computed once on the host
+__device__ __forceinline__ float dev_uniform01(uint64_t key, uint64_t idx) {
+  return (float)(uint32_t)(dev_mix64(key ^ idx) >> 40) * (1.0f / 16777216.0f);
+}
+
+__device__ __forceinline__ float softplus_f(float z) {
+  return fmaxf(z, 0.0f) + log1pf(expf(-fabsf(z)));
+}
+__device__ __forceinline__ float sigmoid_f(float z) { return 1.0f / (1.0f + expf(-z)); }
+
+// gamma of one ray into a bf16 row (E_pad entries, pad = 0).  sin/cos(2^k pi x) via sincospif
+// of the exactly scaled argument (ldexp), so high bands keep full fp32 accuracy.
+__device__ __forceinline__ void encode_vec_bf16(const float v[3], int nfreq, __nv_bfloat16* row) {
+  row[0] = __float2bfloat16_rn(v[0]); row[1] = __float2bfloat16_rn(v[1]); row[2] = __float2bfloat16_rn(v[2]);
+  for (int k = 0; k < nfreq; ++k) {
+    #pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      float s, co;
+      sincospif(ldexpf(v[c], k), &s, &co);
+      row[3 + 6 * k + c] = __float2bfloat16_rn(s);
+      row[6 + 6 * k + c] = __float2bfloat16_rn(co);
+    }
+  }
+}
+#endif
+
+}  // namespace ddf

@@ -1,0 +1,472 @@
+// ddf_tc.cu - the tcgen05 path: ONE persistent, warp-specialised kernel that runs the whole DDF
+// forward pass (encode -> n_hidden x [GEMM + bias + ReLU + bf16] -> heads) for tiles of 128 rays
+// per CTA (256 per CTA pair with cta_group::2).
+//
+//   warp 0      TMA producer  : streams activation (A) and weight (B) K-blocks into a smem ring
+//   warp 1      MMA issuer    : tcgen05.mma (bf16 x bf16 -> fp32 in TMEM), 128x256 (or 256x256 per
+//                               pair) x K accumulators, double-buffered in the 512 TMEM columns
+//   warp 2      TMEM allocator
+//   warps 4-7   epilogue      : tcgen05.ld -> +bias, ReLU, bf16 -> next layer's operand; the last
+//                               layer feeds the fused heads (softplus / sigmoid / AO reduction)
+//   warps 8-11  encoder       : gamma(o, d) of the NEXT tile, in registers, written as bf16
+//
+// Layer hand-off: a 128 x width bf16 activation tile does not fit next to a weight pipeline in
+// 227 KB of shared memory (320 KB at width 1280), so the epilogue writes it to a per-CTA scratch
+// tile that is re-read by TMA as the next layer's A operand.  The scratch (148 CTAs x 2 x 320 KB)
+// is written once and re-read at once by the same SM, i.e. it lives in the 126 MB L2; no
+// activation makes a round trip through a separate kernel launch.  Producer gating is per
+// 256-column output chunk (mbarriers), so layer l+1 starts its K loop while layer l's last
+// chunk is still in the epilogue: the tensor pipe never drains between layers or tiles.
+//
+// Operation: include/ddf.h header comment (Eq.1).
+#include "ddf_common.cuh"
+#include "ddf_tc_ptx.cuh"
+#include <cuda.h>
+#include <stdlib.h>
+#include <string.h>
+#include <new>
+
+namespace ddf {
+
+constexpr int kTileM = 128;          // rays per CTA
+constexpr int kChunkN = 256;         // output columns per accumulator
+constexpr int kMaxTcLayers = 16;
+constexpr int kMaxChunks = 8;
+constexpr int kABytes = kTileM * kKBlock * 2;           // 16 KB
+constexpr int kThreads = 384;
+
+template <int CG> struct TcCfg {
+  static constexpr int kBBytes = (CG == 2 ? 128 : 256) * kKBlock * 2;
+  static constexpr int kStageBytes = kABytes + kBBytes;
+  static constexpr int kStages = (CG == 2) ? 6 : 4;
+  static constexpr int kBarBytes = 1024;
+  static constexpr int kSmemBytes = kStages * kStageBytes + kBarBytes + 1024;   // + alignment slack
+};
+
+struct TcParams {
+  CUtensorMap w[kMaxTcLayers];
+  CUtensorMap x0, x1, g;
+  const float* o; const float* d;
+  int64_t n; const int64_t* n_dev;
+  const float* bias; const float* head_w;
+  __nv_bfloat16 *x0p, *x1p, *gp;
+  float* out0; float* out1;
+  uint32_t* dbg;
+  int n_hidden, width, n_chunks, skip_layer, n_out, input_kind, Lo, Ld, E, E_pad;
+  int mode_out, spp; float ao_radius;
+  int g_last_nk16;
+  int b_off[kMaxTcLayers + 1];
+  int nkb0[kMaxTcLayers], nkb1[kMaxTcLayers];
+};
+
+struct TcPlan {
+  int cg;
+  int grid;
+  __nv_bfloat16 *x0, *x1, *g;
+  uint32_t* dbg_host; uint32_t* dbg_dev;
+  TcParams base;
+};
+
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint64_t globaltimer_ns() {
+  uint64_t t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t;
+}
+
+// Bounded wait: a protocol error becomes a trap with a code in mapped host memory, not a hang.
+template <bool CLUSTER>
+__device__ __forceinline__ void wait_bar(uint32_t bar, uint32_t parity, uint32_t* dbg, uint32_t code) {
+  uint32_t spins = 0; uint64_t t0 = 0;
+  while (true) {
+    bool ok = CLUSTER ? ptx::mbar_try_wait_cluster(bar, parity) : ptx::mbar_try_wait(bar, parity);
+    if (ok) return;
+    if ((++spins & 1023u) == 0) {
+      uint64_t now = globaltimer_ns();
+      if (t0 == 0) t0 = now;
+      else if (now - t0 > 4000000000ull) {
+        if (dbg && atomicCAS(dbg, 0u, code) == 0u) { dbg[1] = blockIdx.x; dbg[2] = parity; dbg[3] = threadIdx.x; __threadfence_system(); }
+        __trap();
+      }
+    }
+  }
+}
+
+template <int CG>
+__global__ void __launch_bounds__(kThreads, 1) ddf_tc_kernel(const __grid_constant__ TcParams p) {
+  using Cfg = TcCfg<CG>;
+  constexpr int S = Cfg::kStages;
+  extern __shared__ uint8_t smem_raw[];
+  const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
+  const uint32_t bar_base = smem_base + S * Cfg::kStageBytes;
+  // barrier map (8 bytes each)
+  auto full_bar   = [&](int s) { return bar_base + 8u * s; };
+  auto empty_bar  = [&](int s) { return bar_base + 8u * (8 + s); };
+  auto tfull_bar  = [&](int b) { return bar_base + 8u * (16 + b); };
+  auto tempty_bar = [&](int b) { return bar_base + 8u * (18 + b); };
+  auto act_bar    = [&](int j) { return bar_base + 8u * (20 + j); };
+  auto gready_bar = [&](int b) { return bar_base + 8u * (28 + b); };
+  auto gfree_bar  = [&](int b) { return bar_base + 8u * (30 + b); };
+  const uint32_t tmem_slot = bar_base + 8u * 32;
+  auto a_smem = [&](int s) { return smem_base + s * Cfg::kStageBytes; };
+  auto b_smem = [&](int s) { return smem_base + s * Cfg::kStageBytes + kABytes; };
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const uint32_t rank = (CG == 2) ? ptx::cluster_ctarank() : 0u;
+  const bool leader = (rank == 0);
+  const int pid = blockIdx.x / CG, num_pairs = gridDim.x / CG;
+  const int cta_global = blockIdx.x;
+  const int64_t n = p.n_dev ? *p.n_dev : p.n;
+  const int64_t tile_rays = (int64_t)kTileM * CG;
+  const int64_t num_tiles = (n + tile_rays - 1) / tile_rays;
+  const int last_layer = p.n_hidden - 1;
+  const int gamma_layer = p.skip_layer >= 0 ? p.skip_layer : 0;      // last layer that reads gamma
+
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < S; ++s) { ptx::mbar_init(full_bar(s), 1); ptx::mbar_init(empty_bar(s), 1); }
+    for (int b = 0; b < 2; ++b) {
+      ptx::mbar_init(tfull_bar(b), 1); ptx::mbar_init(tempty_bar(b), 128 * CG);
+      ptx::mbar_init(gready_bar(b), 128); ptx::mbar_init(gfree_bar(b), 1);
+    }
+    for (int j = 0; j < kMaxChunks; ++j) ptx::mbar_init(act_bar(j), 128);
+    ptx::fence_mbar_init();
+  }
+  if (warp == 0 && lane == 0) {
+    for (int l = 0; l < p.n_hidden; ++l) ptx::prefetch_tmap(&p.w[l]);
+    ptx::prefetch_tmap(&p.x0); ptx::prefetch_tmap(&p.x1); ptx::prefetch_tmap(&p.g);
+  }
+  if (warp == 2) { ptx::tmem_alloc<CG>(tmem_slot, 512); ptx::tmem_relinquish<CG>(); }
+  ptx::tc_fence_before();
+  if (CG == 2) ptx::cluster_sync(); else __syncthreads();
+  ptx::tc_fence_after();
+  uint32_t tmem_base;
+  asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
+
+  if (warp == 0) {
+    // ================================================================ TMA producer
+    if (lane == 0) {
+      const uint32_t full_target = (CG == 2) ? 0u : 0u;  (void)full_target;
+      uint32_t it = 0, act_phase = 0;                    // bit j of act_phase: parity for act_bar(j)
+      int tile_local = 0;
+      for (int64_t tile = pid; tile < num_tiles; tile += num_pairs, ++tile_local) {
+        const int gb = tile_local & 1;
+        const int g_row = (cta_global * 2 + gb) * kTileM;
+        for (int l = 0; l < p.n_hidden; ++l) {
+          const int nk0 = p.nkb0[l], nk1 = p.nkb1[l];
+          const CUtensorMap* amap = (l == 0) ? &p.g : (((l - 1) & 1) ? &p.x1 : &p.x0);
+          const int a_row = (l == 0) ? g_row : cta_global * kTileM;
+          for (int c = 0; c < p.n_chunks; ++c) {
+            for (int kb = 0; kb < nk0 + nk1; ++kb) {
+              if (c == 0 && kb < nk0) {
+                if (l == 0) {
+                  if (kb == 0) wait_bar<false>(gready_bar(gb), (tile_local >> 1) & 1, p.dbg, 0x100 + gb);
+                } else if ((kb & 3) == 0) {
+                  const int j = kb >> 2;
+                  wait_bar<false>(act_bar(j), (act_phase >> j) & 1u, p.dbg, 0x200 + j);
+                  act_phase ^= (1u << j);
+                }
+              }
+              const int s = it % S; const uint32_t ph = (it / S) & 1u;
+              wait_bar<CG == 2>(empty_bar(s), ph ^ 1u, p.dbg, 0x300 + s);
+              const int brow = c * kChunkN + (CG == 2 ? (int)rank * 128 : 0);
+              if (CG == 2) {
+                if (leader) ptx::mbar_arrive_expect_tx(full_bar(s), 2u * Cfg::kStageBytes);
+                const uint32_t fb = ptx::mapa(full_bar(s), 0);
+                if (kb < nk0) ptx::tma_load_2d_cg2(a_smem(s), amap, fb, kb * kKBlock, a_row);
+                else          ptx::tma_load_2d_cg2(a_smem(s), &p.g, fb, (kb - nk0) * kKBlock, g_row);
+                ptx::tma_load_2d_cg2(b_smem(s), &p.w[l], fb, kb * kKBlock, brow);
+              } else {
+                ptx::mbar_arrive_expect_tx(full_bar(s), (uint32_t)Cfg::kStageBytes);
+                if (kb < nk0) ptx::tma_load_2d(a_smem(s), amap, full_bar(s), kb * kKBlock, a_row);
+                else          ptx::tma_load_2d(a_smem(s), &p.g, full_bar(s), (kb - nk0) * kKBlock, g_row);
+                ptx::tma_load_2d(b_smem(s), &p.w[l], full_bar(s), kb * kKBlock, brow);
+                ptx::tma_load_2d(b_smem(s) + 128 * kKBlock * 2, &p.w[l], full_bar(s), kb * kKBlock, brow + 128);
+              }
+              ++it;
+            }
+          }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ================================================================ MMA issuer
+    if (lane == 0 && leader) {
+      constexpr uint32_t idesc = ptx::idesc_bf16_f32(128 * CG, kChunkN);
+      uint32_t it = 0, cc = 0;
+      int tile_local = 0;
+      for (int64_t tile = pid; tile < num_tiles; tile += num_pairs, ++tile_local) {
+        const int gb = tile_local & 1;
+        for (int l = 0; l < p.n_hidden; ++l) {
+          const int nk0 = p.nkb0[l], nk1 = p.nkb1[l], nk = nk0 + nk1;
+          for (int c = 0; c < p.n_chunks; ++c, ++cc) {
+            const uint32_t buf = cc & 1u, use = cc >> 1;
+            wait_bar<CG == 2>(tempty_bar(buf), (use & 1u) ^ 1u, p.dbg, 0x400 + buf);
+            ptx::tc_fence_after();
+            const uint32_t d_tmem = tmem_base + buf * kChunkN;
+            for (int kb = 0; kb < nk; ++kb, ++it) {
+              const int s = it % S; const uint32_t ph = (it / S) & 1u;
+              wait_bar<CG == 2>(full_bar(s), ph, p.dbg, 0x500 + s);
+              ptx::tc_fence_after();
+              const bool g_last = (l == 0) ? (kb == nk0 - 1) : (kb == nk - 1 && nk1 > 0);
+              const int nk16 = g_last ? p.g_last_nk16 : 4;
+              const uint64_t adesc = ptx::smem_desc_k_sw128(a_smem(s));
+              const uint64_t bdesc = ptx::smem_desc_k_sw128(b_smem(s));
+              for (int k = 0; k < nk16; ++k)
+                ptx::umma_bf16<CG>(d_tmem, adesc + 2u * k, bdesc + 2u * k, idesc, (uint32_t)((kb | k) != 0));
+              ptx::umma_commit<CG>(empty_bar(s));
+              if (l == gamma_layer && c == p.n_chunks - 1 && kb == nk - 1) ptx::umma_commit<CG>(gfree_bar(gb));
+            }
+            ptx::umma_commit<CG>(tfull_bar(buf));
+          }
+        }
+      }
+    }
+  } else if (warp >= 4 && warp < 8) {
+    // ================================================================ epilogue
+    const int q = warp & 3;
+    const int row = q * 32 + lane;
+    const uint32_t tempty_remote = (CG == 2) ? ptx::mapa(tempty_bar(0), 0) : 0u;
+    uint32_t cc = 0;
+    for (int64_t tile = pid; tile < num_tiles; tile += num_pairs) {
+      const int64_t grow = tile * tile_rays + (int64_t)rank * kTileM + row;
+      const bool valid = grow < n;
+      float z0 = 0.0f, z1 = 0.0f;
+      for (int l = 0; l < p.n_hidden; ++l) {
+        __nv_bfloat16* xout = ((l & 1) ? p.x1p : p.x0p) + ((size_t)cta_global * kTileM + row) * p.width;
+        const float* bias = p.bias + p.b_off[l];
+        for (int c = 0; c < p.n_chunks; ++c, ++cc) {
+          const uint32_t buf = cc & 1u, use = cc >> 1;
+          wait_bar<CG == 2>(tfull_bar(buf), use & 1u, p.dbg, 0x600 + buf);
+          ptx::tc_fence_after();
+          const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + buf * kChunkN;
+          #pragma unroll 1
+          for (int piece = 0; piece < kChunkN / 32; ++piece) {
+            uint32_t r[32];
+            ptx::tmem_ld32(taddr + piece * 32, r);
+            ptx::tmem_ld_wait();
+            if (piece == kChunkN / 32 - 1) {
+              ptx::tc_fence_before();
+              if (CG == 2) ptx::mbar_arrive_cluster(tempty_remote + 8u * buf);
+              else ptx::mbar_arrive(tempty_bar(buf));
+            }
+            const int col = c * kChunkN + piece * 32;
+            const float4* b4 = reinterpret_cast<const float4*>(bias + col);
+            float v[32];
+            #pragma unroll
+            for (int i = 0; i < 8; ++i) {
+              float4 bb = __ldg(b4 + i);
+              v[4 * i + 0] = fmaxf(__uint_as_float(r[4 * i + 0]) + bb.x, 0.0f);
+              v[4 * i + 1] = fmaxf(__uint_as_float(r[4 * i + 1]) + bb.y, 0.0f);
+              v[4 * i + 2] = fmaxf(__uint_as_float(r[4 * i + 2]) + bb.z, 0.0f);
+              v[4 * i + 3] = fmaxf(__uint_as_float(r[4 * i + 3]) + bb.w, 0.0f);
+            }
+            if (l < last_layer) {
+              uint4* dst = reinterpret_cast<uint4*>(xout + col);
+              #pragma unroll
+              for (int i = 0; i < 4; ++i) {
+                uint4 pk;
+                __nv_bfloat162 t0 = __floats2bfloat162_rn(v[8 * i + 0], v[8 * i + 1]);
+                __nv_bfloat162 t1 = __floats2bfloat162_rn(v[8 * i + 2], v[8 * i + 3]);
+                __nv_bfloat162 t2 = __floats2bfloat162_rn(v[8 * i + 4], v[8 * i + 5]);
+                __nv_bfloat162 t3 = __floats2bfloat162_rn(v[8 * i + 6], v[8 * i + 7]);
+                pk.x = *reinterpret_cast<uint32_t*>(&t0); pk.y = *reinterpret_cast<uint32_t*>(&t1);
+                pk.z = *reinterpret_cast<uint32_t*>(&t2); pk.w = *reinterpret_cast<uint32_t*>(&t3);
+                dst[i] = pk;
+              }
+            } else {
+              const float4* w0 = reinterpret_cast<const float4*>(p.head_w + col);
+              #pragma unroll
+              for (int i = 0; i < 8; ++i) {
+                float4 ww = __ldg(w0 + i);
+                z0 = fmaf(v[4 * i + 0], ww.x, z0); z0 = fmaf(v[4 * i + 1], ww.y, z0);
+                z0 = fmaf(v[4 * i + 2], ww.z, z0); z0 = fmaf(v[4 * i + 3], ww.w, z0);
+              }
+              if (p.n_out == 2) {
+                const float4* w1 = reinterpret_cast<const float4*>(p.head_w + p.width + col);
+                #pragma unroll
+                for (int i = 0; i < 8; ++i) {
+                  float4 ww = __ldg(w1 + i);
+                  z1 = fmaf(v[4 * i + 0], ww.x, z1); z1 = fmaf(v[4 * i + 1], ww.y, z1);
+                  z1 = fmaf(v[4 * i + 2], ww.z, z1); z1 = fmaf(v[4 * i + 3], ww.w, z1);
+                }
+              }
+            }
+          }
+          if (l < last_layer) {
+            ptx::fence_proxy_async();
+            __threadfence();
+            ptx::mbar_arrive(act_bar(c));
+          }
+        }
+      }
+      // ---- fused heads (t = distance, xi = visibility)
+      z0 += p.bias[p.b_off[p.n_hidden]];
+      if (p.n_out == 2) z1 += p.bias[p.b_off[p.n_hidden] + 1];
+      if (p.mode_out == 1) {
+        if (valid) { p.out0[grow * p.n_out] = z0; if (p.n_out == 2) p.out0[grow * p.n_out + 1] = z1; }
+      } else if (p.mode_out == 0) {
+        if (valid) {
+          if (p.n_out == 2) { p.out0[grow] = softplus_f(z0); if (p.out1) p.out1[grow] = sigmoid_f(z1); }
+          else p.out0[grow] = z0;
+        }
+      } else {
+        // AO: 1 - mean over the pixel's spp consecutive rays of (xi > 0.5 and t < ao_radius)
+        const bool hit = valid && (sigmoid_f(z1) > 0.5f) && (softplus_f(z0) < p.ao_radius);
+        const uint32_t m = __ballot_sync(0xffffffffu, hit);
+        const int g0 = (lane / p.spp) * p.spp;
+        const uint32_t bits = (p.spp == 32) ? m : ((m >> g0) & ((1u << p.spp) - 1u));
+        if (valid && (lane % p.spp) == 0) p.out0[grow / p.spp] = 1.0f - (float)__popc(bits) / (float)p.spp;
+      }
+    }
+  } else if (warp >= 8) {
+    // ================================================================ encoder
+    const int row = (warp - 8) * 32 + lane;
+    int tile_local = 0;
+    for (int64_t tile = pid; tile < num_tiles; tile += num_pairs, ++tile_local) {
+      const int gb = tile_local & 1;
+      wait_bar<CG == 2>(gfree_bar(gb), ((tile_local >> 1) & 1) ^ 1, p.dbg, 0x700 + gb);
+      const int64_t grow = tile * tile_rays + (int64_t)rank * kTileM + row;
+      __align__(16) __nv_bfloat16 enc[256];
+      #pragma unroll 1
+      for (int k = 0; k < p.E_pad; ++k) enc[k] = __float2bfloat16_rn(0.0f);
+      if (grow < n) {
+        float v[3] = { p.o[3 * grow], p.o[3 * grow + 1], p.o[3 * grow + 2] };
+        encode_vec_bf16(v, p.Lo, enc);
+        if (p.input_kind == 0) {
+          float w[3] = { p.d[3 * grow], p.d[3 * grow + 1], p.d[3 * grow + 2] };
+          encode_vec_bf16(w, p.Ld, enc + 3 + 6 * p.Lo);
+        }
+      }
+      uint4* dst = reinterpret_cast<uint4*>(p.gp + ((size_t)(cta_global * 2 + gb) * kTileM + row) * p.E_pad);
+      const uint4* src = reinterpret_cast<const uint4*>(enc);
+      #pragma unroll 1
+      for (int k = 0; k < p.E_pad / 8; ++k) dst[k] = src[k];
+      ptx::fence_proxy_async();
+      __threadfence();
+      ptx::mbar_arrive(gready_bar(gb));
+    }
+  }
+
+  ptx::tc_fence_before();
+  if (CG == 2) ptx::cluster_sync(); else __syncthreads();
+  if (warp == 2) ptx::tmem_dealloc<CG>(tmem_base, 512);
+}
+
+// ------------------------------------------------------------------------------------------ host
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static EncodeTiledFn get_encode_fn() {
+  static EncodeTiledFn fn = nullptr;
+  if (!fn) {
+    void* sym = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &sym, cudaEnableDefault, &qres) != cudaSuccess ||
+        qres != cudaDriverEntryPointSuccess)
+      return nullptr;
+    fn = (EncodeTiledFn)sym;
+  }
+  return fn;
+}
+
+// bf16 row-major [rows][cols] with row pitch `pitch_elems`; box = 64 columns x 128 rows, 128B swizzle
+static int make_map(CUtensorMap* out, void* base, uint64_t cols, uint64_t rows, uint64_t pitch_elems) {
+  EncodeTiledFn fn = get_encode_fn();
+  if (!fn) return DDF_E_UNSUPPORTED;
+  cuuint64_t dims[2] = { cols, rows };
+  cuuint64_t strides[1] = { pitch_elems * 2 };
+  cuuint32_t box[2] = { (cuuint32_t)kKBlock, 128u };
+  cuuint32_t estr[2] = { 1u, 1u };
+  CUresult r = fn(out, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, base, dims, strides, box, estr,
+                  CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                  CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return r == CUDA_SUCCESS ? DDF_OK : DDF_E_CUDA;
+}
+
+void tc_plan_destroy(Model* m) {
+  if (!m->tc) return;
+  cudaFree(m->tc->x0); cudaFree(m->tc->x1); cudaFree(m->tc->g);
+  if (m->tc->dbg_host) cudaFreeHost(m->tc->dbg_host);
+  delete m->tc;
+  m->tc = nullptr;
+}
+
+int tc_plan_create(Model* m) {
+  m->tc = nullptr;
+  const ddf_layout& L = m->lay;
+  // shapes this kernel serves: width a multiple of 256 (whole accumulator chunks), <= 16 layers
+  if (L.width % kChunkN != 0 || L.width / kChunkN > (uint32_t)kMaxChunks) return DDF_OK;
+  if (L.n_hidden > (uint32_t)kMaxTcLayers || m->E_pad > 256) return DDF_OK;
+  TcPlan* t = new (std::nothrow) TcPlan();
+  if (!t) return DDF_E_NOMEM;
+  memset(t, 0, sizeof(TcPlan));
+  m->tc = t;
+  const char* env = getenv("DDF_TC_CTA_GROUP");
+  t->cg = (env && env[0] == '1') ? 1 : 2;
+  t->grid = (m->sm_count / 2) * 2;
+  const size_t rows = (size_t)t->grid * kTileM;
+  DDF_CUDA_TRY(cudaMalloc(&t->x0, rows * L.width * 2));
+  DDF_CUDA_TRY(cudaMalloc(&t->x1, rows * L.width * 2));
+  DDF_CUDA_TRY(cudaMalloc(&t->g, rows * 2 * m->E_pad * 2));
+  DDF_CUDA_TRY(cudaMemset(t->x0, 0, rows * L.width * 2));
+  DDF_CUDA_TRY(cudaMemset(t->x1, 0, rows * L.width * 2));
+  DDF_CUDA_TRY(cudaMemset(t->g, 0, rows * 2 * m->E_pad * 2));
+  DDF_CUDA_TRY(cudaHostAlloc(&t->dbg_host, 64, cudaHostAllocMapped));
+  memset(t->dbg_host, 0, 64);
+  DDF_CUDA_TRY(cudaHostGetDevicePointer((void**)&t->dbg_dev, t->dbg_host, 0));
+
+  TcParams& p = t->base;
+  int rc;
+  for (int l = 0; l < (int)L.n_hidden; ++l) {
+    const LayerDesc& d = m->layers[l];
+    rc = make_map(&p.w[l], m->d_w + d.w_off, (uint64_t)d.k_pad, (uint64_t)round_up(d.n_out, 128), (uint64_t)d.k_pad);
+    if (rc != DDF_OK) return rc;
+    p.nkb0[l] = d.k0_pad / kKBlock; p.nkb1[l] = d.k1_pad / kKBlock;
+    p.b_off[l] = (int)d.b_off;
+  }
+  p.b_off[L.n_hidden] = (int)m->layers[L.n_hidden].b_off;
+  if ((rc = make_map(&p.x0, t->x0, L.width, rows, L.width)) != DDF_OK) return rc;
+  if ((rc = make_map(&p.x1, t->x1, L.width, rows, L.width)) != DDF_OK) return rc;
+  if ((rc = make_map(&p.g, t->g, (uint64_t)m->E_pad, rows * 2, (uint64_t)m->E_pad)) != DDF_OK) return rc;
+  p.bias = m->d_b; p.head_w = m->d_head_w;
+  p.x0p = t->x0; p.x1p = t->x1; p.gp = t->g;
+  p.dbg = t->dbg_dev;
+  p.n_hidden = (int)L.n_hidden; p.width = (int)L.width; p.n_chunks = (int)L.width / kChunkN;
+  p.skip_layer = L.skip_layer; p.n_out = (int)L.n_out; p.input_kind = (int)L.input_kind;
+  p.Lo = (int)L.n_freq_origin; p.Ld = (int)L.n_freq_dir; p.E = m->E; p.E_pad = m->E_pad;
+  p.g_last_nk16 = (m->E - (m->E_pad - kKBlock) + 15) / 16;
+  DDF_CUDA_TRY(cudaFuncSetAttribute(ddf_tc_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, TcCfg<1>::kSmemBytes));
+  DDF_CUDA_TRY(cudaFuncSetAttribute(ddf_tc_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, TcCfg<2>::kSmemBytes));
+  return DDF_OK;
+}
+
+int tc_forward(Model* m, const float* o, const float* d, int64_t n, const int64_t* n_dev, int mode_out,
+               float* out0, float* out1, int spp, float ao_radius, cudaStream_t st) {
+  TcPlan* t = m->tc;
+  if (!t) return DDF_E_UNSUPPORTED;
+  if (t->dbg_host[0] != 0) return DDF_E_CUDA;           // an earlier launch tripped a bounded wait
+  TcParams p = t->base;
+  p.o = o; p.d = d; p.n = n; p.n_dev = n_dev;
+  p.out0 = out0; p.out1 = out1; p.mode_out = mode_out; p.spp = spp > 0 ? spp : 1; p.ao_radius = ao_radius;
+  const int64_t tile_rays = (int64_t)kTileM * t->cg;
+  int64_t tiles = (n + tile_rays - 1) / tile_rays;
+  int grid = t->grid;
+  if (tiles * t->cg < grid) grid = (int)tiles * t->cg;   // n_dev can only shrink n
+  cudaLaunchConfig_t cfg;
+  memset(&cfg, 0, sizeof(cfg));
+  cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3(kThreads); cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeClusterDimension;
+  attr[0].val.clusterDim.x = (unsigned)t->cg; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+  cfg.attrs = attr; cfg.numAttrs = 1;
+  if (t->cg == 2) {
+    cfg.dynamicSmemBytes = TcCfg<2>::kSmemBytes;
+    DDF_CUDA_TRY(cudaLaunchKernelEx(&cfg, ddf_tc_kernel<2>, p));
+  } else {
+    cfg.dynamicSmemBytes = TcCfg<1>::kSmemBytes;
+    DDF_CUDA_TRY(cudaLaunchKernelEx(&cfg, ddf_tc_kernel<1>, p));
+  }
+  m->last_launches = 1;
+  return DDF_OK;
+}
+
+}  // namespace ddf

@@ -1,0 +1,138 @@
+// ddf_trace.cu - sphere tracing of an SDF MLP, the comparison point of PAPER.md:19 / 112 and
+// Table IV: "a sequential loop, and each iteration is a full evaluation".
+// Step rule and the traced function s(p) = (|p| - R) + alpha MLP(p): include/ddf.h.
+// Per step: points kernel -> MLP forward (same kernels as ddf_query) -> update kernel.  With
+// early_exit the live rays are compacted into an index list whose length stays on the device.
+#include "ddf_common.cuh"
+#include <math.h>
+
+namespace ddf {
+
+struct TraceWs {
+  float* pts;        // [n][3] compacted points of the current step
+  float* z;          // [n]    MLP output for them
+  int32_t* idx[2];   // live-ray lists (ping-pong)
+  int64_t* counts;   // [max_steps + 2] live count entering each step; last = total evals
+  uint8_t* done;     // [n]
+};
+
+__global__ void trace_init_kernel(int64_t n, float* t, uint8_t* hit, int32_t* steps, uint8_t* done,
+                                  int32_t* idx0, int64_t* counts, int n_counts,
+                                  float* trace_p, float* trace_s, int max_steps) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i == 0) { for (int k = 0; k < n_counts; ++k) counts[k] = 0; counts[0] = n; }
+  const float qnan = __int_as_float(0x7fc00000);
+  if (i < n) { t[i] = 0.0f; hit[i] = 0; steps[i] = 0; done[i] = 0; idx0[i] = (int32_t)i; }
+  if (trace_s) for (int64_t k = i; k < n * max_steps; k += (int64_t)gridDim.x * blockDim.x) trace_s[k] = qnan;
+  if (trace_p) for (int64_t k = i; k < n * max_steps * 3; k += (int64_t)gridDim.x * blockDim.x) trace_p[k] = qnan;
+}
+
+__global__ void trace_points_kernel(const int32_t* __restrict__ idx, const int64_t* __restrict__ count,
+                                    const float* __restrict__ o, const float* __restrict__ d,
+                                    const float* __restrict__ t, float* __restrict__ pts, int64_t* total) {
+  int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int64_t cnt = *count;
+  if (j == 0 && total) *total += cnt;
+  if (j >= cnt) return;
+  int64_t i = idx[j];
+  float tt = t[i];
+  #pragma unroll
+  for (int a = 0; a < 3; ++a) pts[3 * j + a] = fmaf(tt, d[3 * i + a], o[3 * i + a]);
+}
+
+__global__ void trace_update_kernel(const int32_t* __restrict__ idx_in, const int64_t* __restrict__ count_in,
+                                    const float* __restrict__ pts, const float* __restrict__ z,
+                                    int step, sdf_trace_params prm,
+                                    float* __restrict__ t, uint8_t* __restrict__ hit, int32_t* __restrict__ steps,
+                                    uint8_t* __restrict__ done, int32_t* __restrict__ idx_out, int64_t* count_out,
+                                    float* __restrict__ trace_p, float* __restrict__ trace_s) {
+  int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= *count_in) return;
+  int64_t i = idx_in[j];
+  if (done[i]) return;                                   // fixed-step mode keeps finished rays in the list
+  float px = pts[3 * j], py = pts[3 * j + 1], pz = pts[3 * j + 2];
+  float n2 = fmaf(pz, pz, fmaf(py, py, px * px));
+  float s = fmaf(prm.alpha, z[j], sqrtf(n2) - prm.base_radius);
+  steps[i] = step + 1;
+  if (trace_s) trace_s[i * prm.max_steps + step] = s;
+  if (trace_p) { float* q = trace_p + (i * prm.max_steps + step) * 3; q[0] = px; q[1] = py; q[2] = pz; }
+  bool fin = false;
+  if (fabsf(s) < prm.eps) { hit[i] = 1; fin = true; }
+  else {
+    float tt = t[i] + s;
+    t[i] = tt;
+    if (tt > prm.t_max || tt < 0.0f) fin = true;
+  }
+  if (fin) done[i] = 1;
+  else if (prm.early_exit) {
+    unsigned long long pos = atomicAdd((unsigned long long*)count_out, 1ull);
+    idx_out[pos] = (int32_t)i;
+  }
+}
+
+}  // namespace ddf
+
+using namespace ddf;
+
+extern "C" int sdf_sphere_trace(ddf_model* model, const float* o, const float* d, int64_t n,
+                                const sdf_trace_params* prm, float* out_t, uint8_t* out_hit,
+                                int32_t* out_steps, float* trace_p, float* trace_s, int64_t* total_evals,
+                                void* stream) {
+  if (!model || !prm || n < 0 || n > 0x7fffffff) return DDF_E_INVALID_ARG;
+  Model* m = reinterpret_cast<Model*>(model);
+  if (m->lay.input_kind != 1 || m->lay.n_out != 1) return DDF_E_INVALID_ARG;
+  if (prm->max_steps < 1 || prm->max_steps > 4096) return DDF_E_INVALID_ARG;
+  if (n == 0) return DDF_OK;
+  if (!o || !d || !out_t || !out_hit || !out_steps) return DDF_E_INVALID_ARG;
+  cudaStream_t st = (cudaStream_t)stream;
+  const int S = prm->max_steps;
+  // workspace: pts 12n, z 4n, idx 2*4n, done n, counts
+  const size_t a = (size_t)((n + 63) / 64 * 64);
+  const size_t need = a * 12 + a * 4 + a * 8 + a + (size_t)(S + 2) * 8;
+  if (need > m->trace_ws_bytes) {
+    cudaFree(m->trace_ws); m->trace_ws = nullptr; m->trace_ws_bytes = 0;
+    DDF_CUDA_TRY(cudaMalloc(&m->trace_ws, need));
+    m->trace_ws_bytes = need;
+  }
+  uint8_t* base = (uint8_t*)m->trace_ws;
+  TraceWs w;
+  w.pts = (float*)base;                 base += a * 12;
+  w.z = (float*)base;                   base += a * 4;
+  w.idx[0] = (int32_t*)base;            base += a * 4;
+  w.idx[1] = (int32_t*)base;            base += a * 4;
+  w.counts = (int64_t*)base;            base += (size_t)(S + 2) * 8;
+  w.done = base;
+
+  const unsigned nb = (unsigned)((n + 255) / 256);
+  trace_init_kernel<<<nb, 256, 0, st>>>(n, out_t, out_hit, out_steps, w.done, w.idx[0], w.counts, S + 2,
+                                        trace_p, trace_s, S);
+  int launches = 1;
+  const bool use_tc = (m->tc && m->path != 1);
+  int64_t live = n;
+  for (int step = 0; step < S; ++step) {
+    const int cur = prm->early_exit ? (step & 1) : 0;
+    int64_t* cnt_in = prm->early_exit ? w.counts + step : w.counts;          // fixed mode: always n
+    int64_t* cnt_out = w.counts + step + 1;
+    const unsigned gb = (unsigned)((live + 255) / 256);
+    trace_points_kernel<<<gb, 256, 0, st>>>(w.idx[cur], cnt_in, o, d, out_t, w.pts, w.counts + S + 1);
+    int rc;
+    if (use_tc) rc = tc_forward(m, w.pts, nullptr, live, cnt_in, 1, w.z, nullptr, 0, 0.0f, st);
+    else rc = simt_forward(m, w.pts, nullptr, live, 1, w.z, nullptr, st);
+    if (rc != DDF_OK) return rc;
+    launches += 1 + m->last_launches;
+    trace_update_kernel<<<gb, 256, 0, st>>>(w.idx[cur], cnt_in, w.pts, w.z, step, *prm, out_t, out_hit,
+                                           out_steps, w.done, w.idx[cur ^ 1], cnt_out, trace_p, trace_s);
+    ++launches;
+    if (prm->early_exit && !use_tc) {
+      // the SIMT path sizes its grids on the host: read the live count back (synchronises)
+      DDF_CUDA_TRY(cudaMemcpyAsync(&live, cnt_out, 8, cudaMemcpyDeviceToHost, st));
+      DDF_CUDA_TRY(cudaStreamSynchronize(st));
+      if (live == 0) break;
+    }
+  }
+  if (total_evals)
+    DDF_CUDA_TRY(cudaMemcpyAsync(total_evals, w.counts + S + 1, 8, cudaMemcpyDeviceToDevice, st));
+  DDF_CUDA_TRY(cudaGetLastError());
+  m->last_launches = launches;
+  return DDF_OK;
+}

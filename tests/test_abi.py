@@ -1,0 +1,110 @@
+"""The C-ABI library loads and exports every symbol include/ddf.h declares; argument checks that
+need no GPU (host logic).  No compute call is made here."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def libddf():
+    from paper_2606_00817_b200 import build, lib
+    build()
+    return lib()
+
+
+def _declared_symbols():
+    src = open(os.path.join(ROOT, "include", "ddf.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    names = re.findall(r"\b((?:ddf|sdf)_[a-z_0-9]+)\s*\(", src)
+    return sorted(set(names))
+
+
+def test_every_declared_symbol_is_exported(libddf):
+    from paper_2606_00817_b200 import EXPORTED_SYMBOLS
+    decl = _declared_symbols()
+    assert len(decl) >= 19
+    for name in decl:
+        assert hasattr(libddf, name), name
+    assert sorted(EXPORTED_SYMBOLS) == decl
+
+
+def test_binding_mirrors_the_header():
+    import paper_2606_00817_b200 as pkg
+    for name in _declared_symbols():
+        if name in ("ddf_last_cuda_error",):
+            continue
+        assert hasattr(pkg, name), name
+
+
+def test_status_strings(libddf):
+    from paper_2606_00817_b200 import ddf_status_string
+    assert ddf_status_string(0) == "ok"
+    assert ddf_status_string(-1) == "invalid argument"
+    assert ddf_status_string(-2) == "bad layout"
+    assert "unknown" in ddf_status_string(-99)
+
+
+def test_layout_struct_matches_header():
+    from paper_2606_00817_b200 import DdfLayout, DdfCamera, DdfScene, SdfTraceParams
+    assert C.sizeof(DdfLayout) == 44 and C.sizeof(DdfCamera) == 28 and C.sizeof(DdfScene) == 40
+    assert C.sizeof(SdfTraceParams) == 24
+
+
+def test_argument_errors_without_gpu(libddf):
+    from paper_2606_00817_b200 import DdfLayout, DdfCamera
+    h = C.c_void_p(0)
+    assert libddf.ddf_create(None, None, C.byref(h)) == -1
+    bad = DdfLayout(44, 99, 0, 4, 4, 3, 64, -1, 2, 0, 0)                 # wrong version
+    w = np.zeros(16, np.float32)
+    assert libddf.ddf_create(w.ctypes.data_as(C.c_void_p), C.byref(bad), C.byref(h)) == -2
+    bad = DdfLayout(44, 1, 0, 4, 4, 3, 64, 3, 2, 0, 0)                   # skip_layer out of range
+    assert libddf.ddf_create(w.ctypes.data_as(C.c_void_p), C.byref(bad), C.byref(h)) == -2
+    bad = DdfLayout(44, 1, 0, 4, 4, 3, 64, -1, 3, 0, 0)                  # n_out
+    assert libddf.ddf_create(w.ctypes.data_as(C.c_void_p), C.byref(bad), C.byref(h)) == -2
+    assert libddf.ddf_destroy(None) == 0
+    assert libddf.ddf_query(None, None, None, C.c_int64(0), None, None, None) == -1
+    assert libddf.ddf_gen_camera(None, 4, 4, None, None, None) == -1
+    cam = DdfCamera()
+    assert libddf.ddf_gen_camera(C.byref(cam), 0, 0, None, None, None) == 0     # n == 0 is a no-op
+    assert libddf.ddf_gen_sphere_points(C.c_uint64(1), C.c_uint64(1), C.c_int64(-1), C.c_float(1), None, None, None) == -1
+    assert libddf.ddf_ao_reduce(None, None, C.c_int64(0), 16, C.c_float(1), None, None) == 0
+    assert libddf.ddf_ao_reduce(None, None, C.c_int64(4), 0, C.c_float(1), None, None) == -1
+
+
+def test_camera_from_seed_matches_oracle_twin(libddf, orc):
+    from ddf_inputs import MASTER_SEED, STREAMS
+    from paper_2606_00817_b200 import ddf_camera_from_seed
+    cam = ddf_camera_from_seed(MASTER_SEED, STREAMS["camera_pos"], 2.5)
+    want = orc.camera_from_seed(MASTER_SEED, STREAMS["camera_pos"], 2.5)
+    assert np.allclose(list(cam.pos), list(want.pos), atol=3e-7)
+    assert cam.fov_deg == 50.0 and list(cam.look_at) == [0, 0, 0]
+
+
+def test_no_gpu_means_loud_failure(libddf):
+    """Without a CUDA device ddf_create must fail (no CPU fallback)."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    from ddf_inputs import layout_c0, make_weights
+    from paper_2606_00817_b200 import ddf_create, DdfError
+    with pytest.raises(DdfError):
+        ddf_create(make_weights(layout_c0()), layout_c0())
+
+
+def test_product_does_not_import_oracle():
+    pkg = os.path.join(ROOT, "paper_2606_00817_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                src = open(os.path.join(dirpath, f)).read()
+                assert "import oracle" not in src and "from oracle" not in src and "ddf_oracle" not in src, f
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith((".py", ".c", ".h")):
+            src = open(os.path.join(ROOT, "oracle", f)).read()
+            assert "paper_2606_00817_b200" not in src.replace("under paper_2606_00817_b200/", "").replace(
+                "the product (paper_2606_00817_b200)", ""), f
