@@ -1,0 +1,328 @@
+#!/usr/bin/env python
+"""bench.py - DDF ray queries/s on B200 (BASELINE.json metric), one JSON line on stdout.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--extras]
+
+A step = one pass of the hot path over one batch: the camera generator writes
+2^20 primary rays, then ONE fused launch (rows a1-a8: load, encode, 8 layers, heads, store) answers
+them.  Workload = BASELINE.json configs[1].  `value` is device-timed (CUDA events on the launching
+stream, inputs resident in HBM); `e2e` goes through ddf_query_host with pinned HOST buffers.
+N > 1 (torchrun): every rank runs the same per-GPU batch with its own camera (weak scaling, no
+data-path collective: rays are independent, weights replicated - DESIGN.md "Multi-GPU").
+"""
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+FLOP_PER_RAY = 23_403_520            # 2*(90*1280 + 6*1280^2 + 1370*1280 + 1280*2), DESIGN.md
+METRIC = "DDF ray queries/s"
+UNIT = "Mrays/s"
+WORKLOAD = "configs[1]: paper-scale DDF (90-dim enc, 8x1280, skip@4, bf16), 2^20 camera rays 1024x1024"
+# dram__bytes_read.sum + dram__bytes_write.sum of ddf_tc_kernel<2> for one 2^20-ray launch, from
+# the ncu --set full capture summarised in profiles/r01_ncu_summary.md (None until captured)
+NCU_DRAM_TRAFFIC_BYTES = None
+
+
+def _peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        j = json.load(open(p))
+        return dict(burst=float(j["bf16_tflops"]), sustained=float(j.get("bf16_tflops_sustained", j["bf16_tflops"])),
+                    hbm=float(j["hbm_gbs"]), source="measured (MEASURED_PEAKS.json)")
+    return dict(burst=1590.0, sustained=1400.0, hbm=6650.0, source="fallback (B200_PROFILING.md)")
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), [x.strip() for x in line.split(",")]))
+
+    def stop(self, t0, t1):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        rows = [r for (t, r) in self.rows if t0 <= t <= t1 + 0.1 and len(r) >= 7] or [r for (_, r) in self.rows if len(r) >= 7]
+        if not rows:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [nm for k, nm in enumerate(names) if any(r[3 + k].lower().startswith("active") for r in rows)]
+        f = lambda s: float(s) if s.replace(".", "", 1).isdigit() else float("nan")
+        return {"sm_mhz": statistics.median(f(r[0]) for r in rows), "sm_max_mhz": f(rows[0][1]),
+                "power_w_max": max(f(r[2]) for r in rows), "samples": len(rows), "reasons": reasons}
+
+
+def oracle_rate(seconds_target=12.0, mode=0):
+    """rays/s of the oracle as it stands on this box's host cores, on a bounded sample of the
+    configs[1] workload (camera rays through the paper-scale network)."""
+    import oracle
+    from ddf_inputs import MASTER_SEED, STREAMS, layout_c1, make_weights
+    oracle.build()
+    lay = layout_c1()
+    blob = make_weights(lay)
+    cam = oracle.camera_from_seed(MASTER_SEED, STREAMS["camera_pos"], 2.5)
+    o, d = oracle.gen_camera(cam, 1024, 1024)
+    cores = oracle.default_threads()
+    probe = max(2 * cores, 64)
+    t0 = time.time(); oracle.forward(lay, blob, o[:probe], d[:probe], mode); tp = time.time() - t0
+    ns = int(min(1 << 17, max(probe, probe * seconds_target / max(tp, 1e-3))))
+    stride = (1 << 20) // ns
+    t0 = time.time(); oracle.forward(lay, blob, o[::stride][:ns], d[::stride][:ns], mode); dt = time.time() - t0
+    return ns / dt, cores, "%d camera rays (every %d-th pixel of the 1024x1024 batch), %.1f s" % (ns, stride, dt)
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores (rank 0 only)."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    rates = []
+    per = max(2.0, min(20.0, 60.0 / max(1, args.steps + args.warmup)))
+    sample = ""
+    for i in range(args.warmup + args.steps):
+        r, cores, sample = oracle_rate(per)
+        if i >= args.warmup:
+            rates.append(r)
+    v = statistics.mean(rates) / 1e6
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * per, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": WORKLOAD, "note": "CPU oracle (oracle/ddf_oracle.c), each step a bounded sample"},
+        "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+def shard_plan(world, rank, rays_per_gpu):
+    """Weak scaling: every rank answers its own `rays_per_gpu` camera batch (its own seeded camera);
+    no exchange step.  Returns (camera seed, first global ray index, rays)."""
+    from ddf_inputs import MASTER_SEED
+    return MASTER_SEED + rank, rank * rays_per_gpu, rays_per_gpu
+
+
+def aggregate(times_ms_local, rays_local, dist_mod, world):
+    """max-over-ranks time, sum-over-ranks rays -> whole-job Mrays/s (host logic, gloo-testable)."""
+    import torch
+    t = torch.tensor([float(times_ms_local)], dtype=torch.float64)
+    r = torch.tensor([float(rays_local)], dtype=torch.float64)
+    if world > 1:
+        dev = "cuda" if dist_mod.get_backend() == "nccl" else "cpu"
+        t, r = t.to(dev), r.to(dev)
+        dist_mod.all_reduce(t, op=dist_mod.ReduceOp.MAX)
+        dist_mod.all_reduce(r, op=dist_mod.ReduceOp.SUM)
+    return float(r.item()) / float(t.item()) / 1e3, float(t.item())
+
+
+def run_gpu(args):
+    import torch
+    import torch.distributed as dist
+    import paper_2606_00817_b200 as ddf
+    from ddf_inputs import STREAMS, layout_c1, layout_sdf, make_weights, random_rays
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device - there is no CPU fallback (use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl")
+    ddf.build()
+    K, W = args.steps, max(args.warmup, 3)
+    n = 1 << 20
+    seed, _, _ = shard_plan(world, rank, n)
+    lay = layout_c1()
+    model = ddf.ddf_create(make_weights(lay), lay)
+    assert ddf.ddf_get_info(model, 0) == 1
+    cam = ddf.ddf_camera_from_seed(seed, STREAMS["camera_pos"], 2.5)
+    o = torch.empty((n, 3), device="cuda"); d = torch.empty((n, 3), device="cuda")
+    dist_o = torch.empty(n, device="cuda"); vis_o = torch.empty(n, device="cuda")
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")          # > 126 MB L2
+
+    def step(ev=None):
+        if ev: ev[0].record()
+        ddf.ddf_gen_camera(cam, 1024, 1024, o, d)
+        if ev: ev[1].record()
+        ddf.ddf_query(model, o, d, n, dist_o, vis_o)
+        if ev: ev[2].record()
+
+    for _ in range(W):
+        flush.zero_(); step()
+    torch.cuda.synchronize()
+    if world > 1: dist.barrier()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local); sampler.start(); t_wall0 = time.time()
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(K)]
+    for k in range(K):
+        flush.zero_()                       # L2 flush between timed iterations (outside the event pairs)
+        step(evs[k])
+    torch.cuda.synchronize()
+    if world > 1: dist.barrier()
+    torch.cuda.synchronize()
+    t_wall1 = time.time()
+    clocks = sampler.stop(t_wall0, t_wall1)
+    step_ms = [e[0].elapsed_time(e[2]) for e in evs]
+    kern_ms = [e[1].elapsed_time(e[2]) for e in evs]
+    value, t_max = aggregate(sum(step_ms), n * K, dist, world)
+    launches = K * 2                        # gen_camera_kernel + ddf_tc_kernel per step
+
+    # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
+    oh, dh = o.cpu().pin_memory(), d.cpu().pin_memory()
+    dist_h, vis_h = torch.empty(n).pin_memory(), torch.empty(n).pin_memory()
+    for _ in range(2): ddf.ddf_query_host(model, oh, dh, n, dist_h, vis_h)
+    torch.cuda.synchronize()
+    if world > 1: dist.barrier()
+    t0 = time.perf_counter()
+    for _ in range(K): ddf.ddf_query_host(model, oh, dh, n, dist_h, vis_h)
+    torch.cuda.synchronize()
+    e2e_ms = (time.perf_counter() - t0) * 1e3
+    e2e_value, _ = aggregate(e2e_ms, n * K, dist, world)
+    assert torch.equal(dist_h, dist_o.cpu())
+
+    peaks = _peaks()
+    kern_avg = statistics.mean(kern_ms)
+    achieved = n * FLOP_PER_RAY / (kern_avg * 1e-3) / 1e12
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+        "ms_per_step": t_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "bf16", "data": "synthetic",
+        "config": {"workload": WORKLOAD, "rays_per_gpu": n, "parallelism": "replicas x%d, rays sharded" % world,
+                   "flop_per_ray": FLOP_PER_RAY, "l2": "512 MB memset between timed steps (L2 flush)",
+                   "step": "ddf_gen_camera + ddf_query"},
+        "clocks": clocks,
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 24 * n, "d2h_bytes_per_step": 8 * n},
+        "gpu_launches": launches,
+        "roofline": {"bound": "tensor", "kernel": "ddf_tc_kernel<2>", "achieved": achieved, "peak": peaks["burst"],
+                     "unit": "TFLOP/s", "frac": achieved / peaks["burst"], "traffic": NCU_DRAM_TRAFFIC_BYTES,
+                     "frac_of_sustained_peak": achieved / peaks["sustained"], "peak_source": peaks["source"],
+                     "kernel_ms": kern_avg, "kernel_share_of_step": kern_avg / statistics.mean(step_ms),
+                     "ray_io_GBps": 32 * n / (kern_avg * 1e-3) / 1e9},
+    }
+    if rank == 0:
+        if world == 1:
+            r, cores, sample = oracle_rate(12.0)
+            out["cpu_baseline"] = {"value": r / 1e6, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
+        if args.extras and world == 1:
+            out["extra"] = run_extras(ddf, torch, model, peaks)
+        print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def _time_ms(torch, fn, reps=3, warm=1):
+    for _ in range(warm): fn()
+    torch.cuda.synchronize()
+    ts = []
+    for _ in range(reps):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(); fn(); e1.record(); torch.cuda.synchronize()
+        ts.append(e0.elapsed_time(e1))
+    return statistics.median(ts)
+
+
+def run_extras(ddf, torch, model, peaks):
+    """The other BASELINE.json configs, each measured the same way (median of 3 after 1 warm-up):
+    shadow (configs[2]), AO with the on-GPU reduction (configs[3]), the batch sweep and the
+    sphere-tracing comparison (configs[4])."""
+    from ddf_inputs import MASTER_SEED, STREAMS, layout_sdf, make_weights, random_rays
+    ex = {}
+    tf = lambda n, ms: n * FLOP_PER_RAY / (ms * 1e-3) / 1e12
+    # ---- configs[2]: shadow rays
+    n = 1 << 22
+    p = torch.empty((n, 3), device="cuda"); nr = torch.empty((n, 3), device="cuda")
+    o = torch.empty((n, 3), device="cuda"); d = torch.empty((n, 3), device="cuda"); tm = torch.empty(n, device="cuda")
+    dist = torch.empty(n, device="cuda"); vis = torch.empty(n, device="cuda")
+    gen_ms = _time_ms(torch, lambda: (ddf.ddf_gen_sphere_points(MASTER_SEED, STREAMS["shadow_points"], n, 1.0, p, nr),
+                                      ddf.ddf_gen_shadow(p, nr, n, (3.0, 3.0, 3.0), 1e-3, o, d, tm)))
+    q_ms = _time_ms(torch, lambda: ddf.ddf_query(model, o, d, n, dist, vis))
+    ex["shadow_2^22"] = {"query_ms": q_ms, "Mrays_s": n / q_ms / 1e3, "TFLOPs": tf(n, q_ms), "frac_peak": tf(n, q_ms) / peaks["burst"],
+                         "gen_ms": gen_ms, "gen_GBps": (n * 24 + n * 52) / (gen_ms * 1e-3) / 1e9}
+    del p, nr, tm
+    # ---- configs[3]: AO, 1024x1024 x 16 spp, reduced on the GPU inside the query kernel
+    W = H = 1024; npts = W * H; spp = 16; n = npts * spp
+    cam = ddf.ddf_camera_from_seed(MASTER_SEED, STREAMS["camera_pos"], 2.5)
+    sc = ddf.DdfScene((0.0, 0.0, 0.0), 0.6, (-3.0, -3.0, -3.0), (3.0, 3.0, 3.0))
+    gp = torch.empty((npts, 3), device="cuda"); gn = torch.empty((npts, 3), device="cuda")
+    o = torch.empty((n, 3), device="cuda"); d = torch.empty((n, 3), device="cuda"); ao = torch.empty(npts, device="cuda")
+    gen_ms = _time_ms(torch, lambda: (ddf.ddf_gen_gbuffer(cam, sc, W, H, gp, gn, None),
+                                      ddf.ddf_gen_ao(gp, gn, npts, spp, MASTER_SEED, STREAMS["ao_samples"], 1e-3, o, d)))
+    q_ms = _time_ms(torch, lambda: ddf.ddf_query_ao(model, o, d, npts, spp, float("inf"), ao), reps=2)
+    ex["ao_16.7M"] = {"query_ao_ms": q_ms, "Mrays_s": n / q_ms / 1e3, "TFLOPs": tf(n, q_ms), "frac_peak": tf(n, q_ms) / peaks["burst"],
+                      "gen_ms": gen_ms, "gen_GBps": (n * 24 + npts * 24 * 2) / (gen_ms * 1e-3) / 1e9,
+                      "gen_frac_hbm": (n * 24 + npts * 24 * 2) / (gen_ms * 1e-3) / 1e9 / peaks["hbm"]}
+    # ---- configs[4]: batch sweep 2^10 .. 2^24 (prefixes of the AO ray buffer, incoherent rays)
+    sweep = {}
+    dist = torch.empty(n, device="cuda"); vis = torch.empty(n, device="cuda")
+    for lg in range(10, 25):
+        m = 1 << lg
+        ms = _time_ms(torch, lambda: ddf.ddf_query(model, o, d, m, dist, vis), reps=3 if lg > 20 else 7)
+        sweep["2^%d" % lg] = {"ms": ms, "ns_per_ray": ms * 1e6 / m, "Mrays_s": m / ms / 1e3, "frac_peak": tf(m, ms) / peaks["burst"]}
+    ex["sweep"] = sweep
+    del o, d, dist, vis, ao
+    # ---- configs[4]: sphere tracing an SDF MLP of the same width and depth on the camera rays
+    n = 1 << 20
+    lay = layout_sdf()
+    sdf = ddf.ddf_create(make_weights(lay), lay)
+    o = torch.empty((n, 3), device="cuda"); d = torch.empty((n, 3), device="cuda")
+    ddf.ddf_gen_camera(cam, 1024, 1024, o, d)
+    t = torch.empty(n, device="cuda"); hit = torch.empty(n, dtype=torch.uint8, device="cuda")
+    st = torch.empty(n, dtype=torch.int32, device="cuda"); tot = torch.zeros(1, dtype=torch.int64, device="cuda")
+    dist = torch.empty(n, device="cuda"); vis = torch.empty(n, device="cuda")
+    ddf_ms = _time_ms(torch, lambda: ddf.ddf_query(model, o, d, n, dist, vis))
+    SDF_FLOP = 23_262_720
+    for name, early in (("fixed64", 0), ("early_exit", 1)):
+        prm = ddf.SdfTraceParams(64, 1e-3, 6.0, 1.0, 0.05, early)
+        ms = _time_ms(torch, lambda: ddf.sdf_sphere_trace(sdf, o, d, n, prm, t, hit, st, None, None, tot), reps=2)
+        evals = int(tot.item())
+        ex["sphere_trace_" + name] = {"ms": ms, "Mrays_s": n / ms / 1e3, "mlp_evals": evals, "mean_steps": float(st.float().mean()),
+                                      "hit_rate": float(hit.float().mean()), "TFLOPs": evals * SDF_FLOP / (ms * 1e-3) / 1e12,
+                                      "ddf_speedup": ms / ddf_ms}
+    ex["ddf_camera_2^20_ms"] = ddf_ms
+    ddf.ddf_destroy(sdf)
+    return ex
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--extras", action="store_true", help="also measure shadow / AO / sweep / sphere tracing")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_gpu(args)
+
+
+if __name__ == "__main__":
+    main()

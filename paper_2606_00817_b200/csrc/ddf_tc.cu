@@ -39,13 +39,14 @@ template <int CG> struct TcCfg {
   static constexpr int kBBytes = (CG == 2 ? 128 : 256) * kKBlock * 2;
   static constexpr int kStageBytes = kABytes + kBBytes;
   static constexpr int kStages = (CG == 2) ? 6 : 4;
-  static constexpr int kBarBytes = 1024;
-  static constexpr int kSmemBytes = kStages * kStageBytes + kBarBytes + 1024;   // + alignment slack
+  static constexpr int kBarBytes = 2048;
+  static constexpr int kSmemBytes = kStages * kStageBytes + 8 * 4096 + kBarBytes + 1024;   // + alignment slack
 };
 
 struct TcParams {
   CUtensorMap w[kMaxTcLayers];
   CUtensorMap x0, x1, g;
+  CUtensorMap xs0, xs1;              // store maps (32-row boxes) on the same activation buffers
   const float* o; const float* d;
   int64_t n; const int64_t* n_dev;
   const float* bias; const float* head_w;
@@ -96,7 +97,8 @@ __global__ void __launch_bounds__(kThreads, 1) ddf_tc_kernel(const __grid_consta
   constexpr int S = Cfg::kStages;
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
-  const uint32_t bar_base = smem_base + S * Cfg::kStageBytes;
+  const uint32_t stg_base = smem_base + S * Cfg::kStageBytes;          // 8 x 4 KB epilogue staging boxes
+  const uint32_t bar_base = stg_base + 8u * 4096u;
   // barrier map (8 bytes each)
   auto full_bar   = [&](int s) { return bar_base + 8u * s; };
   auto empty_bar  = [&](int s) { return bar_base + 8u * (8 + s); };
@@ -106,6 +108,7 @@ __global__ void __launch_bounds__(kThreads, 1) ddf_tc_kernel(const __grid_consta
   auto gready_bar = [&](int b) { return bar_base + 8u * (28 + b); };
   auto gfree_bar  = [&](int b) { return bar_base + 8u * (30 + b); };
   const uint32_t tmem_slot = bar_base + 8u * 32;
+  const uint32_t zbuf = bar_base + 8u * 40;                            // 128 x float2 head partials
   auto a_smem = [&](int s) { return smem_base + s * Cfg::kStageBytes; };
   auto b_smem = [&](int s) { return smem_base + s * Cfg::kStageBytes + kABytes; };
 
@@ -123,15 +126,16 @@ __global__ void __launch_bounds__(kThreads, 1) ddf_tc_kernel(const __grid_consta
   if (threadIdx.x == 0) {
     for (int s = 0; s < S; ++s) { ptx::mbar_init(full_bar(s), 1); ptx::mbar_init(empty_bar(s), 1); }
     for (int b = 0; b < 2; ++b) {
-      ptx::mbar_init(tfull_bar(b), 1); ptx::mbar_init(tempty_bar(b), 128 * CG);
-      ptx::mbar_init(gready_bar(b), 128); ptx::mbar_init(gfree_bar(b), 1);
+      ptx::mbar_init(tfull_bar(b), 1); ptx::mbar_init(tempty_bar(b), 8 * CG);
+      ptx::mbar_init(gready_bar(b), 64); ptx::mbar_init(gfree_bar(b), 1);
     }
-    for (int j = 0; j < kMaxChunks; ++j) ptx::mbar_init(act_bar(j), 128);
+    for (int j = 0; j < kMaxChunks; ++j) ptx::mbar_init(act_bar(j), 8);
     ptx::fence_mbar_init();
   }
   if (warp == 0 && lane == 0) {
     for (int l = 0; l < p.n_hidden; ++l) ptx::prefetch_tmap(&p.w[l]);
     ptx::prefetch_tmap(&p.x0); ptx::prefetch_tmap(&p.x1); ptx::prefetch_tmap(&p.g);
+    ptx::prefetch_tmap(&p.xs0); ptx::prefetch_tmap(&p.xs1);
   }
   if (warp == 2) { ptx::tmem_alloc<CG>(tmem_slot, 512); ptx::tmem_relinquish<CG>(); }
   ptx::tc_fence_before();
@@ -219,10 +223,14 @@ __global__ void __launch_bounds__(kThreads, 1) ddf_tc_kernel(const __grid_consta
         }
       }
     }
-  } else if (warp >= 4 && warp < 8) {
-    // ================================================================ epilogue
-    const int q = warp & 3;
+  } else if (warp >= 4) {
+    // ================================================================ epilogue (8 warps)
+    // warp w owns TMEM lanes 32*(w%4).. (hardware rule) and columns 128*h.. of each 256-column
+    // chunk, h = (w-4)/4.  Output rows go through a 32x64 bf16 staging box (128B swizzle) and a
+    // TMA store, so the next layer's TMA loads read what the async proxy itself wrote.
+    const int q = warp & 3, h = (warp - 4) >> 2;
     const int row = q * 32 + lane;
+    const uint32_t stage = stg_base + (uint32_t)(warp - 4) * 4096u;
     const uint32_t tempty_remote = (CG == 2) ? ptx::mapa(tempty_bar(0), 0) : 0u;
     uint32_t cc = 0;
     for (int64_t tile = pid; tile < num_tiles; tile += num_pairs) {
@@ -230,115 +238,137 @@ __global__ void __launch_bounds__(kThreads, 1) ddf_tc_kernel(const __grid_consta
       const bool valid = grow < n;
       float z0 = 0.0f, z1 = 0.0f;
       for (int l = 0; l < p.n_hidden; ++l) {
-        __nv_bfloat16* xout = ((l & 1) ? p.x1p : p.x0p) + ((size_t)cta_global * kTileM + row) * p.width;
+        const CUtensorMap* smap = (l & 1) ? &p.xs1 : &p.xs0;
         const float* bias = p.bias + p.b_off[l];
         for (int c = 0; c < p.n_chunks; ++c, ++cc) {
           const uint32_t buf = cc & 1u, use = cc >> 1;
           wait_bar<CG == 2>(tfull_bar(buf), use & 1u, p.dbg, 0x600 + buf);
           ptx::tc_fence_after();
-          const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + buf * kChunkN;
+          const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + buf * kChunkN + h * 128;
           #pragma unroll 1
-          for (int piece = 0; piece < kChunkN / 32; ++piece) {
-            uint32_t r[32];
-            ptx::tmem_ld32(taddr + piece * 32, r);
+          for (int box = 0; box < 2; ++box) {
+            uint32_t r[64];
+            ptx::tmem_ld32(taddr + box * 64, *reinterpret_cast<uint32_t(*)[32]>(&r[0]));
+            ptx::tmem_ld32(taddr + box * 64 + 32, *reinterpret_cast<uint32_t(*)[32]>(&r[32]));
             ptx::tmem_ld_wait();
-            if (piece == kChunkN / 32 - 1) {
+            if (box == 1) {                       // accumulator fully read: hand it back to the MMA warp
               ptx::tc_fence_before();
-              if (CG == 2) ptx::mbar_arrive_cluster(tempty_remote + 8u * buf);
-              else ptx::mbar_arrive(tempty_bar(buf));
+              __syncwarp();
+              if (lane == 0) {
+                if (CG == 2) ptx::mbar_arrive_cluster(tempty_remote + 8u * buf);
+                else ptx::mbar_arrive(tempty_bar(buf));
+              }
             }
-            const int col = c * kChunkN + piece * 32;
+            const int col = c * kChunkN + h * 128 + box * 64;
             const float4* b4 = reinterpret_cast<const float4*>(bias + col);
-            float v[32];
             #pragma unroll
-            for (int i = 0; i < 8; ++i) {
+            for (int i = 0; i < 16; ++i) {
               float4 bb = __ldg(b4 + i);
-              v[4 * i + 0] = fmaxf(__uint_as_float(r[4 * i + 0]) + bb.x, 0.0f);
-              v[4 * i + 1] = fmaxf(__uint_as_float(r[4 * i + 1]) + bb.y, 0.0f);
-              v[4 * i + 2] = fmaxf(__uint_as_float(r[4 * i + 2]) + bb.z, 0.0f);
-              v[4 * i + 3] = fmaxf(__uint_as_float(r[4 * i + 3]) + bb.w, 0.0f);
+              r[4 * i + 0] = __float_as_uint(fmaxf(__uint_as_float(r[4 * i + 0]) + bb.x, 0.0f));
+              r[4 * i + 1] = __float_as_uint(fmaxf(__uint_as_float(r[4 * i + 1]) + bb.y, 0.0f));
+              r[4 * i + 2] = __float_as_uint(fmaxf(__uint_as_float(r[4 * i + 2]) + bb.z, 0.0f));
+              r[4 * i + 3] = __float_as_uint(fmaxf(__uint_as_float(r[4 * i + 3]) + bb.w, 0.0f));
             }
             if (l < last_layer) {
-              uint4* dst = reinterpret_cast<uint4*>(xout + col);
+              if (lane == 0) ptx::bulk_wait_read<0>();          // staging box free again
+              __syncwarp();
               #pragma unroll
-              for (int i = 0; i < 4; ++i) {
+              for (int j = 0; j < 8; ++j) {
                 uint4 pk;
-                __nv_bfloat162 t0 = __floats2bfloat162_rn(v[8 * i + 0], v[8 * i + 1]);
-                __nv_bfloat162 t1 = __floats2bfloat162_rn(v[8 * i + 2], v[8 * i + 3]);
-                __nv_bfloat162 t2 = __floats2bfloat162_rn(v[8 * i + 4], v[8 * i + 5]);
-                __nv_bfloat162 t3 = __floats2bfloat162_rn(v[8 * i + 6], v[8 * i + 7]);
+                __nv_bfloat162 t0 = __floats2bfloat162_rn(__uint_as_float(r[8 * j + 0]), __uint_as_float(r[8 * j + 1]));
+                __nv_bfloat162 t1 = __floats2bfloat162_rn(__uint_as_float(r[8 * j + 2]), __uint_as_float(r[8 * j + 3]));
+                __nv_bfloat162 t2 = __floats2bfloat162_rn(__uint_as_float(r[8 * j + 4]), __uint_as_float(r[8 * j + 5]));
+                __nv_bfloat162 t3 = __floats2bfloat162_rn(__uint_as_float(r[8 * j + 6]), __uint_as_float(r[8 * j + 7]));
                 pk.x = *reinterpret_cast<uint32_t*>(&t0); pk.y = *reinterpret_cast<uint32_t*>(&t1);
                 pk.z = *reinterpret_cast<uint32_t*>(&t2); pk.w = *reinterpret_cast<uint32_t*>(&t3);
-                dst[i] = pk;
+                ptx::st_shared_v4(stage + (uint32_t)lane * 128u + (uint32_t)((j ^ (lane & 7)) << 4), pk);
+              }
+              ptx::fence_proxy_async_smem();
+              __syncwarp();
+              if (lane == 0) {
+                ptx::tma_store_2d(smap, stage, col, cta_global * kTileM + q * 32);
+                ptx::bulk_commit();
               }
             } else {
               const float4* w0 = reinterpret_cast<const float4*>(p.head_w + col);
               #pragma unroll
-              for (int i = 0; i < 8; ++i) {
+              for (int i = 0; i < 16; ++i) {
                 float4 ww = __ldg(w0 + i);
-                z0 = fmaf(v[4 * i + 0], ww.x, z0); z0 = fmaf(v[4 * i + 1], ww.y, z0);
-                z0 = fmaf(v[4 * i + 2], ww.z, z0); z0 = fmaf(v[4 * i + 3], ww.w, z0);
+                z0 = fmaf(__uint_as_float(r[4 * i + 0]), ww.x, z0); z0 = fmaf(__uint_as_float(r[4 * i + 1]), ww.y, z0);
+                z0 = fmaf(__uint_as_float(r[4 * i + 2]), ww.z, z0); z0 = fmaf(__uint_as_float(r[4 * i + 3]), ww.w, z0);
               }
               if (p.n_out == 2) {
                 const float4* w1 = reinterpret_cast<const float4*>(p.head_w + p.width + col);
                 #pragma unroll
-                for (int i = 0; i < 8; ++i) {
+                for (int i = 0; i < 16; ++i) {
                   float4 ww = __ldg(w1 + i);
-                  z1 = fmaf(v[4 * i + 0], ww.x, z1); z1 = fmaf(v[4 * i + 1], ww.y, z1);
-                  z1 = fmaf(v[4 * i + 2], ww.z, z1); z1 = fmaf(v[4 * i + 3], ww.w, z1);
+                  z1 = fmaf(__uint_as_float(r[4 * i + 0]), ww.x, z1); z1 = fmaf(__uint_as_float(r[4 * i + 1]), ww.y, z1);
+                  z1 = fmaf(__uint_as_float(r[4 * i + 2]), ww.z, z1); z1 = fmaf(__uint_as_float(r[4 * i + 3]), ww.w, z1);
                 }
               }
             }
           }
-          if (l < last_layer) {
-            ptx::fence_proxy_async();
-            __threadfence();
+          if (l < last_layer && lane == 0) {
+            ptx::bulk_wait<0>();                  // this warp's part of chunk c is in global memory
             ptx::mbar_arrive(act_bar(c));
           }
         }
       }
-      // ---- fused heads (t = distance, xi = visibility)
-      z0 += p.bias[p.b_off[p.n_hidden]];
-      if (p.n_out == 2) z1 += p.bias[p.b_off[p.n_hidden] + 1];
-      if (p.mode_out == 1) {
-        if (valid) { p.out0[grow * p.n_out] = z0; if (p.n_out == 2) p.out0[grow * p.n_out + 1] = z1; }
-      } else if (p.mode_out == 0) {
-        if (valid) {
-          if (p.n_out == 2) { p.out0[grow] = softplus_f(z0); if (p.out1) p.out1[grow] = sigmoid_f(z1); }
-          else p.out0[grow] = z0;
+      // ---- fused heads (t = distance, xi = visibility); the two column halves
+      // of a row meet through shared memory, always added in the same order
+      if (h == 1) { asm volatile("st.shared.v2.f32 [%0], {%1, %2};" :: "r"(zbuf + (uint32_t)row * 8u), "f"(z0), "f"(z1) : "memory"); }
+      ptx::named_bar_sync(1, 256);
+      if (h == 0) {
+        float y0, y1;
+        asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(y0), "=f"(y1) : "r"(zbuf + (uint32_t)row * 8u) : "memory");
+        z0 = (z0 + y0) + p.bias[p.b_off[p.n_hidden]];
+        if (p.n_out == 2) z1 = (z1 + y1) + p.bias[p.b_off[p.n_hidden] + 1];
+        if (p.mode_out == 1) {
+          if (valid) { p.out0[grow * p.n_out] = z0; if (p.n_out == 2) p.out0[grow * p.n_out + 1] = z1; }
+        } else if (p.mode_out == 0) {
+          if (valid) {
+            if (p.n_out == 2) { p.out0[grow] = softplus_f(z0); if (p.out1) p.out1[grow] = sigmoid_f(z1); }
+            else p.out0[grow] = z0;
+          }
+        } else {
+          // AO: 1 - mean over the pixel's spp consecutive rays of (xi > 0.5 and t < ao_radius)
+          const bool hit = valid && (sigmoid_f(z1) > 0.5f) && (softplus_f(z0) < p.ao_radius);
+          const uint32_t m = __ballot_sync(0xffffffffu, hit);
+          const int g0 = (lane / p.spp) * p.spp;
+          const uint32_t bits = (p.spp == 32) ? m : ((m >> g0) & ((1u << p.spp) - 1u));
+          if (valid && (lane % p.spp) == 0) p.out0[grow / p.spp] = 1.0f - (float)__popc(bits) / (float)p.spp;
         }
-      } else {
-        // AO: 1 - mean over the pixel's spp consecutive rays of (xi > 0.5 and t < ao_radius)
-        const bool hit = valid && (sigmoid_f(z1) > 0.5f) && (softplus_f(z0) < p.ao_radius);
-        const uint32_t m = __ballot_sync(0xffffffffu, hit);
-        const int g0 = (lane / p.spp) * p.spp;
-        const uint32_t bits = (p.spp == 32) ? m : ((m >> g0) & ((1u << p.spp) - 1u));
-        if (valid && (lane % p.spp) == 0) p.out0[grow / p.spp] = 1.0f - (float)__popc(bits) / (float)p.spp;
       }
+      ptx::named_bar_sync(1, 256);
     }
-  } else if (warp >= 8) {
-    // ================================================================ encoder
-    const int row = (warp - 8) * 32 + lane;
+  } else {
+    // ================================================================ encoder (warps 2, 3)
+    // gamma(o, d) of this CTA's 128 rays, two rays per thread, one tile ahead of the MMAs
+    const int t64 = (warp - 2) * 32 + lane;
     int tile_local = 0;
     for (int64_t tile = pid; tile < num_tiles; tile += num_pairs, ++tile_local) {
       const int gb = tile_local & 1;
       wait_bar<CG == 2>(gfree_bar(gb), ((tile_local >> 1) & 1) ^ 1, p.dbg, 0x700 + gb);
-      const int64_t grow = tile * tile_rays + (int64_t)rank * kTileM + row;
-      __align__(16) __nv_bfloat16 enc[256];
       #pragma unroll 1
-      for (int k = 0; k < p.E_pad; ++k) enc[k] = __float2bfloat16_rn(0.0f);
-      if (grow < n) {
-        float v[3] = { p.o[3 * grow], p.o[3 * grow + 1], p.o[3 * grow + 2] };
-        encode_vec_bf16(v, p.Lo, enc);
-        if (p.input_kind == 0) {
-          float w[3] = { p.d[3 * grow], p.d[3 * grow + 1], p.d[3 * grow + 2] };
-          encode_vec_bf16(w, p.Ld, enc + 3 + 6 * p.Lo);
+      for (int rr = 0; rr < 2; ++rr) {
+        const int row = t64 + rr * 64;
+        const int64_t grow = tile * tile_rays + (int64_t)rank * kTileM + row;
+        __align__(16) __nv_bfloat16 enc[256];
+        #pragma unroll 1
+        for (int k = 0; k < p.E_pad; ++k) enc[k] = __float2bfloat16_rn(0.0f);
+        if (grow < n) {
+          float v[3] = { p.o[3 * grow], p.o[3 * grow + 1], p.o[3 * grow + 2] };
+          encode_vec_bf16(v, p.Lo, enc);
+          if (p.input_kind == 0) {
+            float w[3] = { p.d[3 * grow], p.d[3 * grow + 1], p.d[3 * grow + 2] };
+            encode_vec_bf16(w, p.Ld, enc + 3 + 6 * p.Lo);
+          }
         }
+        uint4* dst = reinterpret_cast<uint4*>(p.gp + ((size_t)(cta_global * 2 + gb) * kTileM + row) * p.E_pad);
+        const uint4* src = reinterpret_cast<const uint4*>(enc);
+        #pragma unroll 1
+        for (int k = 0; k < p.E_pad / 8; ++k) dst[k] = src[k];
       }
-      uint4* dst = reinterpret_cast<uint4*>(p.gp + ((size_t)(cta_global * 2 + gb) * kTileM + row) * p.E_pad);
-      const uint4* src = reinterpret_cast<const uint4*>(enc);
-      #pragma unroll 1
-      for (int k = 0; k < p.E_pad / 8; ++k) dst[k] = src[k];
       ptx::fence_proxy_async();
       __threadfence();
       ptx::mbar_arrive(gready_bar(gb));
@@ -369,12 +399,12 @@ static EncodeTiledFn get_encode_fn() {
 }
 
 // bf16 row-major [rows][cols] with row pitch `pitch_elems`; box = 64 columns x 128 rows, 128B swizzle
-static int make_map(CUtensorMap* out, void* base, uint64_t cols, uint64_t rows, uint64_t pitch_elems) {
+static int make_map(CUtensorMap* out, void* base, uint64_t cols, uint64_t rows, uint64_t pitch_elems, uint32_t box_rows = 128u) {
   EncodeTiledFn fn = get_encode_fn();
   if (!fn) return DDF_E_UNSUPPORTED;
   cuuint64_t dims[2] = { cols, rows };
   cuuint64_t strides[1] = { pitch_elems * 2 };
-  cuuint32_t box[2] = { (cuuint32_t)kKBlock, 128u };
+  cuuint32_t box[2] = { (cuuint32_t)kKBlock, box_rows };
   cuuint32_t estr[2] = { 1u, 1u };
   CUresult r = fn(out, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, base, dims, strides, box, estr,
                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
@@ -426,6 +456,8 @@ int tc_plan_create(Model* m) {
   p.b_off[L.n_hidden] = (int)m->layers[L.n_hidden].b_off;
   if ((rc = make_map(&p.x0, t->x0, L.width, rows, L.width)) != DDF_OK) return rc;
   if ((rc = make_map(&p.x1, t->x1, L.width, rows, L.width)) != DDF_OK) return rc;
+  if ((rc = make_map(&p.xs0, t->x0, L.width, rows, L.width, 32u)) != DDF_OK) return rc;
+  if ((rc = make_map(&p.xs1, t->x1, L.width, rows, L.width, 32u)) != DDF_OK) return rc;
   if ((rc = make_map(&p.g, t->g, (uint64_t)m->E_pad, rows * 2, (uint64_t)m->E_pad)) != DDF_OK) return rc;
   p.bias = m->d_b; p.head_w = m->d_head_w;
   p.x0p = t->x0; p.x1p = t->x1; p.gp = t->g;

@@ -1,0 +1,312 @@
+"""GPU tests: closed forms through the kernels (pins P1, P4, P5), the API contract (T4), the two
+kernel paths against each other, the host-buffer entry point, and the sphere tracer (P12)."""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+from ddf_inputs import (MASTER_SEED, STREAMS, Layout, layout_c0, layout_c1, layout_sdf, make_weights,
+                        random_rays, blob_layer_shapes, blob_num_elements, f32_to_bf16_bits)
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def ddf():
+    import paper_2606_00817_b200 as pkg
+    pkg.build()
+    return pkg
+
+
+def _cuda(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def _logits(ddf, m, o, d):
+    n = o.shape[0]
+    z = torch.full((n, m.layout.n_out), float("nan"), device="cuda")
+    ddf.ddf_query_logits(m, _cuda(o), _cuda(d) if d is not None else None, n, z)
+    torch.cuda.synchronize()
+    return z.cpu().numpy()
+
+
+def _heads(ddf, m, o, d):
+    n = o.shape[0]
+    dist = torch.full((n,), float("nan"), device="cuda"); vis = torch.full((n,), float("nan"), device="cuda")
+    ddf.ddf_query(m, _cuda(o), _cuda(d), n, dist, vis)
+    torch.cuda.synchronize()
+    return dist.cpu().numpy(), vis.cpu().numpy()
+
+
+def _blob(lay, layers):
+    parts = []
+    for (W, b), (o, i) in zip(layers, blob_layer_shapes(lay)):
+        W = np.asarray(W, np.float64); assert W.shape == (o, i)
+        parts += [W.reshape(-1), np.asarray(b, np.float64).reshape(o)]
+    return np.concatenate(parts).astype(np.float32)
+
+
+# ------------------------------------------------------------------ closed forms on the GPU
+
+@pytest.mark.parametrize("width", [64, 256])            # SIMT path / tcgen05 path
+def test_zero_weights_give_head_of_bias(ddf, width):
+    lay = Layout(0, 4, 4, 3, width, 1, 2, 0)
+    blob = np.zeros(blob_num_elements(lay), np.float32)
+    blob[-2:] = [1.25, -0.5]
+    m = ddf.ddf_create(blob, lay)
+    o, d = random_rays(300)
+    dist, vis = _heads(ddf, m, o, d)
+    assert np.allclose(dist, 1.25 + math.log1p(math.exp(-1.25)), rtol=2e-7)
+    assert np.allclose(vis, 1.0 / (1.0 + math.exp(0.5)), rtol=2e-7)
+    blob[-2:] = 0
+    m2 = ddf.ddf_create(blob, lay)
+    dist, vis = _heads(ddf, m2, o, d)
+    assert np.allclose(dist, math.log(2.0), rtol=2e-7) and np.all(vis == 0.5)
+
+
+@pytest.mark.parametrize("width", [64, 256])
+def test_all_ones_layer_exposes_pad_lanes(ddf, orc, width):
+    """P4 shape: W0 = all ones => every hidden unit = ReLU(sum gamma); K = 90 is padded to 128 on
+    the GPU, so any pad lane that is not zero changes the sum."""
+    lay = Layout(0, 10, 4, 1, width, -1, 2, 0)
+    head = np.zeros((2, width)); head[0, :] = 1.0 / width; head[1, 0] = -0.25
+    blob = _blob(lay, [(np.ones((width, 90)), np.zeros(width)), (head, [0, 1])])
+    m = ddf.ddf_create(blob, lay)
+    o, d = random_rays(513)
+    z = _logits(ddf, m, o, d)
+    g = orc.encode(lay, o, d)
+    gq = np.vectorize(orc.round_bf16)(g)
+    s = np.maximum(gq.sum(1), 0.0)
+    assert np.allclose(z[:, 0], s, atol=2e-5, rtol=1e-5)
+    assert np.allclose(z[:, 1], 1.0 - 0.25 * s, atol=2e-5, rtol=1e-5)
+
+
+@pytest.mark.parametrize("through_skip", [False, True])
+def test_selector_layers_pass_encoding_through(ddf, orc, through_skip):
+    """P5 on the tcgen05 path: width 256 >= 2E (E = 90); z = c . gamma (bf16-rounded gamma)."""
+    lay = Layout(0, 10, 4, 3, 256, 1, 2, 0)
+    E, W = 90, 256
+    rng = np.random.default_rng(5)
+    c = [np.vectorize(orc.round_bf16)(rng.standard_normal(E)) for _ in range(2)]
+    sel = np.zeros((W, E)); sel[:E] = np.eye(E); sel[E:2 * E] = -np.eye(E)
+    ident = np.zeros((W, W)); ident[:2 * E, :2 * E] = np.eye(2 * E)
+    layers = []
+    for l in range(3):
+        nin = E if l == 0 else (W + E if l == 1 else W)
+        Wl = np.zeros((W, nin))
+        if through_skip:
+            if l == 1: Wl[:, W:] = sel
+            elif l == 2: Wl[:, :W] = ident
+        else:
+            if l == 0: Wl[:, :E] = sel
+            else: Wl[:, :W] = ident
+        layers.append((Wl, np.zeros(W)))
+    head = np.zeros((2, W))
+    for j in range(2):
+        head[j, :E] = c[j]; head[j, E:2 * E] = -c[j]
+    layers.append((head, np.zeros(2)))
+    m = ddf.ddf_create(_blob(lay, layers), lay)
+    assert ddf.ddf_get_info(m, 0) == 1
+    o, d = random_rays(700)
+    z = _logits(ddf, m, o, d)
+    gq = np.vectorize(orc.round_bf16)(orc.encode(lay, o, d))
+    assert np.allclose(z[:, 0], gq @ c[0], atol=3e-5) and np.allclose(z[:, 1], gq @ c[1], atol=3e-5)
+
+
+def test_encoding_on_gpu_matches_definition(ddf, orc):
+    """gamma read back through an identity-selector network, including origins at radius 2.5 where
+    the top band's phase is ~4000 rad (exact power-of-two scaling)."""
+    lay = Layout(0, 10, 4, 1, 256, -1, 2, 0)
+    E, W = 90, 256
+    o, d = random_rays(256)
+    o = (o * 2.5).astype(np.float32)
+    g = orc.encode(lay, o, d)
+    for k in range(0, E, 2):
+        W0 = np.zeros((W, E)); W0[0, k] = 1; W0[1, k] = -1; W0[2, k + 1] = 1; W0[3, k + 1] = -1
+        head = np.zeros((2, W)); head[0, 0] = 1; head[0, 1] = -1; head[1, 2] = 1; head[1, 3] = -1
+        m = ddf.ddf_create(_blob(lay, [(W0, np.zeros(W)), (head, [0, 0])]), lay)
+        z = _logits(ddf, m, o, d)
+        ddf.ddf_destroy(m)
+        assert np.allclose(z, np.vectorize(orc.round_bf16)(g[:, k:k + 2]), atol=1e-6), k
+
+
+# ------------------------------------------------------------------ API contract
+
+@pytest.fixture(scope="module")
+def c1(ddf):
+    lay = layout_c1()
+    m = ddf.ddf_create(make_weights(lay), lay)
+    yield lay, m
+    ddf.ddf_destroy(m)
+
+
+def test_edge_sizes_permutation_determinism(ddf, c1):
+    lay, m = c1
+    N = 256 * 148 + 257
+    o, d = random_rays(N)
+    od, dd = _cuda(o), _cuda(d)
+    full_d = torch.empty(N, device="cuda"); full_v = torch.empty(N, device="cuda")
+    ddf.ddf_query(m, od, dd, N, full_d, full_v)
+    again_d = torch.empty(N, device="cuda"); again_v = torch.empty(N, device="cuda")
+    ddf.ddf_query(m, od, dd, N, again_d, again_v)
+    assert torch.equal(full_d, again_d) and torch.equal(full_v, again_v)          # bit-reproducible
+    for n in (0, 1, 127, 128, 129, 255, 256, 257, 1009):
+        dist = torch.full((max(n, 1) + 8,), -7.0, device="cuda"); vis = torch.full((max(n, 1) + 8,), -7.0, device="cuda")
+        ddf.ddf_query(m, od, dd, n, dist, vis)
+        torch.cuda.synchronize()
+        assert torch.equal(dist[:n], full_d[:n]) and torch.equal(vis[:n], full_v[:n]), n
+        assert bool((dist[n:] == -7.0).all()) and bool((vis[n:] == -7.0).all()), n    # no write past n
+    perm = torch.randperm(N, device="cuda", generator=torch.Generator(device="cuda").manual_seed(1))
+    pd = torch.empty(N, device="cuda"); pv = torch.empty(N, device="cuda")
+    ddf.ddf_query(m, od[perm].contiguous(), dd[perm].contiguous(), N, pd, pv)
+    assert torch.equal(pd, full_d[perm]) and torch.equal(pv, full_v[perm])
+    # out_vis may be NULL
+    only_d = torch.empty(N, device="cuda")
+    ddf.ddf_query(m, od, dd, N, only_d, None)
+    assert torch.equal(only_d, full_d)
+    # unaligned (4-byte aligned only) buffers
+    ou = torch.empty(3 * 1001 + 1, device="cuda")[1:].view(1001, 3); ou.copy_(od[:1001])
+    du = torch.empty(3 * 1001 + 1, device="cuda")[1:].view(1001, 3); du.copy_(dd[:1001])
+    outu = torch.empty(1002, device="cuda")[1:]
+    from paper_2606_00817_b200.binding import lib, _stream
+    import ctypes as C
+    rc = lib().ddf_query(m.handle, C.c_void_p(ou.data_ptr()), C.c_void_p(du.data_ptr()), C.c_int64(1001),
+                         C.c_void_p(outu.data_ptr()), None, _stream(None))
+    assert rc == 0
+    assert torch.equal(outu, full_d[:1001])
+
+
+def test_bad_arguments(ddf, c1):
+    lay, m = c1
+    from paper_2606_00817_b200.binding import lib, _stream
+    import ctypes as C
+    x = torch.zeros((4, 3), device="cuda"); y = torch.zeros(4, device="cuda")
+    p = lambda t: C.c_void_p(t.data_ptr())
+    assert lib().ddf_query(m.handle, p(x), p(x), C.c_int64(-1), p(y), p(y), _stream(None)) == -1
+    assert lib().ddf_query(m.handle, None, p(x), C.c_int64(4), p(y), p(y), _stream(None)) == -1
+    assert lib().ddf_query(m.handle, p(x), None, C.c_int64(4), p(y), p(y), _stream(None)) == -1
+    assert lib().ddf_query(m.handle, p(x), p(x), C.c_int64(4), None, p(y), _stream(None)) == -1
+    assert lib().ddf_query(m.handle, None, None, C.c_int64(0), None, None, _stream(None)) == 0
+    bad = Layout(0, 10, 4, 8, 1280, 4, 2, 1)
+    with pytest.raises(ddf.DdfError):
+        ddf.ddf_set_path(ddf.ddf_create(make_weights(layout_c0()), layout_c0()), 2)   # width 64: no tcgen05 plan
+    prm = ddf.SdfTraceParams(64, 1e-3, 6.0, 1.0, 0.05, 0)
+    t = torch.zeros(4, device="cuda"); h = torch.zeros(4, dtype=torch.uint8, device="cuda"); s = torch.zeros(4, dtype=torch.int32, device="cuda")
+    with pytest.raises(ddf.DdfError):
+        ddf.sdf_sphere_trace(m, x, x, 4, prm, t, h, s)         # a DDF model is not an SDF model
+
+
+def test_simt_and_tcgen05_paths_agree(ddf, orc):
+    lay = Layout(0, 6, 3, 4, 512, 2, 2, 1)
+    blob = make_weights(lay, seed=17, bias_scale=0.2)
+    m = ddf.ddf_create(blob, lay)
+    o, d = random_rays(2000, seed=5)
+    ddf.ddf_set_path(m, 2); z_tc = _logits(ddf, m, o, d); assert ddf.ddf_get_info(m, 1) == 1
+    ddf.ddf_set_path(m, 1); z_si = _logits(ddf, m, o, d); assert ddf.ddf_get_info(m, 1) > 1
+    zq, _, _ = orc.forward(lay, blob, o, d, mode=1)
+    ze, _, _ = orc.forward(lay, blob, o, d, mode=0)
+    assert np.abs(z_tc - z_si).max() < 4e-2 and np.abs(z_tc - z_si).mean() < 3e-3
+    for z in (z_tc, z_si):
+        assert np.abs(z - zq).max() < 4e-2 and np.abs(z - zq).mean() < 3e-3
+        assert np.abs(z - ze).max() < 4e-2
+
+
+def test_query_host_matches_device_query(ddf, c1):
+    lay, m = c1
+    n = 5000
+    o, d = random_rays(n)
+    oh, dh = torch.from_numpy(o).pin_memory(), torch.from_numpy(d).pin_memory()
+    dist_h = torch.empty(n).pin_memory(); vis_h = torch.empty(n).pin_memory()
+    ddf.ddf_query_host(m, oh, dh, n, dist_h, vis_h)
+    dist = torch.empty(n, device="cuda"); vis = torch.empty(n, device="cuda")
+    ddf.ddf_query(m, oh.cuda(), dh.cuda(), n, dist, vis)
+    assert torch.equal(dist.cpu(), dist_h) and torch.equal(vis.cpu(), vis_h)
+
+
+def test_model_from_device_fp32_blob(ddf, orc):
+    lay = Layout(0, 4, 4, 2, 256, -1, 2, 0)
+    blob = make_weights(lay, bias_scale=0.1)
+    m_host = ddf.ddf_create(blob, lay)
+    m_dev = ddf.ddf_create(torch.from_numpy(blob).cuda(), lay)
+    o, d = random_rays(300)
+    assert np.array_equal(_logits(ddf, m_host, o, d), _logits(ddf, m_dev, o, d))
+    zq, _, _ = orc.forward(lay, blob, o, d, mode=1)
+    assert np.abs(_logits(ddf, m_host, o, d) - zq).max() < 1e-3
+
+
+# ------------------------------------------------------------------ sphere tracer
+
+@pytest.fixture(scope="module")
+def sdf(ddf):
+    lay = layout_sdf()
+    blob = make_weights(lay)
+    m = ddf.ddf_create(blob, lay)
+    yield lay, blob, m
+    ddf.ddf_destroy(m)
+
+
+def _trace(ddf, m, o, d, prm, want_trace=False):
+    n = o.shape[0]
+    t = torch.empty(n, device="cuda"); hit = torch.empty(n, dtype=torch.uint8, device="cuda")
+    steps = torch.empty(n, dtype=torch.int32, device="cuda"); tot = torch.zeros(1, dtype=torch.int64, device="cuda")
+    tp = torch.empty((n, prm.max_steps, 3), device="cuda") if want_trace else None
+    ts = torch.empty((n, prm.max_steps), device="cuda") if want_trace else None
+    ddf.sdf_sphere_trace(m, _cuda(o), _cuda(d), n, prm, t, hit, steps, tp, ts, tot)
+    torch.cuda.synchronize()
+    out = [t.cpu().numpy(), hit.cpu().numpy(), steps.cpu().numpy(), int(tot.item())]
+    if want_trace:
+        out += [tp.cpu().numpy(), ts.cpu().numpy()]
+    return out
+
+
+def test_sphere_trace_alpha0_is_bit_identical_to_the_cpu_tracer(ddf, orc, sdf):
+    """P12: with the MLP term off the step rule alone decides everything: t, hit and steps must
+    equal the CPU tracer's exactly (both carry the ray state in fp32 with the same fma order),
+    and t reaches the analytic ray-sphere distance."""
+    lay, blob, m = sdf
+    cam = orc.camera_from_seed(MASTER_SEED, STREAMS["camera_pos"], 2.5)
+    o, d = orc.gen_camera(cam, 64, 64)
+    for early in (0, 1):
+        prm = ddf.SdfTraceParams(64, 1e-3, 6.0, 1.0, 0.0, early)
+        t, hit, steps, tot = _trace(ddf, m, o, d, prm)
+        rt, rhit, rsteps = orc.sphere_trace(lay, blob, o, d, 64, 1e-3, 6.0, 1.0, 0.0)
+        assert np.array_equal(hit, rhit) and np.array_equal(steps, rsteps) and np.array_equal(t, rt)
+        assert tot == (64 * len(o) if not early else int(steps.sum()))
+    want = np.array([orc.ray_sphere(o[i], d[i], [0, 0, 0], 1.0) for i in range(len(o))])
+    h = hit == 1
+    assert h.sum() > 1000 and np.all(want[h] > 0) and np.all(np.abs(want[h] - t[h]) < 1e-3 / 0.05)
+
+
+def test_sphere_trace_teacher_forcing(ddf, orc, sdf):
+    """MLP on: trajectories are chaotic under bf16, so the oracle re-evaluates s at the kernel's
+    own visited points (same tolerance per step); end results are compared statistically."""
+    lay, blob, m = sdf
+    cam = orc.camera_from_seed(MASTER_SEED, STREAMS["camera_pos"], 2.5)
+    o, d = orc.gen_camera(cam, 24, 24)
+    prm = ddf.SdfTraceParams(64, 1e-3, 6.0, 1.0, 0.05, 0)
+    t, hit, steps, tot, tp, ts = _trace(ddf, m, o, d, prm, want_trace=True)
+    prm1 = ddf.SdfTraceParams(64, 1e-3, 6.0, 1.0, 0.05, 1)
+    t1, hit1, steps1, tot1, tp1, ts1 = _trace(ddf, m, o, d, prm1, want_trace=True)
+    assert np.array_equal(t, t1) and np.array_equal(hit, hit1) and np.array_equal(steps, steps1)
+    assert np.array_equal(np.nan_to_num(ts, nan=-9.0), np.nan_to_num(ts1, nan=-9.0))
+    assert tot == 64 * len(o) and tot1 == int(steps.sum())
+    visited = ~np.isnan(ts)
+    assert np.array_equal(visited.sum(1), steps)
+    rows, cols = np.nonzero(visited)
+    pick = np.random.default_rng(0).choice(len(rows), 1200, replace=False)
+    pts = tp[rows[pick], cols[pick]]
+    s_ref = orc.sdf_eval(lay, blob, pts, 1.0, 0.05, mode=0)
+    assert np.abs(ts[rows[pick], cols[pick]] - s_ref).max() < 0.05 * 4e-2 + 1e-6      # alpha * logit tolerance
+    # the step rule applied to the kernel's own s reproduces its decisions
+    for i in np.random.default_rng(1).choice(len(o), 64, replace=False):
+        tt = np.float32(0.0); h = 0; k = 0
+        for k in range(64):
+            s = ts[i, k]
+            if abs(s) < 1e-3: h = 1; break
+            tt = np.float32(tt + s)
+            if tt > 6.0 or tt < 0: break
+        assert (h, k + 1, tt) == (hit[i], steps[i], t[i])
+    # statistics against the CPU tracer run end to end
+    rt, rhit, rsteps = orc.sphere_trace(lay, blob, o, d, 64, 1e-3, 6.0, 1.0, 0.05)
+    assert abs(hit.mean() - rhit.mean()) < 0.02 and abs(steps.mean() - rsteps.mean()) < 1.0
