@@ -192,7 +192,9 @@ __global__ void __launch_bounds__(kThreads, 1) ddf_tc_kernel(const __grid_consta
     }
   } else if (warp == 1) {
     // ================================================================ MMA issuer
-    if (lane == 0 && leader) {
+    // the whole warp walks the schedule (warp-uniform control flow and operands); one elected
+    // lane issues the tcgen05 instructions
+    if (leader) {
       constexpr uint32_t idesc = ptx::idesc_bf16_f32(128 * CG, kChunkN);
       uint32_t it = 0, cc = 0;
       int tile_local = 0;
@@ -213,12 +215,23 @@ __global__ void __launch_bounds__(kThreads, 1) ddf_tc_kernel(const __grid_consta
               const int nk16 = g_last ? p.g_last_nk16 : 4;
               const uint64_t adesc = ptx::smem_desc_k_sw128(a_smem(s));
               const uint64_t bdesc = ptx::smem_desc_k_sw128(b_smem(s));
-              for (int k = 0; k < nk16; ++k)
-                ptx::umma_bf16<CG>(d_tmem, adesc + 2u * k, bdesc + 2u * k, idesc, (uint32_t)((kb | k) != 0));
-              ptx::umma_commit<CG>(empty_bar(s));
-              if (l == gamma_layer && c == p.n_chunks - 1 && kb == nk - 1) ptx::umma_commit<CG>(gfree_bar(gb));
+              const bool free_gamma = (l == gamma_layer && c == p.n_chunks - 1 && kb == nk - 1);
+              if (ptx::elect_one()) {
+                if (nk16 == 4) {
+                  ptx::umma_bf16<CG>(d_tmem, adesc, bdesc, idesc, (uint32_t)(kb != 0));
+                  ptx::umma_bf16<CG>(d_tmem, adesc + 2u, bdesc + 2u, idesc, 1u);
+                  ptx::umma_bf16<CG>(d_tmem, adesc + 4u, bdesc + 4u, idesc, 1u);
+                  ptx::umma_bf16<CG>(d_tmem, adesc + 6u, bdesc + 6u, idesc, 1u);
+                } else {
+                  for (int k = 0; k < nk16; ++k)
+                    ptx::umma_bf16<CG>(d_tmem, adesc + 2u * k, bdesc + 2u * k, idesc, (uint32_t)((kb | k) != 0));
+                }
+                ptx::umma_commit<CG>(empty_bar(s));
+                if (free_gamma) ptx::umma_commit<CG>(gfree_bar(gb));
+                if (kb == nk - 1) ptx::umma_commit<CG>(tfull_bar(buf));
+              }
+              __syncwarp();
             }
-            ptx::umma_commit<CG>(tfull_bar(buf));
           }
         }
       }
