@@ -5,10 +5,11 @@
 //   warp 0      TMA producer  : streams activation (A) and weight (B) K-blocks into a smem ring
 //   warp 1      MMA issuer    : tcgen05.mma (bf16 x bf16 -> fp32 in TMEM), 128x256 (or 256x256 per
 //                               pair) x K accumulators, double-buffered in the 512 TMEM columns
-//   warp 2      TMEM allocator
-//   warps 4-7   epilogue      : tcgen05.ld -> +bias, ReLU, bf16 -> next layer's operand; the last
-//                               layer feeds the fused heads (softplus / sigmoid / AO reduction)
-//   warps 8-11  encoder       : gamma(o, d) of the NEXT tile, in registers, written as bf16
+//   warps 2-3   encoder       : gamma(o, d) of the NEXT tile, in registers, written as bf16
+//                               (warp 2 also owns the TMEM allocation)
+//   warps 4-11  epilogue      : tcgen05.ld -> +bias, ReLU, bf16 -> swizzled smem box -> TMA store
+//                               = next layer's operand; the last layer feeds the fused heads
+//                               (softplus / sigmoid / AO reduction)
 //
 // Layer hand-off: a 128 x width bf16 activation tile does not fit next to a weight pipeline in
 // 227 KB of shared memory (320 KB at width 1280), so the epilogue writes it to a per-CTA scratch
@@ -146,8 +147,7 @@ __global__ void __launch_bounds__(kThreads, 1) ddf_tc_kernel(const __grid_consta
 
   if (warp == 0) {
     // ================================================================ TMA producer
-    if (lane == 0) {
-      const uint32_t full_target = (CG == 2) ? 0u : 0u;  (void)full_target;
+    {
       uint32_t it = 0, act_phase = 0;                    // bit j of act_phase: parity for act_bar(j)
       int tile_local = 0;
       for (int64_t tile = pid; tile < num_tiles; tile += num_pairs, ++tile_local) {
@@ -171,19 +171,22 @@ __global__ void __launch_bounds__(kThreads, 1) ddf_tc_kernel(const __grid_consta
               const int s = it % S; const uint32_t ph = (it / S) & 1u;
               wait_bar<CG == 2>(empty_bar(s), ph ^ 1u, p.dbg, 0x300 + s);
               const int brow = c * kChunkN + (CG == 2 ? (int)rank * 128 : 0);
-              if (CG == 2) {
-                if (leader) ptx::mbar_arrive_expect_tx(full_bar(s), 2u * Cfg::kStageBytes);
-                const uint32_t fb = ptx::mapa(full_bar(s), 0);
-                if (kb < nk0) ptx::tma_load_2d_cg2(a_smem(s), amap, fb, kb * kKBlock, a_row);
-                else          ptx::tma_load_2d_cg2(a_smem(s), &p.g, fb, (kb - nk0) * kKBlock, g_row);
-                ptx::tma_load_2d_cg2(b_smem(s), &p.w[l], fb, kb * kKBlock, brow);
-              } else {
-                ptx::mbar_arrive_expect_tx(full_bar(s), (uint32_t)Cfg::kStageBytes);
-                if (kb < nk0) ptx::tma_load_2d(a_smem(s), amap, full_bar(s), kb * kKBlock, a_row);
-                else          ptx::tma_load_2d(a_smem(s), &p.g, full_bar(s), (kb - nk0) * kKBlock, g_row);
-                ptx::tma_load_2d(b_smem(s), &p.w[l], full_bar(s), kb * kKBlock, brow);
-                ptx::tma_load_2d(b_smem(s) + 128 * kKBlock * 2, &p.w[l], full_bar(s), kb * kKBlock, brow + 128);
+              if (ptx::elect_one()) {
+                if (CG == 2) {
+                  if (leader) ptx::mbar_arrive_expect_tx(full_bar(s), 2u * Cfg::kStageBytes);
+                  const uint32_t fb = ptx::mapa(full_bar(s), 0);
+                  if (kb < nk0) ptx::tma_load_2d_cg2(a_smem(s), amap, fb, kb * kKBlock, a_row);
+                  else          ptx::tma_load_2d_cg2(a_smem(s), &p.g, fb, (kb - nk0) * kKBlock, g_row);
+                  ptx::tma_load_2d_cg2(b_smem(s), &p.w[l], fb, kb * kKBlock, brow);
+                } else {
+                  ptx::mbar_arrive_expect_tx(full_bar(s), (uint32_t)Cfg::kStageBytes);
+                  if (kb < nk0) ptx::tma_load_2d(a_smem(s), amap, full_bar(s), kb * kKBlock, a_row);
+                  else          ptx::tma_load_2d(a_smem(s), &p.g, full_bar(s), (kb - nk0) * kKBlock, g_row);
+                  ptx::tma_load_2d(b_smem(s), &p.w[l], full_bar(s), kb * kKBlock, brow);
+                  ptx::tma_load_2d(b_smem(s) + 128 * kKBlock * 2, &p.w[l], full_bar(s), kb * kKBlock, brow + 128);
+                }
               }
+              __syncwarp();
               ++it;
             }
           }
