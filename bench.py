@@ -30,7 +30,7 @@ UNIT = "Mrays/s"
 WORKLOAD = "configs[1]: paper-scale DDF (90-dim enc, 8x1280, skip@4, bf16), 2^20 camera rays 1024x1024"
 # dram__bytes_read.sum + dram__bytes_write.sum of ddf_tc_kernel<2> for one 2^20-ray launch, from
 # the ncu --set full capture summarised in profiles/r01_ncu_summary.md (None until captured)
-NCU_DRAM_TRAFFIC_BYTES = None
+NCU_DRAM_TRAFFIC_BYTES = 18.22e9
 
 
 def _peaks():
