@@ -124,8 +124,9 @@ int  ddf_gen_ao(const float* p, const float* nrm, int64_t n_pts, int spp, uint64
 /* ao[i] = 1 - mean_s( vis > 0.5 and dist < ao_radius ) ("average the hit flag"). */
 int  ddf_ao_reduce(const float* vis, const float* dist, int64_t n_pts, int spp, float ao_radius,
                    float* ao, void* stream);
-/* Query + reduce in one call; the per-ray results never reach global memory when the tile size
- * is a multiple of spp (else a workspace of 8 bytes per ray owned by the model is used). */
+/* Query + reduce in one call; the per-ray results never reach global memory when spp divides
+ * 32 (a pixel's rays then sit in one warp of a tile); otherwise a workspace of 8 bytes per ray
+ * owned by the model is used and ddf_ao_reduce runs as a second launch. */
 int  ddf_query_ao(ddf_model* model, const float* o, const float* d, int64_t n_pts, int spp,
                   float ao_radius, float* ao, void* stream);
 /* shadow[i] = 1 if vis > 0.5 and dist < tmax ("occluded within the distance to the light"). */

@@ -230,7 +230,7 @@ extern "C" int ddf_query_ao(ddf_model* model, const float* o, const float* d, in
   if (!o || !d || !ao || m->lay.n_out != 2 || m->lay.input_kind != 0) return DDF_E_INVALID_ARG;
   const int64_t n = n_pts * spp;
   cudaStream_t st = (cudaStream_t)stream;
-  if (m->tc && m->path != 1 && 256 % spp == 0)
+  if (m->tc && m->path != 1 && spp <= 32 && 32 % spp == 0)   // a pixel's rays sit in one warp of a tile
     return tc_forward(m, o, d, n, nullptr, 2, ao, nullptr, spp, ao_radius, st);
   if (n > m->ws_out_rows) {
     cudaFree(m->ws_dist); cudaFree(m->ws_vis); m->ws_dist = m->ws_vis = nullptr; m->ws_out_rows = 0;
