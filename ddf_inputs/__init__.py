@@ -10,12 +10,14 @@ Random numbers (reading A8): a counter-based SplitMix64-style mixer ke
 (seed, stream, index); u = (top 24 bits) * 2^-24 in [0, 1).
 """
 from .rng import mix64, u64_at, uniform01, MASTER_SEED, STREAMS
-from .layouts import Layout, layout_c0, layout_c1, layout_sdf, blob_layer_shapes, blob_num_elements
-from .weights import make_weights, f32_to_bf16_bits, bf16_bits_to_f32
+from .layouts import (Layout, layout_c0, layout_c1, layout_sdf, blob_layer_shapes, blob_num_elements,
+                      HashLayout, layout_hash_paper, hash_mlp_shapes)
+from .weights import make_weights, f32_to_bf16_bits, bf16_bits_to_f32, make_hash_table, make_hash_mlp, f32_to_f16_bits
 from .rays import random_rays
 
 __all__ = [
     "mix64", "u64_at", "uniform01", "MASTER_SEED", "STREAMS",
     "Layout", "layout_c0", "layout_c1", "layout_sdf", "blob_layer_shapes", "blob_num_elements",
     "make_weights", "f32_to_bf16_bits", "bf16_bits_to_f32", "random_rays",
+    "HashLayout", "layout_hash_paper", "hash_mlp_shapes", "make_hash_table", "make_hash_mlp", "f32_to_f16_bits",
 ]

@@ -58,3 +58,41 @@ def blob_layer_shapes(lay):
 
 def blob_num_elements(lay):
     return sum(o * i + o for o, i in blob_layer_shapes(lay))
+
+
+@dataclass(frozen=True)
+class HashLayout:
+    """The paper's own field: multiresolution hash grid on the origin, L_d
+    sinusoidal direction bands, a small ReLU MLP.  Field names follow `ddf_hashgrid_layout`."""
+    n_levels: int = 16
+    n_features: int = 2
+    log2_table: int = 19
+    base_res: int = 16
+    growth: float = 1.5
+    box_min: tuple = (-3.0, -3.0, -3.0)
+    box_max: tuple = (3.0, 3.0, 3.0)
+    n_freq_dir: int = 4
+    n_hidden: int = 2
+    width: int = 64
+    n_out: int = 2
+    table_dtype: int = 0       # 0 = fp32, 2 = fp16 (raw uint16)
+    mlp_dtype: int = 0         # 0 = fp32, 1 = bf16 (raw uint16)
+
+    @property
+    def mlp_in(self):
+        return self.n_levels * self.n_features + 3 + 6 * self.n_freq_dir
+
+
+def layout_hash_paper():
+    """16 levels x 2 features, T = 2^19, base 16, growth 1.5, 4 direction bands,
+    2 x 64 MLP; fp32 table (the paper's 52 MB).  Box: DESIGN.md reading H7."""
+    return HashLayout()
+
+
+def hash_mlp_shapes(lay):
+    shapes, fan_in = [], lay.mlp_in
+    for _ in range(lay.n_hidden):
+        shapes.append((lay.width, fan_in))
+        fan_in = lay.width
+    shapes.append((lay.n_out, fan_in))
+    return shapes

@@ -8,7 +8,7 @@ fp32 values are rounded to bf16 (round-to-nearest-even) and returned as raw uint
 import numpy as np
 
 from .rng import uniform01, MASTER_SEED, STREAMS
-from .layouts import blob_layer_shapes
+from .layouts import blob_layer_shapes, hash_mlp_shapes
 
 
 def f32_to_bf16_bits(x):
@@ -44,3 +44,38 @@ def make_weights(lay, seed=MASTER_SEED, stream=None, bias_scale=0.0):
     if lay.weight_dtype == 1:
         return f32_to_bf16_bits(blob)
     return blob
+
+
+def f32_to_f16_bits(x):
+    return np.ascontiguousarray(x, dtype=np.float32).astype(np.float16).view(np.uint16)
+
+
+def make_hash_table(lay, n_entries, seed=MASTER_SEED, stream=None, scale=1.0):
+    """Seeded feature table: `n_entries` x n_features values U(-scale, scale) (stand-ins for trained
+    features), fp32 or fp16 bits per lay.table_dtype.  The entry count is passed in by the caller
+    (from the oracle in tests, from the library in bench.py): this module holds no grid arithmetic."""
+    if stream is None:
+        stream = STREAMS["hash_table"]
+    idx = np.arange(int(n_entries) * lay.n_features, dtype=np.uint64)
+    t = ((2.0 * uniform01(seed, stream, idx) - 1.0) * scale).astype(np.float32)
+    return f32_to_f16_bits(t) if lay.table_dtype == 2 else t
+
+
+def make_hash_mlp(lay, seed=MASTER_SEED, stream=None, bias_scale=0.0):
+    """MLP blob of the hash-grid field: layers then head, W[out][in] row-major then b[out];
+    U(+-sqrt(6/fan_in)) weights (reading A7), zero or seeded biases."""
+    if stream is None:
+        stream = STREAMS["hash_mlp"]
+    parts, off = [], 0
+    for (o, i) in hash_mlp_shapes(lay):
+        bound = np.sqrt(6.0 / i)
+        w = ((2.0 * uniform01(seed, stream, np.arange(off, off + o * i, dtype=np.uint64)) - 1.0) * bound).astype(np.float32)
+        off += o * i
+        if bias_scale > 0.0:
+            b = ((2.0 * uniform01(seed, stream, np.arange(off, off + o, dtype=np.uint64)) - 1.0) * bias_scale).astype(np.float32)
+        else:
+            b = np.zeros(o, dtype=np.float32)
+        off += o
+        parts += [w, b]
+    blob = np.concatenate(parts)
+    return f32_to_bf16_bits(blob) if lay.mlp_dtype == 1 else blob

@@ -12,22 +12,32 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "ddf_oracle.c")
+_SRCS = [_SRC, os.path.join(_HERE, "ddf_hash_oracle.c")]
+_HDRS = [os.path.join(_HERE, "ddf_oracle.h"), os.path.join(_HERE, "ddf_hash_oracle.h")]
 _LIB = os.path.join(_HERE, "libddf_oracle.so")
 
 
 def build(force=False):
-    """gcc -O2, OpenMP, no fast-math."""
+    """gcc -O2, OpenMP, no fast-math, no FMA contraction."""
     if (not force and os.path.exists(_LIB)
-            and os.path.getmtime(_LIB) >= max(os.path.getmtime(_SRC),
-                                              os.path.getmtime(os.path.join(_HERE, "ddf_oracle.h")))):
+            and os.path.getmtime(_LIB) >= max(os.path.getmtime(f) for f in _SRCS + _HDRS)):
         return _LIB
-    subprocess.check_call(["gcc", "-O2", "-Wall", "-fopenmp", "-fPIC", "-shared", "-o", _LIB, _SRC, "-lm"])
+    subprocess.check_call(["gcc", "-O2", "-Wall", "-ffp-contract=off", "-fopenmp", "-fPIC", "-shared",
+                           "-o", _LIB] + _SRCS + ["-lm"])
     return _LIB
 
 
 class OrcLayout(C.Structure):
     _fields_ = [(k, C.c_int32) for k in ("input_kind", "n_freq_origin", "n_freq_dir", "n_hidden",
                                          "width", "skip_layer", "n_out", "weight_dtype")]
+
+
+class OrcHashLayout(C.Structure):
+    _fields_ = [("n_levels", C.c_int32), ("n_features", C.c_int32), ("log2_table", C.c_int32),
+                ("base_res", C.c_int32), ("growth", C.c_double), ("box_min", C.c_float * 3),
+                ("box_max", C.c_float * 3), ("n_freq_dir", C.c_int32), ("n_hidden", C.c_int32),
+                ("width", C.c_int32), ("n_out", C.c_int32), ("table_dtype", C.c_int32),
+                ("mlp_dtype", C.c_int32)]
 
 
 class OrcCamera(C.Structure):
@@ -58,6 +68,9 @@ def lib():
         _lib.orc_u64_at.argtypes = [C.c_uint64] * 3
         _lib.orc_uniform01.restype = C.c_double
         _lib.orc_uniform01.argtypes = [C.c_uint64] * 3
+        _lib.orc_hash_table_entries.restype = C.c_int64
+        _lib.orc_hash_mlp_params.restype = C.c_int64
+        _lib.orc_hash_index.restype = C.c_int64
         _lib.orc_ray_sphere.restype = C.c_double
         _lib.orc_ray_box_exit.restype = C.c_double
     return _lib
@@ -259,3 +272,77 @@ def sphere_trace(lay, blob, o, d, max_steps=64, eps=1e-3, t_max=6.0, base_radius
     if rc != 0:
         raise ValueError("oracle: bad SDF layout")
     return (t, hit, steps, tp, ts) if want_trace else (t, hit, steps)
+
+
+# ------------------------------------------------------------------ hash-grid DDF (ddf_hash_oracle.h)
+
+def _hlayout(lay):
+    return OrcHashLayout(lay.n_levels, lay.n_features, lay.log2_table, lay.base_res, float(lay.growth),
+                         (C.c_float * 3)(*lay.box_min), (C.c_float * 3)(*lay.box_max), lay.n_freq_dir,
+                         lay.n_hidden, lay.width, lay.n_out, lay.table_dtype, lay.mlp_dtype)
+
+
+def hash_level(lay, level):
+    """(resolution N_l, stored entries, entry offset, hashed?) of one level."""
+    L = _hlayout(lay)
+    res, ent, off, hs = C.c_int64(), C.c_int64(), C.c_int64(), C.c_int()
+    rc = lib().orc_hash_level(C.byref(L), C.c_int(level), C.byref(res), C.byref(ent), C.byref(off), C.byref(hs))
+    if rc != 0:
+        raise ValueError("oracle: bad hash layout / level")
+    return res.value, ent.value, off.value, bool(hs.value)
+
+
+def hash_table_entries(lay):
+    L = _hlayout(lay)
+    return lib().orc_hash_table_entries(C.byref(L))
+
+
+def hash_mlp_in(lay):
+    L = _hlayout(lay)
+    return lib().orc_hash_mlp_in(C.byref(L))
+
+
+def hash_mlp_params(lay):
+    L = _hlayout(lay)
+    return lib().orc_hash_mlp_params(C.byref(L))
+
+
+def hash_index(lay, level, ix, iy, iz):
+    L = _hlayout(lay)
+    return lib().orc_hash_index(C.byref(L), C.c_int(level), C.c_uint32(ix), C.c_uint32(iy), C.c_uint32(iz))
+
+
+def _table(lay, table):
+    t = np.ascontiguousarray(table)
+    assert t.dtype == (np.uint16 if lay.table_dtype == 2 else np.float32), t.dtype
+    return t
+
+
+def hash_encode(lay, table, x):
+    x = _f32(x)
+    n = x.shape[0]
+    L = _hlayout(lay)
+    t = _table(lay, table)
+    feat = np.zeros((n, lay.n_levels * lay.n_features), dtype=np.float64)
+    rc = lib().orc_hash_encode(C.byref(L), _p(t), _p(x), C.c_int64(n), _p(feat))
+    if rc != 0:
+        raise ValueError("oracle: bad hash layout")
+    return feat
+
+
+def hash_forward(lay, table, mlp, o, d, mode=0, nthreads=0):
+    """Returns (z[n][n_out], dist[n], vis[n]) in float64."""
+    o, d = _f32(o), _f32(d)
+    n = o.shape[0]
+    L = _hlayout(lay)
+    t = _table(lay, table)
+    m = np.ascontiguousarray(mlp)
+    assert m.dtype == (np.uint16 if lay.mlp_dtype == 1 else np.float32), m.dtype
+    z = np.zeros((n, lay.n_out), dtype=np.float64)
+    dist = np.zeros(n, dtype=np.float64)
+    vis = np.zeros(n, dtype=np.float64) if lay.n_out == 2 else None
+    rc = lib().orc_hash_forward(C.byref(L), _p(t), _p(m), _p(o), _p(d), C.c_int64(n), C.c_int(mode),
+                                _p(z), _p(dist), _p(vis) if vis is not None else None, C.c_int(nthreads))
+    if rc != 0:
+        raise ValueError("oracle: bad hash layout")
+    return z, dist, vis

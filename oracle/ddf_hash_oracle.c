@@ -1,0 +1,185 @@
+/* ddf_hash_oracle.c - CPU oracle of the hash-grid DDF.  TEST INFRASTRUCTURE, NOT PRODUCT.
+ * Definitions, citations and pins: ddf_hash_oracle.h.  Built into libddf_oracle.so together
+ * with ddf_oracle.c (gcc -O2 -ffp-contract=off, no fast-math). */
+#include "ddf_hash_oracle.h"
+#include "ddf_oracle.h"
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define HPI 3.14159265358979323846
+
+static int hl_ok(const orc_hash_layout* L) {
+  if (L->n_levels < 1 || L->n_levels > 32 || L->n_features < 1 || L->n_features > 8) return 0;
+  if (L->log2_table < 4 || L->log2_table > 28 || L->base_res < 1 || !(L->growth >= 1.0)) return 0;
+  if (L->n_freq_dir < 0 || L->n_hidden < 1 || L->width < 1 || L->n_out < 1 || L->n_out > 2) return 0;
+  if (!(L->table_dtype == 0 || L->table_dtype == 2) || L->mlp_dtype < 0 || L->mlp_dtype > 1) return 0;
+  for (int a = 0; a < 3; ++a) if (!(L->box_max[a] > L->box_min[a])) return 0;
+  return 1;
+}
+
+/* H1: N_l = floor(base * growth^l) */
+static int64_t level_res(const orc_hash_layout* L, int level) {
+  return (int64_t)floor((double)L->base_res * pow(L->growth, (double)level));
+}
+
+int orc_hash_level(const orc_hash_layout* L, int level, int64_t* res, int64_t* entries,
+                   int64_t* offset, int* hashed) {
+  if (!hl_ok(L) || level < 0 || level >= L->n_levels) return -1;
+  const int64_t T = (int64_t)1 << L->log2_table;
+  int64_t off = 0;
+  for (int l = 0; l <= level; ++l) {
+    const int64_t N = level_res(L, l), V = N + 1;
+    /* (N+1)^3 <= T without overflow: V is at most a few hundred thousand here */
+    const int dense = (V <= 2097151) && (V * V * V <= T);
+    const int64_t cnt = dense ? V * V * V : T;
+    if (l == level) {
+      if (res) *res = N;
+      if (entries) *entries = cnt;
+      if (offset) *offset = off;
+      if (hashed) *hashed = !dense;
+    }
+    off += cnt;
+  }
+  return 0;
+}
+
+int64_t orc_hash_table_entries(const orc_hash_layout* L) {
+  int64_t e = 0, o = 0;
+  if (orc_hash_level(L, L->n_levels - 1, NULL, &e, &o, NULL)) return -1;
+  return o + e;
+}
+
+int orc_hash_mlp_in(const orc_hash_layout* L) { return L->n_levels * L->n_features + 3 + 6 * L->n_freq_dir; }
+
+int64_t orc_hash_mlp_params(const orc_hash_layout* L) {
+  int64_t p = 0, in = orc_hash_mlp_in(L);
+  for (int l = 0; l < L->n_hidden; ++l) { p += (int64_t)L->width * in + L->width; in = L->width; }
+  return p + (int64_t)L->n_out * in + L->n_out;
+}
+
+/* H4 */
+int64_t orc_hash_index(const orc_hash_layout* L, int level, uint32_t ix, uint32_t iy, uint32_t iz) {
+  int64_t N = 0; int hashed = 0;
+  if (orc_hash_level(L, level, &N, NULL, NULL, &hashed)) return -1;
+  if (!hashed) { const int64_t V = N + 1; return (int64_t)ix + V * ((int64_t)iy + V * (int64_t)iz); }
+  const uint32_t h = (ix * 1u) ^ (iy * 2654435761u) ^ (iz * 805459861u);      /* mod 2^32 products */
+  return (int64_t)(h & (uint32_t)(((int64_t)1 << L->log2_table) - 1));
+}
+
+static double half_bits_to_double(uint16_t h) {
+  const int s = h >> 15, e = (h >> 10) & 31, m = h & 1023;
+  double v;
+  if (e == 0) v = ldexp((double)m, -24);
+  else if (e == 31) v = m ? NAN : INFINITY;
+  else v = ldexp((double)(1024 + m), e - 25);
+  return s ? -v : v;
+}
+
+static double table_at(const orc_hash_layout* L, const void* table, int64_t entry, int f) {
+  const size_t i = (size_t)entry * L->n_features + f;
+  return L->table_dtype == 2 ? half_bits_to_double(((const uint16_t*)table)[i]) : (double)((const float*)table)[i];
+}
+
+/* features of one point (H2, H3, H5) */
+static void encode_point(const orc_hash_layout* L, const void* table, const float* x, double* feat) {
+  float x01[3];
+  for (int a = 0; a < 3; ++a) {
+    /* H2, in fp32: one subtraction, one subtraction, one division, each correctly rounded */
+    const float num = x[a] - L->box_min[a];
+    const float den = L->box_max[a] - L->box_min[a];
+    float v = num / den;
+    v = v < 0.0f ? 0.0f : (v > 1.0f ? 1.0f : v);
+    x01[a] = v;
+  }
+  for (int l = 0; l < L->n_levels; ++l) {
+    int64_t N = 0, off = 0;
+    orc_hash_level(L, l, &N, NULL, &off, NULL);
+    uint32_t c0[3]; double w[3];
+    for (int a = 0; a < 3; ++a) {
+      const float pos = x01[a] * (float)N;                      /* H3, fp32 product */
+      float fl = floorf(pos);
+      if (fl > (float)(N - 1)) fl = (float)(N - 1);
+      c0[a] = (uint32_t)fl;
+      w[a] = (double)(pos - fl);                                /* exact in fp32 */
+    }
+    for (int f = 0; f < L->n_features; ++f) feat[l * L->n_features + f] = 0.0;
+    for (int corner = 0; corner < 8; ++corner) {
+      const int bx = corner & 1, by = (corner >> 1) & 1, bz = (corner >> 2) & 1;
+      const double wt = (bx ? w[0] : 1.0 - w[0]) * (by ? w[1] : 1.0 - w[1]) * (bz ? w[2] : 1.0 - w[2]);
+      const int64_t idx = off + orc_hash_index(L, l, c0[0] + bx, c0[1] + by, c0[2] + bz);
+      for (int f = 0; f < L->n_features; ++f) feat[l * L->n_features + f] += wt * table_at(L, table, idx, f);
+    }
+  }
+}
+
+int orc_hash_encode(const orc_hash_layout* L, const void* table, const float* x, int64_t n, double* feat) {
+  if (!hl_ok(L)) return -1;
+  const int F = L->n_levels * L->n_features;
+  #pragma omp parallel for schedule(static)
+  for (int64_t i = 0; i < n; ++i) encode_point(L, table, x + 3 * i, feat + (size_t)F * i);
+  return 0;
+}
+
+static double mlp_at(const orc_hash_layout* L, const void* mlp, size_t i, int quantise) {
+  if (L->mlp_dtype == 1) {
+    uint32_t b = ((uint32_t)((const uint16_t*)mlp)[i]) << 16; float f; memcpy(&f, &b, 4); return (double)f;
+  }
+  const float f = ((const float*)mlp)[i];
+  return quantise ? orc_round_bf16((double)f) : (double)f;
+}
+
+int orc_hash_forward(const orc_hash_layout* L, const void* table, const void* mlp,
+                     const float* o, const float* d, int64_t n, int mode,
+                     double* z, double* dist, double* vis, int nthreads) {
+  if (!hl_ok(L)) return -1;
+  const int F = L->n_levels * L->n_features, E = orc_hash_mlp_in(L), W = L->width;
+  const int S = (E > W ? E : W);
+#ifdef _OPENMP
+  if (nthreads > 0) omp_set_num_threads(nthreads);
+#endif
+  #pragma omp parallel
+  {
+    double* in = (double*)malloc(sizeof(double) * S);
+    double* h  = (double*)malloc(sizeof(double) * S);
+    #pragma omp for schedule(dynamic, 64)
+    for (int64_t i = 0; i < n; ++i) {
+      /* H6: [hash features ; gamma(d)] */
+      encode_point(L, table, o + 3 * i, in);
+      int m = F;
+      for (int c = 0; c < 3; ++c) in[m++] = (double)d[3 * i + c];
+      for (int k = 0; k < L->n_freq_dir; ++k) {
+        for (int c = 0; c < 3; ++c) in[m++] = sin(HPI * ldexp((double)d[3 * i + c], k));
+        for (int c = 0; c < 3; ++c) in[m++] = cos(HPI * ldexp((double)d[3 * i + c], k));
+      }
+      if (mode) for (int k = 0; k < E; ++k) in[k] = orc_round_bf16(in[k]);
+      int nin = E; size_t off = 0;
+      for (int l = 0; l < L->n_hidden; ++l) {
+        const size_t boff = off + (size_t)W * nin;
+        for (int j = 0; j < W; ++j) {
+          double acc = mlp_at(L, mlp, boff + j, 0);
+          for (int k = 0; k < nin; ++k) acc += mlp_at(L, mlp, off + (size_t)j * nin + k, mode) * in[k];
+          acc = acc > 0.0 ? acc : 0.0;
+          h[j] = (mode && l != L->n_hidden - 1) ? orc_round_bf16(acc) : acc;
+        }
+        for (int j = 0; j < W; ++j) in[j] = h[j];
+        off = boff + W; nin = W;
+      }
+      const size_t boff = off + (size_t)L->n_out * nin;
+      double zz[2] = {0.0, 0.0};
+      for (int j = 0; j < L->n_out; ++j) {
+        double acc = mlp_at(L, mlp, boff + j, 0);
+        for (int k = 0; k < nin; ++k) acc += mlp_at(L, mlp, off + (size_t)j * nin + k, mode) * in[k];
+        zz[j] = acc;
+      }
+      for (int j = 0; j < L->n_out; ++j) z[(size_t)i * L->n_out + j] = zz[j];
+      if (dist) dist[i] = orc_softplus(zz[0]);                     /* (t, xi) */
+      if (vis && L->n_out == 2) vis[i] = orc_sigmoid(zz[1]);
+    }
+    free(in); free(h);
+  }
+  return 0;
+}

@@ -1,0 +1,73 @@
+/* ddf_hash_oracle.h - CPU oracle for the paper's own DDF architecture:
+ * multiresolution hash grid on the ray origin + sinusoidal direction bands + a small MLP.
+ * TEST INFRASTRUCTURE, NOT PRODUCT (same rules as ddf_oracle.h).
+ *
+ * PAPER.md:64 (Sec. III-A): "a multiresolution hash grid that encodes the point x, following
+ * [8], together with a small encoding of the direction d.  A two-layer MLP of width 64 reads
+ * this code and outputs t and xi."   PAPER.md:84 (Sec. III-D): "16 levels, two features per
+ * level, a table of 2^19 entries per level, base resolution 16, and growth 1.5, over a box that
+ * bounds the normalized object ... direction d with four sinusoidal bands ... The hash table
+ * holds about 13M parameters and the MLP about 8k, for a stored field of 52 MB."
+ *
+ * What [8] (the multiresolution hash encoding the paper follows) defines, restated (DESIGN.md
+ * readings H1-H6):
+ *   H1  level l has resolution N_l = floor(base * growth^l); its grid has (N_l + 1)^3 vertices.
+ *   H2  x01 = clamp((x - box_min) / (box_max - box_min), 0, 1), evaluated in fp32.
+ *   H3  pos = x01 * N_l (fp32); cell = min(floor(pos), N_l - 1); w = pos - cell  (per axis).
+ *   H4  a vertex (ix, iy, iz) is stored at  ix + (N_l+1) * (iy + (N_l+1) * iz)  when the whole
+ *       grid fits the table ((N_l+1)^3 <= T), else at
+ *       (ix ^ iy * 2654435761 ^ iz * 805459861) mod T   (32-bit wrap-around products).
+ *   H5  feature_f = sum over the 8 cell corners of  prod_axis (w or 1-w) * table[l][index][f].
+ *   H6  MLP input = [features of level 0, level 1, ... ; gamma_Ld(d)]  (gamma as in
+ *       ddf_oracle.h: identity, then per band 3 sines and 3 cosines of 2^k pi d).
+ * Everything after the integer decisions of H2-H4 (which the paper's fp32 inputs fix) is fp64.
+ *
+ * Pins (tests/test_hash_oracle_pins.py): the paper's own counts (13.06M table parameters,
+ * 52.2 MB, 8130 MLP parameters); partition of unity; exact reproduction of linear fields on
+ * dense levels; table value at a vertex; hand-computed dense and hashed indices; continuity
+ * across cell faces; brute-force numpy re-evaluation.  Parity unpinned: the absolute (t, xi) of
+ * the seeded random field (no trained field exists in the container).
+ */
+#ifndef DDF_HASH_ORACLE_H
+#define DDF_HASH_ORACLE_H
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct orc_hash_layout {
+  int32_t n_levels;        /* 16 */
+  int32_t n_features;      /* 2 */
+  int32_t log2_table;      /* 19: T = 2^19 entries per level */
+  int32_t base_res;        /* 16 */
+  double  growth;          /* 1.5 */
+  float   box_min[3], box_max[3];
+  int32_t n_freq_dir;      /* 4 */
+  int32_t n_hidden;        /* 2 */
+  int32_t width;           /* 64 */
+  int32_t n_out;           /* 2 */
+  int32_t table_dtype;     /* 0 = fp32, 2 = fp16 (raw uint16) */
+  int32_t mlp_dtype;       /* 0 = fp32, 1 = bf16 (raw uint16) */
+} orc_hash_layout;
+
+/* resolution N_l, number of stored entries, entry offset of the level in the table, hashed? */
+int  orc_hash_level(const orc_hash_layout* L, int level, int64_t* res, int64_t* entries,
+                    int64_t* offset, int* hashed);
+int64_t orc_hash_table_entries(const orc_hash_layout* L);       /* all levels */
+int  orc_hash_mlp_in(const orc_hash_layout* L);                 /* n_levels*n_features + 3 + 6*L_d */
+int64_t orc_hash_mlp_params(const orc_hash_layout* L);          /* weights + biases */
+/* storage index of vertex (ix, iy, iz) of `level` within that level (H4) */
+int64_t orc_hash_index(const orc_hash_layout* L, int level, uint32_t ix, uint32_t iy, uint32_t iz);
+/* feat[n][n_levels*n_features] (fp64) of the points x[n][3] */
+int  orc_hash_encode(const orc_hash_layout* L, const void* table, const float* x, int64_t n, double* feat);
+/* mode 0 exact fp64; 1 quantised (features, gamma(d) and hidden activations but the last rounded
+ * to bf16; fp32 MLP weights rounded to bf16).  mlp blob: layers then head, W[out][in] + b[out]. */
+int  orc_hash_forward(const orc_hash_layout* L, const void* table, const void* mlp,
+                      const float* o, const float* d, int64_t n, int mode,
+                      double* z, double* dist, double* vis, int nthreads);
+
+#ifdef __cplusplus
+}
+#endif
+#endif
