@@ -88,6 +88,40 @@ int  ddf_set_path(ddf_model* model, int path);
  * last query call on this model; 2: E (encoded input width); 3: rays per tile of the path. */
 int64_t ddf_get_info(const ddf_model* model, int which);
 
+/* ---------------------------------------------------------------- the paper's own field
+ * PAPER.md:64 (Sec. III-A) / PAPER.md:84 (Sec. III-D): "a multiresolution hash grid that encodes
+ * the point x, following [8] ... 16 levels, two features per level, a table of 2^19 entries per
+ * level, base resolution 16, and growth 1.5, over a box that bounds the normalized object",
+ * direction d with "four sinusoidal bands", "a two-layer MLP of width 64 reads the joined code
+ * and outputs t and xi".  Definition used here (readings H1-H7):
+ *   N_l = floor(base_resolution * growth^l); the level stores (N_l+1)^3 vertices when that fits
+ *   T = 2^log2_table_size entries (index ix + (N_l+1)(iy + (N_l+1) iz)), else T hashed entries
+ *   (index (ix ^ iy*2654435761 ^ iz*805459861) mod T, 32-bit products);
+ *   x01 = clamp((x - box_min)/(box_max - box_min), 0, 1); pos = x01 * N_l; cell = min(floor(pos),
+ *   N_l - 1); trilinear interpolation of the 8 cell corners, n_features values per vertex;
+ *   MLP input = [level 0 features, level 1 features, ... ; gamma_{L_d}(d)], then Linear+ReLU
+ *   layers and the same heads as above.
+ * table: entries of all levels back to back, n_features values each, fp32 or fp16 (raw uint16).
+ * mlp: layers 0..n_hidden-1 then the head, W[out][in] row-major then b[out], fp32 (rounded to
+ * bf16 at create) or bf16.  Arithmetic: interpolation in fp32, bf16 MLP operands, fp32 accumulate.
+ * This build serves n_features == 2, n_levels <= 16, L_d <= 4, width == 64, n_hidden 1..4.
+ * The resulting model is used with ddf_query / ddf_query_host / ddf_query_logits / ddf_query_ao. */
+typedef struct ddf_hashgrid_layout {
+  uint32_t struct_size;        /* sizeof(ddf_hashgrid_layout) */
+  uint32_t version;            /* DDF_LAYOUT_VERSION */
+  uint32_t n_levels, n_features, log2_table_size, base_resolution;
+  float    growth;
+  float    box_min[3], box_max[3];
+  uint32_t n_freq_dir, n_hidden, width, n_out;
+  uint32_t table_dtype;        /* 0 = fp32, 2 = fp16 */
+  uint32_t mlp_dtype;          /* 0 = fp32, 1 = bf16 */
+  uint32_t weights_on_device;  /* both pointers: 0 = host, 1 = device */
+} ddf_hashgrid_layout;
+/* total number of table entries (vertices stored over all levels), or a negative ddf_status */
+int64_t ddf_hashgrid_table_entries(const ddf_hashgrid_layout* layout);
+int  ddf_create_hashgrid(const void* table, const void* mlp, const ddf_hashgrid_layout* layout,
+                         ddf_model** out);
+
 /* ---------------------------------------------------------------- the query
  * origins, dirs: [device] float[n][3].  out_dist, out_vis: [device] float[n]
  * (out_vis may be NULL; for n_out == 1 models out_dist receives the linear value z_0). */

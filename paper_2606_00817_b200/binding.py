@@ -16,6 +16,7 @@ EXPORTED_SYMBOLS = [
     "ddf_get_info", "ddf_query", "ddf_query_host", "ddf_query_logits", "ddf_camera_from_seed",
     "ddf_gen_camera", "ddf_gen_sphere_points", "ddf_gen_shadow", "ddf_gen_gbuffer", "ddf_gen_ao",
     "ddf_ao_reduce", "ddf_query_ao", "ddf_shadow_test", "sdf_sphere_trace",
+    "ddf_hashgrid_table_entries", "ddf_create_hashgrid",
 ]
 
 
@@ -28,6 +29,14 @@ class DdfLayout(C.Structure):
                 ("n_freq_origin", C.c_uint32), ("n_freq_dir", C.c_uint32), ("n_hidden", C.c_uint32),
                 ("width", C.c_uint32), ("skip_layer", C.c_int32), ("n_out", C.c_uint32),
                 ("weight_dtype", C.c_uint32), ("weights_on_device", C.c_uint32)]
+
+
+class DdfHashgridLayout(C.Structure):
+    _fields_ = [("struct_size", C.c_uint32), ("version", C.c_uint32), ("n_levels", C.c_uint32),
+                ("n_features", C.c_uint32), ("log2_table_size", C.c_uint32), ("base_resolution", C.c_uint32),
+                ("growth", C.c_float), ("box_min", C.c_float * 3), ("box_max", C.c_float * 3),
+                ("n_freq_dir", C.c_uint32), ("n_hidden", C.c_uint32), ("width", C.c_uint32), ("n_out", C.c_uint32),
+                ("table_dtype", C.c_uint32), ("mlp_dtype", C.c_uint32), ("weights_on_device", C.c_uint32)]
 
 
 class DdfCamera(C.Structure):
@@ -61,6 +70,7 @@ def lib():
         _lib = C.CDLL(_LIB_PATH)
         _lib.ddf_status_string.restype = C.c_char_p
         _lib.ddf_get_info.restype = C.c_int64
+        _lib.ddf_hashgrid_table_entries.restype = C.c_int64
     return _lib
 
 
@@ -134,6 +144,39 @@ def ddf_create(weights, lay):
         ptr = weights.ctypes.data_as(C.c_void_p)
     h = C.c_void_p(0)
     _check(lib().ddf_create(ptr, C.byref(L), C.byref(h)), "ddf_create")
+    return Model(h, lay)
+
+
+def make_hashgrid_layout(lay, weights_on_device=0):
+    """lay: any object with the ddf_hashgrid_layout field names (e.g. ddf_inputs.HashLayout)."""
+    return DdfHashgridLayout(C.sizeof(DdfHashgridLayout), 1, lay.n_levels, lay.n_features, lay.log2_table,
+                             lay.base_res, float(lay.growth), (C.c_float * 3)(*lay.box_min),
+                             (C.c_float * 3)(*lay.box_max), lay.n_freq_dir, lay.n_hidden, lay.width, lay.n_out,
+                             lay.table_dtype, lay.mlp_dtype, weights_on_device)
+
+
+def ddf_hashgrid_table_entries(lay):
+    L = make_hashgrid_layout(lay)
+    n = int(lib().ddf_hashgrid_table_entries(C.byref(L)))
+    if n < 0:
+        _check(n, "ddf_hashgrid_table_entries")
+    return n
+
+
+def ddf_create_hashgrid(table, mlp, lay):
+    """table, mlp: numpy arrays (host) or CUDA tensors (both on the device)."""
+    import numpy as np
+    if isinstance(table, torch.Tensor):
+        if not (table.is_cuda and isinstance(mlp, torch.Tensor) and mlp.is_cuda):
+            raise DdfError("table and mlp must both be host arrays or both CUDA tensors")
+        L = make_hashgrid_layout(lay, 1)
+        pt, pm = C.c_void_p(table.data_ptr()), C.c_void_p(mlp.data_ptr())
+    else:
+        table, mlp = np.ascontiguousarray(table), np.ascontiguousarray(mlp)
+        L = make_hashgrid_layout(lay, 0)
+        pt, pm = table.ctypes.data_as(C.c_void_p), mlp.ctypes.data_as(C.c_void_p)
+    h = C.c_void_p(0)
+    _check(lib().ddf_create_hashgrid(pt, pm, C.byref(L), C.byref(h)), "ddf_create_hashgrid")
     return Model(h, lay)
 
 

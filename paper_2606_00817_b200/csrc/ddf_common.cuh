@@ -38,6 +38,7 @@ struct LayerDesc {
 };
 
 struct TcPlan;          // tcgen05 path state (ddf_tc.cu)
+struct HashPlan;        // hash-grid field state (ddf_hash.cu)
 
 struct Model {
   ddf_layout lay;
@@ -63,6 +64,7 @@ struct Model {
   void* trace_ws; size_t trace_ws_bytes;
   int path;                        // 0 auto, 1 SIMT, 2 tcgen05
   TcPlan* tc;                      // non-null when the tcgen05 path can serve the layout
+  HashPlan* hg;                    // non-null: this model is a hash-grid field (ddf_create_hashgrid)
   int sm_count;
   int last_launches;
 };
@@ -78,6 +80,11 @@ void tc_plan_destroy(Model* m);
 // mode_out: 0 = heads (dist, vis), 1 = raw logits into out0 [n][n_out], 2 = AO reduce into out0
 int tc_forward(Model* m, const float* o, const float* d, int64_t n, const int64_t* n_dev,
                int mode_out, float* out0, float* out1, int spp, float ao_radius, cudaStream_t st);
+
+// ---- hash-grid field (ddf_hash.cu)
+void hash_plan_destroy(Model* m);
+int hash_forward(Model* m, const float* o, const float* d, int64_t n, int mode_out,
+                 float* out0, float* out1, int spp, float ao_radius, cudaStream_t st);
 
 // ---- device helpers -------------------------------------------------------------------------
 #ifdef __CUDACC__

@@ -108,3 +108,25 @@ def test_product_does_not_import_oracle():
             src = open(os.path.join(ROOT, "oracle", f)).read()
             assert "paper_2606_00817_b200" not in src.replace("under paper_2606_00817_b200/", "").replace(
                 "the product (paper_2606_00817_b200)", ""), f
+
+
+def test_hashgrid_host_logic_without_gpu(libddf, orc):
+    """Level sizing of the hash-grid field is host logic: the library's count must be
+    the paper's 6,529,022 entries (13.06M parameters) and agree with the oracle on other shapes."""
+    from ddf_inputs import HashLayout, layout_hash_paper
+    from paper_2606_00817_b200 import DdfHashgridLayout, make_hashgrid_layout, ddf_hashgrid_table_entries, DdfError
+    assert C.sizeof(DdfHashgridLayout) == 80
+    assert ddf_hashgrid_table_entries(layout_hash_paper()) == 6_529_022
+    for lay in (HashLayout(n_levels=5, base_res=3, growth=2.0, log2_table=10), HashLayout(n_levels=12, growth=1.3819, log2_table=14)):
+        assert ddf_hashgrid_table_entries(lay) == orc.hash_table_entries(lay)
+    bad = make_hashgrid_layout(layout_hash_paper()); bad.version = 7
+    assert libddf.ddf_hashgrid_table_entries(C.byref(bad)) == -2
+    bad = make_hashgrid_layout(HashLayout(box_min=(1.0, 0.0, 0.0), box_max=(1.0, 1.0, 1.0)))
+    assert libddf.ddf_hashgrid_table_entries(C.byref(bad)) == -2
+    h = C.c_void_p(0)
+    assert libddf.ddf_create_hashgrid(None, None, None, C.byref(h)) == -1
+    w = np.zeros(16, np.float32)
+    wide = make_hashgrid_layout(HashLayout(width=128))                     # shape this build does not serve
+    assert libddf.ddf_create_hashgrid(w.ctypes.data_as(C.c_void_p), w.ctypes.data_as(C.c_void_p), C.byref(wide), C.byref(h)) == -3
+    with pytest.raises(DdfError):
+        ddf_hashgrid_table_entries(HashLayout(n_out=5))

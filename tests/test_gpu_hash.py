@@ -1,0 +1,178 @@
+"""GPU parity of the paper's own field (hash grid + direction bands + 2x64 MLP)
+against oracle/ddf_hash_oracle.c, through the C ABI.  Tolerances as for the dense network
+(BASELINE.json north_star): |dd| <= 1e-2 (1+|d|), |dv| <= 1e-2, >= 99.9 % hit/miss agreement outside
+|xi - 0.5| < 1e-2, against the EXACT fp64 oracle; logits within 2e-2 (mean 2e-3) of the oracle's
+quantised mode.  The integer decisions (cell, index) are taken in fp32 on both sides (reading H2/H3)."""
+import numpy as np
+import pytest
+import torch
+
+from ddf_inputs import (MASTER_SEED, STREAMS, HashLayout, layout_hash_paper, make_hash_table, make_hash_mlp,
+                        random_rays)
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def ddf():
+    import paper_2606_00817_b200 as pkg
+    pkg.build()
+    assert torch.cuda.is_available()
+    return pkg
+
+
+def _field(ddf, lay, bias_scale=0.0):
+    n = ddf.ddf_hashgrid_table_entries(lay)
+    table, mlp = make_hash_table(lay, n), make_hash_mlp(lay, bias_scale=bias_scale)
+    return table, mlp, ddf.ddf_create_hashgrid(table, mlp, lay)
+
+
+def _cuda(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def _check(dist, vis, t, xi, what):
+    ed = np.abs(dist - t) / (1.0 + np.abs(t)); ev = np.abs(vis - xi)
+    band = np.abs(xi - 0.5) < 1e-2
+    agree = ((vis > 0.5) == (xi > 0.5))[~band].mean()
+    assert np.isfinite(dist).all() and np.isfinite(vis).all(), what
+    assert ed.max() <= 1e-2 and ev.max() <= 1e-2 and agree >= 0.999 and band.mean() < 0.2, (what, ed.max(), ev.max(), agree, band.mean())
+
+
+@pytest.fixture(scope="module")
+def paper(ddf):
+    lay = layout_hash_paper()
+    table, mlp, m = _field(ddf, lay)
+    yield lay, table, mlp, m
+    ddf.ddf_destroy(m)
+
+
+def _parity(ddf, orc, field, od, dd, n, what, k=6000):
+    lay, table, mlp, m = field
+    dist = torch.full((n,), float("nan"), device="cuda"); vis = torch.full((n,), float("nan"), device="cuda")
+    ddf.ddf_query(m, od, dd, n, dist, vis)
+    torch.cuda.synchronize()
+    assert ddf.ddf_get_info(m, 1) == 1
+    assert bool(torch.isfinite(dist).all()) and bool(torch.isfinite(vis).all())
+    idx = np.unique(np.concatenate([np.arange(0, min(n, 300)), np.arange(max(0, n - 300), n),
+                                    np.arange(0, n, max(1, n // k))]))
+    it = torch.from_numpy(idx).cuda()
+    o, d = od[it].cpu().numpy(), dd[it].cpu().numpy()
+    z, t, xi = orc.hash_forward(lay, table, mlp, o, d, mode=0)
+    _check(dist[it].cpu().numpy(), vis[it].cpu().numpy(), t, xi, what)
+    zg = torch.empty((len(idx), 2), device="cuda")
+    ddf.ddf_query_logits(m, od[it].contiguous(), dd[it].contiguous(), len(idx), zg)
+    zq, _, _ = orc.hash_forward(lay, table, mlp, o, d, mode=1)
+    e = np.abs(zg.cpu().numpy() - zq)
+    assert e.max() <= 2e-2 and e.mean() <= 2e-3, (what, e.max(), e.mean())
+    # batch independence, bit exact
+    d2 = torch.empty(len(idx), device="cuda"); v2 = torch.empty(len(idx), device="cuda")
+    ddf.ddf_query(m, od[it].contiguous(), dd[it].contiguous(), len(idx), d2, v2)
+    assert torch.equal(d2, dist[it]) and torch.equal(v2, vis[it])
+
+
+def test_paper_field_random_origins_all_rays(ddf, orc, paper):
+    """origins uniform in the box (incoherent gathers), every one of 20000 rays checked"""
+    o, d = random_rays(20000)
+    o = (o * 2.9).astype(np.float32)
+    _parity(ddf, orc, paper, _cuda(o), _cuda(d), 20000, "hash random", k=20000)
+
+
+def test_paper_field_camera_shadow_ao_batches(ddf, orc, paper):
+    lay, table, mlp, m = paper
+    # 2^20 primary rays (one shared origin)
+    cam = ddf.ddf_camera_from_seed(MASTER_SEED, STREAMS["camera_pos"], 2.5)
+    n = 1 << 20
+    od = torch.empty((n, 3), device="cuda"); dd = torch.empty((n, 3), device="cuda")
+    ddf.ddf_gen_camera(cam, 1024, 1024, od, dd)
+    _parity(ddf, orc, paper, od, dd, n, "hash camera")
+    # 2^22 shadow rays from the unit sphere
+    n = 1 << 22
+    p = torch.empty((n, 3), device="cuda"); nr = torch.empty((n, 3), device="cuda")
+    od = torch.empty((n, 3), device="cuda"); dd = torch.empty((n, 3), device="cuda")
+    ddf.ddf_gen_sphere_points(MASTER_SEED, STREAMS["shadow_points"], n, 1.0, p, nr)
+    ddf.ddf_gen_shadow(p, nr, n, (3.0, 3.0, 3.0), 1e-3, od, dd, None)
+    _parity(ddf, orc, paper, od, dd, n, "hash shadow")
+    # AO: 512x512 G-buffer x 16 samples, fused reduce = reducer on the per-ray outputs, bit exact
+    W = H = 512; npts = W * H; spp = 16; n = npts * spp
+    sc = ddf.DdfScene((0.0, 0.0, 0.0), 0.6, (-3.0, -3.0, -3.0), (3.0, 3.0, 3.0))
+    gp = torch.empty((npts, 3), device="cuda"); gn = torch.empty((npts, 3), device="cuda")
+    ddf.ddf_gen_gbuffer(cam, sc, W, H, gp, gn, None)
+    od = torch.empty((n, 3), device="cuda"); dd = torch.empty((n, 3), device="cuda")
+    ddf.ddf_gen_ao(gp, gn, npts, spp, MASTER_SEED, STREAMS["ao_samples"], 1e-3, od, dd)
+    _parity(ddf, orc, paper, od, dd, n, "hash AO")
+    ao = torch.full((npts,), float("nan"), device="cuda"); ao2 = torch.empty(npts, device="cuda")
+    ddf.ddf_query_ao(m, od, dd, npts, spp, float("inf"), ao)
+    assert ddf.ddf_get_info(m, 1) == 1
+    dist = torch.empty(n, device="cuda"); vis = torch.empty(n, device="cuda")
+    ddf.ddf_query(m, od, dd, n, dist, vis)
+    ddf.ddf_ao_reduce(vis, dist, npts, spp, float("inf"), ao2)
+    assert torch.equal(ao, ao2)
+
+
+def test_edge_sizes_determinism_and_host_entry(ddf, orc, paper):
+    lay, table, mlp, m = paper
+    N = 128 * 148 * 5 + 77
+    o, d = random_rays(N)
+    od, dd = _cuda(o * 2.0), _cuda(d)
+    full_d = torch.empty(N, device="cuda"); full_v = torch.empty(N, device="cuda")
+    ddf.ddf_query(m, od, dd, N, full_d, full_v)
+    a_d = torch.empty(N, device="cuda"); a_v = torch.empty(N, device="cuda")
+    ddf.ddf_query(m, od, dd, N, a_d, a_v)
+    assert torch.equal(full_d, a_d) and torch.equal(full_v, a_v)
+    for n in (0, 1, 127, 128, 129, 1009):
+        dist = torch.full((n + 8,), -7.0, device="cuda"); vis = torch.full((n + 8,), -7.0, device="cuda")
+        ddf.ddf_query(m, od, dd, n, dist, vis)
+        torch.cuda.synchronize()
+        assert torch.equal(dist[:n], full_d[:n]) and torch.equal(vis[:n], full_v[:n]), n
+        assert bool((dist[n:] == -7.0).all()) and bool((vis[n:] == -7.0).all()), n
+    perm = torch.randperm(N, device="cuda", generator=torch.Generator(device="cuda").manual_seed(2))
+    pd = torch.empty(N, device="cuda"); pv = torch.empty(N, device="cuda")
+    ddf.ddf_query(m, od[perm].contiguous(), dd[perm].contiguous(), N, pd, pv)
+    assert torch.equal(pd, full_d[perm]) and torch.equal(pv, full_v[perm])
+    oh, dh = od.cpu().pin_memory(), dd.cpu().pin_memory()
+    hd, hv = torch.empty(N).pin_memory(), torch.empty(N).pin_memory()
+    ddf.ddf_query_host(m, oh, dh, N, hd, hv)
+    assert torch.equal(hd, full_d.cpu()) and torch.equal(hv, full_v.cpu())
+
+
+@pytest.mark.parametrize("kw", [dict(table_dtype=2), dict(mlp_dtype=1), dict(n_levels=8, n_freq_dir=2, n_hidden=3, log2_table=14),
+                                dict(n_levels=5, base_res=3, growth=2.0, log2_table=10, n_hidden=1, n_freq_dir=0,
+                                     box_min=(-2.0, -1.0, 0.0), box_max=(1.0, 3.0, 0.5))])
+def test_other_field_shapes(ddf, orc, kw):
+    lay = HashLayout(**kw)
+    table, mlp, m = _field(ddf, lay, bias_scale=0.3)
+    o, d = random_rays(5000)
+    o = (o * 3.5).astype(np.float32)                                       # some origins outside the box: clamped
+    _parity(ddf, orc, (lay, table, mlp, m), _cuda(o), _cuda(d), 5000, str(kw), k=5000)
+    ddf.ddf_destroy(m)
+
+
+def test_closed_forms_on_gpu(ddf, orc):
+    """zero MLP => heads of the bias; constant table => features = the constant (partition of unity)
+    so the output is the same for every origin; device-resident blobs give the same field."""
+    lay = layout_hash_paper()
+    n_ent = ddf.ddf_hashgrid_table_entries(lay)
+    table = make_hash_table(lay, n_ent)
+    mlp = np.zeros(8130, np.float32); mlp[-2:] = [2.0, -1.0]
+    m = ddf.ddf_create_hashgrid(table, mlp, lay)
+    o, d = random_rays(1000)
+    dist = torch.empty(1000, device="cuda"); vis = torch.empty(1000, device="cuda")
+    ddf.ddf_query(m, _cuda(o), _cuda(d), 1000, dist, vis)
+    assert np.allclose(dist.cpu().numpy(), 2.1269280110429727, atol=1e-6) and np.allclose(vis.cpu().numpy(), 0.2689414213699951, atol=1e-6)
+    ddf.ddf_destroy(m)
+    const = np.full(2 * n_ent, 0.375, np.float32)
+    mlp = make_hash_mlp(lay, bias_scale=0.2)
+    m = ddf.ddf_create_hashgrid(const, mlp, lay)
+    dsame = np.tile(d[:1], (1000, 1))
+    ddf.ddf_query(m, _cuda(o * 2.5), _cuda(dsame), 1000, dist, vis)
+    assert float(dist.max() - dist.min()) == 0.0 and float(vis.max() - vis.min()) == 0.0
+    z, t, xi = orc.hash_forward(lay, const, mlp, o[:1] * 2.5, dsame[:1])
+    assert abs(float(dist[0]) - t[0]) < 1e-2 and abs(float(vis[0]) - xi[0]) < 1e-2
+    ddf.ddf_destroy(m)
+    m1 = ddf.ddf_create_hashgrid(table, mlp, lay)
+    m2 = ddf.ddf_create_hashgrid(_cuda(table), _cuda(mlp), lay)
+    d1 = torch.empty(1000, device="cuda"); d2 = torch.empty(1000, device="cuda")
+    ddf.ddf_query(m1, _cuda(o), _cuda(d), 1000, d1, None); ddf.ddf_query(m2, _cuda(o), _cuda(d), 1000, d2, None)
+    assert torch.equal(d1, d2)
+    ddf.ddf_destroy(m1); ddf.ddf_destroy(m2)
