@@ -307,7 +307,60 @@ def run_extras(ddf, torch, model, peaks):
                                       "ddf_speedup": ms / ddf_ms}
     ex["ddf_camera_2^20_ms"] = ddf_ms
     ddf.ddf_destroy(sdf)
+    del o, d, t, hit, st, dist, vis
+    ex["hashgrid_field"] = run_hashgrid(ddf, torch, peaks)
     return ex
+
+
+def run_hashgrid(ddf, torch, peaks):
+    """the paper's own field (hash grid 16 x 2 x 2^19 + 4 direction bands + 2 x 64
+    MLP, 52 MB fp32) on the same batch shapes.  Bound: 128 random 8-byte gathers per ray (one 32-byte
+    sector each) served by L1/L2; `gather_GBps` counts the 1024 B/ray actually used, `sector_GBps`
+    the 4096 B/ray of sectors moved.  The paper's own figure for this field (tiny-cuda-nn on an
+    A100) is quoted as context only."""
+    from ddf_inputs import MASTER_SEED, STREAMS, layout_hash_paper, make_hash_table, make_hash_mlp, random_rays
+    lay = layout_hash_paper()
+    n_ent = ddf.ddf_hashgrid_table_entries(lay)
+    table, mlp = make_hash_table(lay, n_ent), make_hash_mlp(lay)
+    m = ddf.ddf_create_hashgrid(table, mlp, lay)
+    out = {"table_entries": n_ent, "field_MB": (2 * n_ent + 8130) * 4 / 1e6,
+           "paper_context": {"Mrays_s": 333.0, "what": "tiny-cuda-nn, A100, 1M rays (PAPER.md:202: 0.0030 us/ray)"}}
+    cam = ddf.ddf_camera_from_seed(MASTER_SEED, STREAMS["camera_pos"], 2.5)
+
+    def rec(name, n, ms):
+        out[name] = {"ms": ms, "Mrays_s": n / ms / 1e3, "gather_GBps": n * 1024 / (ms * 1e-3) / 1e9,
+                     "sector_GBps": n * 4096 / (ms * 1e-3) / 1e9}
+    n = 1 << 22
+    o_np, d_np = random_rays(n)
+    o = torch.from_numpy(o_np).cuda() * 2.9; d = torch.from_numpy(d_np).cuda()
+    dist = torch.empty(n, device="cuda"); vis = torch.empty(n, device="cuda")
+    rec("random_origins_2^22", n, _time_ms(torch, lambda: ddf.ddf_query(m, o, d, n, dist, vis), reps=7))
+    for lg in (10, 14, 18):
+        k = 1 << lg
+        rec("random_origins_2^%d" % lg, k, _time_ms(torch, lambda: ddf.ddf_query(m, o, d, k, dist, vis), reps=7))
+    oc = torch.empty((1 << 20, 3), device="cuda"); dc = torch.empty((1 << 20, 3), device="cuda")
+    ddf.ddf_gen_camera(cam, 1024, 1024, oc, dc)
+    rec("camera_2^20", 1 << 20, _time_ms(torch, lambda: ddf.ddf_query(m, oc, dc, 1 << 20, dist, vis), reps=7))
+    p = torch.empty((n, 3), device="cuda"); nr = torch.empty((n, 3), device="cuda")
+    ddf.ddf_gen_sphere_points(MASTER_SEED, STREAMS["shadow_points"], n, 1.0, p, nr)
+    ddf.ddf_gen_shadow(p, nr, n, (3.0, 3.0, 3.0), 1e-3, o, d, None)
+    rec("shadow_2^22", n, _time_ms(torch, lambda: ddf.ddf_query(m, o, d, n, dist, vis), reps=7))
+    del p, nr, o, d
+    W = H = 1024; npts = W * H; spp = 16; na = npts * spp
+    sc = ddf.DdfScene((0.0, 0.0, 0.0), 0.6, (-3.0, -3.0, -3.0), (3.0, 3.0, 3.0))
+    gp = torch.empty((npts, 3), device="cuda"); gn = torch.empty((npts, 3), device="cuda")
+    ddf.ddf_gen_gbuffer(cam, sc, W, H, gp, gn, None)
+    oa = torch.empty((na, 3), device="cuda"); da = torch.empty((na, 3), device="cuda"); ao = torch.empty(npts, device="cuda")
+    ddf.ddf_gen_ao(gp, gn, npts, spp, MASTER_SEED, STREAMS["ao_samples"], 1e-3, oa, da)
+    rec("ao_16.7M_fused", na, _time_ms(torch, lambda: ddf.ddf_query_ao(m, oa, da, npts, spp, float("inf"), ao), reps=5))
+    del oa, da
+    ddf.ddf_destroy(m)
+    # the oracle on the host cores, bounded sample
+    import oracle
+    k = 1 << 17
+    t0 = time.time(); oracle.hash_forward(lay, table, mlp, o_np[:k] * 2.9, d_np[:k]); dt = time.time() - t0
+    out["cpu_oracle"] = {"Mrays_s": k / dt / 1e6, "cores": oracle.default_threads(), "sample": "%d random-origin rays, %.2f s" % (k, dt)}
+    return out
 
 
 def main():

@@ -19,6 +19,7 @@
 #include "ddf_tc_ptx.cuh"
 #include <cuda_fp16.h>
 #include <math.h>
+#include <stdio.h>
 #include <stdlib.h>
 #include <string.h>
 #include <new>
@@ -293,6 +294,7 @@ int hash_forward(Model* m, const float* o, const float* d, int64_t n, int mode_o
   if (tiles < grid) grid = tiles;
   if (p.table_f16) ddf_hash_kernel<true><<<(unsigned)grid, kHgThreads, h->smem_bytes, st>>>(p);
   else             ddf_hash_kernel<false><<<(unsigned)grid, kHgThreads, h->smem_bytes, st>>>(p);
+  if (getenv("DDF_DEBUG")) fprintf(stderr, "[ddf_hash] grid %lld ctas %d\n", (long long)grid, h->ctas_per_sm);
   DDF_CUDA_TRY(cudaGetLastError());
   m->last_launches = 1;
   return DDF_OK;
@@ -404,12 +406,33 @@ extern "C" int ddf_create_hashgrid(const void* table, const void* mlp, const ddf
   if ((e = cudaFuncSetAttribute(ddf_hash_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_bytes)) != cudaSuccess ||
       (e = cudaFuncSetAttribute(ddf_hash_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_bytes)) != cudaSuccess)
     return fail(DDF_E_CUDA, e);
-  int occ = 0;
-  if ((e = (L.table_dtype == 2 ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, ddf_hash_kernel<true>, kHgThreads, h->smem_bytes)
-                               : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, ddf_hash_kernel<false>, kHgThreads, h->smem_bytes))) != cudaSuccess)
+  // resident CTAs per SM from the kernel's own resource use (the runtime's occupancy query answers
+  // for the current carve-out, which another library in the process may have left at "prefer L1")
+  cudaFuncAttributes fa;
+  if ((e = (L.table_dtype == 2 ? cudaFuncGetAttributes(&fa, ddf_hash_kernel<true>) : cudaFuncGetAttributes(&fa, ddf_hash_kernel<false>))) != cudaSuccess ||
+      false)
     return fail(DDF_E_CUDA, e);
+  const int regs_cta = ((fa.numRegs * 32 + 255) / 256 * 256) * (kHgThreads / 32);
+  int occ = prop.regsPerMultiprocessor / (regs_cta > 0 ? regs_cta : 1);
+  const int by_smem = (int)(prop.sharedMemPerMultiprocessor / (h->smem_bytes + prop.reservedSharedMemPerBlock));
+  if (by_smem < occ) occ = by_smem;
   if (occ < 1) return fail(DDF_E_UNSUPPORTED, cudaSuccess);
-  h->ctas_per_sm = occ > 8 ? 8 : occ;                   // 8 x 64 TMEM columns = all 512
+  // measured on B200: 4 resident CTAs is the best trade between latency hiding
+  // and the L1 left for the coarse levels (8 x 64 TMEM columns would be the hard limit)
+  h->ctas_per_sm = occ > 4 ? 4 : occ;
+  if (const char* ev = getenv("DDF_HASH_CTAS")) { int v = atoi(ev); if (v >= 1 && v <= h->ctas_per_sm) h->ctas_per_sm = v; }
+  // shared-memory carve-out: just what the resident CTAs need; the rest of the 256 KB stays L1,
+  // which is what serves the coarse (small) levels of the grid
+  {
+    int pct = (int)((h->ctas_per_sm * (h->smem_bytes + prop.reservedSharedMemPerBlock) * 100 + prop.sharedMemPerMultiprocessor - 1) / prop.sharedMemPerMultiprocessor);
+    if (const char* ev = getenv("DDF_HASH_CARVEOUT")) pct = atoi(ev);
+    if (pct > 100) pct = 100;
+    if ((e = cudaFuncSetAttribute(ddf_hash_kernel<false>, cudaFuncAttributePreferredSharedMemoryCarveout, pct)) != cudaSuccess ||
+        (e = cudaFuncSetAttribute(ddf_hash_kernel<true>, cudaFuncAttributePreferredSharedMemoryCarveout, pct)) != cudaSuccess)
+      return fail(DDF_E_CUDA, e);
+    if (getenv("DDF_DEBUG")) fprintf(stderr, "[ddf_hash] carveout %d %%\n", pct);
+  }
+  if (getenv("DDF_DEBUG")) fprintf(stderr, "[ddf_hash] regs %d ctas/SM %d smem %zu\n", fa.numRegs, h->ctas_per_sm, h->smem_bytes);
   if ((e = cudaDeviceSynchronize()) != cudaSuccess) return fail(DDF_E_CUDA, e);
   *out = reinterpret_cast<ddf_model*>(m);
   return DDF_OK;
