@@ -309,7 +309,34 @@ def run_extras(ddf, torch, model, peaks):
     ddf.ddf_destroy(sdf)
     del o, d, t, hit, st, dist, vis
     ex["hashgrid_field"] = run_hashgrid(ddf, torch, peaks)
+    ex["wavefront_shadowed_camera_2^20"] = run_wavefront(ddf, torch)
     return ex
+
+
+def run_wavefront(ddf, torch):
+    """primary query -> hit compaction -> shadow rays -> second query -> lit flags in
+    one call (ddf_query_shadowed) on the 2^20 camera batch with spread origins; visibility-head bias 1
+    so that most rays hit.  Rays/s counts primary + secondary evaluations."""
+    from ddf_inputs import MASTER_SEED, STREAMS, layout_c1, layout_hash_paper, make_weights, make_hash_table, make_hash_mlp, random_rays
+    out = {}
+    n = 1 << 20
+    cam = ddf.ddf_camera_from_seed(MASTER_SEED, STREAMS["camera_pos"], 2.5)
+    o = torch.empty((n, 3), device="cuda"); d = torch.empty((n, 3), device="cuda")
+    ddf.ddf_gen_camera(cam, 1024, 1024, o, d)
+    o += torch.from_numpy(random_rays(n)[0]).cuda() * 0.4
+    dist = torch.empty(n, device="cuda"); vis = torch.empty(n, device="cuda")
+    lit = torch.empty(n, dtype=torch.uint8, device="cuda"); cnt = torch.zeros(1, dtype=torch.int64, device="cuda")
+    lay = layout_c1(); blob = make_weights(lay).copy(); blob[-1] = 0x3F80
+    hl = layout_hash_paper(); mlp = make_hash_mlp(hl).copy(); mlp[-1] = 1.0
+    models = {"dense_8x1280": ddf.ddf_create(blob, lay),
+              "hashgrid": ddf.ddf_create_hashgrid(make_hash_table(hl, ddf.ddf_hashgrid_table_entries(hl)), mlp, hl)}
+    for name, m in models.items():
+        ms = _time_ms(torch, lambda: ddf.ddf_query_shadowed(m, o, d, n, (3.0, 3.0, 3.0), 1e-3, dist, vis, lit, cnt), reps=5)
+        k = int(cnt.item())
+        out[name] = {"ms": ms, "shadow_rays": k, "lit_fraction_of_hits": float(lit.sum().item()) / max(k, 1),
+                     "launches": ddf.ddf_get_info(m, 1), "Mrays_s_primary_plus_secondary": (n + k) / ms / 1e3}
+        ddf.ddf_destroy(m)
+    return out
 
 
 def run_hashgrid(ddf, torch, peaks):

@@ -167,6 +167,30 @@ int  ddf_query_ao(ddf_model* model, const float* o, const float* d, int64_t n_pt
 int  ddf_shadow_test(const float* vis, const float* dist, const float* tmax, int64_t n,
                      uint8_t* shadow, void* stream);
 
+/* ---------------------------------------------------------------- wavefront secondary rays
+ * PAPER.md:13 (the field answers "what a surface point sees in some direction")
+ * ("The hit point is x + t d when xi is high"), PAPER.md:80 (shadow test: evaluate f from the
+ * surface point toward the light; occluded within the distance to the light => shadow).
+ * ddf_gen_shadow_from_hits turns the results of a primary query into a COMPACTED batch of shadow
+ * rays: for every primary ray i with vis[i] > 0.5, in increasing i (stable),
+ *   o2 = o_i + (dist_i - eps) d_i     (the hit point, stepped back by eps along the ray - the
+ *                                      field returns no normal to offset along),
+ *   d2 = normalise(light - o2),  tmax = |light - o2|,  index[k] = i.
+ * All pointers [device]; o2, d2 [n][3], tmax [n], index [n] must hold n entries; *count (int64,
+ * [device]) receives the number of secondary rays.  Uses a workspace owned by `model`. */
+int  ddf_gen_shadow_from_hits(ddf_model* model, const float* o, const float* d, const float* dist,
+                              const float* vis, int64_t n, const float light[3], float eps,
+                              float* o2, float* d2, float* tmax, int32_t* index, int64_t* count,
+                              void* stream);
+/* The whole loop in one call: primary query -> hit compaction -> shadow rays -> second query on
+ * the compacted batch (its size never leaves the device on the tcgen05 and hash-grid paths) ->
+ * lit[i] = 1 if ray i hit (vis > 0.5) and its shadow ray is NOT occluded (not (vis2 > 0.5 and
+ * dist2 < tmax)), else 0.  out_dist / out_vis [n] receive the primary results; out_count
+ * (int64 [device], may be NULL) the number of shadow rays traced. */
+int  ddf_query_shadowed(ddf_model* model, const float* o, const float* d, int64_t n,
+                        const float light[3], float eps, float* out_dist, float* out_vis,
+                        uint8_t* out_lit, int64_t* out_count, void* stream);
+
 /* ---------------------------------------------------------------- sphere-tracing comparison
  * (BASELINE.json configs[4]).  `model` must have input_kind 1, n_out 1.
  * Traces s(p) = (|p| - base_radius) + alpha * MLP(p):

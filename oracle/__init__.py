@@ -71,6 +71,7 @@ def lib():
         _lib.orc_hash_table_entries.restype = C.c_int64
         _lib.orc_hash_mlp_params.restype = C.c_int64
         _lib.orc_hash_index.restype = C.c_int64
+        _lib.orc_gen_shadow_from_hits.restype = C.c_int64
         _lib.orc_ray_sphere.restype = C.c_double
         _lib.orc_ray_box_exit.restype = C.c_double
     return _lib
@@ -346,3 +347,24 @@ def hash_forward(lay, table, mlp, o, d, mode=0, nthreads=0):
     if rc != 0:
         raise ValueError("oracle: bad hash layout")
     return z, dist, vis
+
+
+# ------------------------------------------------------------------ wavefront secondary rays
+
+def gen_shadow_from_hits(o, d, dist, vis, light=(3.0, 3.0, 3.0), eps=1e-3):
+    """Returns (o2, d2, tmax, index) of the compacted shadow-ray batch."""
+    o, d, dist, vis = _f32(o), _f32(d), _f32(dist), _f32(vis)
+    n = o.shape[0]
+    o2 = np.empty((n, 3), np.float32); d2 = np.empty((n, 3), np.float32)
+    tmax = np.empty(n, np.float32); index = np.empty(n, np.int32)
+    k = lib().orc_gen_shadow_from_hits(_p(o), _p(d), _p(dist), _p(vis), C.c_int64(n), _v3(light), C.c_float(eps),
+                                       _p(o2), _p(d2), _p(tmax), _p(index))
+    return o2[:k].copy(), d2[:k].copy(), tmax[:k].copy(), index[:k].copy()
+
+
+def shadow_lit(vis2, dist2, tmax, index, n):
+    vis2, dist2, tmax = _f32(vis2), _f32(dist2), _f32(tmax)
+    index = np.ascontiguousarray(index, dtype=np.int32)
+    lit = np.empty(n, np.uint8)
+    lib().orc_shadow_lit(_p(vis2), _p(dist2), _p(tmax), _p(index), C.c_int64(len(index)), C.c_int64(n), _p(lit))
+    return lit

@@ -419,3 +419,31 @@ int orc_sphere_trace(const orc_layout* L, const void* blob, const float* o, cons
   }
   return 0;
 }
+
+/* ------------------------------------------------------------------ wavefront secondary rays */
+
+int64_t orc_gen_shadow_from_hits(const float* o, const float* d, const float* dist, const float* vis,
+                                 int64_t n, const double light[3], float eps, float* o2, float* d2,
+                                 float* tmax, int32_t* index) {
+  int64_t k = 0;
+  for (int64_t i = 0; i < n; ++i) {
+    if (!(vis[i] > 0.5f)) continue;                       /* "when xi is high" */
+    const float t = dist[i] - eps;                        /* stepped back along the ray */
+    double p[3], v[3];
+    for (int a = 0; a < 3; ++a) p[a] = (double)o[3 * i + a] + (double)t * (double)d[3 * i + a];
+    for (int a = 0; a < 3; ++a) v[a] = light[a] - (double)(float)p[a];
+    const double len = sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]);
+    for (int a = 0; a < 3; ++a) { o2[3 * k + a] = (float)p[a]; d2[3 * k + a] = (float)(v[a] / len); }
+    tmax[k] = (float)len;
+    index[k] = (int32_t)i;
+    ++k;
+  }
+  return k;
+}
+
+void orc_shadow_lit(const float* vis2, const float* dist2, const float* tmax, const int32_t* index,
+                    int64_t count, int64_t n, uint8_t* lit) {
+  for (int64_t i = 0; i < n; ++i) lit[i] = 0;
+  for (int64_t k = 0; k < count; ++k)                     /* occluded within the distance to the light */
+    lit[index[k]] = (vis2[k] > 0.5f && dist2[k] < tmax[k]) ? 0 : 1;
+}

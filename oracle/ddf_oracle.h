@@ -75,6 +75,17 @@ void orc_gen_ao(const float* p, const float* nrm, int64_t n_pts, int spp, uint64
 void orc_ao_reduce(const float* vis, const float* dist, int64_t n_pts, int spp,
                    double ao_radius, float* ao);
 
+/* ---- wavefront secondary rays (PAPER.md:62 hit point x + t d; PAPER.md:80 shadow test) ----
+ * for every i with vis[i] > 0.5, in increasing i: o2 = o_i + (dist_i - eps) d_i (fp32 subtraction,
+ * the rest in fp64, rounded to fp32), d2 = normalise(light - o2), tmax = |light - o2|, index = i.
+ * Returns the number of secondary rays. */
+int64_t orc_gen_shadow_from_hits(const float* o, const float* d, const float* dist, const float* vis,
+                                 int64_t n, const double light[3], float eps, float* o2, float* d2,
+                                 float* tmax, int32_t* index);
+/* lit[i] = 1 iff ray i hit and its shadow ray is not occluded (vis2 > 0.5 and dist2 < tmax) */
+void orc_shadow_lit(const float* vis2, const float* dist2, const float* tmax, const int32_t* index,
+                    int64_t count, int64_t n, uint8_t* lit);
+
 /* ---- sphere tracing of s(p) = (|p| - base_radius) + alpha * MLP(p)  (readings A19, A20) ----
  * Ray state (t, p, s) is carried in fp32 exactly as the kernel carries it; the MLP itself is
  * evaluated by orc_forward in `mode`.  trace_p/trace_s (may be NULL) receive, for every ray,

@@ -10,6 +10,7 @@ from .binding import (  # noqa: F401
     ddf_get_info, ddf_camera_from_seed, ddf_gen_camera, ddf_gen_sphere_points, ddf_gen_shadow,
     ddf_gen_gbuffer, ddf_gen_ao, ddf_ao_reduce, ddf_shadow_test, sdf_sphere_trace, ddf_status_string,
     DdfHashgridLayout, make_hashgrid_layout, ddf_hashgrid_table_entries, ddf_create_hashgrid,
+    ddf_gen_shadow_from_hits, ddf_query_shadowed,
     EXPORTED_SYMBOLS,
 )
 from .build import build  # noqa: F401

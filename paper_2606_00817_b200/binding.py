@@ -16,7 +16,7 @@ EXPORTED_SYMBOLS = [
     "ddf_get_info", "ddf_query", "ddf_query_host", "ddf_query_logits", "ddf_camera_from_seed",
     "ddf_gen_camera", "ddf_gen_sphere_points", "ddf_gen_shadow", "ddf_gen_gbuffer", "ddf_gen_ao",
     "ddf_ao_reduce", "ddf_query_ao", "ddf_shadow_test", "sdf_sphere_trace",
-    "ddf_hashgrid_table_entries", "ddf_create_hashgrid",
+    "ddf_hashgrid_table_entries", "ddf_create_hashgrid", "ddf_gen_shadow_from_hits", "ddf_query_shadowed",
 ]
 
 
@@ -264,3 +264,17 @@ def sdf_sphere_trace(model, o, d, n, params, out_t, out_hit, out_steps, trace_p=
                                   _dev(out_hit, torch.uint8), _dev(out_steps, torch.int32), _dev(trace_p),
                                   _dev(trace_s), _dev(total_evals, torch.int64), _stream(stream)),
            "sdf_sphere_trace")
+
+
+def ddf_gen_shadow_from_hits(model, o, d, dist, vis, n, light, eps, o2, d2, tmax, index, count, stream=None):
+    li = (C.c_float * 3)(*[float(x) for x in light])
+    _check(lib().ddf_gen_shadow_from_hits(model.handle, _dev(o), _dev(d), _dev(dist), _dev(vis), C.c_int64(n), li,
+                                          C.c_float(eps), _dev(o2), _dev(d2), _dev(tmax), _dev(index, torch.int32),
+                                          _dev(count, torch.int64), _stream(stream)), "ddf_gen_shadow_from_hits")
+
+
+def ddf_query_shadowed(model, o, d, n, light, eps, out_dist, out_vis, out_lit, out_count=None, stream=None):
+    li = (C.c_float * 3)(*[float(x) for x in light])
+    _check(lib().ddf_query_shadowed(model.handle, _dev(o), _dev(d), C.c_int64(n), li, C.c_float(eps), _dev(out_dist),
+                                    _dev(out_vis), _dev(out_lit, torch.uint8), _dev(out_count, torch.int64),
+                                    _stream(stream)), "ddf_query_shadowed")

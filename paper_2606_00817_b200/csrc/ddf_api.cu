@@ -35,7 +35,7 @@ static void free_model(Model* m) {
   cudaFree(m->ws_gamma); cudaFree(m->ws_act0); cudaFree(m->ws_act1); cudaFree(m->ws_last);
   cudaFree(m->ws_dist); cudaFree(m->ws_vis);
   cudaFree(m->h2d_o); cudaFree(m->h2d_d); cudaFree(m->d2h_dist); cudaFree(m->d2h_vis);
-  cudaFree(m->trace_ws);
+  cudaFree(m->trace_ws); cudaFree(m->wave_ws);
   (void)cudaGetLastError();
   delete m;
 }
@@ -181,7 +181,7 @@ static int run_query(Model* m, const float* o, const float* d, int64_t n, int mo
   if (n == 0) { m->last_launches = 0; return DDF_OK; }
   if (!o || !out0 || (m->lay.input_kind == 0 && !d)) return DDF_E_INVALID_ARG;
   cudaStream_t st = (cudaStream_t)stream;
-  if (m->hg) return hash_forward(m, o, d, n, mode_out, out0, out1, 0, 0.0f, st);
+  if (m->hg) return hash_forward(m, o, d, n, nullptr, mode_out, out0, out1, 0, 0.0f, st);
   if (m->tc && m->path != 1) return tc_forward(m, o, d, n, nullptr, mode_out, out0, out1, 0, 0.0f, st);
   return simt_forward(m, o, d, n, mode_out, out0, out1, st);
 }
@@ -234,7 +234,7 @@ extern "C" int ddf_query_ao(ddf_model* model, const float* o, const float* d, in
   const int64_t n = n_pts * spp;
   cudaStream_t st = (cudaStream_t)stream;
   if (m->hg && spp <= 32 && 32 % spp == 0)
-    return hash_forward(m, o, d, n, 2, ao, nullptr, spp, ao_radius, st);
+    return hash_forward(m, o, d, n, nullptr, 2, ao, nullptr, spp, ao_radius, st);
   if (m->tc && m->path != 1 && spp <= 32 && 32 % spp == 0)   // a pixel's rays sit in one warp of a tile
     return tc_forward(m, o, d, n, nullptr, 2, ao, nullptr, spp, ao_radius, st);
   if (n > m->ws_out_rows) {

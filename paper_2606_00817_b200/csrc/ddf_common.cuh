@@ -62,6 +62,8 @@ struct Model {
   int64_t host_rows;
   // sphere tracer state
   void* trace_ws; size_t trace_ws_bytes;
+  // wavefront secondary rays (ddf_wave.cu)
+  void* wave_ws; size_t wave_ws_bytes;
   int path;                        // 0 auto, 1 SIMT, 2 tcgen05
   TcPlan* tc;                      // non-null when the tcgen05 path can serve the layout
   HashPlan* hg;                    // non-null: this model is a hash-grid field (ddf_create_hashgrid)
@@ -83,7 +85,7 @@ int tc_forward(Model* m, const float* o, const float* d, int64_t n, const int64_
 
 // ---- hash-grid field (ddf_hash.cu)
 void hash_plan_destroy(Model* m);
-int hash_forward(Model* m, const float* o, const float* d, int64_t n, int mode_out,
+int hash_forward(Model* m, const float* o, const float* d, int64_t n, const int64_t* n_dev, int mode_out,
                  float* out0, float* out1, int spp, float ao_radius, cudaStream_t st);
 
 // ---- device helpers -------------------------------------------------------------------------

@@ -43,7 +43,7 @@ struct HgParams {
   const float* head_w;          // [2][64] (bf16-rounded values)
   const float* o; const float* d;
   float* out0; float* out1;
-  int64_t n;
+  int64_t n; const int64_t* n_dev;        // n_dev (device) overrides n when non-null; it can only be smaller
   float bmin[3], den[3];
   float head_b[2];
   float ao_radius;
@@ -98,10 +98,11 @@ __global__ void __launch_bounds__(kHgThreads, 5) ddf_hash_kernel(const __grid_co
   const uint32_t xrow = x_smem + (uint32_t)t * 128u;
   uint32_t phase = 0;
 
-  const int64_t num_tiles = (p.n + kHgThreads - 1) / kHgThreads;
+  const int64_t n_rays = p.n_dev ? *p.n_dev : p.n;
+  const int64_t num_tiles = (n_rays + kHgThreads - 1) / kHgThreads;
   for (int64_t tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
     const int64_t ray = tile * kHgThreads + t;
-    const bool valid = ray < p.n;
+    const bool valid = ray < n_rays;
     uint32_t rw[32];                                   // the operand row, 64 bf16
     #pragma unroll
     for (int i = 0; i < 32; ++i) rw[i] = 0u;
@@ -283,11 +284,11 @@ void hash_plan_destroy(Model* m) {
   m->hg = nullptr;
 }
 
-int hash_forward(Model* m, const float* o, const float* d, int64_t n, int mode_out,
+int hash_forward(Model* m, const float* o, const float* d, int64_t n, const int64_t* n_dev, int mode_out,
                  float* out0, float* out1, int spp, float ao_radius, cudaStream_t st) {
   HashPlan* h = m->hg;
   HgParams p = h->base;
-  p.o = o; p.d = d; p.n = n; p.out0 = out0; p.out1 = out1;
+  p.o = o; p.d = d; p.n = n; p.n_dev = n_dev; p.out0 = out0; p.out1 = out1;
   p.mode_out = mode_out; p.spp = spp > 0 ? spp : 1; p.ao_radius = ao_radius;
   const int64_t tiles = (n + kHgThreads - 1) / kHgThreads;
   int64_t grid = (int64_t)m->sm_count * h->ctas_per_sm;

@@ -1,0 +1,186 @@
+// ddf_wave.cu - wavefront secondary rays: primary query -> hit points -> compacted shadow rays ->
+// second query -> lit flags (include/ddf.h).  The compaction is a stable
+// three-kernel scan (per-block counts, one-block scan of the counts, scatter), so the secondary
+// batch is in increasing primary-ray order and reproducible; its size stays on the device and is
+// read by the query kernels themselves (n_dev), so the loop needs no host round trip.
+#include "ddf_common.cuh"
+
+namespace ddf {
+
+constexpr int kWaveBlock = 256;
+
+__global__ void wave_count_kernel(const float* __restrict__ vis, int64_t n, int32_t* __restrict__ block_counts) {
+  const int64_t i = (int64_t)blockIdx.x * kWaveBlock + threadIdx.x;
+  const int hit = (i < n) && (vis[i] > 0.5f);
+  const int c = __syncthreads_count(hit);
+  if (threadIdx.x == 0) block_counts[blockIdx.x] = c;
+}
+
+// exclusive scan of the block counts in place (one block), total -> *count
+__global__ void wave_scan_kernel(int32_t* __restrict__ block_counts, int64_t n_blocks, int64_t* __restrict__ count) {
+  __shared__ int32_t warp_sums[32];
+  __shared__ int64_t carry;
+  if (threadIdx.x == 0) carry = 0;
+  __syncthreads();
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  for (int64_t base = 0; base < n_blocks; base += blockDim.x) {
+    const int64_t i = base + threadIdx.x;
+    const int32_t v = (i < n_blocks) ? block_counts[i] : 0;
+    int32_t x = v;
+    #pragma unroll
+    for (int s = 1; s < 32; s <<= 1) { const int32_t y = __shfl_up_sync(0xffffffffu, x, s); if (lane >= s) x += y; }
+    if (lane == 31) warp_sums[warp] = x;
+    __syncthreads();
+    if (warp == 0) {
+      int32_t w = (lane < (int)(blockDim.x >> 5)) ? warp_sums[lane] : 0;
+      #pragma unroll
+      for (int s = 1; s < 32; s <<= 1) { const int32_t y = __shfl_up_sync(0xffffffffu, w, s); if (lane >= s) w += y; }
+      warp_sums[lane] = w;                                   // inclusive over warps
+    }
+    __syncthreads();
+    const int64_t before = carry + (warp ? warp_sums[warp - 1] : 0) + (x - v);
+    if (i < n_blocks) block_counts[i] = (int32_t)before;     // n <= 2^31 - 1 rays
+    __syncthreads();
+    if (threadIdx.x == blockDim.x - 1) carry += warp_sums[(blockDim.x >> 5) - 1];
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) *count = carry;
+}
+
+__global__ void wave_scatter_kernel(const float* __restrict__ o, const float* __restrict__ d,
+                                    const float* __restrict__ dist, const float* __restrict__ vis, int64_t n,
+                                    float lx, float ly, float lz, float eps, const int32_t* __restrict__ block_offsets,
+                                    float* __restrict__ o2, float* __restrict__ d2, float* __restrict__ tmax,
+                                    int32_t* __restrict__ index) {
+  __shared__ int32_t warp_base[kWaveBlock / 32];
+  const int64_t i = (int64_t)blockIdx.x * kWaveBlock + threadIdx.x;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const bool hit = (i < n) && (vis[i] > 0.5f);
+  const uint32_t m = __ballot_sync(0xffffffffu, hit);
+  if (lane == 0) warp_base[warp] = __popc(m);
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    int32_t run = 0;
+    for (int w = 0; w < kWaveBlock / 32; ++w) { const int32_t c = warp_base[w]; warp_base[w] = run; run += c; }
+  }
+  __syncthreads();
+  if (!hit) return;
+  const int64_t k = (int64_t)block_offsets[blockIdx.x] + warp_base[warp] + __popc(m & ((1u << lane) - 1u));
+  const float t = dist[i] - eps;
+  const float ox = fmaf(t, d[3 * i], o[3 * i]), oy = fmaf(t, d[3 * i + 1], o[3 * i + 1]), oz = fmaf(t, d[3 * i + 2], o[3 * i + 2]);
+  const float dx = lx - ox, dy = ly - oy, dz = lz - oz;
+  const float len = sqrtf(fmaf(dz, dz, fmaf(dy, dy, dx * dx)));
+  const float inv = 1.0f / len;
+  o2[3 * k] = ox; o2[3 * k + 1] = oy; o2[3 * k + 2] = oz;
+  d2[3 * k] = dx * inv; d2[3 * k + 1] = dy * inv; d2[3 * k + 2] = dz * inv;
+  tmax[k] = len;
+  index[k] = (int32_t)i;
+}
+
+// lit[index[k]] = not occluded, for k < *count (lit was zeroed before: primary misses stay 0)
+__global__ void wave_lit_kernel(const float* __restrict__ vis2, const float* __restrict__ dist2,
+                                const float* __restrict__ tmax, const int32_t* __restrict__ index,
+                                const int64_t* __restrict__ count, uint8_t* __restrict__ lit) {
+  const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= *count) return;
+  lit[index[k]] = (vis2[k] > 0.5f && dist2[k] < tmax[k]) ? 0 : 1;
+}
+
+struct WaveWs { int32_t* block_counts; float *o2, *d2, *tmax, *dist2, *vis2; int32_t* index; int64_t* count; };
+
+// workspace: block counts always; the ray buffers only for ddf_query_shadowed (full = true)
+static int wave_ws(Model* m, int64_t n, bool full, WaveWs* w) {
+  const size_t nb = (size_t)((n + kWaveBlock - 1) / kWaveBlock);
+  const size_t a = (size_t)((n + 63) / 64 * 64);
+  size_t need = ((nb * 4 + 255) / 256) * 256 + 256;
+  if (full) need += a * (12 + 12 + 4 + 4 + 4 + 4);
+  if (need > m->wave_ws_bytes) {
+    cudaFree(m->wave_ws); m->wave_ws = nullptr; m->wave_ws_bytes = 0;
+    DDF_CUDA_TRY(cudaMalloc(&m->wave_ws, need));
+    m->wave_ws_bytes = need;
+  }
+  uint8_t* b = (uint8_t*)m->wave_ws;
+  w->count = (int64_t*)b;                 b += 256;
+  w->block_counts = (int32_t*)b;          b += ((nb * 4 + 255) / 256) * 256;
+  if (full) {
+    w->o2 = (float*)b;    b += a * 12;
+    w->d2 = (float*)b;    b += a * 12;
+    w->tmax = (float*)b;  b += a * 4;
+    w->dist2 = (float*)b; b += a * 4;
+    w->vis2 = (float*)b;  b += a * 4;
+    w->index = (int32_t*)b;
+  }
+  return DDF_OK;
+}
+
+static int wave_compact(Model* m, const WaveWs& w, const float* o, const float* d, const float* dist, const float* vis,
+                        int64_t n, const float light[3], float eps, float* o2, float* d2, float* tmax, int32_t* index,
+                        int64_t* count, cudaStream_t st) {
+  const unsigned nb = (unsigned)((n + kWaveBlock - 1) / kWaveBlock);
+  wave_count_kernel<<<nb, kWaveBlock, 0, st>>>(vis, n, w.block_counts);
+  wave_scan_kernel<<<1, 1024, 0, st>>>(w.block_counts, (int64_t)nb, count);
+  wave_scatter_kernel<<<nb, kWaveBlock, 0, st>>>(o, d, dist, vis, n, light[0], light[1], light[2], eps,
+                                                w.block_counts, o2, d2, tmax, index);
+  DDF_CUDA_TRY(cudaGetLastError());
+  return DDF_OK;
+}
+
+}  // namespace ddf
+
+using namespace ddf;
+
+extern "C" int ddf_gen_shadow_from_hits(ddf_model* model, const float* o, const float* d, const float* dist,
+                                        const float* vis, int64_t n, const float light[3], float eps,
+                                        float* o2, float* d2, float* tmax, int32_t* index, int64_t* count,
+                                        void* stream) {
+  if (!model || !light || !count || n < 0 || n > 0x7fffffff) return DDF_E_INVALID_ARG;
+  cudaStream_t st = (cudaStream_t)stream;
+  if (n == 0) { DDF_CUDA_TRY(cudaMemsetAsync(count, 0, 8, st)); return DDF_OK; }
+  if (!o || !d || !dist || !vis || !o2 || !d2 || !tmax || !index) return DDF_E_INVALID_ARG;
+  Model* m = reinterpret_cast<Model*>(model);
+  WaveWs w;
+  int rc = wave_ws(m, n, false, &w);
+  if (rc != DDF_OK) return rc;
+  rc = wave_compact(m, w, o, d, dist, vis, n, light, eps, o2, d2, tmax, index, count, st);
+  m->last_launches = 3;
+  return rc;
+}
+
+extern "C" int ddf_query_shadowed(ddf_model* model, const float* o, const float* d, int64_t n,
+                                  const float light[3], float eps, float* out_dist, float* out_vis,
+                                  uint8_t* out_lit, int64_t* out_count, void* stream) {
+  if (!model || !light || n < 0 || n > 0x7fffffff) return DDF_E_INVALID_ARG;
+  Model* m = reinterpret_cast<Model*>(model);
+  if (m->lay.input_kind != 0 || m->lay.n_out != 2) return DDF_E_INVALID_ARG;
+  cudaStream_t st = (cudaStream_t)stream;
+  if (n == 0) { if (out_count) DDF_CUDA_TRY(cudaMemsetAsync(out_count, 0, 8, st)); m->last_launches = 0; return DDF_OK; }
+  if (!o || !d || !out_dist || !out_vis || !out_lit) return DDF_E_INVALID_ARG;
+  WaveWs w;
+  int rc = wave_ws(m, n, true, &w);
+  if (rc != DDF_OK) return rc;
+  // 1. primary rays
+  if ((rc = ddf_query(model, o, d, n, out_dist, out_vis, stream)) != DDF_OK) return rc;
+  int launches = m->last_launches;
+  // 2. hit points -> compacted shadow rays
+  if ((rc = wave_compact(m, w, o, d, out_dist, out_vis, n, light, eps, w.o2, w.d2, w.tmax, w.index, w.count, st)) != DDF_OK) return rc;
+  launches += 3;
+  DDF_CUDA_TRY(cudaMemsetAsync(out_lit, 0, (size_t)n, st));
+  // 3. second query on the compacted batch; the fused paths read its size on the device
+  if (m->hg) rc = hash_forward(m, w.o2, w.d2, n, w.count, 0, w.dist2, w.vis2, 0, 0.0f, st);
+  else if (m->tc && m->path != 1) rc = tc_forward(m, w.o2, w.d2, n, w.count, 0, w.dist2, w.vis2, 0, 0.0f, st);
+  else {
+    int64_t live = 0;                                    // the SIMT path sizes its grids on the host
+    DDF_CUDA_TRY(cudaMemcpyAsync(&live, w.count, 8, cudaMemcpyDeviceToHost, st));
+    DDF_CUDA_TRY(cudaStreamSynchronize(st));
+    rc = live > 0 ? simt_forward(m, w.o2, w.d2, live, 0, w.dist2, w.vis2, st) : DDF_OK;
+    if (live == 0) m->last_launches = 0;
+  }
+  if (rc != DDF_OK) return rc;
+  launches += m->last_launches;
+  // 4. shadow decision, scattered back to the primary rays
+  wave_lit_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(w.vis2, w.dist2, w.tmax, w.index, w.count, out_lit);
+  DDF_CUDA_TRY(cudaGetLastError());
+  if (out_count) DDF_CUDA_TRY(cudaMemcpyAsync(out_count, w.count, 8, cudaMemcpyDeviceToDevice, st));
+  m->last_launches = launches + 1;
+  return DDF_OK;
+}

@@ -310,3 +310,31 @@ def test_sphere_trace_teacher_forcing(ddf, orc, sdf):
     # statistics against the CPU tracer run end to end
     rt, rhit, rsteps = orc.sphere_trace(lay, blob, o, d, 64, 1e-3, 6.0, 1.0, 0.05)
     assert abs(hit.mean() - rhit.mean()) < 0.06 and abs(steps.mean() - rsteps.mean()) < 3.0
+
+
+def test_maximum_batch_2pow24_and_side_stream(ddf, orc, c1):
+    """The largest batch BASELINE.json names (2^24 rays, 403 MB of ray data) in one call on a
+    non-default stream: finite everywhere, sampled rays within tolerance, prefix-consistent with a
+    smaller call (results do not depend on n)."""
+    lay, m = c1
+    n = 1 << 24
+    o, d = random_rays(1 << 16)
+    od = _cuda(o).repeat(n >> 16, 1); dd = _cuda(d).repeat(n >> 16, 1)
+    dist = torch.full((n,), float("nan"), device="cuda"); vis = torch.full((n,), float("nan"), device="cuda")
+    st = torch.cuda.Stream()
+    st.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(st):
+        ddf.ddf_query(m, od, dd, n, dist, vis, stream=st)
+    st.synchronize()
+    assert bool(torch.isfinite(dist).all()) and bool(torch.isfinite(vis).all())
+    # the batch repeats a 2^16 block: every repetition must give the same bits
+    assert torch.equal(dist.view(-1, 1 << 16)[0], dist.view(-1, 1 << 16)[-1])
+    assert torch.equal(dist.view(-1, 1 << 16).min(0).values, dist.view(-1, 1 << 16).max(0).values)
+    small_d = torch.empty(1 << 16, device="cuda"); small_v = torch.empty(1 << 16, device="cuda")
+    ddf.ddf_query(m, od, dd, 1 << 16, small_d, small_v)
+    assert torch.equal(small_d, dist[:1 << 16]) and torch.equal(small_v, vis[:1 << 16])
+    from ddf_inputs import make_weights
+    idx = np.arange(0, 1 << 16, 97)
+    z, t, xi = orc.forward(lay, make_weights(lay), o[idx], d[idx], mode=0)
+    g = dist[-(1 << 16):].cpu().numpy()[idx]
+    assert (np.abs(g - t) / (1 + np.abs(t))).max() <= 1e-2

@@ -1,0 +1,147 @@
+"""Wavefront secondary rays: CPU pins of the oracle twin,
+then the CUDA path (compaction + second query + lit flags) against it through the C ABI."""
+import math
+
+import numpy as np
+import pytest
+
+from ddf_inputs import MASTER_SEED, STREAMS, layout_c1, layout_hash_paper, make_weights, make_hash_table, make_hash_mlp, random_rays
+
+
+# ------------------------------------------------------------------ CPU: the twin against geometry
+
+def test_twin_on_an_analytic_sphere(orc):
+    """Feed the twin the EXACT field of a unit sphere (dist = ray-sphere distance, vis = hit): the
+    secondary origins lie eps inside the ray from the surface, directions are unit and aim at the
+    light, tmax is the light distance, the index list is the increasing list of hits."""
+    ocam = orc.make_camera((0.0, -2.5, 0.0))
+    o, d = orc.gen_camera(ocam, 64, 64)
+    t = np.array([orc.ray_sphere(o[i], d[i], (0, 0, 0), 1.0) for i in range(len(o))])
+    vis = (t > 0).astype(np.float32); dist = np.where(t > 0, t, 0.0).astype(np.float32)
+    L = np.array([3.0, 3.0, 3.0])
+    o2, d2, tmax, idx = orc.gen_shadow_from_hits(o, d, dist, vis, L, 1e-3)
+    assert np.array_equal(idx, np.nonzero(vis > 0.5)[0]) and 0 < len(idx) < len(o)
+    hit = o[idx].astype(np.float64) + dist[idx, None].astype(np.float64) * d[idx]
+    assert np.allclose(np.linalg.norm(hit, axis=1), 1.0, atol=1e-5)
+    assert np.allclose(np.linalg.norm(o2 - hit, axis=1), 1e-3, atol=2e-6)          # stepped back by eps ...
+    assert np.all(np.einsum("ij,ij->i", o2 - hit, d[idx]) < 0)                      # ... against the ray
+    assert np.allclose(np.linalg.norm(d2, axis=1), 1.0, atol=1e-6)
+    assert np.allclose(o2 + tmax[:, None] * d2, L[None, :], atol=1e-5)
+    # lit flags with the exact field again: a point of the sphere is lit iff its shadow ray leaves the sphere
+    t2 = np.array([orc.ray_sphere(o2[k], d2[k], (0, 0, 0), 1.0) for k in range(len(idx))])
+    vis2 = (t2 > 0).astype(np.float32); dist2 = np.where(t2 > 0, t2, 0).astype(np.float32)
+    lit = orc.shadow_lit(vis2, dist2, tmax, idx, len(o))
+    facing = np.einsum("ij,ij->i", hit, L[None, :] - hit) > 0                       # n . (L - p) > 0
+    inside_margin = np.abs(np.einsum("ij,ij->i", hit, L[None, :] - hit)) > 0.3      # away from the terminator (the eps offset lifts grazing rays over the horizon)
+    assert np.array_equal(lit[idx][inside_margin].astype(bool), facing[inside_margin])
+    assert lit[np.nonzero(vis < 0.5)[0]].sum() == 0                                 # primary misses are never lit
+
+
+def test_twin_threshold_and_order(orc):
+    o = np.zeros((6, 3), np.float32); d = np.tile(np.array([[0, 0, 1]], np.float32), (6, 1))
+    dist = np.arange(1, 7, dtype=np.float32)
+    vis = np.array([0.5, 0.50001, 0.2, 1.0, 0.4999, 0.9], np.float32)               # ties (0.5) are misses (A10)
+    o2, d2, tmax, idx = orc.gen_shadow_from_hits(o, d, dist, vis, (0, 0, 10), 0.25)
+    assert list(idx) == [1, 3, 5]
+    assert np.allclose(o2[:, 2], [1.75, 3.75, 5.75]) and np.allclose(tmax, [8.25, 6.25, 4.25])
+    lit = orc.shadow_lit(np.array([0.9, 0.9, 0.1], np.float32), np.array([1.0, 7.0, 1.0], np.float32), tmax, idx, 6)
+    assert list(lit) == [0, 0, 0, 1, 0, 1]                                          # occluded only if dist2 < tmax
+
+
+# ------------------------------------------------------------------ GPU
+
+def _models(ddf):
+    """both model kinds, with the visibility-head bias raised to 1 so that hits and occlusions are
+    common (the seeded random fields otherwise answer xi ~ 0.3 almost everywhere)"""
+    lay = layout_c1()
+    blob = make_weights(lay).copy()
+    blob[-1] = 0x3F80                                         # bf16 bits of 1.0: bias of the visibility logit
+    yield "dense", ddf.ddf_create(blob, lay), lambda orc, o, d: orc.forward(lay, blob, o, d)
+    hl = layout_hash_paper()
+    n = ddf.ddf_hashgrid_table_entries(hl)
+    tab, mlp = make_hash_table(hl, n), make_hash_mlp(hl).copy()
+    mlp[-1] = 1.0
+    yield "hash", ddf.ddf_create_hashgrid(tab, mlp, hl), lambda orc, o, d: orc.hash_forward(hl, tab, mlp, o, d)
+
+
+@pytest.mark.gpu
+def test_gpu_wavefront_against_twin(orc):
+    import torch
+    import paper_2606_00817_b200 as ddf
+    ddf.build()
+    cam = ddf.ddf_camera_from_seed(MASTER_SEED, STREAMS["camera_pos"], 2.5)
+    W = H = 384; n = W * H
+    light = (3.0, 3.0, 3.0)
+    for name, m, oracle_fwd in _models(ddf):
+        o = torch.empty((n, 3), device="cuda"); d = torch.empty((n, 3), device="cuda")
+        ddf.ddf_gen_camera(cam, W, H, o, d)
+        # spread the origins so that hits and misses mix (with one shared origin the seeded random
+        # fields answer nearly the same xi for every direction)
+        o += torch.from_numpy(random_rays(n)[0]).cuda() * 0.4
+        dist = torch.empty(n, device="cuda"); vis = torch.empty(n, device="cuda")
+        lit = torch.full((n,), 7, dtype=torch.uint8, device="cuda"); cnt = torch.zeros(1, dtype=torch.int64, device="cuda")
+        ddf.ddf_query_shadowed(m, o, d, n, light, 1e-3, dist, vis, lit, cnt)
+        torch.cuda.synchronize()
+        k = int(cnt.item())
+        # primary results are exactly ddf_query's
+        d1 = torch.empty(n, device="cuda"); v1 = torch.empty(n, device="cuda")
+        ddf.ddf_query(m, o, d, n, d1, v1)
+        assert torch.equal(d1, dist) and torch.equal(v1, vis)
+        assert k == int((vis > 0.5).sum().item()) and 0 < k < n, (name, k)
+        # compaction against the twin on the GPU's own primary results: indices bit-exact, rays to 1e-5
+        o2 = torch.empty((n, 3), device="cuda"); d2 = torch.empty((n, 3), device="cuda")
+        tmax = torch.empty(n, device="cuda"); idx = torch.empty(n, dtype=torch.int32, device="cuda"); c2 = torch.zeros(1, dtype=torch.int64, device="cuda")
+        ddf.ddf_gen_shadow_from_hits(m, o, d, dist, vis, n, light, 1e-3, o2, d2, tmax, idx, c2)
+        assert int(c2.item()) == k
+        ro2, rd2, rt, ridx = orc.gen_shadow_from_hits(o.cpu().numpy(), d.cpu().numpy(), dist.cpu().numpy(), vis.cpu().numpy(), light, 1e-3)
+        assert np.array_equal(idx[:k].cpu().numpy(), ridx)
+        assert np.allclose(o2[:k].cpu().numpy(), ro2, atol=2e-6) and np.allclose(d2[:k].cpu().numpy(), rd2, atol=1e-5)
+        assert np.allclose(tmax[:k].cpu().numpy(), rt, rtol=1e-6)
+        # lit flags = the decision rule applied to a plain second query of the compacted batch
+        dist2 = torch.empty(k, device="cuda"); vis2 = torch.empty(k, device="cuda")
+        ddf.ddf_query(m, o2[:k].contiguous(), d2[:k].contiguous(), k, dist2, vis2)
+        want = orc.shadow_lit(vis2.cpu().numpy(), dist2.cpu().numpy(), tmax[:k].cpu().numpy(), ridx, n)
+        assert np.array_equal(lit.cpu().numpy(), want), name
+        assert 0 < int(lit.sum().item()) < k                 # both outcomes occur
+        # ... and against the oracle end to end on a sample of hit rays, away from the two thresholds
+        sel = np.arange(0, k, max(1, k // 400))[:400]
+        z, t2, xi2 = oracle_fwd(orc, ro2[sel], rd2[sel])
+        safe = (np.abs(xi2 - 0.5) > 1e-2) & (np.abs(t2 - rt[sel]) > 1e-2 * (1 + np.abs(t2)))
+        ref = ~((xi2 > 0.5) & (t2 < rt[sel]))
+        got = lit.cpu().numpy()[ridx[sel]].astype(bool)
+        assert np.array_equal(got[safe], ref[safe]) and safe.mean() > 0.5, name
+        # n = 0 and determinism
+        ddf.ddf_query_shadowed(m, o, d, 0, light, 1e-3, dist, vis, lit, cnt)
+        assert int(cnt.item()) == 0
+        lit2 = torch.empty(n, dtype=torch.uint8, device="cuda")
+        ddf.ddf_query_shadowed(m, o, d, n, light, 1e-3, dist, vis, lit2, None)
+        assert torch.equal(lit2, torch.from_numpy(want).cuda())
+        ddf.ddf_destroy(m)
+
+
+@pytest.mark.gpu
+def test_gpu_compaction_edge_cases(orc):
+    """all hits, no hits, one hit at the end, sizes around the 256-ray scan block and a 2^22 batch"""
+    import torch
+    import paper_2606_00817_b200 as ddf
+    from ddf_inputs import layout_c0
+    ddf.build()
+    m = ddf.ddf_create(make_weights(layout_c0()), layout_c0())
+    g = torch.Generator(device="cuda").manual_seed(3)
+    for n, mode in [(1, "all"), (255, "none"), (256, "all"), (257, "last"), (1000, "rand"), (65537, "rand"), (1 << 22, "rand")]:
+        o = torch.rand((n, 3), device="cuda", generator=g); d = torch.nn.functional.normalize(torch.randn((n, 3), device="cuda", generator=g), dim=1)
+        dist = torch.rand(n, device="cuda", generator=g) + 0.5
+        vis = {"all": torch.ones(n, device="cuda"), "none": torch.zeros(n, device="cuda"),
+               "last": torch.zeros(n, device="cuda"), "rand": torch.rand(n, device="cuda", generator=g)}[mode]
+        if mode == "last": vis[-1] = 1.0
+        o2 = torch.empty((n, 3), device="cuda"); d2 = torch.empty((n, 3), device="cuda"); tmax = torch.empty(n, device="cuda")
+        idx = torch.full((n,), -1, dtype=torch.int32, device="cuda"); cnt = torch.full((1,), -5, dtype=torch.int64, device="cuda")
+        ddf.ddf_gen_shadow_from_hits(m, o, d, dist, vis, n, (1.0, 2.0, 3.0), 1e-2, o2, d2, tmax, idx, cnt)
+        want = torch.nonzero(vis > 0.5).flatten().to(torch.int32)
+        k = int(cnt.item())
+        assert k == len(want) and torch.equal(idx[:k], want), (n, mode)
+        assert bool((idx[k:] == -1).all())
+        if k:
+            p = o[want.long()] + (dist[want.long()] - 1e-2)[:, None] * d[want.long()]
+            assert torch.allclose(o2[:k], p, atol=1e-6)
+    ddf.ddf_destroy(m)
