@@ -19,7 +19,6 @@
 #include "ddf_tc_ptx.cuh"
 #include <cuda_fp16.h>
 #include <math.h>
-#include <stdio.h>
 #include <stdlib.h>
 #include <string.h>
 #include <new>
@@ -295,7 +294,6 @@ int hash_forward(Model* m, const float* o, const float* d, int64_t n, const int6
   if (tiles < grid) grid = tiles;
   if (p.table_f16) ddf_hash_kernel<true><<<(unsigned)grid, kHgThreads, h->smem_bytes, st>>>(p);
   else             ddf_hash_kernel<false><<<(unsigned)grid, kHgThreads, h->smem_bytes, st>>>(p);
-  if (getenv("DDF_DEBUG")) fprintf(stderr, "[ddf_hash] grid %lld ctas %d\n", (long long)grid, h->ctas_per_sm);
   DDF_CUDA_TRY(cudaGetLastError());
   m->last_launches = 1;
   return DDF_OK;
@@ -421,19 +419,15 @@ extern "C" int ddf_create_hashgrid(const void* table, const void* mlp, const ddf
   // measured on B200: 4 resident CTAs is the best trade between latency hiding
   // and the L1 left for the coarse levels (8 x 64 TMEM columns would be the hard limit)
   h->ctas_per_sm = occ > 4 ? 4 : occ;
-  if (const char* ev = getenv("DDF_HASH_CTAS")) { int v = atoi(ev); if (v >= 1 && v <= h->ctas_per_sm) h->ctas_per_sm = v; }
   // shared-memory carve-out: just what the resident CTAs need; the rest of the 256 KB stays L1,
   // which is what serves the coarse (small) levels of the grid
   {
     int pct = (int)((h->ctas_per_sm * (h->smem_bytes + prop.reservedSharedMemPerBlock) * 100 + prop.sharedMemPerMultiprocessor - 1) / prop.sharedMemPerMultiprocessor);
-    if (const char* ev = getenv("DDF_HASH_CARVEOUT")) pct = atoi(ev);
     if (pct > 100) pct = 100;
     if ((e = cudaFuncSetAttribute(ddf_hash_kernel<false>, cudaFuncAttributePreferredSharedMemoryCarveout, pct)) != cudaSuccess ||
         (e = cudaFuncSetAttribute(ddf_hash_kernel<true>, cudaFuncAttributePreferredSharedMemoryCarveout, pct)) != cudaSuccess)
       return fail(DDF_E_CUDA, e);
-    if (getenv("DDF_DEBUG")) fprintf(stderr, "[ddf_hash] carveout %d %%\n", pct);
   }
-  if (getenv("DDF_DEBUG")) fprintf(stderr, "[ddf_hash] regs %d ctas/SM %d smem %zu\n", fa.numRegs, h->ctas_per_sm, h->smem_bytes);
   if ((e = cudaDeviceSynchronize()) != cudaSuccess) return fail(DDF_E_CUDA, e);
   *out = reinterpret_cast<ddf_model*>(m);
   return DDF_OK;

@@ -35,14 +35,6 @@ constexpr int kMaxTcLayers = 16;
 constexpr int kMaxChunks = 8;
 constexpr int kABytes = kTileM * kKBlock * 2;           // 16 KB
 constexpr int kThreads = 384;
-// -DDDF_TC_INTERLEAVE_L0: issue layer 0 of tile i+1 between the last-layer chunks of tile i (see the
-// schedule comment in the kernel).  Parity-tested and bit-identical, but measured no faster under
-// the 1 kW power cap, so it is off by default.
-#ifdef DDF_TC_INTERLEAVE_L0
-constexpr bool kInterleaveL0 = true;
-#else
-constexpr bool kInterleaveL0 = false;
-#endif
 
 template <int CG> struct TcCfg {
   static constexpr int kBBytes = (CG == 2 ? 128 : 256) * kKBlock * 2;
@@ -153,65 +145,52 @@ __global__ void __launch_bounds__(kThreads, 1) ddf_tc_kernel(const __grid_consta
   uint32_t tmem_base;
   asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
 
-  // Schedule (identical in the producer, the MMA issuer and the epilogue): a list of work items
-  // (tile, layer, 256-column chunk).  Layer 0 has 6 MMAs per chunk but a full epilogue, so back to
-  // back its five chunks leave the tensor pipe waiting for accumulators; with kInterleaveL0, from
-  // the second tile on, layer 0 of tile i+1 is issued BETWEEN the chunks of the last layer of
-  // tile i.  Its output goes to the activation buffer the last layer does not read, so the
-  // ping-pong parity of a tile's layers alternates with the tile.
-  const bool inter = kInterleaveL0 && p.n_hidden >= 2;
-  auto tile_parity = [&](int tl) { return inter ? ((tl * (p.n_hidden - 1)) & 1) : 0; };
-
   if (warp == 0) {
     // ================================================================ TMA producer
     {
       uint32_t it = 0, act_phase = 0;                    // bit j of act_phase: parity for act_bar(j)
-      // one work item = one 256-column chunk of one layer of the tile with local index tl
-      auto item = [&](int tl, int l, int c) {
-        const int gb = tl & 1, par = tile_parity(tl);
+      int tile_local = 0;
+      for (int64_t tile = pid; tile < num_tiles; tile += num_pairs, ++tile_local) {
+        const int gb = tile_local & 1;
         const int g_row = (cta_global * 2 + gb) * kTileM;
-        const int nk0 = p.nkb0[l], nk1 = p.nkb1[l];
-        const CUtensorMap* amap = (l == 0) ? &p.g : (((l - 1 + par) & 1) ? &p.x1 : &p.x0);
-        const int a_row = (l == 0) ? g_row : cta_global * kTileM;
-        for (int kb = 0; kb < nk0 + nk1; ++kb) {
-          if (c == 0 && kb < nk0) {
-            if (l == 0) {
-              if (kb == 0) wait_bar<false>(gready_bar(gb), (tl >> 1) & 1, p.dbg, 0x100 + gb);
-            } else if ((kb & 3) == 0) {
-              const int j = kb >> 2;
-              wait_bar<false>(act_bar(j), (act_phase >> j) & 1u, p.dbg, 0x200 + j);
-              act_phase ^= (1u << j);
+        for (int l = 0; l < p.n_hidden; ++l) {
+          const int nk0 = p.nkb0[l], nk1 = p.nkb1[l];
+          const CUtensorMap* amap = (l == 0) ? &p.g : (((l - 1) & 1) ? &p.x1 : &p.x0);
+          const int a_row = (l == 0) ? g_row : cta_global * kTileM;
+          for (int c = 0; c < p.n_chunks; ++c) {
+            for (int kb = 0; kb < nk0 + nk1; ++kb) {
+              if (c == 0 && kb < nk0) {
+                if (l == 0) {
+                  if (kb == 0) wait_bar<false>(gready_bar(gb), (tile_local >> 1) & 1, p.dbg, 0x100 + gb);
+                } else if ((kb & 3) == 0) {
+                  const int j = kb >> 2;
+                  wait_bar<false>(act_bar(j), (act_phase >> j) & 1u, p.dbg, 0x200 + j);
+                  act_phase ^= (1u << j);
+                }
+              }
+              const int s = it % S; const uint32_t ph = (it / S) & 1u;
+              wait_bar<CG == 2>(empty_bar(s), ph ^ 1u, p.dbg, 0x300 + s);
+              const int brow = c * kChunkN + (CG == 2 ? (int)rank * 128 : 0);
+              if (ptx::elect_one()) {
+                if (CG == 2) {
+                  if (leader) ptx::mbar_arrive_expect_tx(full_bar(s), 2u * Cfg::kStageBytes);
+                  const uint32_t fb = ptx::mapa(full_bar(s), 0);
+                  if (kb < nk0) ptx::tma_load_2d_cg2(a_smem(s), amap, fb, kb * kKBlock, a_row);
+                  else          ptx::tma_load_2d_cg2(a_smem(s), &p.g, fb, (kb - nk0) * kKBlock, g_row);
+                  ptx::tma_load_2d_cg2(b_smem(s), &p.w[l], fb, kb * kKBlock, brow);
+                } else {
+                  ptx::mbar_arrive_expect_tx(full_bar(s), (uint32_t)Cfg::kStageBytes);
+                  if (kb < nk0) ptx::tma_load_2d(a_smem(s), amap, full_bar(s), kb * kKBlock, a_row);
+                  else          ptx::tma_load_2d(a_smem(s), &p.g, full_bar(s), (kb - nk0) * kKBlock, g_row);
+                  ptx::tma_load_2d(b_smem(s), &p.w[l], full_bar(s), kb * kKBlock, brow);
+                  ptx::tma_load_2d(b_smem(s) + 128 * kKBlock * 2, &p.w[l], full_bar(s), kb * kKBlock, brow + 128);
+                }
+              }
+              __syncwarp();
+              ++it;
             }
           }
-          const int s = it % S; const uint32_t ph = (it / S) & 1u;
-          wait_bar<CG == 2>(empty_bar(s), ph ^ 1u, p.dbg, 0x300 + s);
-          const int brow = c * kChunkN + (CG == 2 ? (int)rank * 128 : 0);
-          if (ptx::elect_one()) {
-            if (CG == 2) {
-              if (leader) ptx::mbar_arrive_expect_tx(full_bar(s), 2u * Cfg::kStageBytes);
-              const uint32_t fb = ptx::mapa(full_bar(s), 0);
-              if (kb < nk0) ptx::tma_load_2d_cg2(a_smem(s), amap, fb, kb * kKBlock, a_row);
-              else          ptx::tma_load_2d_cg2(a_smem(s), &p.g, fb, (kb - nk0) * kKBlock, g_row);
-              ptx::tma_load_2d_cg2(b_smem(s), &p.w[l], fb, kb * kKBlock, brow);
-            } else {
-              ptx::mbar_arrive_expect_tx(full_bar(s), (uint32_t)Cfg::kStageBytes);
-              if (kb < nk0) ptx::tma_load_2d(a_smem(s), amap, full_bar(s), kb * kKBlock, a_row);
-              else          ptx::tma_load_2d(a_smem(s), &p.g, full_bar(s), (kb - nk0) * kKBlock, g_row);
-              ptx::tma_load_2d(b_smem(s), &p.w[l], full_bar(s), kb * kKBlock, brow);
-              ptx::tma_load_2d(b_smem(s) + 128 * kKBlock * 2, &p.w[l], full_bar(s), kb * kKBlock, brow + 128);
-            }
-          }
-          __syncwarp();
-          ++it;
         }
-      };
-      int tl = 0;
-      for (int64_t tile = pid; tile < num_tiles; tile += num_pairs, ++tl) {
-        const bool has_next = tile + num_pairs < num_tiles;
-        if (tl == 0 || !inter) for (int c = 0; c < p.n_chunks; ++c) item(tl, 0, c);
-        for (int l = 1; l < last_layer; ++l) for (int c = 0; c < p.n_chunks; ++c) item(tl, l, c);
-        if (last_layer >= 1)
-          for (int c = 0; c < p.n_chunks; ++c) { item(tl, last_layer, c); if (inter && has_next) item(tl + 1, 0, c); }
       }
     }
   } else if (warp == 1) {
@@ -221,47 +200,43 @@ __global__ void __launch_bounds__(kThreads, 1) ddf_tc_kernel(const __grid_consta
     if (leader) {
       constexpr uint32_t idesc = ptx::idesc_bf16_f32(128 * CG, kChunkN);
       uint32_t it = 0, cc = 0;
-      auto item = [&](int tl, int l, int c) {
-        const int gb = tl & 1;
-        const int nk0 = p.nkb0[l], nk1 = p.nkb1[l], nk = nk0 + nk1;
-        const uint32_t buf = cc & 1u, use = cc >> 1;
-        wait_bar<CG == 2>(tempty_bar(buf), (use & 1u) ^ 1u, p.dbg, 0x400 + buf);
-        ptx::tc_fence_after();
-        const uint32_t d_tmem = tmem_base + buf * kChunkN;
-        for (int kb = 0; kb < nk; ++kb, ++it) {
-          const int s = it % S; const uint32_t ph = (it / S) & 1u;
-          wait_bar<CG == 2>(full_bar(s), ph, p.dbg, 0x500 + s);
-          ptx::tc_fence_after();
-          const bool g_last = (l == 0) ? (kb == nk0 - 1) : (kb == nk - 1 && nk1 > 0);
-          const int nk16 = g_last ? p.g_last_nk16 : 4;
-          const uint64_t adesc = ptx::smem_desc_k_sw128(a_smem(s));
-          const uint64_t bdesc = ptx::smem_desc_k_sw128(b_smem(s));
-          const bool free_gamma = (l == gamma_layer && c == p.n_chunks - 1 && kb == nk - 1);
-          if (ptx::elect_one()) {
-            if (nk16 == 4) {
-              ptx::umma_bf16<CG>(d_tmem, adesc, bdesc, idesc, (uint32_t)(kb != 0));
-              ptx::umma_bf16<CG>(d_tmem, adesc + 2u, bdesc + 2u, idesc, 1u);
-              ptx::umma_bf16<CG>(d_tmem, adesc + 4u, bdesc + 4u, idesc, 1u);
-              ptx::umma_bf16<CG>(d_tmem, adesc + 6u, bdesc + 6u, idesc, 1u);
-            } else {
-              for (int k = 0; k < nk16; ++k)
-                ptx::umma_bf16<CG>(d_tmem, adesc + 2u * k, bdesc + 2u * k, idesc, (uint32_t)((kb | k) != 0));
+      int tile_local = 0;
+      for (int64_t tile = pid; tile < num_tiles; tile += num_pairs, ++tile_local) {
+        const int gb = tile_local & 1;
+        for (int l = 0; l < p.n_hidden; ++l) {
+          const int nk0 = p.nkb0[l], nk1 = p.nkb1[l], nk = nk0 + nk1;
+          for (int c = 0; c < p.n_chunks; ++c, ++cc) {
+            const uint32_t buf = cc & 1u, use = cc >> 1;
+            wait_bar<CG == 2>(tempty_bar(buf), (use & 1u) ^ 1u, p.dbg, 0x400 + buf);
+            ptx::tc_fence_after();
+            const uint32_t d_tmem = tmem_base + buf * kChunkN;
+            for (int kb = 0; kb < nk; ++kb, ++it) {
+              const int s = it % S; const uint32_t ph = (it / S) & 1u;
+              wait_bar<CG == 2>(full_bar(s), ph, p.dbg, 0x500 + s);
+              ptx::tc_fence_after();
+              const bool g_last = (l == 0) ? (kb == nk0 - 1) : (kb == nk - 1 && nk1 > 0);
+              const int nk16 = g_last ? p.g_last_nk16 : 4;
+              const uint64_t adesc = ptx::smem_desc_k_sw128(a_smem(s));
+              const uint64_t bdesc = ptx::smem_desc_k_sw128(b_smem(s));
+              const bool free_gamma = (l == gamma_layer && c == p.n_chunks - 1 && kb == nk - 1);
+              if (ptx::elect_one()) {
+                if (nk16 == 4) {
+                  ptx::umma_bf16<CG>(d_tmem, adesc, bdesc, idesc, (uint32_t)(kb != 0));
+                  ptx::umma_bf16<CG>(d_tmem, adesc + 2u, bdesc + 2u, idesc, 1u);
+                  ptx::umma_bf16<CG>(d_tmem, adesc + 4u, bdesc + 4u, idesc, 1u);
+                  ptx::umma_bf16<CG>(d_tmem, adesc + 6u, bdesc + 6u, idesc, 1u);
+                } else {
+                  for (int k = 0; k < nk16; ++k)
+                    ptx::umma_bf16<CG>(d_tmem, adesc + 2u * k, bdesc + 2u * k, idesc, (uint32_t)((kb | k) != 0));
+                }
+                ptx::umma_commit<CG>(empty_bar(s));
+                if (free_gamma) ptx::umma_commit<CG>(gfree_bar(gb));
+                if (kb == nk - 1) ptx::umma_commit<CG>(tfull_bar(buf));
+              }
+              __syncwarp();
             }
-            ptx::umma_commit<CG>(empty_bar(s));
-            if (free_gamma) ptx::umma_commit<CG>(gfree_bar(gb));
-            if (kb == nk - 1) ptx::umma_commit<CG>(tfull_bar(buf));
           }
-          __syncwarp();
         }
-        ++cc;
-      };
-      int tl = 0;
-      for (int64_t tile = pid; tile < num_tiles; tile += num_pairs, ++tl) {
-        const bool has_next = tile + num_pairs < num_tiles;
-        if (tl == 0 || !inter) for (int c = 0; c < p.n_chunks; ++c) item(tl, 0, c);
-        for (int l = 1; l < last_layer; ++l) for (int c = 0; c < p.n_chunks; ++c) item(tl, l, c);
-        if (last_layer >= 1)
-          for (int c = 0; c < p.n_chunks; ++c) { item(tl, last_layer, c); if (inter && has_next) item(tl + 1, 0, c); }
       }
     }
   } else if (warp >= 4) {
@@ -274,94 +249,87 @@ __global__ void __launch_bounds__(kThreads, 1) ddf_tc_kernel(const __grid_consta
     const uint32_t stage = stg_base + (uint32_t)(warp - 4) * 4096u;
     const uint32_t tempty_remote = (CG == 2) ? ptx::mapa(tempty_bar(0), 0) : 0u;
     uint32_t cc = 0;
-    float z0 = 0.0f, z1 = 0.0f;
-    auto item = [&](int tl, int l, int c) {
-      const int par = tile_parity(tl);
-      const CUtensorMap* smap = ((l + par) & 1) ? &p.xs1 : &p.xs0;
-      const float* bias = p.bias + p.b_off[l];
-      const uint32_t buf = cc & 1u, use = cc >> 1;
-      ++cc;
-      wait_bar<CG == 2>(tfull_bar(buf), use & 1u, p.dbg, 0x600 + buf);
-      ptx::tc_fence_after();
-      const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + buf * kChunkN + h * 128;
-      #pragma unroll 1
-      for (int box = 0; box < 2; ++box) {
-        uint32_t r[64];
-        ptx::tmem_ld32(taddr + box * 64, *reinterpret_cast<uint32_t(*)[32]>(&r[0]));
-        ptx::tmem_ld32(taddr + box * 64 + 32, *reinterpret_cast<uint32_t(*)[32]>(&r[32]));
-        ptx::tmem_ld_wait();
-        if (box == 1) {                       // accumulator fully read: hand it back to the MMA warp
-          ptx::tc_fence_before();
-          __syncwarp();
-          if (lane == 0) {
-            if (CG == 2) ptx::mbar_arrive_cluster(tempty_remote + 8u * buf);
-            else ptx::mbar_arrive(tempty_bar(buf));
-          }
-        }
-        const int col = c * kChunkN + h * 128 + box * 64;
-        const float4* b4 = reinterpret_cast<const float4*>(bias + col);
-        #pragma unroll
-        for (int i = 0; i < 16; ++i) {
-          float4 bb = __ldg(b4 + i);
-          r[4 * i + 0] = __float_as_uint(fmaxf(__uint_as_float(r[4 * i + 0]) + bb.x, 0.0f));
-          r[4 * i + 1] = __float_as_uint(fmaxf(__uint_as_float(r[4 * i + 1]) + bb.y, 0.0f));
-          r[4 * i + 2] = __float_as_uint(fmaxf(__uint_as_float(r[4 * i + 2]) + bb.z, 0.0f));
-          r[4 * i + 3] = __float_as_uint(fmaxf(__uint_as_float(r[4 * i + 3]) + bb.w, 0.0f));
-        }
-        if (l < last_layer) {
-          if (lane == 0) ptx::bulk_wait_read<0>();          // staging box free again
-          __syncwarp();
-          #pragma unroll
-          for (int j = 0; j < 8; ++j) {
-            uint4 pk;
-            __nv_bfloat162 t0 = __floats2bfloat162_rn(__uint_as_float(r[8 * j + 0]), __uint_as_float(r[8 * j + 1]));
-            __nv_bfloat162 t1 = __floats2bfloat162_rn(__uint_as_float(r[8 * j + 2]), __uint_as_float(r[8 * j + 3]));
-            __nv_bfloat162 t2 = __floats2bfloat162_rn(__uint_as_float(r[8 * j + 4]), __uint_as_float(r[8 * j + 5]));
-            __nv_bfloat162 t3 = __floats2bfloat162_rn(__uint_as_float(r[8 * j + 6]), __uint_as_float(r[8 * j + 7]));
-            pk.x = *reinterpret_cast<uint32_t*>(&t0); pk.y = *reinterpret_cast<uint32_t*>(&t1);
-            pk.z = *reinterpret_cast<uint32_t*>(&t2); pk.w = *reinterpret_cast<uint32_t*>(&t3);
-            ptx::st_shared_v4(stage + (uint32_t)lane * 128u + (uint32_t)((j ^ (lane & 7)) << 4), pk);
-          }
-          ptx::fence_proxy_async_smem();
-          __syncwarp();
-          if (lane == 0) {
-            ptx::tma_store_2d(smap, stage, col, cta_global * kTileM + q * 32);
-            ptx::bulk_commit();
-          }
-        } else {
-          const float4* w0 = reinterpret_cast<const float4*>(p.head_w + col);
-          #pragma unroll
-          for (int i = 0; i < 16; ++i) {
-            float4 ww = __ldg(w0 + i);
-            z0 = fmaf(__uint_as_float(r[4 * i + 0]), ww.x, z0); z0 = fmaf(__uint_as_float(r[4 * i + 1]), ww.y, z0);
-            z0 = fmaf(__uint_as_float(r[4 * i + 2]), ww.z, z0); z0 = fmaf(__uint_as_float(r[4 * i + 3]), ww.w, z0);
-          }
-          if (p.n_out == 2) {
-            const float4* w1 = reinterpret_cast<const float4*>(p.head_w + p.width + col);
-            #pragma unroll
-            for (int i = 0; i < 16; ++i) {
-              float4 ww = __ldg(w1 + i);
-              z1 = fmaf(__uint_as_float(r[4 * i + 0]), ww.x, z1); z1 = fmaf(__uint_as_float(r[4 * i + 1]), ww.y, z1);
-              z1 = fmaf(__uint_as_float(r[4 * i + 2]), ww.z, z1); z1 = fmaf(__uint_as_float(r[4 * i + 3]), ww.w, z1);
-            }
-          }
-        }
-      }
-      if (l < last_layer && lane == 0) {
-        ptx::bulk_wait<0>();                  // this warp's part of chunk c is in global memory
-        ptx::mbar_arrive(act_bar(c));
-      }
-    };
-    int tl = 0;
-    for (int64_t tile = pid; tile < num_tiles; tile += num_pairs, ++tl) {
+    for (int64_t tile = pid; tile < num_tiles; tile += num_pairs) {
       const int64_t grow = tile * tile_rays + (int64_t)rank * kTileM + row;
       const bool valid = grow < n;
-      const bool has_next = tile + num_pairs < num_tiles;
-      z0 = 0.0f; z1 = 0.0f;
-      if (tl == 0 || !inter) for (int c = 0; c < p.n_chunks; ++c) item(tl, 0, c);
-      for (int l = 1; l < last_layer; ++l) for (int c = 0; c < p.n_chunks; ++c) item(tl, l, c);
-      if (last_layer >= 1)
-        for (int c = 0; c < p.n_chunks; ++c) { item(tl, last_layer, c); if (inter && has_next) item(tl + 1, 0, c); }
+      float z0 = 0.0f, z1 = 0.0f;
+      for (int l = 0; l < p.n_hidden; ++l) {
+        const CUtensorMap* smap = (l & 1) ? &p.xs1 : &p.xs0;
+        const float* bias = p.bias + p.b_off[l];
+        for (int c = 0; c < p.n_chunks; ++c, ++cc) {
+          const uint32_t buf = cc & 1u, use = cc >> 1;
+          wait_bar<CG == 2>(tfull_bar(buf), use & 1u, p.dbg, 0x600 + buf);
+          ptx::tc_fence_after();
+          const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + buf * kChunkN + h * 128;
+          #pragma unroll 1
+          for (int box = 0; box < 2; ++box) {
+            uint32_t r[64];
+            ptx::tmem_ld32(taddr + box * 64, *reinterpret_cast<uint32_t(*)[32]>(&r[0]));
+            ptx::tmem_ld32(taddr + box * 64 + 32, *reinterpret_cast<uint32_t(*)[32]>(&r[32]));
+            ptx::tmem_ld_wait();
+            if (box == 1) {                       // accumulator fully read: hand it back to the MMA warp
+              ptx::tc_fence_before();
+              __syncwarp();
+              if (lane == 0) {
+                if (CG == 2) ptx::mbar_arrive_cluster(tempty_remote + 8u * buf);
+                else ptx::mbar_arrive(tempty_bar(buf));
+              }
+            }
+            const int col = c * kChunkN + h * 128 + box * 64;
+            const float4* b4 = reinterpret_cast<const float4*>(bias + col);
+            #pragma unroll
+            for (int i = 0; i < 16; ++i) {
+              float4 bb = __ldg(b4 + i);
+              r[4 * i + 0] = __float_as_uint(fmaxf(__uint_as_float(r[4 * i + 0]) + bb.x, 0.0f));
+              r[4 * i + 1] = __float_as_uint(fmaxf(__uint_as_float(r[4 * i + 1]) + bb.y, 0.0f));
+              r[4 * i + 2] = __float_as_uint(fmaxf(__uint_as_float(r[4 * i + 2]) + bb.z, 0.0f));
+              r[4 * i + 3] = __float_as_uint(fmaxf(__uint_as_float(r[4 * i + 3]) + bb.w, 0.0f));
+            }
+            if (l < last_layer) {
+              if (lane == 0) ptx::bulk_wait_read<0>();          // staging box free again
+              __syncwarp();
+              #pragma unroll
+              for (int j = 0; j < 8; ++j) {
+                uint4 pk;
+                __nv_bfloat162 t0 = __floats2bfloat162_rn(__uint_as_float(r[8 * j + 0]), __uint_as_float(r[8 * j + 1]));
+                __nv_bfloat162 t1 = __floats2bfloat162_rn(__uint_as_float(r[8 * j + 2]), __uint_as_float(r[8 * j + 3]));
+                __nv_bfloat162 t2 = __floats2bfloat162_rn(__uint_as_float(r[8 * j + 4]), __uint_as_float(r[8 * j + 5]));
+                __nv_bfloat162 t3 = __floats2bfloat162_rn(__uint_as_float(r[8 * j + 6]), __uint_as_float(r[8 * j + 7]));
+                pk.x = *reinterpret_cast<uint32_t*>(&t0); pk.y = *reinterpret_cast<uint32_t*>(&t1);
+                pk.z = *reinterpret_cast<uint32_t*>(&t2); pk.w = *reinterpret_cast<uint32_t*>(&t3);
+                ptx::st_shared_v4(stage + (uint32_t)lane * 128u + (uint32_t)((j ^ (lane & 7)) << 4), pk);
+              }
+              ptx::fence_proxy_async_smem();
+              __syncwarp();
+              if (lane == 0) {
+                ptx::tma_store_2d(smap, stage, col, cta_global * kTileM + q * 32);
+                ptx::bulk_commit();
+              }
+            } else {
+              const float4* w0 = reinterpret_cast<const float4*>(p.head_w + col);
+              #pragma unroll
+              for (int i = 0; i < 16; ++i) {
+                float4 ww = __ldg(w0 + i);
+                z0 = fmaf(__uint_as_float(r[4 * i + 0]), ww.x, z0); z0 = fmaf(__uint_as_float(r[4 * i + 1]), ww.y, z0);
+                z0 = fmaf(__uint_as_float(r[4 * i + 2]), ww.z, z0); z0 = fmaf(__uint_as_float(r[4 * i + 3]), ww.w, z0);
+              }
+              if (p.n_out == 2) {
+                const float4* w1 = reinterpret_cast<const float4*>(p.head_w + p.width + col);
+                #pragma unroll
+                for (int i = 0; i < 16; ++i) {
+                  float4 ww = __ldg(w1 + i);
+                  z1 = fmaf(__uint_as_float(r[4 * i + 0]), ww.x, z1); z1 = fmaf(__uint_as_float(r[4 * i + 1]), ww.y, z1);
+                  z1 = fmaf(__uint_as_float(r[4 * i + 2]), ww.z, z1); z1 = fmaf(__uint_as_float(r[4 * i + 3]), ww.w, z1);
+                }
+              }
+            }
+          }
+          if (l < last_layer && lane == 0) {
+            ptx::bulk_wait<0>();                  // this warp's part of chunk c is in global memory
+            ptx::mbar_arrive(act_bar(c));
+          }
+        }
+      }
       // ---- fused heads (t = distance, xi = visibility); the two column halves
       // of a row meet through shared memory, always added in the same order
       if (h == 1) { asm volatile("st.shared.v2.f32 [%0], {%1, %2};" :: "r"(zbuf + (uint32_t)row * 8u), "f"(z0), "f"(z1) : "memory"); }
