@@ -40,6 +40,12 @@ class OrcHashLayout(C.Structure):
                 ("mlp_dtype", C.c_int32)]
 
 
+class OrcTrainParams(C.Structure):
+    _fields_ = [("lr0", C.c_double), ("lr_final_frac", C.c_double), ("total_steps", C.c_int32),
+                ("beta1", C.c_double), ("beta2", C.c_double), ("adam_eps", C.c_double),
+                ("dist_clamp", C.c_double), ("ce_weight", C.c_double)]
+
+
 class OrcCamera(C.Structure):
     _fields_ = [("pos", C.c_double * 3), ("look_at", C.c_double * 3), ("fov_deg", C.c_double)]
 
@@ -72,6 +78,9 @@ def lib():
         _lib.orc_hash_mlp_params.restype = C.c_int64
         _lib.orc_hash_index.restype = C.c_int64
         _lib.orc_gen_shadow_from_hits.restype = C.c_int64
+        _lib.orc_hash_loss_grads.restype = C.c_double
+        _lib.orc_lr_at.restype = C.c_double
+        _lib.orc_solid_scene_raycast.restype = C.c_double
         _lib.orc_ray_sphere.restype = C.c_double
         _lib.orc_ray_box_exit.restype = C.c_double
     return _lib
@@ -368,3 +377,39 @@ def shadow_lit(vis2, dist2, tmax, index, n):
     lit = np.empty(n, np.uint8)
     lib().orc_shadow_lit(_p(vis2), _p(dist2), _p(tmax), _p(index), C.c_int64(len(index)), C.c_int64(n), _p(lit))
     return lit
+
+
+# ------------------------------------------------------------------ training (ddf_hash_oracle.h, T1-T5)
+
+def train_params(lr0=3e-3, lr_final_frac=0.05, total_steps=30000, beta1=0.9, beta2=0.999, adam_eps=1e-8,
+                 dist_clamp=6.0, ce_weight=0.3):
+    return OrcTrainParams(lr0, lr_final_frac, total_steps, beta1, beta2, adam_eps, dist_clamp, ce_weight)
+
+
+def hash_loss_grads(lay, table, mlp, o, d, t, hit, P, want_grads=True):
+    """(loss, grad_table[entries*F], grad_mlp) in float64; table and mlp are float32 master copies."""
+    o, d, t = _f32(o), _f32(d), _f32(t)
+    hit = np.ascontiguousarray(hit, dtype=np.uint8)
+    table, mlp = _f32(table), _f32(mlp)
+    n = o.shape[0]
+    L = _hlayout(lay)
+    gt = np.zeros(table.shape[0], np.float64) if want_grads else None
+    gm = np.zeros(mlp.shape[0], np.float64) if want_grads else None
+    loss = lib().orc_hash_loss_grads(C.byref(L), _p(table), _p(mlp), _p(o), _p(d), _p(t), _p(hit), C.c_int64(n),
+                                     C.byref(P), _p(gt) if want_grads else None, _p(gm) if want_grads else None)
+    return loss, gt, gm
+
+
+def lr_at(P, step):
+    return lib().orc_lr_at(C.byref(P), C.c_int64(step))
+
+
+def adam_step(p, g, m, v, step, lr, P):
+    """in place on p (float32), m, v (float64)"""
+    assert p.dtype == np.float32 and m.dtype == np.float64 and v.dtype == np.float64
+    g = np.ascontiguousarray(g, dtype=np.float64)
+    lib().orc_adam_step(_p(p), _p(g), _p(m), _p(v), C.c_int64(p.shape[0]), C.c_int64(step), C.c_double(lr), C.byref(P))
+
+
+def solid_scene_raycast(o, d, sphere_c=(0.0, 0.0, 0.0), sphere_r=0.5, bmin=(-0.9, -0.9, -0.9), bmax=(0.9, 0.9, -0.6)):
+    return lib().orc_solid_scene_raycast(_v3(o), _v3(d), _v3(sphere_c), C.c_double(sphere_r), _v3(bmin), _v3(bmax))

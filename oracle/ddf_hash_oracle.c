@@ -183,3 +183,161 @@ int orc_hash_forward(const orc_hash_layout* L, const void* table, const void* ml
   }
   return 0;
 }
+
+/* ------------------------------------------------------------------ training (readings T1-T5) */
+
+/* corners of one level for a point: indices (into the whole table) and trilinear weights */
+static void level_corners(const orc_hash_layout* L, int l, const float x01[3], int64_t idx[8], double wt[8]) {
+  int64_t N = 0, off = 0;
+  orc_hash_level(L, l, &N, NULL, &off, NULL);
+  uint32_t c0[3]; double w[3];
+  for (int a = 0; a < 3; ++a) {
+    const float pos = x01[a] * (float)N;
+    float fl = floorf(pos);
+    if (fl > (float)(N - 1)) fl = (float)(N - 1);
+    c0[a] = (uint32_t)fl; w[a] = (double)(pos - fl);
+  }
+  for (int c = 0; c < 8; ++c) {
+    const int bx = c & 1, by = (c >> 1) & 1, bz = (c >> 2) & 1;
+    wt[c] = (bx ? w[0] : 1.0 - w[0]) * (by ? w[1] : 1.0 - w[1]) * (bz ? w[2] : 1.0 - w[2]);
+    idx[c] = off + orc_hash_index(L, l, c0[0] + bx, c0[1] + by, c0[2] + bz);
+  }
+}
+
+double orc_hash_loss_grads(const orc_hash_layout* L, const float* table, const float* mlp,
+                           const float* o, const float* d, const float* t, const uint8_t* hit,
+                           int64_t n, const orc_train_params* P, double* grad_table, double* grad_mlp) {
+  if (!hl_ok(L) || L->n_out != 2) return NAN;
+  const int F = L->n_features, NF = L->n_levels * F, E = orc_hash_mlp_in(L), W = L->width, H = L->n_hidden;
+  const int64_t n_mlp = orc_hash_mlp_params(L);
+  if (grad_table) memset(grad_table, 0, sizeof(double) * (size_t)orc_hash_table_entries(L) * F);
+  if (grad_mlp) memset(grad_mlp, 0, sizeof(double) * (size_t)n_mlp);
+  /* activations of every layer for one ray: act[0] = input (E), act[l+1] = output of layer l (W) */
+  const int S = E > W ? E : W;
+  double* act = (double*)malloc(sizeof(double) * (size_t)(H + 1) * S);
+  double* del = (double*)malloc(sizeof(double) * S);
+  double* dprev = (double*)malloc(sizeof(double) * S);
+  double loss = 0.0;
+  for (int64_t i = 0; i < n; ++i) {
+    float x01[3];
+    for (int a = 0; a < 3; ++a) {
+      const float num = o[3 * i + a] - L->box_min[a], den = L->box_max[a] - L->box_min[a];
+      float v = num / den; v = v < 0.0f ? 0.0f : (v > 1.0f ? 1.0f : v); x01[a] = v;
+    }
+    double* in = act;
+    for (int l = 0; l < L->n_levels; ++l) {
+      int64_t idx[8]; double wt[8];
+      level_corners(L, l, x01, idx, wt);
+      for (int f = 0; f < F; ++f) {
+        double s = 0.0;
+        for (int c = 0; c < 8; ++c) s += wt[c] * (double)table[(size_t)idx[c] * F + f];
+        in[l * F + f] = s;
+      }
+    }
+    int m = NF;
+    for (int c = 0; c < 3; ++c) in[m++] = (double)d[3 * i + c];
+    for (int k = 0; k < L->n_freq_dir; ++k) {
+      for (int c = 0; c < 3; ++c) in[m++] = sin(HPI * ldexp((double)d[3 * i + c], k));
+      for (int c = 0; c < 3; ++c) in[m++] = cos(HPI * ldexp((double)d[3 * i + c], k));
+    }
+    /* forward */
+    size_t off = 0; int nin = E;
+    for (int l = 0; l < H; ++l) {
+      const double* a_in = act + (size_t)l * S; double* a_out = act + (size_t)(l + 1) * S;
+      const size_t boff = off + (size_t)W * nin;
+      for (int j = 0; j < W; ++j) {
+        double acc = (double)mlp[boff + j];
+        for (int k = 0; k < nin; ++k) acc += (double)mlp[off + (size_t)j * nin + k] * a_in[k];
+        a_out[j] = acc > 0.0 ? acc : 0.0;
+      }
+      off = boff + W; nin = W;
+    }
+    const size_t head_off = off, head_b = off + (size_t)2 * nin;
+    const double* hl = act + (size_t)H * S;
+    double z[2];
+    for (int j = 0; j < 2; ++j) {
+      double acc = (double)mlp[head_b + j];
+      for (int k = 0; k < nin; ++k) acc += (double)mlp[head_off + (size_t)j * nin + k] * hl[k];
+      z[j] = acc;
+    }
+    /* loss (T1, T2) and its derivative w.r.t. the logits */
+    const double that = orc_softplus(z[0]), err = that - (double)t[i];
+    const int h = hit[i] != 0;
+    double dz[2] = {0.0, 0.0};
+    if (h) {
+      const double ae = fabs(err);
+      loss += ae < P->dist_clamp ? ae : P->dist_clamp;
+      if (ae < P->dist_clamp) dz[0] = (err > 0.0 ? 1.0 : (err < 0.0 ? -1.0 : 0.0)) * orc_sigmoid(z[0]);   /* d softplus = sigmoid */
+    }
+    loss += P->ce_weight * (h ? orc_softplus(-z[1]) : orc_softplus(z[1]));
+    dz[1] = P->ce_weight * (orc_sigmoid(z[1]) - (double)h);
+    dz[0] /= (double)n; dz[1] /= (double)n;
+    /* backward: head */
+    for (int k = 0; k < nin; ++k) del[k] = 0.0;
+    for (int j = 0; j < 2; ++j) {
+      if (grad_mlp) { grad_mlp[head_b + j] += dz[j]; for (int k = 0; k < nin; ++k) grad_mlp[head_off + (size_t)j * nin + k] += dz[j] * hl[k]; }
+      for (int k = 0; k < nin; ++k) del[k] += (double)mlp[head_off + (size_t)j * nin + k] * dz[j];
+    }
+    /* hidden layers, last to first; del = dLoss/d(output of layer l) */
+    for (int l = H - 1; l >= 0; --l) {
+      const int lin = (l == 0) ? E : W;
+      size_t woff = 0; { int q = E; for (int r = 0; r < l; ++r) { woff += (size_t)W * q + W; q = W; } }
+      const size_t boff = woff + (size_t)W * lin;
+      const double* a_in = act + (size_t)l * S; const double* a_out = act + (size_t)(l + 1) * S;
+      for (int k = 0; k < lin; ++k) dprev[k] = 0.0;
+      for (int j = 0; j < W; ++j) {
+        const double g = a_out[j] > 0.0 ? del[j] : 0.0;          /* ReLU */
+        if (grad_mlp) { grad_mlp[boff + j] += g; for (int k = 0; k < lin; ++k) grad_mlp[woff + (size_t)j * lin + k] += g * a_in[k]; }
+        for (int k = 0; k < lin; ++k) dprev[k] += (double)mlp[woff + (size_t)j * lin + k] * g;
+      }
+      for (int k = 0; k < lin; ++k) del[k] = dprev[k];
+    }
+    /* table: d feature / d table value = the trilinear weight */
+    if (grad_table)
+      for (int l = 0; l < L->n_levels; ++l) {
+        int64_t idx[8]; double wt[8];
+        level_corners(L, l, x01, idx, wt);
+        for (int c = 0; c < 8; ++c) for (int f = 0; f < F; ++f) grad_table[(size_t)idx[c] * F + f] += wt[c] * del[l * F + f];
+      }
+  }
+  free(act); free(del); free(dprev);
+  return loss / (double)n;
+}
+
+double orc_lr_at(const orc_train_params* P, int64_t step) {
+  const double s = step < P->total_steps ? (double)step : (double)P->total_steps;
+  const double f = P->lr_final_frac;
+  return P->lr0 * (f + (1.0 - f) * 0.5 * (1.0 + cos(HPI * s / (double)P->total_steps)));
+}
+
+void orc_adam_step(float* p, const double* g, double* m, double* v, int64_t n, int64_t step,
+                   double lr, const orc_train_params* P) {
+  const double c1 = 1.0 - pow(P->beta1, (double)step), c2 = 1.0 - pow(P->beta2, (double)step);
+  for (int64_t i = 0; i < n; ++i) {
+    m[i] = P->beta1 * m[i] + (1.0 - P->beta1) * g[i];
+    v[i] = P->beta2 * v[i] + (1.0 - P->beta2) * g[i] * g[i];
+    p[i] = (float)((double)p[i] - lr * (m[i] / c1) / (sqrt(v[i] / c2) + P->adam_eps));
+  }
+}
+
+double orc_solid_scene_raycast(const double o[3], const double d[3], const double sphere_c[3],
+                               double sphere_r, const double bmin[3], const double bmax[3]) {
+  double best = -1.0;
+  const double ts = orc_ray_sphere(o, d, sphere_c, sphere_r);      /* smallest t > 0, from inside too */
+  if (ts > 0.0) best = ts;
+  /* slabs: the ray is inside the box for t in [tn, tf] */
+  double tn = -INFINITY, tf = INFINITY; int ok = 1;
+  for (int a = 0; a < 3; ++a) {
+    if (d[a] != 0.0) {
+      double t0 = (bmin[a] - o[a]) / d[a], t1 = (bmax[a] - o[a]) / d[a];
+      if (t0 > t1) { const double q = t0; t0 = t1; t1 = q; }
+      if (t0 > tn) tn = t0;
+      if (t1 < tf) tf = t1;
+    } else if (o[a] < bmin[a] || o[a] > bmax[a]) ok = 0;
+  }
+  if (ok && tn <= tf && tf > 0.0) {
+    const double tb = tn > 0.0 ? tn : tf;                          /* entering, or leaving from inside */
+    if (best < 0.0 || tb < best) best = tb;
+  }
+  return best;
+}

@@ -67,6 +67,42 @@ int  orc_hash_forward(const orc_hash_layout* L, const void* table, const void* m
                       const float* o, const float* d, int64_t n, int mode,
                       double* z, double* dist, double* vis, int nthreads);
 
+/* ---------------------------------------------------------------- training
+ * PAPER.md:70 (Sec. III-B): "The loss is an L1 term on distance, clamped to a maximum so far-away
+ * surfaces do not dominate, plus a cross-entropy term on the hit flag."  PAPER.md:86 (Sec. III-D):
+ * "Adam for 30,000 steps, a batch of 16,384 rays, and a learning rate of 3e-3 decayed by cosine to
+ * five percent of its value.  The loss is an L1 term on distance, clamped at the box scale, plus a
+ * cross-entropy term on the hit weighted at 0.3."  Readings T1-T5:
+ *   T1  per ray  l = hit * min(|softplus(z0) - t|, clamp) + ce_weight * CE(sigmoid(z1), hit),
+ *       CE = softplus(-z1) if hit else softplus(z1);  loss = mean over the batch.
+ *   T2  the distance term exists only for rays that hit (a miss has no distance).
+ *   T3  Adam as published (Kingma & Ba): m = b1 m + (1-b1) g; v = b2 v + (1-b2) g^2;
+ *       p -= lr * (m / (1-b1^s)) / (sqrt(v / (1-b2^s)) + eps), s = 1, 2, ...
+ *   T4  lr(s) = lr0 * (f + (1-f) * (1 + cos(pi * min(s, S) / S)) / 2), f = 0.05, s = 0 .. S.
+ *   T5  fp32 master parameters; this oracle evaluates everything in fp64 from them.
+ * Pins (tests/test_train_oracle_pins.py): gradients against central finite differences of the
+ * loss; Adam's first step = -lr * sign(g); constant gradient; schedule end points. */
+typedef struct orc_train_params {
+  double lr0, lr_final_frac; int32_t total_steps;
+  double beta1, beta2, adam_eps, dist_clamp, ce_weight;
+} orc_train_params;
+/* loss (returned) and gradients of the mean loss w.r.t. every table value (grad_table
+ * [entries * n_features]) and every MLP parameter (grad_mlp, blob order); either may be NULL.
+ * table and mlp are fp32 here (table_dtype / mlp_dtype of L are ignored). */
+double orc_hash_loss_grads(const orc_hash_layout* L, const float* table, const float* mlp,
+                           const float* o, const float* d, const float* t, const uint8_t* hit,
+                           int64_t n, const orc_train_params* P, double* grad_table, double* grad_mlp);
+double orc_lr_at(const orc_train_params* P, int64_t step);
+/* one Adam update of n parameters in place; `step` is 1-based (T3) */
+void orc_adam_step(float* p, const double* g, double* m, double* v, int64_t n, int64_t step,
+                   double lr, const orc_train_params* P);
+
+/* ---- analytic supervision (stands in for the paper's mesh ray cast): distance to
+ * the FIRST SURFACE along d of a sphere and an axis-aligned box, from any origin
+ * (inside an object the first surface is where the ray leaves it).  Returns t, or -1 for a miss. */
+double orc_solid_scene_raycast(const double o[3], const double d[3], const double sphere_c[3],
+                               double sphere_r, const double bmin[3], const double bmax[3]);
+
 #ifdef __cplusplus
 }
 #endif

@@ -1,0 +1,94 @@
+"""Pins of the training oracle (oracle/ddf_hash_oracle.c, readings T1-T5): CPU only.
+Gradients are pinned by central finite differences of the oracle's own LOSS (a different code path:
+forward only), Adam and the schedule by their published closed forms, the supervision by textbook
+ray-sphere / ray-box values."""
+import math
+
+import numpy as np
+
+from ddf_inputs import HashLayout, make_hash_table, make_hash_mlp, random_rays
+
+
+def _small():
+    return HashLayout(n_levels=3, n_features=2, log2_table=9, base_res=3, growth=2.0,
+                      box_min=(-1.0, -1.0, -1.0), box_max=(1.0, 1.0, 1.0), n_freq_dir=2, n_hidden=2, width=8)
+
+
+def _batch(orc, lay, n=40):
+    o, d = random_rays(n)
+    rng = np.random.default_rng(3)
+    t = rng.uniform(0.2, 3.0, n).astype(np.float32)
+    hit = (rng.uniform(size=n) < 0.6).astype(np.uint8)
+    table = make_hash_table(lay, orc.hash_table_entries(lay), scale=0.5)
+    mlp = make_hash_mlp(lay, bias_scale=0.3)
+    return o, d, t, hit, table, mlp
+
+
+def test_gradients_match_finite_differences(orc):
+    lay = _small()
+    o, d, t, hit, table, mlp = _batch(orc, lay)
+    P = orc.train_params(dist_clamp=2.0)                  # some rays sit beyond the clamp: zero distance gradient there
+    loss, gt, gm = orc.hash_loss_grads(lay, table, mlp, o, d, t, hit, P)
+    assert np.isfinite(loss) and np.abs(gt).max() > 0 and np.abs(gm).max() > 0
+    rng = np.random.default_rng(0)
+    h = 1e-3                                              # fp32 master copies: the step must survive the cast
+    touched = np.nonzero(gt)[0]
+    for arr, g, picks in ((table, gt, rng.choice(touched, 25, replace=False)), (mlp, gm, rng.choice(len(mlp), 40, replace=False))):
+        for i in picks:
+            a = arr.copy(); b = arr.copy()
+            a[i] += h; b[i] -= h
+            step = float(a[i]) - float(b[i])
+            la = orc.hash_loss_grads(lay, a if arr is table else table, a if arr is mlp else mlp, o, d, t, hit, P, want_grads=False)[0]
+            lb = orc.hash_loss_grads(lay, b if arr is table else table, b if arr is mlp else mlp, o, d, t, hit, P, want_grads=False)[0]
+            fd = (la - lb) / step
+            assert abs(fd - g[i]) <= 2e-4 * max(1.0, abs(g[i])) + 2e-5, (i, fd, g[i])
+    # entries no ray touches have exactly zero gradient
+    assert np.count_nonzero(gt) < len(gt)
+
+
+def test_loss_closed_forms(orc):
+    """zero MLP: softplus(b0) = ln 2 + ..., CE = ln 2; clamp; misses carry no distance term (T1, T2)"""
+    lay = _small()
+    o, d, t, hit, table, mlp = _batch(orc, lay, n=10)
+    mlp = np.zeros_like(mlp)
+    P = orc.train_params(dist_clamp=0.5, ce_weight=0.3)
+    hit[:] = 1; t[:] = math.log(2.0) + 0.25
+    loss, _, gm = orc.hash_loss_grads(lay, table, mlp, o, d, t, hit, P)
+    assert abs(loss - (0.25 + 0.3 * math.log(2.0))) < 1e-7          # |ln2 - t| = 0.25 < clamp
+    t[:] = 5.0
+    loss, _, gm = orc.hash_loss_grads(lay, table, mlp, o, d, t, hit, P)
+    assert abs(loss - (0.5 + 0.3 * math.log(2.0))) < 1e-7           # clamped at 0.5 ...
+    assert gm[-2] == 0.0 and abs(gm[-1] - 0.3 * (0.5 - 1.0)) < 1e-12  # ... and flat there; d CE / d z1 = w (xi - hit)
+    hit[:] = 0
+    loss, _, gm = orc.hash_loss_grads(lay, table, mlp, o, d, t, hit, P)
+    assert abs(loss - 0.3 * math.log(2.0)) < 1e-12 and gm[-2] == 0.0 and abs(gm[-1] - 0.15) < 1e-12
+
+
+def test_adam_and_schedule_closed_forms(orc):
+    P = orc.train_params(lr0=3e-3, lr_final_frac=0.05, total_steps=30000, adam_eps=1e-12)
+    assert abs(orc.lr_at(P, 0) - 3e-3) < 1e-15 and abs(orc.lr_at(P, 30000) - 1.5e-4) < 1e-15     # "decayed by cosine to five percent"
+    assert abs(orc.lr_at(P, 15000) - 3e-3 * 0.525) < 1e-15 and orc.lr_at(P, 99999) == orc.lr_at(P, 30000)
+    g = np.array([0.5, -2.0, 1e-3, -7e-5]); p = np.array([1.0, 1.0, 1.0, 1.0], np.float32)
+    m = np.zeros(4); v = np.zeros(4)
+    orc.adam_step(p, g, m, v, 1, 0.01, P)
+    assert np.allclose(p, 1.0 - 0.01 * np.sign(g), atol=1e-6)        # first step: -lr sign(g)
+    for s in range(2, 11):
+        orc.adam_step(p, g, m, v, s, 0.01, P)
+    assert np.allclose(p, 1.0 - 0.1 * np.sign(g), atol=1e-5)         # constant gradient: every step is -lr sign(g)
+    assert np.allclose(m, (1 - 0.9 ** 10) * g) and np.allclose(v, (1 - 0.999 ** 10) * g * g)
+    # zero gradient after a history: the moments decay, the parameter keeps moving the same way
+    p0 = p.copy(); orc.adam_step(p, np.zeros(4), m, v, 11, 0.01, P)
+    assert np.all(np.sign(p - p0) == -np.sign(g))
+
+
+def test_supervision_raycast_textbook(orc):
+    c, r, bmin, bmax = (0.0, 0.0, 0.0), 0.5, (-0.9, -0.9, -0.9), (0.9, 0.9, -0.6)
+    rc = lambda o, d: orc.solid_scene_raycast(o, d, c, r, bmin, bmax)
+    assert abs(rc((0, 0, 3), (0, 0, -1)) - 2.5) < 1e-12                 # sphere from outside
+    assert abs(rc((0, 0, 0), (0, 0, 1)) - 0.5) < 1e-12                  # from inside: where the ray leaves
+    assert abs(rc((0.8, 0.8, 3), (0, 0, -1)) - 3.6) < 1e-12             # misses the sphere, lands on the slab's top face
+    assert abs(rc((0.8, 0, -0.75), (1, 0, 0)) - 0.1) < 1e-12            # inside the slab: exit face
+    assert rc((2, 2, 2), (0, 0, 1)) == -1.0 and rc((0, 2, 0), (1, 0, 0)) == -1.0     # misses
+    assert abs(rc((0, 0, -3), (0, 0, 1)) - 2.1) < 1e-12                 # slab bottom before the sphere
+    s = 1 / math.sqrt(2)
+    assert abs(rc((-2, 0, -2.75), (s, 0, s)) - (1.85 / s)) < 1e-9       # oblique: x is inside the slab from t = 1.1/s, z only from 1.85/s (at x = -0.15)
