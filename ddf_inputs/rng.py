@@ -14,7 +14,7 @@ import numpy as np
 MASTER_SEED = 20260600817
 STREAMS = {
     "weights_ddf": 1, "weights_sdf": 2, "rays_c0": 3, "camera_pos": 4,
-    "shadow_points": 5, "ao_samples": 6, "biases": 7, "hash_table": 8, "hash_mlp": 9,
+    "shadow_points": 5, "ao_samples": 6, "biases": 7, "hash_table": 8, "hash_mlp": 9, "train_rays": 10,
 }
 
 _M1 = np.uint64(0x9E3779B97F4A7C15)

@@ -191,6 +191,53 @@ int  ddf_query_shadowed(ddf_model* model, const float* o, const float* d, int64_
                         const float light[3], float eps, float* out_dist, float* out_vis,
                         uint8_t* out_lit, int64_t* out_count, void* stream);
 
+/* ---------------------------------------------------------------- training the hash-grid field
+ * PAPER.md:70 / 86: "an L1 term on distance, clamped at the box scale, plus a cross-entropy term
+ * on the hit weighted at 0.3"; "Adam for 30,000 steps, a batch of 16,384 rays, and a learning rate
+ * of 3e-3 decayed by cosine to five percent of its value"; 30 percent of each batch are ray-march
+ * shifted points.  Readings T1-T6:
+ *   per ray  l = hit * min(|softplus(z0) - t|, dist_clamp) + ce_weight * CE(sigmoid(z1), hit),
+ *   loss = mean over the batch; Adam as published, bias-corrected, dense over every parameter;
+ *   lr(s) = lr0 (f + (1-f)(1 + cos(pi min(s,S)/S))/2);  fp32 master parameters and arithmetic.
+ * The trainer owns fp32 copies of the table and the MLP (+ Adam moments and a gradient buffer:
+ * 4 x the field size).  This build trains n_features == 2, width == 64, n_hidden <= 2. */
+typedef struct ddf_train_params {
+  uint32_t struct_size;        /* sizeof(ddf_train_params) */
+  float lr0, lr_final_frac; int32_t total_steps;
+  float beta1, beta2, adam_eps, dist_clamp, ce_weight;
+} ddf_train_params;
+typedef struct ddf_trainer ddf_trainer;
+/* table, mlp: [host] fp32 blobs in the ddf_create_hashgrid order (layout dtypes must be 0). */
+int  ddf_trainer_create(const float* table, const float* mlp, const ddf_hashgrid_layout* layout,
+                        const ddf_train_params* params, ddf_trainer** out);
+int  ddf_trainer_destroy(ddf_trainer* trainer);
+/* One optimisation step on a batch: forward, loss, backward, Adam update (step counter + 1).
+ * o, d [device] float[n][3]; t [device] float[n] target distance; hit [device] uint8[n];
+ * loss [device] float (may be NULL) receives the batch loss BEFORE the update. */
+int  ddf_trainer_step(ddf_trainer* trainer, const float* o, const float* d, const float* t,
+                      const uint8_t* hit, int64_t n, float* loss, void* stream);
+/* Parity aid: loss and gradients of the mean loss, no update.  grad_table [device] float
+ * [entries * 2], grad_mlp [device] float [mlp parameters, blob order]; either may be NULL. */
+int  ddf_trainer_loss_grads(ddf_trainer* trainer, const float* o, const float* d, const float* t,
+                            const uint8_t* hit, int64_t n, float* loss, float* grad_table,
+                            float* grad_mlp, void* stream);
+/* Current parameters to [host] fp32 blobs (synchronises); feed them to ddf_create_hashgrid. */
+int  ddf_trainer_export(ddf_trainer* trainer, float* table, float* mlp);
+int64_t ddf_trainer_steps(const ddf_trainer* trainer);
+/* Analytic supervision (stands in for the paper's mesh ray cast): distance to the
+ * FIRST SURFACE along d of a solid sphere and a solid axis-aligned box, from any
+ * origin (from inside an object that is where the ray leaves it).  t [n] (0 for a miss), hit [n]. */
+int  ddf_scene_raycast(const ddf_scene* scene, const float* o, const float* d, int64_t n,
+                       float* t, uint8_t* hit, void* stream);
+/* One training batch (reading T6): origins uniform in [-sample_half, sample_half]^3 aimed at a
+ * uniform point of [-1,1]^3; half of them re-anchored on the surface they hit (stepped back 1e-3,
+ * new direction uniform on the sphere); targets from ddf_scene_raycast's rule; 30 % of the hit
+ * rays moved forward by u * t with target t - u t (PAPER.md:70 self-consistency).  Ray k of step
+ * s draws counters (s n + k) * 16 + j of (seed, rng_stream). */
+int  ddf_gen_train_batch(const ddf_scene* scene, uint64_t seed, uint64_t rng_stream, int64_t step,
+                         int64_t n, float sample_half, float* o, float* d, float* t, uint8_t* hit,
+                         void* stream);
+
 /* ---------------------------------------------------------------- sphere-tracing comparison
  * (BASELINE.json configs[4]).  `model` must have input_kind 1, n_out 1.
  * Traces s(p) = (|p| - base_radius) + alpha * MLP(p):

@@ -413,3 +413,16 @@ def adam_step(p, g, m, v, step, lr, P):
 
 def solid_scene_raycast(o, d, sphere_c=(0.0, 0.0, 0.0), sphere_r=0.5, bmin=(-0.9, -0.9, -0.9), bmax=(0.9, 0.9, -0.6)):
     return lib().orc_solid_scene_raycast(_v3(o), _v3(d), _v3(sphere_c), C.c_double(sphere_r), _v3(bmin), _v3(bmax))
+
+
+TRAIN_SCENE = dict(sphere_c=(0.0, 0.0, 0.0), sphere_r=0.5, bmin=(-0.9, -0.9, -0.9), bmax=(0.9, 0.9, -0.6))
+
+
+def gen_train_batch(seed, stream, step, n, sample_half=2.0, scene=None):
+    sc = scene or TRAIN_SCENE
+    o = np.empty((n, 3), np.float32); d = np.empty((n, 3), np.float32)
+    t = np.empty(n, np.float32); hit = np.empty(n, np.uint8)
+    lib().orc_gen_train_batch(_v3(sc["sphere_c"]), C.c_double(sc["sphere_r"]), _v3(sc["bmin"]), _v3(sc["bmax"]),
+                              C.c_uint64(int(seed)), C.c_uint64(int(stream)), C.c_int64(step), C.c_int64(n),
+                              C.c_double(sample_half), _p(o), _p(d), _p(t), _p(hit))
+    return o, d, t, hit

@@ -341,3 +341,35 @@ double orc_solid_scene_raycast(const double o[3], const double d[3], const doubl
   }
   return best;
 }
+
+/* reading T6: "Camera rays ... Rays that start on the surface and point in all
+ * directions ... a point moved forward by s should report distance t-s"; "We replace
+ * 30 percent of each batch with the ray-march shifted points". */
+void orc_gen_train_batch(const double sphere_c[3], double sphere_r, const double bmin[3], const double bmax[3],
+                         uint64_t seed, uint64_t stream, int64_t step, int64_t n, double sample_half,
+                         float* o, float* d, float* t, uint8_t* hit) {
+  for (int64_t k = 0; k < n; ++k) {
+    const uint64_t base = ((uint64_t)step * (uint64_t)n + (uint64_t)k) * 16ull;
+    double u[11];
+    for (int j = 0; j < 11; ++j) u[j] = orc_uniform01(seed, stream, base + j);
+    double oo[3], dd[3], q[3];
+    for (int a = 0; a < 3; ++a) oo[a] = (2.0 * u[a] - 1.0) * sample_half;
+    for (int a = 0; a < 3; ++a) q[a] = (2.0 * u[3 + a] - 1.0) - oo[a];
+    const double len = sqrt(q[0]*q[0] + q[1]*q[1] + q[2]*q[2]);
+    if (len > 1e-6) { for (int a = 0; a < 3; ++a) dd[a] = q[a] / len; } else { dd[0] = 0; dd[1] = 0; dd[2] = 1; }
+    double tt = orc_solid_scene_raycast(oo, dd, sphere_c, sphere_r, bmin, bmax);
+    if (u[6] >= 0.5 && tt > 0.0) {                        /* surface-anchored, omnidirectional */
+      for (int a = 0; a < 3; ++a) oo[a] += (tt - 1e-3) * dd[a];
+      orc_dir_from_u(u[7], u[8], dd);
+      tt = orc_solid_scene_raycast(oo, dd, sphere_c, sphere_r, bmin, bmax);
+    }
+    double tf = tt > 0.0 ? tt : 0.0;
+    if (tt > 0.0 && u[9] < 0.3) {                         /* ray-march shifted point */
+      const double s = u[10] * tf;
+      for (int a = 0; a < 3; ++a) oo[a] += s * dd[a];
+      tf -= s;
+    }
+    for (int a = 0; a < 3; ++a) { o[3 * k + a] = (float)oo[a]; d[3 * k + a] = (float)dd[a]; }
+    t[k] = (float)tf; hit[k] = tt > 0.0 ? 1 : 0;
+  }
+}

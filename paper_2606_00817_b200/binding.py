@@ -17,6 +17,8 @@ EXPORTED_SYMBOLS = [
     "ddf_gen_camera", "ddf_gen_sphere_points", "ddf_gen_shadow", "ddf_gen_gbuffer", "ddf_gen_ao",
     "ddf_ao_reduce", "ddf_query_ao", "ddf_shadow_test", "sdf_sphere_trace",
     "ddf_hashgrid_table_entries", "ddf_create_hashgrid", "ddf_gen_shadow_from_hits", "ddf_query_shadowed",
+    "ddf_trainer_create", "ddf_trainer_destroy", "ddf_trainer_step", "ddf_trainer_loss_grads", "ddf_trainer_export",
+    "ddf_trainer_steps", "ddf_scene_raycast", "ddf_gen_train_batch",
 ]
 
 
@@ -37,6 +39,12 @@ class DdfHashgridLayout(C.Structure):
                 ("growth", C.c_float), ("box_min", C.c_float * 3), ("box_max", C.c_float * 3),
                 ("n_freq_dir", C.c_uint32), ("n_hidden", C.c_uint32), ("width", C.c_uint32), ("n_out", C.c_uint32),
                 ("table_dtype", C.c_uint32), ("mlp_dtype", C.c_uint32), ("weights_on_device", C.c_uint32)]
+
+
+class DdfTrainParams(C.Structure):
+    _fields_ = [("struct_size", C.c_uint32), ("lr0", C.c_float), ("lr_final_frac", C.c_float), ("total_steps", C.c_int32),
+                ("beta1", C.c_float), ("beta2", C.c_float), ("adam_eps", C.c_float), ("dist_clamp", C.c_float),
+                ("ce_weight", C.c_float)]
 
 
 class DdfCamera(C.Structure):
@@ -71,6 +79,7 @@ def lib():
         _lib.ddf_status_string.restype = C.c_char_p
         _lib.ddf_get_info.restype = C.c_int64
         _lib.ddf_hashgrid_table_entries.restype = C.c_int64
+        _lib.ddf_trainer_steps.restype = C.c_int64
     return _lib
 
 
@@ -278,3 +287,73 @@ def ddf_query_shadowed(model, o, d, n, light, eps, out_dist, out_vis, out_lit, o
     _check(lib().ddf_query_shadowed(model.handle, _dev(o), _dev(d), C.c_int64(n), li, C.c_float(eps), _dev(out_dist),
                                     _dev(out_vis), _dev(out_lit, torch.uint8), _dev(out_count, torch.int64),
                                     _stream(stream)), "ddf_query_shadowed")
+
+
+# ------------------------------------------------------------------ training
+
+def make_train_params(lr0=3e-3, lr_final_frac=0.05, total_steps=30000, beta1=0.9, beta2=0.999, adam_eps=1e-8,
+                      dist_clamp=6.0, ce_weight=0.3):
+    return DdfTrainParams(C.sizeof(DdfTrainParams), lr0, lr_final_frac, total_steps, beta1, beta2, adam_eps, dist_clamp, ce_weight)
+
+
+class Trainer:
+    def __init__(self, handle, layout):
+        self.handle, self.layout = handle, layout
+
+    def __del__(self):
+        try:
+            if self.handle:
+                ddf_trainer_destroy(self)
+        except Exception:
+            pass
+
+
+def ddf_trainer_create(table, mlp, lay, params):
+    import numpy as np
+    table = np.ascontiguousarray(table, dtype=np.float32); mlp = np.ascontiguousarray(mlp, dtype=np.float32)
+    L = make_hashgrid_layout(lay, 0)
+    h = C.c_void_p(0)
+    _check(lib().ddf_trainer_create(table.ctypes.data_as(C.c_void_p), mlp.ctypes.data_as(C.c_void_p), C.byref(L),
+                                    C.byref(params), C.byref(h)), "ddf_trainer_create")
+    return Trainer(h, lay)
+
+
+def ddf_trainer_destroy(tr):
+    if tr.handle:
+        rc = lib().ddf_trainer_destroy(tr.handle)
+        tr.handle = None
+        _check(rc, "ddf_trainer_destroy")
+
+
+def ddf_trainer_step(tr, o, d, t, hit, n, loss=None, stream=None):
+    _check(lib().ddf_trainer_step(tr.handle, _dev(o), _dev(d), _dev(t), _dev(hit, torch.uint8), C.c_int64(n), _dev(loss),
+                                  _stream(stream)), "ddf_trainer_step")
+
+
+def ddf_trainer_loss_grads(tr, o, d, t, hit, n, loss, grad_table, grad_mlp, stream=None):
+    _check(lib().ddf_trainer_loss_grads(tr.handle, _dev(o), _dev(d), _dev(t), _dev(hit, torch.uint8), C.c_int64(n), _dev(loss),
+                                        _dev(grad_table), _dev(grad_mlp), _stream(stream)), "ddf_trainer_loss_grads")
+
+
+def ddf_trainer_export(tr, n_table, n_mlp):
+    """Returns (table, mlp) as float32 numpy arrays."""
+    import numpy as np
+    table = np.empty(n_table, np.float32); mlp = np.empty(n_mlp, np.float32)
+    _check(lib().ddf_trainer_export(tr.handle, table.ctypes.data_as(C.c_void_p), mlp.ctypes.data_as(C.c_void_p)),
+           "ddf_trainer_export")
+    return table, mlp
+
+
+def ddf_trainer_steps(tr):
+    return int(lib().ddf_trainer_steps(tr.handle))
+
+
+def ddf_scene_raycast(scene, o, d, n, t, hit, stream=None):
+    _check(lib().ddf_scene_raycast(C.byref(scene), _dev(o), _dev(d), C.c_int64(n), _dev(t), _dev(hit, torch.uint8),
+                                   _stream(stream)), "ddf_scene_raycast")
+
+
+def ddf_gen_train_batch(scene, seed, rng_stream, step, n, sample_half, o, d, t, hit, stream=None):
+    _check(lib().ddf_gen_train_batch(C.byref(scene), C.c_uint64(seed), C.c_uint64(rng_stream), C.c_int64(step), C.c_int64(n),
+                                     C.c_float(sample_half), _dev(o), _dev(d), _dev(t), _dev(hit, torch.uint8),
+                                     _stream(stream)), "ddf_gen_train_batch")

@@ -1,0 +1,520 @@
+// ddf_train.cu - training the hash-grid field (include/ddf.h "training"):
+// forward, clamped-L1 + cross-entropy loss, backward, dense Adam, all in fp32.
+//
+// train_fwd_bwd_kernel: one CTA = 128 rays, one thread per ray.  Activations and deltas live in
+// shared memory as [unit][ray] columns (pitch 129 floats: a thread walking its own column and a
+// thread walking a row over the rays are both conflict-free); the MLP weights sit beside them
+// transposed ([k][j], so 4 outputs come from one broadcast 16-byte load).  Per CTA the weight
+// gradients are block-level outer products summed over the 128 rays, added to the global
+// gradient with one atomic per parameter; the table gradient is 8 float2 atomics per level and
+// ray.  adam_kernel then updates every parameter (dense, as the paper's "Adam") and clears the
+// gradient.  Atomics make the sums order-dependent in the last bits: training is reproducible
+// to rounding, not bitwise.
+#include "ddf_common.cuh"
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+#include <new>
+#include <vector>
+
+namespace ddf {
+
+constexpr int kTrThreads = 128;
+constexpr int kTrPitch = 129;
+constexpr int kTrW = 64;
+constexpr int kTrMaxLevels = 16;
+
+struct TrLevel { float scale; uint32_t verts; uint32_t offset; uint32_t hashed; };
+
+struct TrParams {
+  TrLevel lv[kTrMaxLevels];
+  const float* table; const float* mlp;          // fp32 master copies
+  float* g_table; float* g_mlp; float* loss;
+  const float* o; const float* d; const float* t; const uint8_t* hit;
+  int64_t n;
+  float bmin[3], den[3];
+  float dist_clamp, ce_weight;
+  uint32_t tmask;
+  int n_levels, Ld, n_hidden, E, NF;
+  int w_off[3], b_off[3];                        // blob offsets of layer l (l = n_hidden: head)
+};
+
+struct Trainer {
+  ddf_hashgrid_layout lay;
+  ddf_train_params prm;
+  int64_t entries, n_table, n_mlp, step;
+  float *p_table, *p_mlp, *m, *v, *g;            // m, v, g hold table values first, then the MLP
+  float* loss_dev;
+  TrParams base;
+  size_t smem_bytes;
+};
+
+// corner indices (into the table, in float2 units) and weights of one level
+__device__ __forceinline__ void tr_corners(const TrLevel& lv, uint32_t tmask, const float x01[3], uint32_t idx[8], float wt[8]) {
+  uint32_t c0[3]; float w1[3];
+  #pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    const float pos = __fmul_rn(x01[a], lv.scale);
+    const float fl = fminf(floorf(pos), lv.scale - 1.0f);
+    c0[a] = (uint32_t)fl; w1[a] = pos - fl;
+  }
+  uint32_t kx[2], ky[2], kz[2];
+  if (lv.hashed) {
+    kx[0] = c0[0]; kx[1] = c0[0] + 1u;
+    ky[0] = c0[1] * 2654435761u; ky[1] = (c0[1] + 1u) * 2654435761u;
+    kz[0] = c0[2] * 805459861u;  kz[1] = (c0[2] + 1u) * 805459861u;
+  } else {
+    kx[0] = c0[0]; kx[1] = c0[0] + 1u;
+    ky[0] = c0[1] * lv.verts; ky[1] = ky[0] + lv.verts;
+    kz[0] = c0[2] * lv.verts * lv.verts; kz[1] = kz[0] + lv.verts * lv.verts;
+  }
+  #pragma unroll
+  for (int c = 0; c < 8; ++c) {
+    const uint32_t a = kx[c & 1], b = ky[(c >> 1) & 1], e = kz[c >> 2];
+    idx[c] = lv.offset + (lv.hashed ? ((a ^ b ^ e) & tmask) : (a + b + e));
+    wt[c] = ((c & 1) ? w1[0] : 1.0f - w1[0]) * (((c >> 1) & 1) ? w1[1] : 1.0f - w1[1]) * ((c >> 2) ? w1[2] : 1.0f - w1[2]);
+  }
+}
+
+// out[j][t] = relu(b[j] + sum_k Wt[k][j] in[k][t]) for j < 64, 8 outputs per pass
+__device__ __forceinline__ void tr_layer_fwd(const float* __restrict__ Wt, const float* __restrict__ b, int nin,
+                                             const float* in, float* out, int t) {
+  for (int j0 = 0; j0 < kTrW; j0 += 8) {
+    float acc[8];
+    #pragma unroll
+    for (int q = 0; q < 8; ++q) acc[q] = b[j0 + q];
+    for (int k = 0; k < nin; ++k) {
+      const float a = in[k * kTrPitch + t];
+      const float4 w0 = *reinterpret_cast<const float4*>(Wt + k * kTrW + j0);
+      const float4 w1 = *reinterpret_cast<const float4*>(Wt + k * kTrW + j0 + 4);
+      acc[0] = fmaf(w0.x, a, acc[0]); acc[1] = fmaf(w0.y, a, acc[1]); acc[2] = fmaf(w0.z, a, acc[2]); acc[3] = fmaf(w0.w, a, acc[3]);
+      acc[4] = fmaf(w1.x, a, acc[4]); acc[5] = fmaf(w1.y, a, acc[5]); acc[6] = fmaf(w1.z, a, acc[6]); acc[7] = fmaf(w1.w, a, acc[7]);
+    }
+    #pragma unroll
+    for (int q = 0; q < 8; ++q) out[(j0 + q) * kTrPitch + t] = fmaxf(acc[q], 0.0f);
+  }
+}
+
+// din[k][t] = sum_j Wt[k][j] g[j][t]   (g already holds delta * relu')
+__device__ __forceinline__ void tr_layer_bwd(const float* __restrict__ Wt, int nin, const float* g, float* din, int t) {
+  for (int k = 0; k < nin; ++k) din[k * kTrPitch + t] = 0.0f;
+  for (int j0 = 0; j0 < kTrW; j0 += 8) {
+    float gj[8];
+    #pragma unroll
+    for (int q = 0; q < 8; ++q) gj[q] = g[(j0 + q) * kTrPitch + t];
+    for (int k = 0; k < nin; ++k) {
+      const float4 w0 = *reinterpret_cast<const float4*>(Wt + k * kTrW + j0);
+      const float4 w1 = *reinterpret_cast<const float4*>(Wt + k * kTrW + j0 + 4);
+      float s = din[k * kTrPitch + t];
+      s = fmaf(w0.x, gj[0], s); s = fmaf(w0.y, gj[1], s); s = fmaf(w0.z, gj[2], s); s = fmaf(w0.w, gj[3], s);
+      s = fmaf(w1.x, gj[4], s); s = fmaf(w1.y, gj[5], s); s = fmaf(w1.z, gj[6], s); s = fmaf(w1.w, gj[7], s);
+      din[k * kTrPitch + t] = s;
+    }
+  }
+}
+
+// block-level  dW[j][k] += sum_r g[j][r] a[k][r],  db[j] += sum_r g[j][r]; one atomic per entry
+__device__ __forceinline__ void tr_weight_grads(const float* g, const float* a, int nin, float* gW, float* gb, int t) {
+  const int j = t & 63, half = t >> 6;
+  for (int k0 = half * 4; k0 < nin; k0 += 8) {
+    float acc[4] = {0.0f, 0.0f, 0.0f, 0.0f};
+    for (int r = 0; r < kTrThreads; ++r) {
+      const float gv = g[j * kTrPitch + r];
+      #pragma unroll
+      for (int q = 0; q < 4; ++q) if (k0 + q < nin) acc[q] = fmaf(gv, a[(k0 + q) * kTrPitch + r], acc[q]);
+    }
+    #pragma unroll
+    for (int q = 0; q < 4; ++q) if (k0 + q < nin) atomicAdd(gW + j * nin + k0 + q, acc[q]);
+  }
+  if (half == 0) {
+    float s = 0.0f;
+    for (int r = 0; r < kTrThreads; ++r) s += g[j * kTrPitch + r];
+    atomicAdd(gb + j, s);
+  }
+}
+
+__global__ void __launch_bounds__(kTrThreads, 1) train_fwd_bwd_kernel(const __grid_constant__ TrParams p) {
+  extern __shared__ float sm[];
+  const int t = threadIdx.x, H = p.n_hidden, E = p.E;
+  // shared layout: weights (transposed), biases, head; then act[0..H] and two delta buffers
+  float* Wt[2]; float* bs[2];
+  float* cur = sm;
+  for (int l = 0; l < H; ++l) { Wt[l] = cur; cur += (l == 0 ? E : kTrW) * kTrW; }
+  for (int l = 0; l < H; ++l) { bs[l] = cur; cur += kTrW; }
+  float* Wh = cur; cur += 2 * kTrW;
+  float* act[3];
+  for (int l = 0; l <= H; ++l) { act[l] = cur; cur += kTrW * kTrPitch; }
+  float* dA = cur; cur += kTrW * kTrPitch;
+  float* dB = cur;
+  for (int l = 0; l < H; ++l) {
+    const int nin = l == 0 ? E : kTrW;
+    for (int e = t; e < kTrW * nin; e += kTrThreads) { const int j = e / nin, k = e % nin; Wt[l][k * kTrW + j] = p.mlp[p.w_off[l] + e]; }
+    for (int e = t; e < kTrW; e += kTrThreads) bs[l][e] = p.mlp[p.b_off[l] + e];
+  }
+  for (int e = t; e < 2 * kTrW; e += kTrThreads) Wh[e] = p.mlp[p.w_off[H] + e];
+  const float hb0 = p.mlp[p.b_off[H]], hb1 = p.mlp[p.b_off[H] + 1];
+  __syncthreads();
+
+  float block_loss = 0.0f;
+  const int64_t num_tiles = (p.n + kTrThreads - 1) / kTrThreads;
+  for (int64_t tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
+    const int64_t ray = tile * kTrThreads + t;
+    const bool valid = ray < p.n;
+    float x01[3] = {0.0f, 0.0f, 0.0f};
+    // ---- forward: input column
+    for (int k = 0; k < E; ++k) act[0][k * kTrPitch + t] = 0.0f;
+    if (valid) {
+      #pragma unroll
+      for (int a = 0; a < 3; ++a) {
+        const float v = __fdiv_rn(__fsub_rn(p.o[3 * ray + a], p.bmin[a]), p.den[a]);
+        x01[a] = fminf(fmaxf(v, 0.0f), 1.0f);
+      }
+      for (int l = 0; l < p.n_levels; ++l) {
+        uint32_t idx[8]; float wt[8];
+        tr_corners(p.lv[l], p.tmask, x01, idx, wt);
+        float f0 = 0.0f, f1 = 0.0f;
+        #pragma unroll
+        for (int c = 0; c < 8; ++c) { const float2 v = __ldg(reinterpret_cast<const float2*>(p.table) + idx[c]); f0 = fmaf(wt[c], v.x, f0); f1 = fmaf(wt[c], v.y, f1); }
+        act[0][(2 * l) * kTrPitch + t] = f0; act[0][(2 * l + 1) * kTrPitch + t] = f1;
+      }
+      const float dv[3] = { p.d[3 * ray], p.d[3 * ray + 1], p.d[3 * ray + 2] };
+      int m = p.NF;
+      for (int c = 0; c < 3; ++c) act[0][(m++) * kTrPitch + t] = dv[c];
+      for (int k = 0; k < p.Ld; ++k) {
+        float s[3], co[3];
+        for (int c = 0; c < 3; ++c) sincospif(ldexpf(dv[c], k), &s[c], &co[c]);
+        for (int c = 0; c < 3; ++c) act[0][(m++) * kTrPitch + t] = s[c];
+        for (int c = 0; c < 3; ++c) act[0][(m++) * kTrPitch + t] = co[c];
+      }
+    }
+    for (int l = 0; l < H; ++l) tr_layer_fwd(Wt[l], bs[l], l == 0 ? E : kTrW, act[l], act[l + 1], t);
+    float z0 = hb0, z1 = hb1;
+    for (int k = 0; k < kTrW; ++k) { const float hv = act[H][k * kTrPitch + t]; z0 = fmaf(Wh[k], hv, z0); z1 = fmaf(Wh[kTrW + k], hv, z1); }
+    // ---- loss and d loss / d logits (readings T1, T2)
+    float dz0 = 0.0f, dz1 = 0.0f;
+    if (valid) {
+      const int h = p.hit[ray] != 0;
+      const float sp = softplus_f(z0), err = sp - p.t[ray], ae = fabsf(err);
+      if (h) { block_loss += fminf(ae, p.dist_clamp); if (ae < p.dist_clamp) dz0 = (err > 0.0f ? 1.0f : (err < 0.0f ? -1.0f : 0.0f)) * sigmoid_f(z0); }
+      block_loss += p.ce_weight * (h ? softplus_f(-z1) : softplus_f(z1));
+      dz1 = p.ce_weight * (sigmoid_f(z1) - (float)h);
+      const float inv_n = 1.0f / (float)p.n;
+      dz0 *= inv_n; dz1 *= inv_n;
+    }
+    // ---- backward: head.  dA = delta at the last hidden output, masked by ReLU
+    for (int k = 0; k < kTrW; ++k) {
+      const float hv = act[H][k * kTrPitch + t];
+      dA[k * kTrPitch + t] = hv > 0.0f ? fmaf(Wh[k], dz0, Wh[kTrW + k] * dz1) : 0.0f;
+    }
+    // head weight gradients need the block's dz: park them in dB rows 0, 1
+    dB[0 * kTrPitch + t] = dz0; dB[1 * kTrPitch + t] = dz1;
+    __syncthreads();
+    if (t < kTrW) {
+      float s0 = 0.0f, s1 = 0.0f;
+      for (int r = 0; r < kTrThreads; ++r) { const float hv = act[H][t * kTrPitch + r]; s0 = fmaf(dB[r], hv, s0); s1 = fmaf(dB[kTrPitch + r], hv, s1); }
+      atomicAdd(p.g_mlp + p.w_off[H] + t, s0); atomicAdd(p.g_mlp + p.w_off[H] + kTrW + t, s1);
+    } else if (t < kTrW + 2) {
+      float s = 0.0f;
+      for (int r = 0; r < kTrThreads; ++r) s += dB[(t - kTrW) * kTrPitch + r];
+      atomicAdd(p.g_mlp + p.b_off[H] + (t - kTrW), s);
+    }
+    __syncthreads();
+    // ---- hidden layers, last to first
+    float* g = dA; float* din = dB;
+    for (int l = H - 1; l >= 0; --l) {
+      const int nin = l == 0 ? E : kTrW;
+      tr_layer_bwd(Wt[l], nin, g, din, t);                      // own column only
+      __syncthreads();                                          // g, act[l] complete for the whole block
+      tr_weight_grads(g, act[l], nin, p.g_mlp + p.w_off[l], p.g_mlp + p.b_off[l], t);
+      __syncthreads();
+      if (l > 0) for (int k = 0; k < nin; ++k) { if (!(act[l][k * kTrPitch + t] > 0.0f)) din[k * kTrPitch + t] = 0.0f; }
+      float* tmp = g; g = din; din = tmp;
+    }
+    // g now holds d loss / d input; its first NF rows are the level features
+    if (valid)
+      for (int l = 0; l < p.n_levels; ++l) {
+        uint32_t idx[8]; float wt[8];
+        tr_corners(p.lv[l], p.tmask, x01, idx, wt);
+        const float g0 = g[(2 * l) * kTrPitch + t], g1 = g[(2 * l + 1) * kTrPitch + t];
+        #pragma unroll
+        for (int c = 0; c < 8; ++c) atomicAdd(reinterpret_cast<float2*>(p.g_table) + idx[c], make_float2(wt[c] * g0, wt[c] * g1));
+      }
+    __syncthreads();
+  }
+  // ---- batch loss
+  #pragma unroll
+  for (int s = 16; s > 0; s >>= 1) block_loss += __shfl_xor_sync(0xffffffffu, block_loss, s);
+  if ((t & 31) == 0 && p.loss) atomicAdd(p.loss, block_loss / (float)p.n);
+}
+
+// dense Adam (reading T3) over n parameters; clears the gradient
+__global__ void adam_kernel(float* __restrict__ prm, float* __restrict__ m, float* __restrict__ v, float* __restrict__ g,
+                            int64_t n, float lr, float b1, float b2, float eps, float c1, float c2) {
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+    const float gi = g[i];
+    const float mi = b1 * m[i] + (1.0f - b1) * gi;
+    const float vi = b2 * v[i] + (1.0f - b2) * gi * gi;
+    m[i] = mi; v[i] = vi; g[i] = 0.0f;
+    prm[i] -= lr * (mi / c1) / (sqrtf(vi / c2) + eps);
+  }
+}
+
+// ------------------------------------------------------------------------------------------ supervision
+// first surface along d of a solid sphere and a solid box, from any origin; fp64 like the G-buffer
+__device__ double solid_scene_cast(const ddf_scene& sc, const double o[3], const double d[3]) {
+  double best = -1.0;
+  {
+    const double oc[3] = { o[0] - sc.sphere_c[0], o[1] - sc.sphere_c[1], o[2] - sc.sphere_c[2] };
+    const double b = oc[0]*d[0] + oc[1]*d[1] + oc[2]*d[2];
+    const double cc = oc[0]*oc[0] + oc[1]*oc[1] + oc[2]*oc[2] - (double)sc.sphere_r * (double)sc.sphere_r;
+    const double disc = b * b - cc;
+    if (disc >= 0.0) { const double sq = sqrt(disc); const double t0 = -b - sq, t1 = -b + sq; if (t0 > 0.0) best = t0; else if (t1 > 0.0) best = t1; }
+  }
+  double tn = -INFINITY, tf = INFINITY; bool ok = true;
+  #pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    if (d[a] != 0.0) {
+      double t0 = ((double)sc.box_min[a] - o[a]) / d[a], t1 = ((double)sc.box_max[a] - o[a]) / d[a];
+      if (t0 > t1) { const double q = t0; t0 = t1; t1 = q; }
+      tn = fmax(tn, t0); tf = fmin(tf, t1);
+    } else if (o[a] < (double)sc.box_min[a] || o[a] > (double)sc.box_max[a]) ok = false;
+  }
+  if (ok && tn <= tf && tf > 0.0) { const double tb = tn > 0.0 ? tn : tf; if (best < 0.0 || tb < best) best = tb; }
+  return best;
+}
+
+__global__ void scene_raycast_kernel(ddf_scene sc, const float* __restrict__ o, const float* __restrict__ d, int64_t n,
+                                     float* __restrict__ t, uint8_t* __restrict__ hit) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const double oo[3] = { o[3*i], o[3*i+1], o[3*i+2] }, dd[3] = { d[3*i], d[3*i+1], d[3*i+2] };
+  const double tt = solid_scene_cast(sc, oo, dd);
+  t[i] = tt > 0.0 ? (float)tt : 0.0f; hit[i] = tt > 0.0 ? 1 : 0;
+}
+
+__device__ __forceinline__ void tr_dir_from_u(float u1, float u2, float out[3]) {   // reading A9
+  const float z = 2.0f * u1 - 1.0f;
+  const float s = sqrtf(fmaxf(0.0f, 1.0f - z * z));
+  float sn, cs; sincospif(2.0f * u2, &sn, &cs);
+  out[0] = s * cs; out[1] = s * sn; out[2] = z;
+  const float inv = 1.0f / sqrtf(out[0]*out[0] + out[1]*out[1] + out[2]*out[2]);
+  out[0] *= inv; out[1] *= inv; out[2] *= inv;
+}
+
+__global__ void gen_train_batch_kernel(ddf_scene sc, uint64_t key, int64_t step, int64_t n, float sample_half,
+                                       float* __restrict__ o, float* __restrict__ d, float* __restrict__ t, uint8_t* __restrict__ hit) {
+  const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= n) return;
+  const uint64_t base = ((uint64_t)step * (uint64_t)n + (uint64_t)k) * 16ull;
+  float u[11];
+  #pragma unroll
+  for (int j = 0; j < 11; ++j) u[j] = dev_uniform01(key, base + j);
+  float oo[3], dd[3];
+  #pragma unroll
+  for (int a = 0; a < 3; ++a) oo[a] = (2.0f * u[a] - 1.0f) * sample_half;
+  {
+    float q[3] = { 2.0f * u[3] - 1.0f - oo[0], 2.0f * u[4] - 1.0f - oo[1], 2.0f * u[5] - 1.0f - oo[2] };
+    const float len = sqrtf(q[0]*q[0] + q[1]*q[1] + q[2]*q[2]);
+    if (len > 1e-6f) { dd[0] = q[0] / len; dd[1] = q[1] / len; dd[2] = q[2] / len; } else { dd[0] = 0.0f; dd[1] = 0.0f; dd[2] = 1.0f; }
+  }
+  double od[3] = { oo[0], oo[1], oo[2] }, ddd[3] = { dd[0], dd[1], dd[2] };
+  double tt = solid_scene_cast(sc, od, ddd);
+  if (u[6] >= 0.5f && tt > 0.0) {                     // surface-anchored, omnidirectional
+    const float back = (float)tt - 1e-3f;
+    #pragma unroll
+    for (int a = 0; a < 3; ++a) oo[a] = fmaf(back, dd[a], oo[a]);
+    tr_dir_from_u(u[7], u[8], dd);
+    for (int a = 0; a < 3; ++a) { od[a] = oo[a]; ddd[a] = dd[a]; }
+    tt = solid_scene_cast(sc, od, ddd);
+  }
+  float tf = tt > 0.0 ? (float)tt : 0.0f;
+  if (tt > 0.0 && u[9] < 0.3f) {                      // ray-march shifted point: same ray, target t - s
+    const float s = u[10] * tf;
+    #pragma unroll
+    for (int a = 0; a < 3; ++a) oo[a] = fmaf(s, dd[a], oo[a]);
+    tf -= s;
+  }
+  #pragma unroll
+  for (int a = 0; a < 3; ++a) { o[3*k + a] = oo[a]; d[3*k + a] = dd[a]; }
+  t[k] = tf; hit[k] = tt > 0.0 ? 1 : 0;
+}
+
+static inline uint64_t tr_mix64(uint64_t z) {
+  z += 0x9E3779B97F4A7C15ull; z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull; z = (z ^ (z >> 27)) * 0x94D049BB133111EBull; return z ^ (z >> 31);
+}
+
+}  // namespace ddf
+
+using namespace ddf;
+
+extern "C" int ddf_scene_raycast(const ddf_scene* scene, const float* o, const float* d, int64_t n,
+                                 float* t, uint8_t* hit, void* stream) {
+  if (!scene || n < 0) return DDF_E_INVALID_ARG;
+  if (n == 0) return DDF_OK;
+  if (!o || !d || !t || !hit) return DDF_E_INVALID_ARG;
+  scene_raycast_kernel<<<(unsigned)((n + 255) / 256), 256, 0, (cudaStream_t)stream>>>(*scene, o, d, n, t, hit);
+  DDF_CUDA_TRY(cudaGetLastError());
+  return DDF_OK;
+}
+
+extern "C" int ddf_gen_train_batch(const ddf_scene* scene, uint64_t seed, uint64_t rng_stream, int64_t step,
+                                   int64_t n, float sample_half, float* o, float* d, float* t, uint8_t* hit,
+                                   void* stream) {
+  if (!scene || n < 0 || step < 0 || !(sample_half > 0.0f)) return DDF_E_INVALID_ARG;
+  if (n == 0) return DDF_OK;
+  if (!o || !d || !t || !hit) return DDF_E_INVALID_ARG;
+  const uint64_t key = tr_mix64(tr_mix64(seed) ^ rng_stream);
+  gen_train_batch_kernel<<<(unsigned)((n + 255) / 256), 256, 0, (cudaStream_t)stream>>>(*scene, key, step, n, sample_half, o, d, t, hit);
+  DDF_CUDA_TRY(cudaGetLastError());
+  return DDF_OK;
+}
+
+// ------------------------------------------------------------------------------------------ trainer
+static int tr_check(const ddf_hashgrid_layout* L, const ddf_train_params* P) {
+  if (L->struct_size != sizeof(ddf_hashgrid_layout) || L->version != DDF_LAYOUT_VERSION) return DDF_E_BAD_LAYOUT;
+  if (P->struct_size != sizeof(ddf_train_params)) return DDF_E_BAD_LAYOUT;
+  if (!(P->lr0 > 0.0f) || P->total_steps < 1 || !(P->beta1 >= 0.0f && P->beta1 < 1.0f) || !(P->beta2 >= 0.0f && P->beta2 < 1.0f) ||
+      !(P->adam_eps > 0.0f) || !(P->dist_clamp > 0.0f) || !(P->ce_weight >= 0.0f) || !(P->lr_final_frac >= 0.0f)) return DDF_E_INVALID_ARG;
+  if (L->table_dtype != 0 || L->mlp_dtype != 0 || L->weights_on_device != 0) return DDF_E_BAD_LAYOUT;
+  for (int a = 0; a < 3; ++a) if (!(L->box_max[a] > L->box_min[a])) return DDF_E_BAD_LAYOUT;
+  if (L->n_features != 2 || L->n_levels < 1 || L->n_levels > (uint32_t)kTrMaxLevels || L->n_freq_dir > 4 || L->width != (uint32_t)kTrW ||
+      L->n_hidden < 1 || L->n_hidden > 2 || L->n_out != 2)
+    return DDF_E_UNSUPPORTED;
+  return DDF_OK;
+}
+
+static void tr_free(Trainer* T) {
+  if (!T) return;
+  cudaFree(T->p_table); cudaFree(T->p_mlp); cudaFree(T->m); cudaFree(T->v); cudaFree(T->g); cudaFree(T->loss_dev);
+  (void)cudaGetLastError();
+  delete T;
+}
+
+extern "C" int ddf_trainer_create(const float* table, const float* mlp, const ddf_hashgrid_layout* layout,
+                                  const ddf_train_params* params, ddf_trainer** out) {
+  if (out) *out = nullptr;
+  if (!table || !mlp || !layout || !params || !out) return DDF_E_INVALID_ARG;
+  int rc = tr_check(layout, params);
+  if (rc != DDF_OK) return rc;
+  const int64_t entries = ddf_hashgrid_table_entries(layout);
+  if (entries < 0) return (int)entries;
+  int dev = 0; cudaDeviceProp prop;
+  DDF_CUDA_TRY(cudaGetDevice(&dev));
+  DDF_CUDA_TRY(cudaGetDeviceProperties(&prop, dev));
+  if (prop.major != 10) return DDF_E_UNSUPPORTED;
+  Trainer* T = new (std::nothrow) Trainer();
+  if (!T) return DDF_E_NOMEM;
+  memset(T, 0, sizeof(Trainer));
+  T->lay = *layout; T->prm = *params; T->entries = entries; T->n_table = entries * 2;
+  const ddf_hashgrid_layout& L = T->lay;
+  const int NF = (int)L.n_levels * 2, E = NF + 3 + 6 * (int)L.n_freq_dir, H = (int)L.n_hidden;
+  TrParams& p = T->base;
+  int off = 0, nin = E;
+  for (int l = 0; l < H; ++l) { p.w_off[l] = off; off += kTrW * nin; p.b_off[l] = off; off += kTrW; nin = kTrW; }
+  p.w_off[H] = off; off += 2 * kTrW; p.b_off[H] = off; off += 2;
+  T->n_mlp = off;
+  const size_t total = (size_t)(T->n_table + T->n_mlp);
+  cudaError_t e;
+  auto fail = [&](cudaError_t err) { g_last_cuda_error = (int)err; (void)cudaGetLastError(); tr_free(T); return err == cudaErrorMemoryAllocation ? DDF_E_NOMEM : DDF_E_CUDA; };
+  if ((e = cudaMalloc(&T->p_table, (size_t)T->n_table * 4)) != cudaSuccess || (e = cudaMalloc(&T->p_mlp, (size_t)T->n_mlp * 4)) != cudaSuccess ||
+      (e = cudaMalloc(&T->m, total * 4)) != cudaSuccess || (e = cudaMalloc(&T->v, total * 4)) != cudaSuccess ||
+      (e = cudaMalloc(&T->g, total * 4)) != cudaSuccess || (e = cudaMalloc(&T->loss_dev, 4)) != cudaSuccess ||
+      (e = cudaMemcpy(T->p_table, table, (size_t)T->n_table * 4, cudaMemcpyHostToDevice)) != cudaSuccess ||
+      (e = cudaMemcpy(T->p_mlp, mlp, (size_t)T->n_mlp * 4, cudaMemcpyHostToDevice)) != cudaSuccess ||
+      (e = cudaMemset(T->m, 0, total * 4)) != cudaSuccess || (e = cudaMemset(T->v, 0, total * 4)) != cudaSuccess ||
+      (e = cudaMemset(T->g, 0, total * 4)) != cudaSuccess)
+    return fail(e);
+  // level table: the same sizing rule as ddf_create_hashgrid (readings H1, H4)
+  {
+    const int64_t Tn = (int64_t)1 << L.log2_table_size;
+    int64_t o2 = 0;
+    for (uint32_t l = 0; l < L.n_levels; ++l) {
+      const double nd = floor((double)L.base_resolution * pow((double)L.growth, (double)l));
+      const int64_t N = (int64_t)nd, V = N + 1;
+      const bool dense = V <= 1024 && V * V * V <= Tn;
+      p.lv[l].scale = (float)N; p.lv[l].verts = (uint32_t)V; p.lv[l].hashed = dense ? 0u : 1u; p.lv[l].offset = (uint32_t)o2;
+      o2 += dense ? V * V * V : Tn;
+    }
+  }
+  p.table = T->p_table; p.mlp = T->p_mlp; p.g_table = T->g; p.g_mlp = T->g + T->n_table; p.loss = T->loss_dev;
+  for (int a = 0; a < 3; ++a) { p.bmin[a] = L.box_min[a]; p.den[a] = L.box_max[a] - L.box_min[a]; }
+  p.dist_clamp = params->dist_clamp; p.ce_weight = params->ce_weight;
+  p.tmask = (1u << L.log2_table_size) - 1u;
+  p.n_levels = (int)L.n_levels; p.Ld = (int)L.n_freq_dir; p.n_hidden = H; p.E = E; p.NF = NF;
+  T->smem_bytes = (size_t)((E + (H - 1) * kTrW) * kTrW + H * kTrW + 2 * kTrW + (H + 3) * kTrW * kTrPitch) * 4;
+  if ((e = cudaFuncSetAttribute(train_fwd_bwd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T->smem_bytes)) != cudaSuccess) return fail(e);
+  if ((e = cudaDeviceSynchronize()) != cudaSuccess) return fail(e);
+  *out = reinterpret_cast<ddf_trainer*>(T);
+  return DDF_OK;
+}
+
+extern "C" int ddf_trainer_destroy(ddf_trainer* trainer) {
+  if (!trainer) return DDF_OK;
+  cudaDeviceSynchronize();
+  tr_free(reinterpret_cast<Trainer*>(trainer));
+  return DDF_OK;
+}
+
+extern "C" int64_t ddf_trainer_steps(const ddf_trainer* trainer) {
+  return trainer ? reinterpret_cast<const Trainer*>(trainer)->step : (int64_t)DDF_E_INVALID_ARG;
+}
+
+static int tr_launch_grads(Trainer* T, const float* o, const float* d, const float* t, const uint8_t* hit, int64_t n, cudaStream_t st) {
+  TrParams p = T->base;
+  p.o = o; p.d = d; p.t = t; p.hit = hit; p.n = n;
+  DDF_CUDA_TRY(cudaMemsetAsync(T->loss_dev, 0, 4, st));
+  const int64_t tiles = (n + kTrThreads - 1) / kTrThreads;
+  int sms = 0; DDF_CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, 0));
+  const unsigned grid = (unsigned)(tiles < sms ? tiles : sms);
+  train_fwd_bwd_kernel<<<grid, kTrThreads, T->smem_bytes, st>>>(p);
+  DDF_CUDA_TRY(cudaGetLastError());
+  return DDF_OK;
+}
+
+extern "C" int ddf_trainer_loss_grads(ddf_trainer* trainer, const float* o, const float* d, const float* t,
+                                      const uint8_t* hit, int64_t n, float* loss, float* grad_table,
+                                      float* grad_mlp, void* stream) {
+  if (!trainer || n <= 0 || !o || !d || !t || !hit) return DDF_E_INVALID_ARG;
+  Trainer* T = reinterpret_cast<Trainer*>(trainer);
+  cudaStream_t st = (cudaStream_t)stream;
+  const size_t total = (size_t)(T->n_table + T->n_mlp);
+  int rc = tr_launch_grads(T, o, d, t, hit, n, st);
+  if (rc != DDF_OK) return rc;
+  if (loss) DDF_CUDA_TRY(cudaMemcpyAsync(loss, T->loss_dev, 4, cudaMemcpyDeviceToDevice, st));
+  if (grad_table) DDF_CUDA_TRY(cudaMemcpyAsync(grad_table, T->g, (size_t)T->n_table * 4, cudaMemcpyDeviceToDevice, st));
+  if (grad_mlp) DDF_CUDA_TRY(cudaMemcpyAsync(grad_mlp, T->g + T->n_table, (size_t)T->n_mlp * 4, cudaMemcpyDeviceToDevice, st));
+  DDF_CUDA_TRY(cudaMemsetAsync(T->g, 0, total * 4, st));            // leave the accumulator clean: no update happened
+  return DDF_OK;
+}
+
+extern "C" int ddf_trainer_step(ddf_trainer* trainer, const float* o, const float* d, const float* t,
+                                const uint8_t* hit, int64_t n, float* loss, void* stream) {
+  if (!trainer || n <= 0 || !o || !d || !t || !hit) return DDF_E_INVALID_ARG;
+  Trainer* T = reinterpret_cast<Trainer*>(trainer);
+  cudaStream_t st = (cudaStream_t)stream;
+  int rc = tr_launch_grads(T, o, d, t, hit, n, st);
+  if (rc != DDF_OK) return rc;
+  if (loss) DDF_CUDA_TRY(cudaMemcpyAsync(loss, T->loss_dev, 4, cudaMemcpyDeviceToDevice, st));
+  const ddf_train_params& P = T->prm;
+  // reading T4 (schedule evaluated at the 0-based step) and T3 (1-based Adam step), in double on the host
+  const double s0 = (double)(T->step < P.total_steps ? T->step : P.total_steps);
+  const double f = P.lr_final_frac;
+  const double lr = (double)P.lr0 * (f + (1.0 - f) * 0.5 * (1.0 + cos(3.14159265358979323846 * s0 / (double)P.total_steps)));
+  const int64_t s1 = T->step + 1;
+  const double c1 = 1.0 - pow((double)P.beta1, (double)s1), c2 = 1.0 - pow((double)P.beta2, (double)s1);
+  adam_kernel<<<148 * 8, 256, 0, st>>>(T->p_table, T->m, T->v, T->g, T->n_table, (float)lr, P.beta1, P.beta2, P.adam_eps, (float)c1, (float)c2);
+  adam_kernel<<<8, 256, 0, st>>>(T->p_mlp, T->m + T->n_table, T->v + T->n_table, T->g + T->n_table, T->n_mlp, (float)lr, P.beta1, P.beta2, P.adam_eps, (float)c1, (float)c2);
+  DDF_CUDA_TRY(cudaGetLastError());
+  T->step = s1;
+  return DDF_OK;
+}
+
+extern "C" int ddf_trainer_export(ddf_trainer* trainer, float* table, float* mlp) {
+  if (!trainer || !table || !mlp) return DDF_E_INVALID_ARG;
+  Trainer* T = reinterpret_cast<Trainer*>(trainer);
+  DDF_CUDA_TRY(cudaDeviceSynchronize());
+  DDF_CUDA_TRY(cudaMemcpy(table, T->p_table, (size_t)T->n_table * 4, cudaMemcpyDeviceToHost));
+  DDF_CUDA_TRY(cudaMemcpy(mlp, T->p_mlp, (size_t)T->n_mlp * 4, cudaMemcpyDeviceToHost));
+  return DDF_OK;
+}
