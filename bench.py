@@ -306,6 +306,12 @@ def run_extras(ddf, torch, model, peaks):
                                       "hit_rate": float(hit.float().mean()), "TFLOPs": evals * SDF_FLOP / (ms * 1e-3) / 1e12,
                                       "ddf_speedup": ms / ddf_ms}
     ex["ddf_camera_2^20_ms"] = ddf_ms
+    # "across convergence thresholds": the early-exit tracer at three hit thresholds
+    for eps in (1e-2, 1e-4):
+        prm = ddf.SdfTraceParams(64, eps, 6.0, 1.0, 0.05, 1)
+        ms = _time_ms(torch, lambda: ddf.sdf_sphere_trace(sdf, o, d, n, prm, t, hit, st, None, None, tot), reps=2)
+        ex["sphere_trace_early_exit_eps%g" % eps] = {"ms": ms, "mlp_evals": int(tot.item()), "mean_steps": float(st.float().mean()),
+                                                     "hit_rate": float(hit.float().mean()), "ddf_speedup": ms / ddf_ms}
     ddf.ddf_destroy(sdf)
     del o, d, t, hit, st, dist, vis
     ex["hashgrid_field"] = run_hashgrid(ddf, torch, peaks)
@@ -375,6 +381,28 @@ def run_training(ddf, torch, steps=30000, batch=16384):
     out["shadow_fraction_ground_truth"] = float(gt_shadow.float().mean())
     mse = float((((ds > 0).float() - gt_shadow.float()) ** 2).mean())
     out["shadow_mask_psnr_db"] = float(-10.0 * np.log10(max(mse, 1e-12)))
+    # ambient occlusion over the same G-buffer: 16 cosine samples per pixel, "average the hit flag"
+    gp = (po[pix] + gt_t[pix][:, None] * pd[pix]).contiguous()
+    on_sphere = (gp.norm(dim=1) - 0.5).abs() < 1e-4
+    bmin = torch.tensor((-0.9, -0.9, -0.9), device="cuda"); bmax = torch.tensor((0.9, 0.9, -0.6), device="cuda")
+    dlo, dhi = (gp - bmin[None, :]).abs(), (gp - bmax[None, :]).abs()
+    face = torch.cat([dlo, dhi], dim=1).argmin(dim=1)                     # 0..2: min faces, 3..5: max faces
+    gn = torch.zeros_like(gp)
+    gn[torch.arange(k, device="cuda"), face % 3] = torch.where(face < 3, -1.0, 1.0)
+    gn[on_sphere] = gp[on_sphere] / gp[on_sphere].norm(dim=1, keepdim=True)
+    gn = gn.contiguous()
+    spp = 16
+    ao_o = torch.empty((k * spp, 3), device="cuda"); ao_d = torch.empty((k * spp, 3), device="cuda")
+    ddf.ddf_gen_ao(gp, gn, k, spp, MASTER_SEED, STREAMS["ao_samples"], 2e-3, ao_o, ao_d)
+    at = torch.empty(k * spp, device="cuda"); ah = torch.empty(k * spp, dtype=torch.uint8, device="cuda")
+    ddf.ddf_scene_raycast(scene, ao_o, ao_d, k * spp, at, ah)
+    ao_gt = 1.0 - ah.view(k, spp).float().mean(dim=1)
+    ao = torch.empty(k, device="cuda")
+    ddf.ddf_query_ao(m, ao_o, ao_d, k, spp, float("inf"), ao)
+    out["ao_mae"] = float((ao - ao_gt).abs().mean())
+    out["ao_psnr_db"] = float(-10.0 * np.log10(max(float(((ao - ao_gt) ** 2).mean()), 1e-12)))
+    out["ao_mean_ground_truth"] = float(ao_gt.mean())
+    out["paper_context_metrics"] = "shadows 30.3 dB, AO 21.3 dB, AO MAE 0.216 over 142 scanned objects vs Embree (PAPER.md:248-256)"
     # primary rays from the camera itself (one shared origin: only the 27-dim direction code varies)
     pdist = torch.empty(n, device="cuda"); pvis = torch.empty(n, device="cuda")
     ddf.ddf_query(m, po, pd, n, pdist, pvis)
