@@ -130,3 +130,32 @@ def test_hashgrid_host_logic_without_gpu(libddf, orc):
     assert libddf.ddf_create_hashgrid(w.ctypes.data_as(C.c_void_p), w.ctypes.data_as(C.c_void_p), C.byref(wide), C.byref(h)) == -3
     with pytest.raises(DdfError):
         ddf_hashgrid_table_entries(HashLayout(n_out=5))
+
+
+def test_trainer_and_wavefront_argument_errors_without_gpu(libddf):
+    """struct sizes and the argument checks of the training / wavefront entry points that run before
+    any CUDA call"""
+    from ddf_inputs import HashLayout, layout_hash_paper
+    from paper_2606_00817_b200 import DdfTrainParams, make_train_params, make_hashgrid_layout, DdfScene
+    assert C.sizeof(DdfTrainParams) == 36
+    h = C.c_void_p(0)
+    w = np.zeros(16, np.float32); wp = w.ctypes.data_as(C.c_void_p)
+    L = make_hashgrid_layout(layout_hash_paper()); P = make_train_params()
+    assert libddf.ddf_trainer_create(None, wp, C.byref(L), C.byref(P), C.byref(h)) == -1
+    bad = make_train_params(); bad.struct_size = 3
+    assert libddf.ddf_trainer_create(wp, wp, C.byref(L), C.byref(bad), C.byref(h)) == -2
+    assert libddf.ddf_trainer_create(wp, wp, C.byref(L), C.byref(make_train_params(lr0=-1.0)), C.byref(h)) == -1
+    assert libddf.ddf_trainer_create(wp, wp, C.byref(L), C.byref(make_train_params(beta2=1.0)), C.byref(h)) == -1
+    f16 = make_hashgrid_layout(HashLayout(table_dtype=2))                 # training wants fp32 master copies
+    assert libddf.ddf_trainer_create(wp, wp, C.byref(f16), C.byref(P), C.byref(h)) == -2
+    deep = make_hashgrid_layout(HashLayout(n_hidden=3))
+    assert libddf.ddf_trainer_create(wp, wp, C.byref(deep), C.byref(P), C.byref(h)) == -3
+    assert libddf.ddf_trainer_destroy(None) == 0 and libddf.ddf_trainer_steps(None) == -1
+    assert libddf.ddf_trainer_step(None, None, None, None, None, C.c_int64(4), None, None) == -1
+    sc = DdfScene((0.0, 0.0, 0.0), 0.5, (-0.9, -0.9, -0.9), (0.9, 0.9, -0.6))
+    assert libddf.ddf_scene_raycast(C.byref(sc), None, None, C.c_int64(0), None, None, None) == 0
+    assert libddf.ddf_scene_raycast(C.byref(sc), None, None, C.c_int64(5), None, None, None) == -1
+    assert libddf.ddf_gen_train_batch(C.byref(sc), C.c_uint64(1), C.c_uint64(1), C.c_int64(-1), C.c_int64(4), C.c_float(2.0), None, None, None, None, None) == -1
+    li = (C.c_float * 3)(1, 2, 3)
+    assert libddf.ddf_query_shadowed(None, None, None, C.c_int64(4), li, C.c_float(1e-3), None, None, None, None, None) == -1
+    assert libddf.ddf_gen_shadow_from_hits(None, None, None, None, None, C.c_int64(4), li, C.c_float(1e-3), None, None, None, None, None, None) == -1
