@@ -317,7 +317,33 @@ def run_extras(ddf, torch, model, peaks):
     ex["hashgrid_field"] = run_hashgrid(ddf, torch, peaks)
     ex["wavefront_shadowed_camera_2^20"] = run_wavefront(ddf, torch)
     ex["training_hashgrid"] = run_training(ddf, torch)
+    ex["narrow_networks_2^20_random_rays"] = run_narrow(ddf, torch)
     return ex
+
+
+def run_narrow(ddf, torch):
+    """BASELINE.json configs[0] (3 x 64, 54-dim input) and the paper's own sinusoidal MLPs of its encoding
+    ablation (128 x 4 and 256 x 6; band counts as configs[1]) on 2^20 random rays.
+    Widths 64 / 128 run on the shared-memory-resident tcgen05 kernel (ddf_narrow.cu), 256 on the
+    persistent kernel of the headline config."""
+    from ddf_inputs import Layout, layout_c0, make_weights, random_rays, blob_layer_shapes
+    n = 1 << 20
+    o_np, d_np = random_rays(n)
+    o = torch.from_numpy(o_np).cuda(); d = torch.from_numpy(d_np).cuda()
+    dist = torch.empty(n, device="cuda"); vis = torch.empty(n, device="cuda")
+    out = {}
+    for name, lay in (("configs[0]_64x3", layout_c0()), ("paper_128x4", Layout(0, 10, 4, 4, 128, -1, 2, 0)),
+                      ("paper_256x6", Layout(0, 10, 4, 6, 256, -1, 2, 0))):
+        m = ddf.ddf_create(make_weights(lay), lay)
+        ms = _time_ms(torch, lambda: ddf.ddf_query(m, o, d, n, dist, vis), reps=7)
+        flop = 2 * sum(a * b for a, b in blob_layer_shapes(lay))
+        out[name] = {"ms": ms, "Mrays_s": n / ms / 1e3, "TFLOPs": n * flop / (ms * 1e-3) / 1e12, "flop_per_ray": flop,
+                     "launches": ddf.ddf_get_info(m, 1), "tcgen05": ddf.ddf_get_info(m, 0)}
+        ddf.ddf_set_path(m, 1)
+        ms1 = _time_ms(torch, lambda: ddf.ddf_query(m, o, d, n, dist, vis), reps=3)
+        out[name]["cuda_core_path_ms"] = ms1
+        ddf.ddf_destroy(m)
+    return out
 
 
 def run_training(ddf, torch, steps=30000, batch=16384):

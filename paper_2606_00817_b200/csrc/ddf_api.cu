@@ -30,6 +30,7 @@ static int check_layout(const ddf_layout* L) {
 static void free_model(Model* m) {
   if (!m) return;
   tc_plan_destroy(m);
+  narrow_plan_destroy(m);
   hash_plan_destroy(m);
   cudaFree(m->d_w); cudaFree(m->d_b); cudaFree(m->d_head_w);
   cudaFree(m->ws_gamma); cudaFree(m->ws_act0); cudaFree(m->ws_act1); cudaFree(m->ws_last);
@@ -142,6 +143,10 @@ extern "C" int ddf_create(const void* weights, const ddf_layout* layout, ddf_mod
   }
   rc = tc_plan_create(m);
   if (rc != DDF_OK) { free_model(m); return rc; }
+  if (!m->tc) {
+    rc = narrow_plan_create(m, hw.data(), hb.data());
+    if (rc != DDF_OK) { free_model(m); return rc; }
+  }
   DDF_CUDA_TRY(cudaDeviceSynchronize());
   *out = reinterpret_cast<ddf_model*>(m);
   return DDF_OK;
@@ -158,7 +163,7 @@ extern "C" int ddf_set_path(ddf_model* model, int path) {
   if (!model || path < 0 || path > 2) return DDF_E_INVALID_ARG;
   Model* m = reinterpret_cast<Model*>(model);
   if (m->hg) return path == 0 ? DDF_OK : DDF_E_UNSUPPORTED;
-  if (path == 2 && !m->tc) return DDF_E_UNSUPPORTED;
+  if (path == 2 && !m->tc && !m->nw) return DDF_E_UNSUPPORTED;
   m->path = path;
   return DDF_OK;
 }
@@ -167,10 +172,10 @@ extern "C" int64_t ddf_get_info(const ddf_model* model, int which) {
   if (!model) return DDF_E_INVALID_ARG;
   const Model* m = reinterpret_cast<const Model*>(model);
   switch (which) {
-    case 0: return (m->hg || (m->tc && m->path != 1)) ? 1 : 0;
+    case 0: return has_fused_path(m) ? 1 : 0;
     case 1: return m->last_launches;
     case 2: return m->E;
-    case 3: return m->hg ? 128 : ((m->tc && m->path != 1) ? 256 : 64);
+    case 3: return m->hg ? 128 : ((m->tc && m->path != 1) ? 256 : ((m->nw && m->path != 1) ? 128 : 64));
     default: return DDF_E_INVALID_ARG;
   }
 }
@@ -181,8 +186,7 @@ static int run_query(Model* m, const float* o, const float* d, int64_t n, int mo
   if (n == 0) { m->last_launches = 0; return DDF_OK; }
   if (!o || !out0 || (m->lay.input_kind == 0 && !d)) return DDF_E_INVALID_ARG;
   cudaStream_t st = (cudaStream_t)stream;
-  if (m->hg) return hash_forward(m, o, d, n, nullptr, mode_out, out0, out1, 0, 0.0f, st);
-  if (m->tc && m->path != 1) return tc_forward(m, o, d, n, nullptr, mode_out, out0, out1, 0, 0.0f, st);
+  if (has_fused_path(m)) return fused_forward(m, o, d, n, nullptr, mode_out, out0, out1, 0, 0.0f, st);
   return simt_forward(m, o, d, n, mode_out, out0, out1, st);
 }
 
@@ -233,10 +237,8 @@ extern "C" int ddf_query_ao(ddf_model* model, const float* o, const float* d, in
   if (!o || !d || !ao || m->lay.n_out != 2 || m->lay.input_kind != 0) return DDF_E_INVALID_ARG;
   const int64_t n = n_pts * spp;
   cudaStream_t st = (cudaStream_t)stream;
-  if (m->hg && spp <= 32 && 32 % spp == 0)
-    return hash_forward(m, o, d, n, nullptr, 2, ao, nullptr, spp, ao_radius, st);
-  if (m->tc && m->path != 1 && spp <= 32 && 32 % spp == 0)   // a pixel's rays sit in one warp of a tile
-    return tc_forward(m, o, d, n, nullptr, 2, ao, nullptr, spp, ao_radius, st);
+  if (has_fused_path(m) && spp <= 32 && 32 % spp == 0)          // a pixel's rays sit in one warp of a tile
+    return fused_forward(m, o, d, n, nullptr, 2, ao, nullptr, spp, ao_radius, st);
   if (n > m->ws_out_rows) {
     cudaFree(m->ws_dist); cudaFree(m->ws_vis); m->ws_dist = m->ws_vis = nullptr; m->ws_out_rows = 0;
     DDF_CUDA_TRY(cudaMalloc(&m->ws_dist, (size_t)n * 4));

@@ -39,6 +39,7 @@ struct LayerDesc {
 
 struct TcPlan;          // tcgen05 path state (ddf_tc.cu)
 struct HashPlan;        // hash-grid field state (ddf_hash.cu)
+struct NarrowPlan;      // tcgen05 path for narrow networks (ddf_narrow.cu)
 
 struct Model {
   ddf_layout lay;
@@ -66,6 +67,7 @@ struct Model {
   void* wave_ws; size_t wave_ws_bytes;
   int path;                        // 0 auto, 1 SIMT, 2 tcgen05
   TcPlan* tc;                      // non-null when the tcgen05 path can serve the layout
+  NarrowPlan* nw;                  // non-null when the narrow tcgen05 path (width 64 / 128, weights in smem) serves it
   HashPlan* hg;                    // non-null: this model is a hash-grid field (ddf_create_hashgrid)
   int sm_count;
   int last_launches;
@@ -87,6 +89,21 @@ int tc_forward(Model* m, const float* o, const float* d, int64_t n, const int64_
 void hash_plan_destroy(Model* m);
 int hash_forward(Model* m, const float* o, const float* d, int64_t n, const int64_t* n_dev, int mode_out,
                  float* out0, float* out1, int spp, float ao_radius, cudaStream_t st);
+
+// ---- narrow-network tcgen05 path (ddf_narrow.cu)
+int narrow_plan_create(Model* m, const uint16_t* hw_host, const float* hb_host);   // sets m->nw or leaves it null
+void narrow_plan_destroy(Model* m);
+int narrow_forward(Model* m, const float* o, const float* d, int64_t n, const int64_t* n_dev, int mode_out,
+                   float* out0, float* out1, int spp, float ao_radius, cudaStream_t st);
+
+// one dispatch for every fused path: tcgen05 wide, tcgen05 narrow, hash grid (n_dev: device-side count or null)
+inline bool has_fused_path(const Model* m) { return m->hg || ((m->tc || m->nw) && m->path != 1); }
+inline int fused_forward(Model* m, const float* o, const float* d, int64_t n, const int64_t* n_dev, int mode_out,
+                         float* out0, float* out1, int spp, float ao_radius, cudaStream_t st) {
+  if (m->hg) return hash_forward(m, o, d, n, n_dev, mode_out, out0, out1, spp, ao_radius, st);
+  if (m->tc) return tc_forward(m, o, d, n, n_dev, mode_out, out0, out1, spp, ao_radius, st);
+  return narrow_forward(m, o, d, n, n_dev, mode_out, out0, out1, spp, ao_radius, st);
+}
 
 // ---- device helpers -------------------------------------------------------------------------
 #ifdef __CUDACC__

@@ -107,7 +107,7 @@ extern "C" int sdf_sphere_trace(ddf_model* model, const float* o, const float* d
   trace_init_kernel<<<nb, 256, 0, st>>>(n, out_t, out_hit, out_steps, w.done, w.idx[0], w.counts, S + 2,
                                         trace_p, trace_s, S);
   int launches = 1;
-  const bool use_tc = (m->tc && m->path != 1);
+  const bool use_tc = has_fused_path(m);
   int64_t live = n;
   for (int step = 0; step < S; ++step) {
     const int cur = prm->early_exit ? (step & 1) : 0;
@@ -116,7 +116,7 @@ extern "C" int sdf_sphere_trace(ddf_model* model, const float* o, const float* d
     const unsigned gb = (unsigned)((live + 255) / 256);
     trace_points_kernel<<<gb, 256, 0, st>>>(w.idx[cur], cnt_in, o, d, out_t, w.pts, w.counts + S + 1);
     int rc;
-    if (use_tc) rc = tc_forward(m, w.pts, nullptr, live, cnt_in, 1, w.z, nullptr, 0, 0.0f, st);
+    if (use_tc) rc = fused_forward(m, w.pts, nullptr, live, cnt_in, 1, w.z, nullptr, 0, 0.0f, st);
     else rc = simt_forward(m, w.pts, nullptr, live, 1, w.z, nullptr, st);
     if (rc != DDF_OK) return rc;
     launches += 1 + m->last_launches;

@@ -166,8 +166,7 @@ extern "C" int ddf_query_shadowed(ddf_model* model, const float* o, const float*
   launches += 3;
   DDF_CUDA_TRY(cudaMemsetAsync(out_lit, 0, (size_t)n, st));
   // 3. second query on the compacted batch; the fused paths read its size on the device
-  if (m->hg) rc = hash_forward(m, w.o2, w.d2, n, w.count, 0, w.dist2, w.vis2, 0, 0.0f, st);
-  else if (m->tc && m->path != 1) rc = tc_forward(m, w.o2, w.d2, n, w.count, 0, w.dist2, w.vis2, 0, 0.0f, st);
+  if (has_fused_path(m)) rc = fused_forward(m, w.o2, w.d2, n, w.count, 0, w.dist2, w.vis2, 0, 0.0f, st);
   else {
     int64_t live = 0;                                    // the SIMT path sizes its grids on the host
     DDF_CUDA_TRY(cudaMemcpyAsync(&live, w.count, 8, cudaMemcpyDeviceToHost, st));

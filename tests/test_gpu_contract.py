@@ -49,7 +49,7 @@ def _blob(lay, layers):
 
 # ------------------------------------------------------------------ closed forms on the GPU
 
-@pytest.mark.parametrize("width", [64, 256])            # SIMT path / tcgen05 path
+@pytest.mark.parametrize("width", [32, 64, 128, 256])   # SIMT / narrow tcgen05 x2 / wide tcgen05 path
 def test_zero_weights_give_head_of_bias(ddf, width):
     lay = Layout(0, 4, 4, 3, width, 1, 2, 0)
     blob = np.zeros(blob_num_elements(lay), np.float32)
@@ -65,7 +65,7 @@ def test_zero_weights_give_head_of_bias(ddf, width):
     assert np.allclose(dist, math.log(2.0), rtol=2e-7) and np.all(vis == 0.5)
 
 
-@pytest.mark.parametrize("width", [64, 256])
+@pytest.mark.parametrize("width", [32, 64, 128, 256])
 def test_all_ones_layer_exposes_pad_lanes(ddf, orc, width):
     """P4 shape: W0 = all ones => every hidden unit = ReLU(sum gamma); K = 90 is padded to 128 on
     the GPU, so any pad lane that is not zero changes the sum."""
@@ -190,18 +190,25 @@ def test_bad_arguments(ddf, c1):
     assert lib().ddf_query(m.handle, None, None, C.c_int64(0), None, None, _stream(None)) == 0
     bad = Layout(0, 10, 4, 8, 1280, 4, 2, 1)
     with pytest.raises(ddf.DdfError):
-        ddf.ddf_set_path(ddf.ddf_create(make_weights(layout_c0()), layout_c0()), 2)   # width 64: no tcgen05 plan
+        w96 = Layout(0, 4, 4, 3, 96, -1, 2, 0)
+        ddf.ddf_set_path(ddf.ddf_create(make_weights(w96), w96), 2)   # width 96: no tcgen05 plan, SIMT only
     prm = ddf.SdfTraceParams(64, 1e-3, 6.0, 1.0, 0.05, 0)
     t = torch.zeros(4, device="cuda"); h = torch.zeros(4, dtype=torch.uint8, device="cuda"); s = torch.zeros(4, dtype=torch.int32, device="cuda")
     with pytest.raises(ddf.DdfError):
         ddf.sdf_sphere_trace(m, x, x, 4, prm, t, h, s)         # a DDF model is not an SDF model
 
 
-def test_simt_and_tcgen05_paths_agree(ddf, orc):
-    lay = Layout(0, 6, 3, 4, 512, 2, 2, 1)
+@pytest.mark.parametrize("lay", [Layout(0, 6, 3, 4, 512, 2, 2, 1), Layout(0, 6, 3, 4, 128, 2, 2, 0), Layout(0, 4, 4, 3, 64, -1, 2, 1),
+                                 Layout(1, 10, 0, 5, 128, 3, 1, 1)])
+def test_simt_and_tcgen05_paths_agree(ddf, orc, lay):
+    """wide tcgen05 kernel, narrow tcgen05 kernel (width 128 with skip / width 64 / point input with
+    one linear output) against the plain CUDA-core path and both oracle modes"""
     blob = make_weights(lay, seed=17, bias_scale=0.2)
     m = ddf.ddf_create(blob, lay)
+    assert ddf.ddf_get_info(m, 0) == 1
     o, d = random_rays(2000, seed=5)
+    if lay.input_kind == 1:
+        d = None
     ddf.ddf_set_path(m, 2); z_tc = _logits(ddf, m, o, d); assert ddf.ddf_get_info(m, 1) == 1
     ddf.ddf_set_path(m, 1); z_si = _logits(ddf, m, o, d); assert ddf.ddf_get_info(m, 1) > 1
     zq, _, _ = orc.forward(lay, blob, o, d, mode=1)
