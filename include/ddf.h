@@ -81,6 +81,10 @@ int  ddf_create(const void* weights, const ddf_layout* layout, ddf_model** out);
 int  ddf_destroy(ddf_model* model);                       /* NULL is DDF_OK */
 const char* ddf_status_string(int status);
 int  ddf_last_cuda_error(void);                           /* cudaError_t of the last DDF_E_CUDA on this thread */
+/* Which kernel serves a layout: width a multiple of 256 (up to 2048): the persistent tcgen05 kernel;
+ * width 64 or 128 with a weight set that fits in shared memory: the shared-memory-resident tcgen05
+ * kernel; any other width up to 2048 is zero-padded at create to the next such width (padded units
+ * have zero weights and bias, so every result is unchanged); everything else: the CUDA-core path. */
 /* kernel selection: 0 = automatic (tcgen05 path when the layout allows, else the SIMT path),
  * 1 = force the SIMT path, 2 = force the tcgen05 path (DDF_E_UNSUPPORTED if it cannot run). */
 int  ddf_set_path(ddf_model* model, int path);

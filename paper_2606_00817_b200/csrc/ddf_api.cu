@@ -59,11 +59,70 @@ extern "C" const char* ddf_status_string(int s) {
 
 extern "C" int ddf_last_cuda_error(void) { return g_last_cuda_error; }
 
+// Widths the tensor-core kernels do not tile (not 64 / 128 / a multiple of 256) are served by
+// padding the network with zero units up to the next such width: a padded unit has zero weights
+// and zero bias, so it outputs ReLU(0) = 0 and multiplies zero weights in the next layer - every
+// real accumulation sees the same terms in the same order.  Returns 0 when no padding applies.
+static uint32_t padded_width(uint32_t w) {
+  if (w == 64 || w == 128 || w % 256 == 0) return 0;
+  if (w < 64) return 64;
+  if (w < 128) return 128;
+  const uint32_t up = (w + 255) / 256 * 256;
+  return up <= 2048 ? up : 0;
+}
+
+static void pad_blob(const ddf_layout& L, const uint8_t* src, uint32_t w_new, std::vector<uint8_t>* dst) {
+  const size_t esz = L.weight_dtype == 1 ? 2 : 4;
+  const size_t E = 3 + 6 * (size_t)L.n_freq_origin + (L.input_kind == 0 ? 3 + 6 * (size_t)L.n_freq_dir : 0);
+  const size_t W = L.width, Wn = w_new;
+  size_t total = 0;
+  for (uint32_t l = 0; l <= L.n_hidden; ++l) {
+    const bool head = l == L.n_hidden;
+    const size_t k0n = l == 0 ? E : Wn, k1 = ((int32_t)l == L.skip_layer) ? E : 0;
+    total += (head ? L.n_out : Wn) * (k0n + k1 + 1);
+  }
+  dst->assign(total * esz, 0);
+  size_t so = 0, dofs = 0;
+  for (uint32_t l = 0; l <= L.n_hidden; ++l) {
+    const bool head = l == L.n_hidden;
+    const size_t k0 = l == 0 ? E : W, k0n = l == 0 ? E : Wn, k1 = ((int32_t)l == L.skip_layer) ? E : 0;
+    const size_t rows = head ? L.n_out : W, rows_n = head ? L.n_out : Wn;
+    for (size_t j = 0; j < rows; ++j) {
+      memcpy(dst->data() + (dofs + j * (k0n + k1)) * esz, src + (so + j * (k0 + k1)) * esz, k0 * esz);
+      if (k1) memcpy(dst->data() + (dofs + j * (k0n + k1) + k0n) * esz, src + (so + j * (k0 + k1) + k0) * esz, k1 * esz);
+    }
+    so += rows * (k0 + k1); dofs += rows_n * (k0n + k1);
+    memcpy(dst->data() + dofs * esz, src + so * esz, rows * esz);           // biases
+    so += rows; dofs += rows_n;
+  }
+}
+
+static int create_impl(const void* weights, const ddf_layout* layout, ddf_model** out);
+
 extern "C" int ddf_create(const void* weights, const ddf_layout* layout, ddf_model** out) {
   if (out) *out = nullptr;
   if (!weights || !layout || !out) return DDF_E_INVALID_ARG;
   int rc = check_layout(layout);
   if (rc != DDF_OK) return rc;
+  const uint32_t w_new = padded_width(layout->width);
+  if (w_new == 0) return create_impl(weights, layout, out);
+  const ddf_layout& L = *layout;
+  const size_t esz = L.weight_dtype == 1 ? 2 : 4;
+  const size_t E = 3 + 6 * (size_t)L.n_freq_origin + (L.input_kind == 0 ? 3 + 6 * (size_t)L.n_freq_dir : 0);
+  size_t elems = 0;
+  for (uint32_t l = 0; l <= L.n_hidden; ++l)
+    elems += (size_t)(l == L.n_hidden ? L.n_out : L.width) * ((l == 0 ? E : L.width) + ((int32_t)l == L.skip_layer ? E : 0) + 1);
+  std::vector<uint8_t> host(elems * esz), padded;
+  if (L.weights_on_device) DDF_CUDA_TRY(cudaMemcpy(host.data(), weights, elems * esz, cudaMemcpyDeviceToHost));
+  else memcpy(host.data(), weights, elems * esz);
+  pad_blob(L, host.data(), w_new, &padded);
+  ddf_layout Lp = L;
+  Lp.width = w_new; Lp.weights_on_device = 0;
+  return create_impl(padded.data(), &Lp, out);
+}
+
+static int create_impl(const void* weights, const ddf_layout* layout, ddf_model** out) {
+  int rc;
   int dev = 0; cudaDeviceProp prop;
   DDF_CUDA_TRY(cudaGetDevice(&dev));
   DDF_CUDA_TRY(cudaGetDeviceProperties(&prop, dev));

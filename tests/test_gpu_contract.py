@@ -49,12 +49,14 @@ def _blob(lay, layers):
 
 # ------------------------------------------------------------------ closed forms on the GPU
 
-@pytest.mark.parametrize("width", [32, 64, 128, 256])   # SIMT / narrow tcgen05 x2 / wide tcgen05 path
-def test_zero_weights_give_head_of_bias(ddf, width):
+@pytest.mark.parametrize("path", [0, 1])                # the fused kernel that serves the layout / the CUDA-core path
+@pytest.mark.parametrize("width", [32, 64, 128, 256])   # padded to 64 / narrow tcgen05 x2 / wide tcgen05 kernel
+def test_zero_weights_give_head_of_bias(ddf, width, path):
     lay = Layout(0, 4, 4, 3, width, 1, 2, 0)
     blob = np.zeros(blob_num_elements(lay), np.float32)
     blob[-2:] = [1.25, -0.5]
     m = ddf.ddf_create(blob, lay)
+    ddf.ddf_set_path(m, path)
     o, d = random_rays(300)
     dist, vis = _heads(ddf, m, o, d)
     assert np.allclose(dist, 1.25 + math.log1p(math.exp(-1.25)), rtol=2e-7)
@@ -65,14 +67,16 @@ def test_zero_weights_give_head_of_bias(ddf, width):
     assert np.allclose(dist, math.log(2.0), rtol=2e-7) and np.all(vis == 0.5)
 
 
+@pytest.mark.parametrize("path", [0, 1])
 @pytest.mark.parametrize("width", [32, 64, 128, 256])
-def test_all_ones_layer_exposes_pad_lanes(ddf, orc, width):
+def test_all_ones_layer_exposes_pad_lanes(ddf, orc, width, path):
     """P4 shape: W0 = all ones => every hidden unit = ReLU(sum gamma); K = 90 is padded to 128 on
     the GPU, so any pad lane that is not zero changes the sum."""
     lay = Layout(0, 10, 4, 1, width, -1, 2, 0)
     head = np.zeros((2, width)); head[0, :] = 1.0 / width; head[1, 0] = -0.25
     blob = _blob(lay, [(np.ones((width, 90)), np.zeros(width)), (head, [0, 1])])
     m = ddf.ddf_create(blob, lay)
+    ddf.ddf_set_path(m, path)
     o, d = random_rays(513)
     z = _logits(ddf, m, o, d)
     g = orc.encode(lay, o, d)
@@ -190,8 +194,8 @@ def test_bad_arguments(ddf, c1):
     assert lib().ddf_query(m.handle, None, None, C.c_int64(0), None, None, _stream(None)) == 0
     bad = Layout(0, 10, 4, 8, 1280, 4, 2, 1)
     with pytest.raises(ddf.DdfError):
-        w96 = Layout(0, 4, 4, 3, 96, -1, 2, 0)
-        ddf.ddf_set_path(ddf.ddf_create(make_weights(w96), w96), 2)   # width 96: no tcgen05 plan, SIMT only
+        wbig = Layout(0, 4, 4, 1, 2100, -1, 2, 0)
+        ddf.ddf_set_path(ddf.ddf_create(make_weights(wbig), wbig), 2)   # width 2100: beyond the padded tilings, CUDA-core path only
     prm = ddf.SdfTraceParams(64, 1e-3, 6.0, 1.0, 0.05, 0)
     t = torch.zeros(4, device="cuda"); h = torch.zeros(4, dtype=torch.uint8, device="cuda"); s = torch.zeros(4, dtype=torch.int32, device="cuda")
     with pytest.raises(ddf.DdfError):
@@ -199,7 +203,10 @@ def test_bad_arguments(ddf, c1):
 
 
 @pytest.mark.parametrize("lay", [Layout(0, 6, 3, 4, 512, 2, 2, 1), Layout(0, 6, 3, 4, 128, 2, 2, 0), Layout(0, 4, 4, 3, 64, -1, 2, 1),
-                                 Layout(1, 10, 0, 5, 128, 3, 1, 1)])
+                                 Layout(1, 10, 0, 5, 128, 3, 1, 1),
+                                 # widths the kernels do not tile are zero-padded at create (96 -> 128, 200 -> 256, 384 -> 512, 24 -> 64)
+                                 Layout(0, 6, 3, 3, 96, 1, 2, 0), Layout(0, 4, 4, 2, 200, -1, 2, 0), Layout(0, 10, 4, 4, 384, 2, 2, 1),
+                                 Layout(0, 2, 2, 2, 24, 1, 2, 0)])
 def test_simt_and_tcgen05_paths_agree(ddf, orc, lay):
     """wide tcgen05 kernel, narrow tcgen05 kernel (width 128 with skip / width 64 / point input with
     one linear output) against the plain CUDA-core path and both oracle modes"""
