@@ -104,7 +104,19 @@ extern "C" int ddf_create(const void* weights, const ddf_layout* layout, ddf_mod
   if (!weights || !layout || !out) return DDF_E_INVALID_ARG;
   int rc = check_layout(layout);
   if (rc != DDF_OK) return rc;
-  const uint32_t w_new = padded_width(layout->width);
+  uint32_t w_new = padded_width(layout->width);
+  {
+    // a narrow network whose weight set does not fit in shared memory (or whose encoding is wider
+    // than the narrow kernel's two K blocks) goes to the wide kernel instead, padded to 256
+    const uint32_t wt = w_new ? w_new : layout->width;
+    if (wt == 64 || wt == 128) {
+      const size_t E0 = 3 + 6 * (size_t)layout->n_freq_origin + (layout->input_kind == 0 ? 3 + 6 * (size_t)layout->n_freq_dir : 0);
+      const size_t gb = (E0 + 63) / 64, hb = wt / 64;
+      const size_t blocks = gb + (size_t)(layout->n_hidden - 1) * hb + (layout->skip_layer >= 1 ? gb : 0);
+      const size_t smem = (gb + hb) * 16384 + blocks * wt * 128 + (size_t)(layout->n_hidden + 2) * wt * 4 + 64 + 1024;
+      if (gb > 2 || smem > 232448) w_new = 256;
+    }
+  }
   if (w_new == 0) return create_impl(weights, layout, out);
   const ddf_layout& L = *layout;
   const size_t esz = L.weight_dtype == 1 ? 2 : 4;

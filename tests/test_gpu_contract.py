@@ -206,7 +206,9 @@ def test_bad_arguments(ddf, c1):
                                  Layout(1, 10, 0, 5, 128, 3, 1, 1),
                                  # widths the kernels do not tile are zero-padded at create (96 -> 128, 200 -> 256, 384 -> 512, 24 -> 64)
                                  Layout(0, 6, 3, 3, 96, 1, 2, 0), Layout(0, 4, 4, 2, 200, -1, 2, 0), Layout(0, 10, 4, 4, 384, 2, 2, 1),
-                                 Layout(0, 2, 2, 2, 24, 1, 2, 0)])
+                                 Layout(0, 2, 2, 2, 24, 1, 2, 0),
+                                 # narrow but too deep for shared memory (12 x 128, skip): padded to 256, wide kernel
+                                 Layout(0, 10, 4, 12, 128, 5, 2, 1)])
 def test_simt_and_tcgen05_paths_agree(ddf, orc, lay):
     """wide tcgen05 kernel, narrow tcgen05 kernel (width 128 with skip / width 64 / point input with
     one linear output) against the plain CUDA-core path and both oracle modes"""
