@@ -132,7 +132,11 @@ int  ddf_create_hashgrid(const void* table, const void* mlp, const ddf_hashgrid_
 int  ddf_query(ddf_model* model, const float* origins, const float* dirs, int64_t n,
                float* out_dist, float* out_vis, void* stream);
 /* Same through [host] buffers (pinned for full speed): H2D copies, query, D2H copies, and a
- * stream synchronise, all inside the call.  The end-to-end entry point bench.py times. */
+ * stream synchronise, all inside the call.  The end-to-end entry point bench.py times.  Batches of
+ * 2^18 rays or more are cut into 4 (8 from 2^21) tile-aligned chunks: uploads run ahead on a
+ * stream owned by the model, chunk i is answered on `stream` once it has landed, and its results
+ * return on a third stream while chunk i+1 is being answered; results are bit-identical to one
+ * ddf_query over the whole batch. */
 int  ddf_query_host(ddf_model* model, const float* origins, const float* dirs, int64_t n,
                     float* out_dist, float* out_vis, void* stream);
 /* Debug/parity aid: raw logits z[n][n_out] instead of the head nonlinearities. */

@@ -37,6 +37,7 @@ static void free_model(Model* m) {
   cudaFree(m->ws_dist); cudaFree(m->ws_vis);
   cudaFree(m->h2d_o); cudaFree(m->h2d_d); cudaFree(m->d2h_dist); cudaFree(m->d2h_vis);
   cudaFree(m->trace_ws); cudaFree(m->wave_ws);
+  if (m->host_s_in) { cudaStreamDestroy(m->host_s_in); cudaStreamDestroy(m->host_s_out); for (int i = 0; i < 16; ++i) cudaEventDestroy(m->host_ev[i]); }
   (void)cudaGetLastError();
   delete m;
 }
@@ -290,13 +291,49 @@ extern "C" int ddf_query_host(ddf_model* model, const float* origins, const floa
     m->host_rows = n;
   }
   cudaStream_t st = (cudaStream_t)stream;
-  DDF_CUDA_TRY(cudaMemcpyAsync(m->h2d_o, origins, (size_t)n * 12, cudaMemcpyHostToDevice, st));
-  if (ray) DDF_CUDA_TRY(cudaMemcpyAsync(m->h2d_d, dirs, (size_t)n * 12, cudaMemcpyHostToDevice, st));
-  int rc = run_query(m, m->h2d_o, ray ? m->h2d_d : nullptr, n, 0, m->d2h_dist, two ? m->d2h_vis : nullptr, stream);
-  if (rc != DDF_OK) return rc;
-  DDF_CUDA_TRY(cudaMemcpyAsync(out_dist, m->d2h_dist, (size_t)n * 4, cudaMemcpyDeviceToHost, st));
-  if (two && out_vis) DDF_CUDA_TRY(cudaMemcpyAsync(out_vis, m->d2h_vis, (size_t)n * 4, cudaMemcpyDeviceToHost, st));
+  // Large batches are cut into up to 8 tile-aligned chunks: the uploads run ahead on their own
+  // stream, chunk i is answered on `stream` as soon as it has landed, and its results go back
+  // on a third stream while chunk i+1 is being answered (results do not depend on the batching).
+  int chunks = 1;
+  if (n >= (1 << 18)) chunks = n >= (1 << 21) ? 8 : 4;
+  if (chunks > 1 && !m->host_s_in) {
+    DDF_CUDA_TRY(cudaStreamCreateWithFlags(&m->host_s_in, cudaStreamNonBlocking));
+    DDF_CUDA_TRY(cudaStreamCreateWithFlags(&m->host_s_out, cudaStreamNonBlocking));
+    for (int i = 0; i < 16; ++i) DDF_CUDA_TRY(cudaEventCreateWithFlags(&m->host_ev[i], cudaEventDisableTiming));
+  }
+  if (chunks == 1) {
+    DDF_CUDA_TRY(cudaMemcpyAsync(m->h2d_o, origins, (size_t)n * 12, cudaMemcpyHostToDevice, st));
+    if (ray) DDF_CUDA_TRY(cudaMemcpyAsync(m->h2d_d, dirs, (size_t)n * 12, cudaMemcpyHostToDevice, st));
+    int rc = run_query(m, m->h2d_o, ray ? m->h2d_d : nullptr, n, 0, m->d2h_dist, two ? m->d2h_vis : nullptr, stream);
+    if (rc != DDF_OK) return rc;
+    DDF_CUDA_TRY(cudaMemcpyAsync(out_dist, m->d2h_dist, (size_t)n * 4, cudaMemcpyDeviceToHost, st));
+    if (two && out_vis) DDF_CUDA_TRY(cudaMemcpyAsync(out_vis, m->d2h_vis, (size_t)n * 4, cudaMemcpyDeviceToHost, st));
+    DDF_CUDA_TRY(cudaStreamSynchronize(st));
+    return DDF_OK;
+  }
+  const int64_t per = ((n + chunks - 1) / chunks + 255) / 256 * 256;
+  int launches = 0;
+  for (int c = 0; c < chunks; ++c) {
+    const int64_t b = (int64_t)c * per, e = b + per < n ? b + per : n;
+    if (b >= e) { chunks = c; break; }
+    DDF_CUDA_TRY(cudaMemcpyAsync(m->h2d_o + 3 * b, origins + 3 * b, (size_t)(e - b) * 12, cudaMemcpyHostToDevice, m->host_s_in));
+    if (ray) DDF_CUDA_TRY(cudaMemcpyAsync(m->h2d_d + 3 * b, dirs + 3 * b, (size_t)(e - b) * 12, cudaMemcpyHostToDevice, m->host_s_in));
+    DDF_CUDA_TRY(cudaEventRecord(m->host_ev[c], m->host_s_in));
+  }
+  for (int c = 0; c < chunks; ++c) {
+    const int64_t b = (int64_t)c * per, e = b + per < n ? b + per : n;
+    DDF_CUDA_TRY(cudaStreamWaitEvent(st, m->host_ev[c], 0));
+    int rc = run_query(m, m->h2d_o + 3 * b, ray ? m->h2d_d + 3 * b : nullptr, e - b, 0, m->d2h_dist + b, two ? m->d2h_vis + b : nullptr, stream);
+    if (rc != DDF_OK) return rc;
+    launches += m->last_launches;
+    DDF_CUDA_TRY(cudaEventRecord(m->host_ev[8 + c], st));
+    DDF_CUDA_TRY(cudaStreamWaitEvent(m->host_s_out, m->host_ev[8 + c], 0));
+    DDF_CUDA_TRY(cudaMemcpyAsync(out_dist + b, m->d2h_dist + b, (size_t)(e - b) * 4, cudaMemcpyDeviceToHost, m->host_s_out));
+    if (two && out_vis) DDF_CUDA_TRY(cudaMemcpyAsync(out_vis + b, m->d2h_vis + b, (size_t)(e - b) * 4, cudaMemcpyDeviceToHost, m->host_s_out));
+  }
+  m->last_launches = launches;
   DDF_CUDA_TRY(cudaStreamSynchronize(st));
+  DDF_CUDA_TRY(cudaStreamSynchronize(m->host_s_out));
   return DDF_OK;
 }
 

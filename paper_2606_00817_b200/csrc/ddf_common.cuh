@@ -61,6 +61,8 @@ struct Model {
   // staging for ddf_query_host
   float *h2d_o, *h2d_d, *d2h_dist, *d2h_vis;
   int64_t host_rows;
+  cudaStream_t host_s_in, host_s_out;      // ddf_query_host: copy streams (created on first use)
+  cudaEvent_t host_ev[16];                 // [0..7] chunk uploaded, [8..15] chunk computed
   // sphere tracer state
   void* trace_ws; size_t trace_ws_bytes;
   // wavefront secondary rays (ddf_wave.cu)

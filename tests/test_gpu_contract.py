@@ -228,16 +228,24 @@ def test_simt_and_tcgen05_paths_agree(ddf, orc, lay):
         assert np.abs(z - ze).max() < 4e-2
 
 
-def test_query_host_matches_device_query(ddf, c1):
+@pytest.mark.parametrize("n", [5000, (1 << 18) + 77, (1 << 21) + 5])     # one pass / 4 chunks / 8 chunks, ragged tails
+def test_query_host_matches_device_query(ddf, c1, n):
+    """host-buffer entry: uploads, answers and downloads are pipelined in tile-aligned chunks on three
+    streams for large batches; the results must be the device query's, bit for bit"""
     lay, m = c1
-    n = 5000
-    o, d = random_rays(n)
+    o, d = random_rays(min(n, 1 << 16))
+    reps = (n + len(o) - 1) // len(o)
+    o = np.tile(o, (reps, 1))[:n].copy(); d = np.tile(d, (reps, 1))[:n].copy()
     oh, dh = torch.from_numpy(o).pin_memory(), torch.from_numpy(d).pin_memory()
-    dist_h = torch.empty(n).pin_memory(); vis_h = torch.empty(n).pin_memory()
-    ddf.ddf_query_host(m, oh, dh, n, dist_h, vis_h)
+    dist_h = torch.full((n,), float("nan")).pin_memory(); vis_h = torch.full((n,), float("nan")).pin_memory()
+    st = torch.cuda.Stream()
+    with torch.cuda.stream(st):
+        ddf.ddf_query_host(m, oh, dh, n, dist_h, vis_h, stream=st)       # synchronises inside the call
     dist = torch.empty(n, device="cuda"); vis = torch.empty(n, device="cuda")
     ddf.ddf_query(m, oh.cuda(), dh.cuda(), n, dist, vis)
     assert torch.equal(dist.cpu(), dist_h) and torch.equal(vis.cpu(), vis_h)
+    ddf.ddf_query_host(m, oh, dh, n, dist_h, None)                        # default stream, no visibility output
+    assert torch.equal(dist.cpu(), dist_h)
 
 
 def test_model_from_device_fp32_blob(ddf, orc):
