@@ -509,6 +509,14 @@ def run_hashgrid(ddf, torch, peaks):
     rec("ao_16.7M_fused", na, _time_ms(torch, lambda: ddf.ddf_query_ao(m, oa, da, npts, spp, float("inf"), ao), reps=5))
     del oa, da
     ddf.ddf_destroy(m)
+    # the same field with an fp16 table (26 MB): random origins again
+    from ddf_inputs import HashLayout
+    lay16 = HashLayout(table_dtype=2)
+    m16 = ddf.ddf_create_hashgrid(make_hash_table(lay16, n_ent), mlp, lay16)
+    o = torch.from_numpy(o_np).cuda() * 2.9; d = torch.from_numpy(d_np).cuda()
+    rec("random_origins_2^22_fp16_table", n, _time_ms(torch, lambda: ddf.ddf_query(m16, o, d, n, dist, vis), reps=7))
+    ddf.ddf_destroy(m16)
+    del o, d
     # the oracle on the host cores, bounded sample
     import oracle
     k = 1 << 17
