@@ -19,7 +19,8 @@
 
 namespace ddf {
 
-constexpr int kTrThreads = 128;
+constexpr int kTrRays = 128;            // rays per CTA
+constexpr int kTrThreads = 256;         // two threads per ray
 constexpr int kTrPitch = 129;
 constexpr int kTrW = 64;
 constexpr int kTrMaxLevels = 16;
@@ -76,49 +77,51 @@ __device__ __forceinline__ void tr_corners(const TrLevel& lv, uint32_t tmask, co
   }
 }
 
-// out[j][t] = relu(b[j] + sum_k Wt[k][j] in[k][t]) for j < 64, 8 outputs per pass
+// Two threads per ray: thread (r, h) with r = ray in the tile, h = 0 / 1.
+// out[j][r] = relu(b[j] + sum_k Wt[k][j] in[k][r]) for the 32 outputs j of half h, 8 per pass
 __device__ __forceinline__ void tr_layer_fwd(const float* __restrict__ Wt, const float* __restrict__ b, int nin,
-                                             const float* in, float* out, int t) {
-  for (int j0 = 0; j0 < kTrW; j0 += 8) {
+                                             const float* in, float* out, int r, int h) {
+  for (int j0 = 32 * h; j0 < 32 * h + 32; j0 += 8) {
     float acc[8];
     #pragma unroll
     for (int q = 0; q < 8; ++q) acc[q] = b[j0 + q];
     for (int k = 0; k < nin; ++k) {
-      const float a = in[k * kTrPitch + t];
+      const float a = in[k * kTrPitch + r];
       const float4 w0 = *reinterpret_cast<const float4*>(Wt + k * kTrW + j0);
       const float4 w1 = *reinterpret_cast<const float4*>(Wt + k * kTrW + j0 + 4);
       acc[0] = fmaf(w0.x, a, acc[0]); acc[1] = fmaf(w0.y, a, acc[1]); acc[2] = fmaf(w0.z, a, acc[2]); acc[3] = fmaf(w0.w, a, acc[3]);
       acc[4] = fmaf(w1.x, a, acc[4]); acc[5] = fmaf(w1.y, a, acc[5]); acc[6] = fmaf(w1.z, a, acc[6]); acc[7] = fmaf(w1.w, a, acc[7]);
     }
     #pragma unroll
-    for (int q = 0; q < 8; ++q) out[(j0 + q) * kTrPitch + t] = fmaxf(acc[q], 0.0f);
+    for (int q = 0; q < 8; ++q) out[(j0 + q) * kTrPitch + r] = fmaxf(acc[q], 0.0f);
   }
 }
 
-// din[k][t] = sum_j Wt[k][j] g[j][t]   (g already holds delta * relu')
-__device__ __forceinline__ void tr_layer_bwd(const float* __restrict__ Wt, int nin, const float* g, float* din, int t) {
-  for (int k = 0; k < nin; ++k) din[k * kTrPitch + t] = 0.0f;
-  for (int j0 = 0; j0 < kTrW; j0 += 8) {
-    float gj[8];
+// din[k][r] = sum_j Wt[k][j] g[j][r] for the inputs k of half h (g already holds delta * relu')
+__device__ __forceinline__ void tr_layer_bwd(const float* __restrict__ Wt, int nin, const float* g, float* din, int r, int h) {
+  float gj[kTrW];
+  #pragma unroll
+  for (int j = 0; j < kTrW; ++j) gj[j] = g[j * kTrPitch + r];
+  const int mid = (nin + 1) / 2;
+  for (int k = h ? mid : 0; k < (h ? nin : mid); ++k) {
+    float s0 = 0.0f, s1 = 0.0f;
     #pragma unroll
-    for (int q = 0; q < 8; ++q) gj[q] = g[(j0 + q) * kTrPitch + t];
-    for (int k = 0; k < nin; ++k) {
-      const float4 w0 = *reinterpret_cast<const float4*>(Wt + k * kTrW + j0);
-      const float4 w1 = *reinterpret_cast<const float4*>(Wt + k * kTrW + j0 + 4);
-      float s = din[k * kTrPitch + t];
-      s = fmaf(w0.x, gj[0], s); s = fmaf(w0.y, gj[1], s); s = fmaf(w0.z, gj[2], s); s = fmaf(w0.w, gj[3], s);
-      s = fmaf(w1.x, gj[4], s); s = fmaf(w1.y, gj[5], s); s = fmaf(w1.z, gj[6], s); s = fmaf(w1.w, gj[7], s);
-      din[k * kTrPitch + t] = s;
+    for (int j = 0; j < kTrW; j += 8) {
+      const float4 w0 = *reinterpret_cast<const float4*>(Wt + k * kTrW + j);
+      const float4 w1 = *reinterpret_cast<const float4*>(Wt + k * kTrW + j + 4);
+      s0 = fmaf(w0.x, gj[j + 0], s0); s0 = fmaf(w0.y, gj[j + 1], s0); s0 = fmaf(w0.z, gj[j + 2], s0); s0 = fmaf(w0.w, gj[j + 3], s0);
+      s1 = fmaf(w1.x, gj[j + 4], s1); s1 = fmaf(w1.y, gj[j + 5], s1); s1 = fmaf(w1.z, gj[j + 6], s1); s1 = fmaf(w1.w, gj[j + 7], s1);
     }
+    din[k * kTrPitch + r] = s0 + s1;
   }
 }
 
 // block-level  dW[j][k] += sum_r g[j][r] a[k][r],  db[j] += sum_r g[j][r]; one atomic per entry
 __device__ __forceinline__ void tr_weight_grads(const float* g, const float* a, int nin, float* gW, float* gb, int t) {
-  const int j = t & 63, half = t >> 6;
-  for (int k0 = half * 4; k0 < nin; k0 += 8) {
+  const int j = t & 63, quarter = t >> 6;
+  for (int k0 = quarter * 4; k0 < nin; k0 += 16) {
     float acc[4] = {0.0f, 0.0f, 0.0f, 0.0f};
-    for (int r = 0; r < kTrThreads; ++r) {
+    for (int r = 0; r < kTrRays; ++r) {
       const float gv = g[j * kTrPitch + r];
       #pragma unroll
       for (int q = 0; q < 4; ++q) if (k0 + q < nin) acc[q] = fmaf(gv, a[(k0 + q) * kTrPitch + r], acc[q]);
@@ -126,16 +129,16 @@ __device__ __forceinline__ void tr_weight_grads(const float* g, const float* a, 
     #pragma unroll
     for (int q = 0; q < 4; ++q) if (k0 + q < nin) atomicAdd(gW + j * nin + k0 + q, acc[q]);
   }
-  if (half == 0) {
+  if (quarter == 0) {
     float s = 0.0f;
-    for (int r = 0; r < kTrThreads; ++r) s += g[j * kTrPitch + r];
+    for (int r = 0; r < kTrRays; ++r) s += g[j * kTrPitch + r];
     atomicAdd(gb + j, s);
   }
 }
 
 __global__ void __launch_bounds__(kTrThreads, 1) train_fwd_bwd_kernel(const __grid_constant__ TrParams p) {
   extern __shared__ float sm[];
-  const int t = threadIdx.x, H = p.n_hidden, E = p.E;
+  const int t = threadIdx.x, r = t & (kTrRays - 1), h = t >> 7, H = p.n_hidden, E = p.E;
   // shared layout: weights (transposed), biases, head; then act[0..H] and two delta buffers
   float* Wt[2]; float* bs[2];
   float* cur = sm;
@@ -156,66 +159,71 @@ __global__ void __launch_bounds__(kTrThreads, 1) train_fwd_bwd_kernel(const __gr
   __syncthreads();
 
   float block_loss = 0.0f;
-  const int64_t num_tiles = (p.n + kTrThreads - 1) / kTrThreads;
+  const int64_t num_tiles = (p.n + kTrRays - 1) / kTrRays;
   for (int64_t tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
-    const int64_t ray = tile * kTrThreads + t;
+    const int64_t ray = tile * kTrRays + r;
     const bool valid = ray < p.n;
     float x01[3] = {0.0f, 0.0f, 0.0f};
-    // ---- forward: input column
-    for (int k = 0; k < E; ++k) act[0][k * kTrPitch + t] = 0.0f;
+    // ---- forward: input column.  h = 0: even levels and gamma(d); h = 1: odd levels
     if (valid) {
       #pragma unroll
       for (int a = 0; a < 3; ++a) {
         const float v = __fdiv_rn(__fsub_rn(p.o[3 * ray + a], p.bmin[a]), p.den[a]);
         x01[a] = fminf(fmaxf(v, 0.0f), 1.0f);
       }
-      for (int l = 0; l < p.n_levels; ++l) {
+      for (int l = h; l < p.n_levels; l += 2) {
         uint32_t idx[8]; float wt[8];
         tr_corners(p.lv[l], p.tmask, x01, idx, wt);
         float f0 = 0.0f, f1 = 0.0f;
         #pragma unroll
         for (int c = 0; c < 8; ++c) { const float2 v = __ldg(reinterpret_cast<const float2*>(p.table) + idx[c]); f0 = fmaf(wt[c], v.x, f0); f1 = fmaf(wt[c], v.y, f1); }
-        act[0][(2 * l) * kTrPitch + t] = f0; act[0][(2 * l + 1) * kTrPitch + t] = f1;
+        act[0][(2 * l) * kTrPitch + r] = f0; act[0][(2 * l + 1) * kTrPitch + r] = f1;
       }
-      const float dv[3] = { p.d[3 * ray], p.d[3 * ray + 1], p.d[3 * ray + 2] };
-      int m = p.NF;
-      for (int c = 0; c < 3; ++c) act[0][(m++) * kTrPitch + t] = dv[c];
-      for (int k = 0; k < p.Ld; ++k) {
-        float s[3], co[3];
-        for (int c = 0; c < 3; ++c) sincospif(ldexpf(dv[c], k), &s[c], &co[c]);
-        for (int c = 0; c < 3; ++c) act[0][(m++) * kTrPitch + t] = s[c];
-        for (int c = 0; c < 3; ++c) act[0][(m++) * kTrPitch + t] = co[c];
+      if (h == 0) {
+        const float dv[3] = { p.d[3 * ray], p.d[3 * ray + 1], p.d[3 * ray + 2] };
+        int m = p.NF;
+        for (int c = 0; c < 3; ++c) act[0][(m++) * kTrPitch + r] = dv[c];
+        for (int k = 0; k < p.Ld; ++k) {
+          float sn[3], co[3];
+          for (int c = 0; c < 3; ++c) sincospif(ldexpf(dv[c], k), &sn[c], &co[c]);
+          for (int c = 0; c < 3; ++c) act[0][(m++) * kTrPitch + r] = sn[c];
+          for (int c = 0; c < 3; ++c) act[0][(m++) * kTrPitch + r] = co[c];
+        }
       }
+    } else {
+      for (int k = h; k < E; k += 2) act[0][k * kTrPitch + r] = 0.0f;
     }
-    for (int l = 0; l < H; ++l) tr_layer_fwd(Wt[l], bs[l], l == 0 ? E : kTrW, act[l], act[l + 1], t);
-    float z0 = hb0, z1 = hb1;
-    for (int k = 0; k < kTrW; ++k) { const float hv = act[H][k * kTrPitch + t]; z0 = fmaf(Wh[k], hv, z0); z1 = fmaf(Wh[kTrW + k], hv, z1); }
+    __syncthreads();
+    for (int l = 0; l < H; ++l) { tr_layer_fwd(Wt[l], bs[l], l == 0 ? E : kTrW, act[l], act[l + 1], r, h); __syncthreads(); }
+    float z0 = hb0, z1 = hb1;                                    // both threads of a ray compute the same logits
+    for (int k = 0; k < kTrW; ++k) { const float hv = act[H][k * kTrPitch + r]; z0 = fmaf(Wh[k], hv, z0); z1 = fmaf(Wh[kTrW + k], hv, z1); }
     // ---- loss and d loss / d logits (readings T1, T2)
     float dz0 = 0.0f, dz1 = 0.0f;
     if (valid) {
-      const int h = p.hit[ray] != 0;
+      const int hitf = p.hit[ray] != 0;
       const float sp = softplus_f(z0), err = sp - p.t[ray], ae = fabsf(err);
-      if (h) { block_loss += fminf(ae, p.dist_clamp); if (ae < p.dist_clamp) dz0 = (err > 0.0f ? 1.0f : (err < 0.0f ? -1.0f : 0.0f)) * sigmoid_f(z0); }
-      block_loss += p.ce_weight * (h ? softplus_f(-z1) : softplus_f(z1));
-      dz1 = p.ce_weight * (sigmoid_f(z1) - (float)h);
+      float l = p.ce_weight * (hitf ? softplus_f(-z1) : softplus_f(z1));
+      if (hitf) { l += fminf(ae, p.dist_clamp); if (ae < p.dist_clamp) dz0 = (err > 0.0f ? 1.0f : (err < 0.0f ? -1.0f : 0.0f)) * sigmoid_f(z0); }
+      if (h == 0) block_loss += l;
+      dz1 = p.ce_weight * (sigmoid_f(z1) - (float)hitf);
       const float inv_n = 1.0f / (float)p.n;
       dz0 *= inv_n; dz1 *= inv_n;
     }
-    // ---- backward: head.  dA = delta at the last hidden output, masked by ReLU
-    for (int k = 0; k < kTrW; ++k) {
-      const float hv = act[H][k * kTrPitch + t];
-      dA[k * kTrPitch + t] = hv > 0.0f ? fmaf(Wh[k], dz0, Wh[kTrW + k] * dz1) : 0.0f;
+    // ---- backward: head.  dA = delta at the last hidden output, masked by ReLU (half of the units each)
+    for (int k = 32 * h; k < 32 * h + 32; ++k) {
+      const float hv = act[H][k * kTrPitch + r];
+      dA[k * kTrPitch + r] = hv > 0.0f ? fmaf(Wh[k], dz0, Wh[kTrW + k] * dz1) : 0.0f;
     }
     // head weight gradients need the block's dz: park them in dB rows 0, 1
-    dB[0 * kTrPitch + t] = dz0; dB[1 * kTrPitch + t] = dz1;
+    if (h == 0) { dB[0 * kTrPitch + r] = dz0; dB[1 * kTrPitch + r] = dz1; }
     __syncthreads();
     if (t < kTrW) {
       float s0 = 0.0f, s1 = 0.0f;
-      for (int r = 0; r < kTrThreads; ++r) { const float hv = act[H][t * kTrPitch + r]; s0 = fmaf(dB[r], hv, s0); s1 = fmaf(dB[kTrPitch + r], hv, s1); }
+      for (int q = 0; q < kTrRays; ++q) { const float hv = act[H][t * kTrPitch + q]; s0 = fmaf(dB[q], hv, s0); s1 = fmaf(dB[kTrPitch + q], hv, s1); }
       atomicAdd(p.g_mlp + p.w_off[H] + t, s0); atomicAdd(p.g_mlp + p.w_off[H] + kTrW + t, s1);
     } else if (t < kTrW + 2) {
       float s = 0.0f;
-      for (int r = 0; r < kTrThreads; ++r) s += dB[(t - kTrW) * kTrPitch + r];
+      for (int q = 0; q < kTrRays; ++q) s += dB[(t - kTrW) * kTrPitch + q];
       atomicAdd(p.g_mlp + p.b_off[H] + (t - kTrW), s);
     }
     __syncthreads();
@@ -223,19 +231,21 @@ __global__ void __launch_bounds__(kTrThreads, 1) train_fwd_bwd_kernel(const __gr
     float* g = dA; float* din = dB;
     for (int l = H - 1; l >= 0; --l) {
       const int nin = l == 0 ? E : kTrW;
-      tr_layer_bwd(Wt[l], nin, g, din, t);                      // own column only
-      __syncthreads();                                          // g, act[l] complete for the whole block
-      tr_weight_grads(g, act[l], nin, p.g_mlp + p.w_off[l], p.g_mlp + p.b_off[l], t);
+      tr_layer_bwd(Wt[l], nin, g, din, r, h);                   // half of the inputs of the own ray
+      if (l > 0) {                                              // ReLU mask of the layer below, on the entries just written
+        const int mid = (nin + 1) / 2;
+        for (int k = h ? mid : 0; k < (h ? nin : mid); ++k) if (!(act[l][k * kTrPitch + r] > 0.0f)) din[k * kTrPitch + r] = 0.0f;
+      }
+      tr_weight_grads(g, act[l], nin, p.g_mlp + p.w_off[l], p.g_mlp + p.b_off[l], t);   // g, act[l]: complete since the last barrier
       __syncthreads();
-      if (l > 0) for (int k = 0; k < nin; ++k) { if (!(act[l][k * kTrPitch + t] > 0.0f)) din[k * kTrPitch + t] = 0.0f; }
       float* tmp = g; g = din; din = tmp;
     }
     // g now holds d loss / d input; its first NF rows are the level features
     if (valid)
-      for (int l = 0; l < p.n_levels; ++l) {
+      for (int l = h; l < p.n_levels; l += 2) {
         uint32_t idx[8]; float wt[8];
         tr_corners(p.lv[l], p.tmask, x01, idx, wt);
-        const float g0 = g[(2 * l) * kTrPitch + t], g1 = g[(2 * l + 1) * kTrPitch + t];
+        const float g0 = g[(2 * l) * kTrPitch + r], g1 = g[(2 * l + 1) * kTrPitch + r];
         #pragma unroll
         for (int c = 0; c < 8; ++c) atomicAdd(reinterpret_cast<float2*>(p.g_table) + idx[c], make_float2(wt[c] * g0, wt[c] * g1));
       }
@@ -243,7 +253,7 @@ __global__ void __launch_bounds__(kTrThreads, 1) train_fwd_bwd_kernel(const __gr
   }
   // ---- batch loss
   #pragma unroll
-  for (int s = 16; s > 0; s >>= 1) block_loss += __shfl_xor_sync(0xffffffffu, block_loss, s);
+  for (int sft = 16; sft > 0; sft >>= 1) block_loss += __shfl_xor_sync(0xffffffffu, block_loss, sft);
   if ((t & 31) == 0 && p.loss) atomicAdd(p.loss, block_loss / (float)p.n);
 }
 
@@ -251,7 +261,19 @@ __global__ void __launch_bounds__(kTrThreads, 1) train_fwd_bwd_kernel(const __gr
 __global__ void adam_kernel(float* __restrict__ prm, float* __restrict__ m, float* __restrict__ v, float* __restrict__ g,
                             int64_t n, float lr, float b1, float b2, float eps, float c1, float c2) {
   const int64_t stride = (int64_t)gridDim.x * blockDim.x;
-  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+  const bool aligned = ((reinterpret_cast<uintptr_t>(prm) | reinterpret_cast<uintptr_t>(m) | reinterpret_cast<uintptr_t>(v) |
+                         reinterpret_cast<uintptr_t>(g)) & 15) == 0;
+  const int64_t n4 = aligned ? (n >> 2) : 0;                  // the MLP slice of m / v / g may start on an 8-byte boundary
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n4; i += stride) {
+    float4 gi = reinterpret_cast<float4*>(g)[i], mi = reinterpret_cast<float4*>(m)[i], vi = reinterpret_cast<float4*>(v)[i], pi = reinterpret_cast<float4*>(prm)[i];
+    #define ADAM1(c) { mi.c = b1 * mi.c + (1.0f - b1) * gi.c; vi.c = b2 * vi.c + (1.0f - b2) * gi.c * gi.c; \
+                       pi.c -= lr * (mi.c / c1) / (sqrtf(vi.c / c2) + eps); }
+    ADAM1(x) ADAM1(y) ADAM1(z) ADAM1(w)
+    #undef ADAM1
+    reinterpret_cast<float4*>(m)[i] = mi; reinterpret_cast<float4*>(v)[i] = vi; reinterpret_cast<float4*>(prm)[i] = pi;
+    reinterpret_cast<float4*>(g)[i] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+  }
+  for (int64_t i = (n4 << 2) + (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
     const float gi = g[i];
     const float mi = b1 * m[i] + (1.0f - b1) * gi;
     const float vi = b2 * v[i] + (1.0f - b2) * gi * gi;
@@ -464,7 +486,7 @@ static int tr_launch_grads(Trainer* T, const float* o, const float* d, const flo
   TrParams p = T->base;
   p.o = o; p.d = d; p.t = t; p.hit = hit; p.n = n;
   DDF_CUDA_TRY(cudaMemsetAsync(T->loss_dev, 0, 4, st));
-  const int64_t tiles = (n + kTrThreads - 1) / kTrThreads;
+  const int64_t tiles = (n + kTrRays - 1) / kTrRays;
   int sms = 0; DDF_CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, 0));
   const unsigned grid = (unsigned)(tiles < sms ? tiles : sms);
   train_fwd_bwd_kernel<<<grid, kTrThreads, T->smem_bytes, st>>>(p);
