@@ -27,6 +27,8 @@
  *  - n == 0 is DDF_OK and a no-op; n < 0 or a NULL pointer with n > 0 is DDF_E_INVALID_ARG.
  *  - Results are a pure function of (weights, ray): independent of n and of the ray's position
  *    in the batch, bit-reproducible run to run.  Directions must be unit length (not checked).
+ *  - A model (and a trainer) owns device workspaces that its calls reuse: use one model from one
+ *    stream / host thread at a time; different models are independent.
  *  - There is no CPU fallback: without a CUDA device of compute capability 10.x the calls
  *    return DDF_E_UNSUPPORTED / DDF_E_CUDA.
  */
