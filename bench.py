@@ -495,6 +495,8 @@ def run_hashgrid(ddf, torch, peaks):
     oc = torch.empty((1 << 20, 3), device="cuda"); dc = torch.empty((1 << 20, 3), device="cuda")
     ddf.ddf_gen_camera(cam, 1024, 1024, oc, dc)
     rec("camera_2^20", 1 << 20, _time_ms(torch, lambda: ddf.ddf_query(m, oc, dc, 1 << 20, dist, vis), reps=7))
+    # the same frame through ddf_query_camera: rays generated in the kernel, origin features once per CTA
+    rec("camera_2^20_fused_generator", 1 << 20, _time_ms(torch, lambda: ddf.ddf_query_camera(m, cam, 1024, 1024, dist, vis), reps=7))
     p = torch.empty((n, 3), device="cuda"); nr = torch.empty((n, 3), device="cuda")
     ddf.ddf_gen_sphere_points(MASTER_SEED, STREAMS["shadow_points"], n, 1.0, p, nr)
     ddf.ddf_gen_shadow(p, nr, n, (3.0, 3.0, 3.0), 1e-3, o, d, None)

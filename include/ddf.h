@@ -141,6 +141,13 @@ int  ddf_query(ddf_model* model, const float* origins, const float* dirs, int64_
  * ddf_query over the whole batch. */
 int  ddf_query_host(ddf_model* model, const float* origins, const float* dirs, int64_t n,
                     float* out_dist, float* out_vis, void* stream);
+/* Primary rays ("To trace a primary ray we evaluate f at the camera and read t and
+ * xi"): the width x height rays of ddf_gen_camera answered in one call, row-major, bit-identical
+ * to ddf_gen_camera + ddf_query.  For a hash-grid model the rays are generated inside the query
+ * kernel and the level features of the shared origin are computed once per CTA (8 bytes of HBM
+ * traffic per ray instead of 32 and no per-ray gathers); other models use a workspace. */
+int  ddf_query_camera(ddf_model* model, const ddf_camera* cam, int width, int height,
+                      float* out_dist, float* out_vis, void* stream);
 /* Debug/parity aid: raw logits z[n][n_out] instead of the head nonlinearities. */
 int  ddf_query_logits(ddf_model* model, const float* origins, const float* dirs, int64_t n,
                       float* out_z, void* stream);

@@ -18,7 +18,7 @@ EXPORTED_SYMBOLS = [
     "ddf_ao_reduce", "ddf_query_ao", "ddf_shadow_test", "sdf_sphere_trace",
     "ddf_hashgrid_table_entries", "ddf_create_hashgrid", "ddf_gen_shadow_from_hits", "ddf_query_shadowed",
     "ddf_trainer_create", "ddf_trainer_destroy", "ddf_trainer_step", "ddf_trainer_loss_grads", "ddf_trainer_export",
-    "ddf_trainer_steps", "ddf_scene_raycast", "ddf_gen_train_batch",
+    "ddf_trainer_steps", "ddf_scene_raycast", "ddf_gen_train_batch", "ddf_query_camera",
 ]
 
 
@@ -357,3 +357,8 @@ def ddf_gen_train_batch(scene, seed, rng_stream, step, n, sample_half, o, d, t, 
     _check(lib().ddf_gen_train_batch(C.byref(scene), C.c_uint64(seed), C.c_uint64(rng_stream), C.c_int64(step), C.c_int64(n),
                                      C.c_float(sample_half), _dev(o), _dev(d), _dev(t), _dev(hit, torch.uint8),
                                      _stream(stream)), "ddf_gen_train_batch")
+
+
+def ddf_query_camera(model, cam, width, height, out_dist, out_vis, stream=None):
+    _check(lib().ddf_query_camera(model.handle, C.byref(cam), C.c_int(width), C.c_int(height), _dev(out_dist), _dev(out_vis),
+                                  _stream(stream)), "ddf_query_camera")

@@ -36,7 +36,7 @@ static void free_model(Model* m) {
   cudaFree(m->ws_gamma); cudaFree(m->ws_act0); cudaFree(m->ws_act1); cudaFree(m->ws_last);
   cudaFree(m->ws_dist); cudaFree(m->ws_vis);
   cudaFree(m->h2d_o); cudaFree(m->h2d_d); cudaFree(m->d2h_dist); cudaFree(m->d2h_vis);
-  cudaFree(m->trace_ws); cudaFree(m->wave_ws);
+  cudaFree(m->trace_ws); cudaFree(m->wave_ws); cudaFree(m->cam_o); cudaFree(m->cam_d);
   if (m->host_s_in) { cudaStreamDestroy(m->host_s_in); cudaStreamDestroy(m->host_s_out); for (int i = 0; i < 16; ++i) cudaEventDestroy(m->host_ev[i]); }
   (void)cudaGetLastError();
   delete m;
@@ -335,6 +335,29 @@ extern "C" int ddf_query_host(ddf_model* model, const float* origins, const floa
   DDF_CUDA_TRY(cudaStreamSynchronize(st));
   DDF_CUDA_TRY(cudaStreamSynchronize(m->host_s_out));
   return DDF_OK;
+}
+
+extern "C" int ddf_query_camera(ddf_model* model, const ddf_camera* cam, int width, int height,
+                                float* out_dist, float* out_vis, void* stream) {
+  if (!model || !cam || width < 0 || height < 0) return DDF_E_INVALID_ARG;
+  Model* m = reinterpret_cast<Model*>(model);
+  if (m->lay.input_kind != 0) return DDF_E_INVALID_ARG;
+  const int64_t n = (int64_t)width * height;
+  if (n == 0) { m->last_launches = 0; return DDF_OK; }
+  if (!out_dist) return DDF_E_INVALID_ARG;
+  cudaStream_t st = (cudaStream_t)stream;
+  if (m->hg) return hash_forward_camera(m, cam, width, height, out_dist, out_vis, st);
+  if (n > m->cam_rows) {
+    cudaFree(m->cam_o); cudaFree(m->cam_d); m->cam_o = m->cam_d = nullptr; m->cam_rows = 0;
+    DDF_CUDA_TRY(cudaMalloc(&m->cam_o, (size_t)n * 12));
+    DDF_CUDA_TRY(cudaMalloc(&m->cam_d, (size_t)n * 12));
+    m->cam_rows = n;
+  }
+  int rc = ddf_gen_camera(cam, width, height, m->cam_o, m->cam_d, stream);
+  if (rc != DDF_OK) return rc;
+  rc = run_query(m, m->cam_o, m->cam_d, n, 0, out_dist, out_vis, stream);
+  if (rc == DDF_OK) m->last_launches += 1;
+  return rc;
 }
 
 extern "C" int ddf_query_ao(ddf_model* model, const float* o, const float* d, int64_t n_pts, int spp,

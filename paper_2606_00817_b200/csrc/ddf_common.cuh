@@ -61,6 +61,7 @@ struct Model {
   // staging for ddf_query_host
   float *h2d_o, *h2d_d, *d2h_dist, *d2h_vis;
   int64_t host_rows;
+  float *cam_o, *cam_d; int64_t cam_rows;  // ddf_query_camera workspace for the kernels that read rays from memory
   cudaStream_t host_s_in, host_s_out;      // ddf_query_host: copy streams (created on first use)
   cudaEvent_t host_ev[16];                 // [0..7] chunk uploaded, [8..15] chunk computed
   // sphere tracer state
@@ -91,6 +92,8 @@ int tc_forward(Model* m, const float* o, const float* d, int64_t n, const int64_
 void hash_plan_destroy(Model* m);
 int hash_forward(Model* m, const float* o, const float* d, int64_t n, const int64_t* n_dev, int mode_out,
                  float* out0, float* out1, int spp, float ao_radius, cudaStream_t st);
+
+int hash_forward_camera(Model* m, const ddf_camera* cam, int width, int height, float* out0, float* out1, cudaStream_t st);
 
 // ---- narrow-network tcgen05 path (ddf_narrow.cu)
 int narrow_plan_create(Model* m, const uint16_t* hw_host, const float* hb_host);   // sets m->nw or leaves it null

@@ -17,6 +17,7 @@
 // Operation and readings H1-H7: include/ddf.h, DESIGN.md.
 #include "ddf_common.cuh"
 #include "ddf_tc_ptx.cuh"
+#include "ddf_camera.cuh"
 #include <cuda_fp16.h>
 #include <math.h>
 #include <stdlib.h>
@@ -48,6 +49,10 @@ struct HgParams {
   float ao_radius;
   uint32_t tmask;
   int n_levels, Ld, n_hidden, n_out, table_f16, mode_out, spp;
+  // primary rays generated in the kernel (ddf_query_camera): every ray starts at cam.pos, so the
+  // level features are computed once per CTA; o and d are not read
+  int cam_mode, cam_w, cam_h;
+  CamFrame cam;
 };
 
 struct HashPlan {
@@ -60,6 +65,44 @@ struct HashPlan {
 __device__ __forceinline__ uint32_t pack_bf16(float a, float b) {
   __nv_bfloat162 t = __floats2bfloat162_rn(a, b);
   return *reinterpret_cast<uint32_t*>(&t);
+}
+
+// features (2 values, packed bf16) of one level at the point x01 (readings H3-H5)
+template <bool F16>
+__device__ __forceinline__ uint32_t hg_level_feature(const HgLevel lv, uint32_t tmask, const void* table, const float x01[3]) {
+  uint32_t c0[3]; float w1[3];
+  #pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    const float pos = __fmul_rn(x01[a], lv.scale);
+    const float fl = fminf(floorf(pos), lv.scale - 1.0f);
+    c0[a] = (uint32_t)fl; w1[a] = pos - fl;
+  }
+  uint32_t kx[2], ky[2], kz[2];
+  if (lv.hashed) {
+    kx[0] = c0[0];                  kx[1] = c0[0] + 1u;
+    ky[0] = c0[1] * 2654435761u;    ky[1] = (c0[1] + 1u) * 2654435761u;
+    kz[0] = c0[2] * 805459861u;     kz[1] = (c0[2] + 1u) * 805459861u;
+  } else {
+    kx[0] = c0[0];                          kx[1] = c0[0] + 1u;
+    ky[0] = c0[1] * lv.verts;               ky[1] = ky[0] + lv.verts;
+    kz[0] = c0[2] * lv.verts * lv.verts;    kz[1] = kz[0] + lv.verts * lv.verts;
+  }
+  float2 v[8];
+  #pragma unroll
+  for (int c = 0; c < 8; ++c) {
+    const uint32_t a = kx[c & 1], b = ky[(c >> 1) & 1], e = kz[c >> 2];
+    const uint32_t idx = lv.offset + (lv.hashed ? ((a ^ b ^ e) & tmask) : (a + b + e));
+    if (F16) v[c] = __half22float2(__ldg(reinterpret_cast<const __half2*>(table) + idx));
+    else     v[c] = __ldg(reinterpret_cast<const float2*>(table) + idx);
+  }
+  float f0 = 0.0f, f1 = 0.0f;
+  #pragma unroll
+  for (int c = 0; c < 8; ++c) {
+    const float wt = ((c & 1) ? w1[0] : 1.0f - w1[0]) * (((c >> 1) & 1) ? w1[1] : 1.0f - w1[1])
+                   * ((c >> 2) ? w1[2] : 1.0f - w1[2]);
+    f0 = fmaf(wt, v[c].x, f0); f1 = fmaf(wt, v[c].y, f1);
+  }
+  return pack_bf16(f0, f1);
 }
 
 template <bool F16>
@@ -97,6 +140,21 @@ __global__ void __launch_bounds__(kHgThreads, 5) ddf_hash_kernel(const __grid_co
   const uint32_t xrow = x_smem + (uint32_t)t * 128u;
   uint32_t phase = 0;
 
+  // shared origin: thread l computes level l once for the whole CTA
+  uint32_t* cam_feat = nullptr;
+  if (p.cam_mode) {
+    cam_feat = reinterpret_cast<uint32_t*>(gen + (bar - smem_base) + 16);
+    if (t < p.n_levels) {
+      float x01[3];
+      #pragma unroll
+      for (int a = 0; a < 3; ++a) {
+        const float v = __fdiv_rn(__fsub_rn(p.cam.pos[a], p.bmin[a]), p.den[a]);
+        x01[a] = fminf(fmaxf(v, 0.0f), 1.0f);
+      }
+      cam_feat[t] = hg_level_feature<F16>(p.lv[t], p.tmask, p.table, x01);
+    }
+    __syncthreads();
+  }
   const int64_t n_rays = p.n_dev ? *p.n_dev : p.n;
   const int64_t num_tiles = (n_rays + kHgThreads - 1) / kHgThreads;
   for (int64_t tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
@@ -110,7 +168,9 @@ __global__ void __launch_bounds__(kHgThreads, 5) ddf_hash_kernel(const __grid_co
       float g[32];
       #pragma unroll
       for (int i = 0; i < 32; ++i) g[i] = 0.0f;
-      const float dv[3] = { p.d[3 * ray], p.d[3 * ray + 1], p.d[3 * ray + 2] };
+      float dv[3];
+      if (p.cam_mode) pixel_dir(p.cam, p.cam_w, p.cam_h, (int)(ray % p.cam_w), (int)(ray / p.cam_w), dv);
+      else { dv[0] = p.d[3 * ray]; dv[1] = p.d[3 * ray + 1]; dv[2] = p.d[3 * ray + 2]; }
       g[0] = dv[0]; g[1] = dv[1]; g[2] = dv[2];
       #pragma unroll
       for (int k = 0; k < 4; ++k) {
@@ -126,49 +186,18 @@ __global__ void __launch_bounds__(kHgThreads, 5) ddf_hash_kernel(const __grid_co
       #pragma unroll
       for (int i = 0; i < 16; ++i) rw[i] = pack_bf16(g[2 * i], g[2 * i + 1]);
       // ---- hash grid on the origin (readings H1-H5)
-      float x01[3];
-      #pragma unroll
-      for (int a = 0; a < 3; ++a) {
-        const float v = __fdiv_rn(__fsub_rn(p.o[3 * ray + a], p.bmin[a]), p.den[a]);
-        x01[a] = fminf(fmaxf(v, 0.0f), 1.0f);
+      float x01[3] = {0.0f, 0.0f, 0.0f};
+      if (!p.cam_mode) {
+        #pragma unroll
+        for (int a = 0; a < 3; ++a) {
+          const float v = __fdiv_rn(__fsub_rn(p.o[3 * ray + a], p.bmin[a]), p.den[a]);
+          x01[a] = fminf(fmaxf(v, 0.0f), 1.0f);
+        }
       }
       #pragma unroll
       for (int l = 0; l < kHgMaxLevels; ++l) {
         if (l < p.n_levels) {
-          const HgLevel lv = p.lv[l];
-          uint32_t c0[3]; float w1[3];
-          #pragma unroll
-          for (int a = 0; a < 3; ++a) {
-            const float pos = __fmul_rn(x01[a], lv.scale);
-            const float fl = fminf(floorf(pos), lv.scale - 1.0f);
-            c0[a] = (uint32_t)fl; w1[a] = pos - fl;
-          }
-          uint32_t kx[2], ky[2], kz[2];
-          if (lv.hashed) {
-            kx[0] = c0[0];                  kx[1] = c0[0] + 1u;
-            ky[0] = c0[1] * 2654435761u;    ky[1] = (c0[1] + 1u) * 2654435761u;
-            kz[0] = c0[2] * 805459861u;     kz[1] = (c0[2] + 1u) * 805459861u;
-          } else {
-            kx[0] = c0[0];                          kx[1] = c0[0] + 1u;
-            ky[0] = c0[1] * lv.verts;               ky[1] = ky[0] + lv.verts;
-            kz[0] = c0[2] * lv.verts * lv.verts;    kz[1] = kz[0] + lv.verts * lv.verts;
-          }
-          float2 v[8];
-          #pragma unroll
-          for (int c = 0; c < 8; ++c) {
-            const uint32_t a = kx[c & 1], b = ky[(c >> 1) & 1], e = kz[c >> 2];
-            const uint32_t idx = lv.offset + (lv.hashed ? ((a ^ b ^ e) & p.tmask) : (a + b + e));
-            if (F16) v[c] = __half22float2(__ldg(reinterpret_cast<const __half2*>(p.table) + idx));
-            else     v[c] = __ldg(reinterpret_cast<const float2*>(p.table) + idx);
-          }
-          float f0 = 0.0f, f1 = 0.0f;
-          #pragma unroll
-          for (int c = 0; c < 8; ++c) {
-            const float wt = ((c & 1) ? w1[0] : 1.0f - w1[0]) * (((c >> 1) & 1) ? w1[1] : 1.0f - w1[1])
-                           * ((c >> 2) ? w1[2] : 1.0f - w1[2]);
-            f0 = fmaf(wt, v[c].x, f0); f1 = fmaf(wt, v[c].y, f1);
-          }
-          rw[kHgFeatCol / 2 + l] = pack_bf16(f0, f1);
+          rw[kHgFeatCol / 2 + l] = cam_feat ? cam_feat[l] : hg_level_feature<F16>(p.lv[l], p.tmask, p.table, x01);
         }
       }
     }
@@ -281,6 +310,23 @@ void hash_plan_destroy(Model* m) {
   cudaFree(m->hg->d_table); cudaFree(m->hg->d_w); cudaFree(m->hg->d_bias); cudaFree(m->hg->d_head_w);
   delete m->hg;
   m->hg = nullptr;
+}
+
+int hash_forward_camera(Model* m, const ddf_camera* cam, int width, int height, float* out0, float* out1, cudaStream_t st) {
+  HashPlan* h = m->hg;
+  HgParams p = h->base;
+  const int64_t n = (int64_t)width * height;
+  p.o = nullptr; p.d = nullptr; p.n = n; p.n_dev = nullptr; p.out0 = out0; p.out1 = out1;
+  p.mode_out = 0; p.spp = 1; p.ao_radius = 0.0f;
+  p.cam_mode = 1; p.cam_w = width; p.cam_h = height; p.cam = make_frame(cam);
+  const int64_t tiles = (n + kHgThreads - 1) / kHgThreads;
+  int64_t grid = (int64_t)m->sm_count * h->ctas_per_sm;
+  if (tiles < grid) grid = tiles;
+  if (p.table_f16) ddf_hash_kernel<true><<<(unsigned)grid, kHgThreads, h->smem_bytes, st>>>(p);
+  else             ddf_hash_kernel<false><<<(unsigned)grid, kHgThreads, h->smem_bytes, st>>>(p);
+  DDF_CUDA_TRY(cudaGetLastError());
+  m->last_launches = 1;
+  return DDF_OK;
 }
 
 int hash_forward(Model* m, const float* o, const float* d, int64_t n, const int64_t* n_dev, int mode_out,
@@ -401,7 +447,7 @@ extern "C" int ddf_create_hashgrid(const void* table, const void* mlp, const ddf
   p.tmask = (1u << L.log2_table_size) - 1u;
   p.n_levels = (int)L.n_levels; p.Ld = (int)L.n_freq_dir; p.n_hidden = (int)L.n_hidden; p.n_out = (int)L.n_out;
   p.table_f16 = L.table_dtype == 2;
-  h->smem_bytes = 16384 + (size_t)L.n_hidden * 8192 + (L.n_hidden + 2) * 256 + 64 + 1024;
+  h->smem_bytes = 16384 + (size_t)L.n_hidden * 8192 + (L.n_hidden + 2) * 256 + 128 + 1024;
   if ((e = cudaFuncSetAttribute(ddf_hash_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_bytes)) != cudaSuccess ||
       (e = cudaFuncSetAttribute(ddf_hash_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_bytes)) != cudaSuccess)
     return fail(DDF_E_CUDA, e);

@@ -176,3 +176,32 @@ def test_closed_forms_on_gpu(ddf, orc):
     ddf.ddf_query(m1, _cuda(o), _cuda(d), 1000, d1, None); ddf.ddf_query(m2, _cuda(o), _cuda(d), 1000, d2, None)
     assert torch.equal(d1, d2)
     ddf.ddf_destroy(m1); ddf.ddf_destroy(m2)
+
+
+@pytest.mark.parametrize("kind", ["hash_fp32", "hash_fp16", "dense_narrow", "dense_wide"])
+def test_query_camera_is_generator_plus_query(ddf, kind):
+    """ddf_query_camera (rays generated in the kernel, shared-origin features computed once per CTA for
+    the hash-grid field) must give the bits of ddf_gen_camera + ddf_query, for any image size."""
+    from ddf_inputs import Layout, make_weights
+    if kind.startswith("hash"):
+        lay = HashLayout(table_dtype=2 if kind == "hash_fp16" else 0)
+        m = ddf.ddf_create_hashgrid(make_hash_table(lay, ddf.ddf_hashgrid_table_entries(lay)), make_hash_mlp(lay, bias_scale=0.2), lay)
+    else:
+        lay = Layout(0, 6, 3, 3, 64 if kind == "dense_narrow" else 256, 1, 2, 0)
+        m = ddf.ddf_create(make_weights(lay, bias_scale=0.2), lay)
+    cam = ddf.ddf_camera_from_seed(MASTER_SEED, STREAMS["camera_pos"], 2.5)
+    for (W, H) in ((333, 77), (1024, 512), (1, 1)):
+        n = W * H
+        o = torch.empty((n, 3), device="cuda"); d = torch.empty((n, 3), device="cuda")
+        ddf.ddf_gen_camera(cam, W, H, o, d)
+        d0 = torch.empty(n, device="cuda"); v0 = torch.empty(n, device="cuda")
+        ddf.ddf_query(m, o, d, n, d0, v0)
+        d1 = torch.full((n + 4,), -7.0, device="cuda"); v1 = torch.full((n + 4,), -7.0, device="cuda")
+        ddf.ddf_query_camera(m, cam, W, H, d1, v1)
+        torch.cuda.synchronize()
+        assert torch.equal(d1[:n], d0) and torch.equal(v1[:n], v0), (kind, W, H)
+        assert bool((d1[n:] == -7.0).all()) and bool((v1[n:] == -7.0).all())
+        if kind.startswith("hash"):
+            assert ddf.ddf_get_info(m, 1) == 1                # one launch, no generator
+    ddf.ddf_query_camera(m, cam, 0, 5, d1, v1)                 # empty image: a no-op
+    ddf.ddf_destroy(m)
