@@ -117,6 +117,9 @@ extern "C" int ddf_create(const void* weights, const ddf_layout* layout, ddf_mod
       const size_t smem = (gb + hb) * 16384 + blocks * wt * 128 + (size_t)(layout->n_hidden + 2) * wt * 4 + 64 + 1024;
       if (gb > 2 || smem > 232448) w_new = 256;
     }
+    // padding only pays if the wide kernel will take the padded network (<= 16 layers, encoding <= 256)
+    const size_t E1 = 3 + 6 * (size_t)layout->n_freq_origin + (layout->input_kind == 0 ? 3 + 6 * (size_t)layout->n_freq_dir : 0);
+    if (w_new >= 256 && (layout->n_hidden > 16 || E1 > 256)) w_new = 0;
   }
   if (w_new == 0) return create_impl(weights, layout, out);
   const ddf_layout& L = *layout;
