@@ -264,7 +264,7 @@ def sdf_eval(lay, blob, p, base_radius=1.0, alpha=0.05, mode=0, nthreads=0):
 
 
 def sphere_trace(lay, blob, o, d, max_steps=64, eps=1e-3, t_max=6.0, base_radius=1.0, alpha=0.05,
-                 mode=0, want_trace=False, nthreads=0):
+                 mode=0, want_trace=False, nthreads=0, omega=1.0):
     o, d = _f32(o), _f32(d)
     n = o.shape[0]
     L = _layout(lay)
@@ -274,9 +274,9 @@ def sphere_trace(lay, blob, o, d, max_steps=64, eps=1e-3, t_max=6.0, base_radius
     steps = np.empty(n, np.int32)
     tp = np.empty((n, max_steps, 3), np.float32) if want_trace else None
     ts = np.empty((n, max_steps), np.float32) if want_trace else None
-    rc = lib().orc_sphere_trace(C.byref(L), _p(b), _p(o), _p(d), C.c_int64(n), C.c_int(max_steps),
+    rc = lib().orc_sphere_trace_relaxed(C.byref(L), _p(b), _p(o), _p(d), C.c_int64(n), C.c_int(max_steps),
                                 C.c_float(eps), C.c_float(t_max), C.c_float(base_radius),
-                                C.c_float(alpha), C.c_int(mode), _p(t), _p(hit), _p(steps),
+                                C.c_float(alpha), C.c_float(omega), C.c_int(mode), _p(t), _p(hit), _p(steps),
                                 _p(tp) if want_trace else None, _p(ts) if want_trace else None,
                                 C.c_int(nthreads))
     if rc != 0:

@@ -387,6 +387,18 @@ int orc_sphere_trace(const orc_layout* L, const void* blob, const float* o, cons
                      int64_t n, int max_steps, float eps, float t_max, float base_radius,
                      float alpha, int mode, float* out_t, uint8_t* out_hit, int32_t* out_steps,
                      float* trace_p, float* trace_s, int nthreads) {
+  return orc_sphere_trace_relaxed(L, blob, o, d, n, max_steps, eps, t_max, base_radius, alpha, 1.0f, mode,
+                                  out_t, out_hit, out_steps, trace_p, trace_s, nthreads);
+}
+
+/* Over-relaxed sphere tracing (reading A19'): steps of omega * s with 1 <= omega < 2; when the
+ * spheres at the previous and at the current point do not touch (|s| + |s_prev| < t - t_prev) the
+ * relaxed step may have jumped a surface: go back to the plain position t_prev + s_prev and never
+ * relax this ray again.  omega = 1 is the plain rule of A19, bit for bit. */
+int orc_sphere_trace_relaxed(const orc_layout* L, const void* blob, const float* o, const float* d,
+                             int64_t n, int max_steps, float eps, float t_max, float base_radius,
+                             float alpha, float omega, int mode, float* out_t, uint8_t* out_hit, int32_t* out_steps,
+                             float* trace_p, float* trace_s, int nthreads) {
   if (!layout_ok(L) || L->input_kind != 1 || L->n_out != 1) return -1;
   const int E = orc_enc_dim(L), S = L->width + E > 2 * E ? L->width + E : 2 * E;
 #ifdef _OPENMP
@@ -399,7 +411,7 @@ int orc_sphere_trace(const orc_layout* L, const void* blob, const float* o, cons
     double* hin = (double*)malloc(sizeof(double) * S);
     #pragma omp for schedule(dynamic, 1)
     for (int64_t i = 0; i < n; ++i) {
-      float t = 0.0f; int hit = 0, steps = 0;
+      float t = 0.0f, t_prev = 0.0f, s_prev = 0.0f, om = omega > 1.0f ? omega : 1.0f; int hit = 0, steps = 0, have_prev = 0;
       if (trace_p) for (int k = 0; k < 3 * max_steps; ++k) trace_p[(size_t)i * 3 * max_steps + k] = NAN;
       if (trace_s) for (int k = 0; k < max_steps; ++k) trace_s[(size_t)i * max_steps + k] = NAN;
       for (int step = 0; step < max_steps; ++step) {
@@ -409,8 +421,14 @@ int orc_sphere_trace(const orc_layout* L, const void* blob, const float* o, cons
         steps = step + 1;
         if (trace_p) for (int a = 0; a < 3; ++a) trace_p[((size_t)i * max_steps + step) * 3 + a] = p[a];
         if (trace_s) trace_s[(size_t)i * max_steps + step] = s;
+        if (om > 1.0f && have_prev && fabsf(s) + fabsf(s_prev) < t - t_prev) {
+          t = t_prev + s_prev; om = 1.0f; have_prev = 0;          /* redo from the plain position */
+          if (t > t_max || t < 0.0f) break;
+          continue;
+        }
         if (fabsf(s) < eps) { hit = 1; break; }
-        t += s;
+        t_prev = t; s_prev = s; have_prev = 1;
+        t = fmaf(om, s, t);
         if (t > t_max || t < 0.0f) break;
       }
       out_t[i] = t; out_hit[i] = (uint8_t)hit; out_steps[i] = steps;

@@ -94,6 +94,11 @@ int orc_sphere_trace(const orc_layout* L, const void* blob, const float* o, cons
                      int64_t n, int max_steps, float eps, float t_max, float base_radius,
                      float alpha, int mode, float* out_t, uint8_t* out_hit, int32_t* out_steps,
                      float* trace_p, float* trace_s, int nthreads);
+/* the same with over-relaxed steps (rule in ddf_oracle.c); omega <= 1: plain */
+int orc_sphere_trace_relaxed(const orc_layout* L, const void* blob, const float* o, const float* d,
+                             int64_t n, int max_steps, float eps, float t_max, float base_radius,
+                             float alpha, float omega, int mode, float* out_t, uint8_t* out_hit,
+                             int32_t* out_steps, float* trace_p, float* trace_s, int nthreads);
 /* value of s at given points (teacher forcing, pin P12) */
 int orc_sdf_eval(const orc_layout* L, const void* blob, const float* p, int64_t n,
                  float base_radius, float alpha, int mode, double* s, int nthreads);

@@ -199,6 +199,38 @@ def test_sphere_trace_alpha0_reaches_analytic_distance(orc):
     assert np.all(steps >= 2) and np.all(np.isnan(ts[np.arange(len(o)), np.minimum(steps, 63)]) | (steps == 64))
 
 
+def test_over_relaxed_sphere_trace_is_safe_and_shorter(orc):
+    """reading A19': with the exact SDF of the unit sphere, steps of omega * s reach
+    the same hits at the analytic distance and fall back when a relaxed step jumps the surface (the
+    spheres at t_prev and t no longer touch); omega = 1 is the plain tracer bit for bit.  On this
+    scene relaxation only pays for omega = 1.1: from the camera the first step is 1.5 and almost
+    normal to the surface, so omega >= 1.2 overshoots, falls back and costs one evaluation more per
+    ray - which is why the CUDA tracer does not implement it."""
+    lay = Layout(1, 2, 0, 1, 4, -1, 1, 1)
+    blob = make_weights(lay)
+    cam = orc.camera_from_seed(MASTER_SEED, STREAMS["camera_pos"], 2.5)
+    o, d = orc.gen_camera(cam, 48, 48)
+    t1, h1, s1 = orc.sphere_trace(lay, blob, o, d, 64, 1e-3, 6.0, 1.0, 0.0)
+    ta, ha, sa = orc.sphere_trace(lay, blob, o, d, 64, 1e-3, 6.0, 1.0, 0.0, omega=1.0)
+    assert np.array_equal(t1, ta) and np.array_equal(h1, ha) and np.array_equal(s1, sa)
+    want = np.array([orc.ray_sphere(o[i], d[i], [0, 0, 0], 1.0) for i in range(len(o))])
+    ang = np.arccos(np.clip(d.astype(np.float64) @ (-np.array(list(cam.pos)) / 2.5), -1, 1))
+    lim = math.asin(1 / 2.5)
+    sure_hit, sure_miss = ang < lim - 0.02, ang > lim + 0.02
+    for om in (1.1, 1.2, 1.6, 1.9):
+        t, hit, steps, tp, ts = orc.sphere_trace(lay, blob, o, d, 64, 1e-3, 6.0, 1.0, 0.0, want_trace=True, omega=om)
+        assert np.all(hit[sure_hit] == 1) and np.all(hit[sure_miss] == 0)
+        gap = want[sure_hit] - t[sure_hit]
+        assert np.all(np.abs(gap) < 1e-3 / 0.19 + 1e-5)               # stops within eps of the surface, on either side
+        assert (steps.sum() < s1.sum()) == (om < 1.15), (om, steps.sum(), s1.sum())
+        # a ray through the centre: s_0 = 1.5, the relaxed step lands at t = 1.5 om; for om = 1.9 that is past the
+        # far side reach: |s_1| + |s_0| < 1.5 om  =>  fall back to t = 1.5 (the plain position)
+        c = int(np.argmin(ang))
+        if om == 1.9:
+            assert abs(ts[c, 0] - 1.5) < 1e-3 and abs(np.linalg.norm(tp[c, 2] - (o[c] + 1.5 * d[c]))) < 2e-3
+        assert np.all(t[sure_miss] > 6.0)
+
+
 def test_sphere_trace_mlp_term_is_orc_forward(orc):
     """s(p) = (|p| - R) + alpha * MLP(p): the MLP part is exactly the (pinned) forward pass."""
     lay = Layout(1, 3, 0, 2, 8, 1, 1, 1)
