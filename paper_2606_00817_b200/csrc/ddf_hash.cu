@@ -230,7 +230,13 @@ __global__ void __launch_bounds__(kHgThreads, 5) ddf_hash_kernel(const __grid_co
       ptx::tmem_ld_wait();
       const float* bl = fsm + l * 64;
       #pragma unroll
-      for (int i = 0; i < 64; ++i) r[i] = __float_as_uint(fmaxf(__uint_as_float(r[i]) + bl[i], 0.0f));
+      for (int i = 0; i < 16; ++i) {                                    // bias: broadcast 16-byte loads
+        const float4 b4 = reinterpret_cast<const float4*>(bl)[i];
+        r[4 * i + 0] = __float_as_uint(fmaxf(__uint_as_float(r[4 * i + 0]) + b4.x, 0.0f));
+        r[4 * i + 1] = __float_as_uint(fmaxf(__uint_as_float(r[4 * i + 1]) + b4.y, 0.0f));
+        r[4 * i + 2] = __float_as_uint(fmaxf(__uint_as_float(r[4 * i + 2]) + b4.z, 0.0f));
+        r[4 * i + 3] = __float_as_uint(fmaxf(__uint_as_float(r[4 * i + 3]) + b4.w, 0.0f));
+      }
       if (l < p.n_hidden - 1) {
         // MMA l has completed (the commit arrived), so the operand tile may be overwritten
         #pragma unroll
@@ -245,7 +251,13 @@ __global__ void __launch_bounds__(kHgThreads, 5) ddf_hash_kernel(const __grid_co
       } else {
         const float* hw = fsm + p.n_hidden * 64;
         #pragma unroll
-        for (int i = 0; i < 64; ++i) { z0 = fmaf(__uint_as_float(r[i]), hw[i], z0); z1 = fmaf(__uint_as_float(r[i]), hw[64 + i], z1); }
+        for (int i = 0; i < 16; ++i) {
+          const float4 a4 = reinterpret_cast<const float4*>(hw)[i], c4 = reinterpret_cast<const float4*>(hw + 64)[i];
+          z0 = fmaf(__uint_as_float(r[4 * i + 0]), a4.x, z0); z1 = fmaf(__uint_as_float(r[4 * i + 0]), c4.x, z1);
+          z0 = fmaf(__uint_as_float(r[4 * i + 1]), a4.y, z0); z1 = fmaf(__uint_as_float(r[4 * i + 1]), c4.y, z1);
+          z0 = fmaf(__uint_as_float(r[4 * i + 2]), a4.z, z0); z1 = fmaf(__uint_as_float(r[4 * i + 2]), c4.z, z1);
+          z0 = fmaf(__uint_as_float(r[4 * i + 3]), a4.w, z0); z1 = fmaf(__uint_as_float(r[4 * i + 3]), c4.w, z1);
+        }
       }
     }
     // ---- heads (t = distance, xi = visibility)

@@ -148,7 +148,13 @@ __global__ void __launch_bounds__(kNwThreads) ddf_narrow_kernel(const __grid_con
         ptx::tmem_ld32(taddr + hb * 64 + 32, *reinterpret_cast<uint32_t(*)[32]>(&r[32]));
         ptx::tmem_ld_wait();
         #pragma unroll
-        for (int i = 0; i < 64; ++i) r[i] = __float_as_uint(fmaxf(__uint_as_float(r[i]) + bl[hb * 64 + i], 0.0f));
+        for (int i = 0; i < 16; ++i) {                                  // bias: broadcast 16-byte loads
+          const float4 b4 = reinterpret_cast<const float4*>(bl + hb * 64)[i];
+          r[4 * i + 0] = __float_as_uint(fmaxf(__uint_as_float(r[4 * i + 0]) + b4.x, 0.0f));
+          r[4 * i + 1] = __float_as_uint(fmaxf(__uint_as_float(r[4 * i + 1]) + b4.y, 0.0f));
+          r[4 * i + 2] = __float_as_uint(fmaxf(__uint_as_float(r[4 * i + 2]) + b4.z, 0.0f));
+          r[4 * i + 3] = __float_as_uint(fmaxf(__uint_as_float(r[4 * i + 3]) + b4.w, 0.0f));
+        }
         if (l < last_layer) {
           // every MMA of this layer has completed (commit observed): the H tile may be overwritten
           #pragma unroll
@@ -163,7 +169,13 @@ __global__ void __launch_bounds__(kNwThreads) ddf_narrow_kernel(const __grid_con
         } else {
           const float* hw = fsm + p.n_hidden * W + hb * 64;
           #pragma unroll
-          for (int i = 0; i < 64; ++i) { z0 = fmaf(__uint_as_float(r[i]), hw[i], z0); z1 = fmaf(__uint_as_float(r[i]), hw[W + i], z1); }
+          for (int i = 0; i < 16; ++i) {
+            const float4 a4 = reinterpret_cast<const float4*>(hw)[i], c4 = reinterpret_cast<const float4*>(hw + W)[i];
+            z0 = fmaf(__uint_as_float(r[4 * i + 0]), a4.x, z0); z1 = fmaf(__uint_as_float(r[4 * i + 0]), c4.x, z1);
+            z0 = fmaf(__uint_as_float(r[4 * i + 1]), a4.y, z0); z1 = fmaf(__uint_as_float(r[4 * i + 1]), c4.y, z1);
+            z0 = fmaf(__uint_as_float(r[4 * i + 2]), a4.z, z0); z1 = fmaf(__uint_as_float(r[4 * i + 2]), c4.z, z1);
+            z0 = fmaf(__uint_as_float(r[4 * i + 3]), a4.w, z0); z1 = fmaf(__uint_as_float(r[4 * i + 3]), c4.w, z1);
+          }
         }
       }
     }
