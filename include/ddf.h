@@ -22,11 +22,14 @@
  *    contiguous, 4-byte aligned (16-byte alignment enables the vectorised path); [host] are
  *    host pointers.  Inputs and outputs must not alias.
  *  - All work is enqueued on `stream` (a cudaStream_t passed as void*; NULL = default stream);
- *    no call synchronises the stream except ddf_create / ddf_destroy / *_host variants.
+ *    no call synchronises the stream except ddf_create / ddf_destroy / ddf_trainer_create /
+ *    ddf_trainer_export / the *_host variants, and - only for models served by the CUDA-core path -
+ *    sdf_sphere_trace with early_exit and ddf_query_shadowed (their grids are sized on the host).
  *    Results are valid once the stream reaches the point after the call.
  *  - n == 0 is DDF_OK and a no-op; n < 0 or a NULL pointer with n > 0 is DDF_E_INVALID_ARG.
  *  - Results are a pure function of (weights, ray): independent of n and of the ray's position
- *    in the batch, bit-reproducible run to run.  Directions must be unit length (not checked).
+ *    in the batch, bit-reproducible run to run (training steps accumulate gradients with atomics
+ *    and are reproducible to rounding only).  Directions must be unit length (not checked).
  *  - A model (and a trainer) owns device workspaces that its calls reuse: use one model from one
  *    stream / host thread at a time; different models are independent.
  *  - There is no CPU fallback: without a CUDA device of compute capability 10.x the calls
