@@ -32,6 +32,16 @@ def test_paper_counts(orc):
     assert abs((2 * n + 8130) * 4 / 1e6 - 52.0) < 0.5             # "52 MB"
     offs = [orc.hash_level(lay, l)[2] for l in range(16)]
     assert offs == list(np.cumsum([0] + ent[:-1]))
+    # the same facts as a cited fixture (tests/golden/hashgrid_paper_counts.txt)
+    import os
+    gold = {}
+    for line in open(os.path.join(os.path.dirname(__file__), "golden", "hashgrid_paper_counts.txt")):
+        if line.strip() and not line.startswith("#"):
+            k, *v = line.split(); gold[k] = v
+    assert [int(x) for x in gold["resolutions"]] == res and int(gold["table_entries"][0]) == n
+    assert int(gold["table_parameters"][0]) == 2 * n and round(2 * n / 1e6) == int(gold["paper_table_parameters_millions"][0])
+    assert int(gold["mlp_parameters"][0]) == orc.hash_mlp_params(lay) and round(8130 / 1e3) == int(gold["paper_mlp_parameters_thousands"][0])
+    assert round((2 * n + 8130) * 4 / 1e6) == int(gold["paper_field_megabytes"][0])
 
 
 def test_index_formulas_by_hand(orc):
