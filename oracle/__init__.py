@@ -400,6 +400,17 @@ def hash_loss_grads(lay, table, mlp, o, d, t, hit, P, want_grads=True):
     return loss, gt, gm
 
 
+def hash_relu_margin(lay, table, mlp, o, d):
+    """min |pre-activation| over the hidden units, per ray (float64): the distance from a ReLU kink."""
+    o, d = _f32(o), _f32(d)
+    table, mlp = _f32(table), _f32(mlp)
+    L = _hlayout(lay)
+    out = np.empty(o.shape[0], np.float64)
+    rc = lib().orc_hash_relu_margin(C.byref(L), _p(table), _p(mlp), _p(o), _p(d), C.c_int64(o.shape[0]), _p(out))
+    assert rc == 0
+    return out
+
+
 def lr_at(P, step):
     return lib().orc_lr_at(C.byref(P), C.c_int64(step))
 

@@ -304,6 +304,45 @@ double orc_hash_loss_grads(const orc_hash_layout* L, const float* table, const f
   return loss / (double)n;
 }
 
+/* Distance of a ray from the nearest ReLU kink: min over all hidden units of |pre-activation|, fp64,
+ * the same forward pass as orc_hash_loss_grads.  The loss is not differentiable where a
+ * pre-activation is 0, and an implementation whose forward pass is rounded differently picks the
+ * other side of the kink for a ray within its rounding error of one (reading T7); the
+ * gradient parity tests use this to keep such rays out of large batches. */
+int orc_hash_relu_margin(const orc_hash_layout* L, const float* table, const float* mlp,
+                         const float* o, const float* d, int64_t n, double* margin) {
+  if (!hl_ok(L)) return -1;
+  const int E = orc_hash_mlp_in(L), W = L->width, H = L->n_hidden, NF = L->n_levels * L->n_features;
+  const int S = E > W ? E : W;
+  double* in = (double*)malloc(sizeof(double) * S);
+  double* out = (double*)malloc(sizeof(double) * S);
+  for (int64_t i = 0; i < n; ++i) {
+    encode_point(L, table, o + 3 * i, in);
+    int m = NF;
+    for (int c = 0; c < 3; ++c) in[m++] = (double)d[3 * i + c];
+    for (int k = 0; k < L->n_freq_dir; ++k) {
+      for (int c = 0; c < 3; ++c) in[m++] = sin(HPI * ldexp((double)d[3 * i + c], k));
+      for (int c = 0; c < 3; ++c) in[m++] = cos(HPI * ldexp((double)d[3 * i + c], k));
+    }
+    double best = INFINITY;
+    size_t off = 0; int nin = E;
+    for (int l = 0; l < H; ++l) {
+      const size_t boff = off + (size_t)W * nin;
+      for (int j = 0; j < W; ++j) {
+        double acc = (double)mlp[boff + j];
+        for (int k = 0; k < nin; ++k) acc += (double)mlp[off + (size_t)j * nin + k] * in[k];
+        if (fabs(acc) < best) best = fabs(acc);
+        out[j] = acc > 0.0 ? acc : 0.0;
+      }
+      for (int j = 0; j < W; ++j) in[j] = out[j];
+      off = boff + W; nin = W;
+    }
+    margin[i] = best;
+  }
+  free(in); free(out);
+  return 0;
+}
+
 double orc_lr_at(const orc_train_params* P, int64_t step) {
   const double s = step < P->total_steps ? (double)step : (double)P->total_steps;
   const double f = P->lr_final_frac;

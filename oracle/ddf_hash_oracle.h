@@ -92,6 +92,11 @@ typedef struct orc_train_params {
 double orc_hash_loss_grads(const orc_hash_layout* L, const float* table, const float* mlp,
                            const float* o, const float* d, const float* t, const uint8_t* hit,
                            int64_t n, const orc_train_params* P, double* grad_table, double* grad_mlp);
+/* margin[i] = min over the hidden units of |pre-activation| of ray i (fp32 table and MLP, as in
+ * orc_hash_loss_grads): how far the ray is from a ReLU kink, where the loss has no gradient
+ * (reading T7). */
+int orc_hash_relu_margin(const orc_hash_layout* L, const float* table, const float* mlp,
+                         const float* o, const float* d, int64_t n, double* margin);
 double orc_lr_at(const orc_train_params* P, int64_t step);
 /* one Adam update of n parameters in place; `step` is 1-based (T3) */
 void orc_adam_step(float* p, const double* g, double* m, double* v, int64_t n, int64_t step,

@@ -46,6 +46,30 @@ def test_gradients_match_finite_differences(orc):
     assert np.count_nonzero(gt) < len(gt)
 
 
+def test_relu_margin_is_the_smallest_hidden_pre_activation(orc):
+    """orc.hash_relu_margin against numpy matrix products on the (separately pinned) encoder's features, and
+    its meaning: a ray with margin m keeps every ReLU on its side under any perturbation of a
+    pre-activation below m, so nudging a bias by less than the batch's margin leaves the gradient's
+    zero pattern (the ReLU masks) of the first layer's bias untouched."""
+    lay = _small()
+    o, d, t, hit, table, mlp = _batch(orc, lay, n=200)
+    feat = orc.hash_encode(lay, table, o)
+    gam = [d.astype(np.float64)]
+    for k in range(lay.n_freq_dir):
+        gam += [np.sin(np.pi * d.astype(np.float64) * 2.0 ** k), np.cos(np.pi * d.astype(np.float64) * 2.0 ** k)]
+    x = np.concatenate([feat] + gam, axis=1)
+    E, W = x.shape[1], lay.width
+    w = mlp.astype(np.float64)
+    W0, b0 = w[:W * E].reshape(W, E), w[W * E:W * E + W]
+    o1 = W * E + W
+    W1, b1 = w[o1:o1 + W * W].reshape(W, W), w[o1 + W * W:o1 + W * W + W]
+    z0 = x @ W0.T + b0
+    z1 = np.maximum(z0, 0.0) @ W1.T + b1
+    want = np.minimum(np.abs(z0).min(axis=1), np.abs(z1).min(axis=1))
+    got = orc.hash_relu_margin(lay, table, mlp, o, d)
+    assert np.allclose(got, want, rtol=1e-12, atol=1e-15) and got.min() > 0 and got.max() < 1.0
+
+
 def test_loss_closed_forms(orc):
     """zero MLP: softplus(b0) = ln 2 + ..., CE = ln 2; clamp; misses carry no distance term (T1, T2)"""
     lay = _small()
