@@ -317,6 +317,7 @@ def run_extras(ddf, torch, model, peaks):
     ex["hashgrid_field"] = run_hashgrid(ddf, torch, peaks)
     ex["wavefront_shadowed_camera_2^20"] = run_wavefront(ddf, torch)
     ex["training_hashgrid"] = run_training(ddf, torch)
+    ex["training_hashgrid_fp32_cuda_cores"] = run_training(ddf, torch, arithmetic=1)
     ex["narrow_networks_2^20_random_rays"] = run_narrow(ddf, torch)
     return ex
 
@@ -346,7 +347,7 @@ def run_narrow(ddf, torch):
     return out
 
 
-def run_training(ddf, torch, steps=30000, batch=16384):
+def run_training(ddf, torch, steps=30000, batch=16384, arithmetic=0):
     """the paper's recipe (Adam, 30,000 steps, batch 16,384, lr 3e-3 with
     cosine decay to 5 %, clamped L1 + 0.3 CE, 30 % ray-march shifted samples) on an ANALYTIC scene (a
     sphere over a slab; the paper's scanned objects are not in the container), then the paper-style
@@ -357,7 +358,7 @@ def run_training(ddf, torch, steps=30000, batch=16384):
     lay = layout_hash_paper()
     n_ent = ddf.ddf_hashgrid_table_entries(lay)
     table, mlp = make_hash_table(lay, n_ent, scale=1e-4), make_hash_mlp(lay)
-    tr = ddf.ddf_trainer_create(table, mlp, lay, ddf.make_train_params(total_steps=steps))
+    tr = ddf.ddf_trainer_create(table, mlp, lay, ddf.make_train_params(total_steps=steps, arithmetic=arithmetic))
     scene = ddf.DdfScene((0.0, 0.0, 0.0), 0.5, (-0.9, -0.9, -0.9), (0.9, 0.9, -0.6))
     o = torch.empty((batch, 3), device="cuda"); d = torch.empty((batch, 3), device="cuda")
     t = torch.empty(batch, device="cuda"); hit = torch.empty(batch, dtype=torch.uint8, device="cuda")
@@ -371,7 +372,7 @@ def run_training(ddf, torch, steps=30000, batch=16384):
     e1.record(); torch.cuda.synchronize()
     sec = e0.elapsed_time(e1) / 1e3
     l = losses.cpu().numpy()
-    out = {"steps": steps, "batch": batch, "seconds": sec, "steps_per_s": steps / sec, "Mrays_per_s": steps * batch / sec / 1e6,
+    out = {"arithmetic": ["bf16x3 tensor cores", "fp32 CUDA cores"][arithmetic], "steps": steps, "batch": batch, "seconds": sec, "steps_per_s": steps / sec, "Mrays_per_s": steps * batch / sec / 1e6,
            "loss_first_100": float(l[:100].mean()), "loss_last_100": float(l[-100:].mean()),
            "paper_context": "30,000 steps x 16,384 rays in under an hour on one A100 (PAPER.md:86), PyTorch"}
     tt, mm = ddf.ddf_trainer_export(tr, 2 * n_ent, len(mlp))

@@ -225,7 +225,16 @@ typedef struct ddf_train_params {
   uint32_t struct_size;        /* sizeof(ddf_train_params) */
   float lr0, lr_final_frac; int32_t total_steps;
   float beta1, beta2, adam_eps, dist_clamp, ce_weight;
+  uint32_t arithmetic;         /* how the MLP products of the forward / backward pass are formed.
+                                * DDF_TRAIN_BF16X3: on the tensor cores; each fp32 operand is split into two
+                                * bf16 terms (16 mantissa bits together) and a product is three bf16 MMAs with
+                                * fp32 accumulation, relative error ~2^-16 per term.  DDF_TRAIN_FP32: on the
+                                * CUDA cores.  Parameters, moments, gradients, the loss, the head and the table
+                                * interpolation are fp32 either way (the paper trains in half precision,
+                                * PAPER.md:86; both choices here are tighter). */
 } ddf_train_params;
+#define DDF_TRAIN_BF16X3 0u
+#define DDF_TRAIN_FP32 1u
 typedef struct ddf_trainer ddf_trainer;
 /* table, mlp: [host] fp32 blobs in the ddf_create_hashgrid order (layout dtypes must be 0). */
 int  ddf_trainer_create(const float* table, const float* mlp, const ddf_hashgrid_layout* layout,

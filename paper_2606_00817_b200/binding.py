@@ -44,7 +44,7 @@ class DdfHashgridLayout(C.Structure):
 class DdfTrainParams(C.Structure):
     _fields_ = [("struct_size", C.c_uint32), ("lr0", C.c_float), ("lr_final_frac", C.c_float), ("total_steps", C.c_int32),
                 ("beta1", C.c_float), ("beta2", C.c_float), ("adam_eps", C.c_float), ("dist_clamp", C.c_float),
-                ("ce_weight", C.c_float)]
+                ("ce_weight", C.c_float), ("arithmetic", C.c_uint32)]
 
 
 class DdfCamera(C.Structure):
@@ -292,8 +292,10 @@ def ddf_query_shadowed(model, o, d, n, light, eps, out_dist, out_vis, out_lit, o
 # ------------------------------------------------------------------ training
 
 def make_train_params(lr0=3e-3, lr_final_frac=0.05, total_steps=30000, beta1=0.9, beta2=0.999, adam_eps=1e-8,
-                      dist_clamp=6.0, ce_weight=0.3):
-    return DdfTrainParams(C.sizeof(DdfTrainParams), lr0, lr_final_frac, total_steps, beta1, beta2, adam_eps, dist_clamp, ce_weight)
+                      dist_clamp=6.0, ce_weight=0.3, arithmetic=0):
+    """arithmetic: DDF_TRAIN_BF16X3 (0, tensor cores) or DDF_TRAIN_FP32 (1, CUDA cores); include/ddf.h."""
+    return DdfTrainParams(C.sizeof(DdfTrainParams), lr0, lr_final_frac, total_steps, beta1, beta2, adam_eps, dist_clamp,
+                          ce_weight, arithmetic)
 
 
 class Trainer:

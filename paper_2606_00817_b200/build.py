@@ -6,7 +6,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libddf.so")
-SOURCES = ["ddf_api.cu", "ddf_simt.cu", "ddf_gen.cu", "ddf_trace.cu", "ddf_tc.cu", "ddf_hash.cu", "ddf_wave.cu", "ddf_train.cu", "ddf_narrow.cu"]
+SOURCES = ["ddf_api.cu", "ddf_simt.cu", "ddf_gen.cu", "ddf_trace.cu", "ddf_tc.cu", "ddf_hash.cu", "ddf_wave.cu", "ddf_train.cu", "ddf_train_tc.cu", "ddf_narrow.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
          "-Xcompiler", "-fPIC", "-Wno-deprecated-gpu-targets"]

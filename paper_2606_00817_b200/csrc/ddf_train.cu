@@ -10,7 +10,7 @@
 // ray.  adam_kernel then updates every parameter (dense, as the paper's "Adam") and clears the
 // gradient.  Atomics make the sums order-dependent in the last bits: training is reproducible
 // to rounding, not bitwise.
-#include "ddf_common.cuh"
+#include "ddf_train.cuh"
 #include <math.h>
 #include <stdlib.h>
 #include <string.h>
@@ -18,64 +18,6 @@
 #include <vector>
 
 namespace ddf {
-
-constexpr int kTrRays = 128;            // rays per CTA
-constexpr int kTrThreads = 256;         // two threads per ray
-constexpr int kTrPitch = 129;
-constexpr int kTrW = 64;
-constexpr int kTrMaxLevels = 16;
-
-struct TrLevel { float scale; uint32_t verts; uint32_t offset; uint32_t hashed; };
-
-struct TrParams {
-  TrLevel lv[kTrMaxLevels];
-  const float* table; const float* mlp;          // fp32 master copies
-  float* g_table; float* g_mlp; float* loss;
-  const float* o; const float* d; const float* t; const uint8_t* hit;
-  int64_t n;
-  float bmin[3], den[3];
-  float dist_clamp, ce_weight;
-  uint32_t tmask;
-  int n_levels, Ld, n_hidden, E, NF;
-  int w_off[3], b_off[3];                        // blob offsets of layer l (l = n_hidden: head)
-};
-
-struct Trainer {
-  ddf_hashgrid_layout lay;
-  ddf_train_params prm;
-  int64_t entries, n_table, n_mlp, step;
-  float *p_table, *p_mlp, *m, *v, *g;            // m, v, g hold table values first, then the MLP
-  float* loss_dev;
-  TrParams base;
-  size_t smem_bytes;
-};
-
-// corner indices (into the table, in float2 units) and weights of one level
-__device__ __forceinline__ void tr_corners(const TrLevel& lv, uint32_t tmask, const float x01[3], uint32_t idx[8], float wt[8]) {
-  uint32_t c0[3]; float w1[3];
-  #pragma unroll
-  for (int a = 0; a < 3; ++a) {
-    const float pos = __fmul_rn(x01[a], lv.scale);
-    const float fl = fminf(floorf(pos), lv.scale - 1.0f);
-    c0[a] = (uint32_t)fl; w1[a] = pos - fl;
-  }
-  uint32_t kx[2], ky[2], kz[2];
-  if (lv.hashed) {
-    kx[0] = c0[0]; kx[1] = c0[0] + 1u;
-    ky[0] = c0[1] * 2654435761u; ky[1] = (c0[1] + 1u) * 2654435761u;
-    kz[0] = c0[2] * 805459861u;  kz[1] = (c0[2] + 1u) * 805459861u;
-  } else {
-    kx[0] = c0[0]; kx[1] = c0[0] + 1u;
-    ky[0] = c0[1] * lv.verts; ky[1] = ky[0] + lv.verts;
-    kz[0] = c0[2] * lv.verts * lv.verts; kz[1] = kz[0] + lv.verts * lv.verts;
-  }
-  #pragma unroll
-  for (int c = 0; c < 8; ++c) {
-    const uint32_t a = kx[c & 1], b = ky[(c >> 1) & 1], e = kz[c >> 2];
-    idx[c] = lv.offset + (lv.hashed ? ((a ^ b ^ e) & tmask) : (a + b + e));
-    wt[c] = ((c & 1) ? w1[0] : 1.0f - w1[0]) * (((c >> 1) & 1) ? w1[1] : 1.0f - w1[1]) * ((c >> 2) ? w1[2] : 1.0f - w1[2]);
-  }
-}
 
 // Two threads per ray: thread (r, h) with r = ray in the tile, h = 0 / 1.
 // out[j][r] = relu(b[j] + sum_k Wt[k][j] in[k][r]) for the 32 outputs j of half h, 8 per pass
@@ -264,14 +206,18 @@ __global__ void adam_kernel(float* __restrict__ prm, float* __restrict__ m, floa
   const bool aligned = ((reinterpret_cast<uintptr_t>(prm) | reinterpret_cast<uintptr_t>(m) | reinterpret_cast<uintptr_t>(v) |
                          reinterpret_cast<uintptr_t>(g)) & 15) == 0;
   const int64_t n4 = aligned ? (n >> 2) : 0;                  // the MLP slice of m / v / g may start on an 8-byte boundary
+  // The moments are touched once per step: stream them (evict-first), which leaves more of the parameters and of
+  // the gradient accumulator - what the next forward / backward pass gathers from and scatters to - in L2.
+  // (Explicit evict-last policies on those two made no further difference: DESIGN.md 13.)
   for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n4; i += stride) {
-    float4 gi = reinterpret_cast<float4*>(g)[i], mi = reinterpret_cast<float4*>(m)[i], vi = reinterpret_cast<float4*>(v)[i], pi = reinterpret_cast<float4*>(prm)[i];
+    float4 gi = reinterpret_cast<float4*>(g)[i], mi = __ldcs(reinterpret_cast<float4*>(m) + i), vi = __ldcs(reinterpret_cast<float4*>(v) + i),
+           pi = reinterpret_cast<float4*>(prm)[i];
     #define ADAM1(c) { mi.c = b1 * mi.c + (1.0f - b1) * gi.c; vi.c = b2 * vi.c + (1.0f - b2) * gi.c * gi.c; \
                        pi.c -= lr * (mi.c / c1) / (sqrtf(vi.c / c2) + eps); }
     ADAM1(x) ADAM1(y) ADAM1(z) ADAM1(w)
     #undef ADAM1
-    reinterpret_cast<float4*>(m)[i] = mi; reinterpret_cast<float4*>(v)[i] = vi; reinterpret_cast<float4*>(prm)[i] = pi;
-    reinterpret_cast<float4*>(g)[i] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+    __stcs(reinterpret_cast<float4*>(m) + i, mi); __stcs(reinterpret_cast<float4*>(v) + i, vi); reinterpret_cast<float4*>(prm)[i] = pi;
+    if (gi.x != 0.0f || gi.y != 0.0f || gi.z != 0.0f || gi.w != 0.0f) reinterpret_cast<float4*>(g)[i] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
   }
   for (int64_t i = (n4 << 2) + (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
     const float gi = g[i];
@@ -397,7 +343,8 @@ static int tr_check(const ddf_hashgrid_layout* L, const ddf_train_params* P) {
   if (L->struct_size != sizeof(ddf_hashgrid_layout) || L->version != DDF_LAYOUT_VERSION) return DDF_E_BAD_LAYOUT;
   if (P->struct_size != sizeof(ddf_train_params)) return DDF_E_BAD_LAYOUT;
   if (!(P->lr0 > 0.0f) || P->total_steps < 1 || !(P->beta1 >= 0.0f && P->beta1 < 1.0f) || !(P->beta2 >= 0.0f && P->beta2 < 1.0f) ||
-      !(P->adam_eps > 0.0f) || !(P->dist_clamp > 0.0f) || !(P->ce_weight >= 0.0f) || !(P->lr_final_frac >= 0.0f)) return DDF_E_INVALID_ARG;
+      !(P->adam_eps > 0.0f) || !(P->dist_clamp > 0.0f) || !(P->ce_weight >= 0.0f) || !(P->lr_final_frac >= 0.0f) ||
+      P->arithmetic > DDF_TRAIN_FP32) return DDF_E_INVALID_ARG;
   if (L->table_dtype != 0 || L->mlp_dtype != 0 || L->weights_on_device != 0) return DDF_E_BAD_LAYOUT;
   for (int a = 0; a < 3; ++a) if (!(L->box_max[a] > L->box_min[a])) return DDF_E_BAD_LAYOUT;
   if (L->n_features != 2 || L->n_levels < 1 || L->n_levels > (uint32_t)kTrMaxLevels || L->n_freq_dir > 4 || L->width != (uint32_t)kTrW ||
@@ -409,6 +356,7 @@ static int tr_check(const ddf_hashgrid_layout* L, const ddf_train_params* P) {
 static void tr_free(Trainer* T) {
   if (!T) return;
   cudaFree(T->p_table); cudaFree(T->p_mlp); cudaFree(T->m); cudaFree(T->v); cudaFree(T->g); cudaFree(T->loss_dev);
+  cudaFree(T->ws_feat); cudaFree(T->ws_dfeat); cudaFree(T->ws_slab);
   (void)cudaGetLastError();
   delete T;
 }
@@ -466,6 +414,10 @@ extern "C" int ddf_trainer_create(const float* table, const float* mlp, const dd
   p.n_levels = (int)L.n_levels; p.Ld = (int)L.n_freq_dir; p.n_hidden = H; p.E = E; p.NF = NF;
   T->smem_bytes = (size_t)((E + (H - 1) * kTrW) * kTrW + H * kTrW + 2 * kTrW + (H + 3) * kTrW * kTrPitch) * 4;
   if ((e = cudaFuncSetAttribute(train_fwd_bwd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T->smem_bytes)) != cudaSuccess) return fail(e);
+  if ((e = train_tc_prepare()) != cudaSuccess) return fail(e);
+  T->sms = prop.multiProcessorCount;
+  if (params->arithmetic == DDF_TRAIN_BF16X3 &&
+      (e = cudaMalloc(&T->ws_slab, (size_t)T->sms * train_tc_slab_floats() * 4)) != cudaSuccess) return fail(e);
   if ((e = cudaDeviceSynchronize()) != cudaSuccess) return fail(e);
   *out = reinterpret_cast<ddf_trainer*>(T);
   return DDF_OK;
@@ -485,11 +437,23 @@ extern "C" int64_t ddf_trainer_steps(const ddf_trainer* trainer) {
 static int tr_launch_grads(Trainer* T, const float* o, const float* d, const float* t, const uint8_t* hit, int64_t n, cudaStream_t st) {
   TrParams p = T->base;
   p.o = o; p.d = d; p.t = t; p.hit = hit; p.n = n;
-  DDF_CUDA_TRY(cudaMemsetAsync(T->loss_dev, 0, 4, st));
   const int64_t tiles = (n + kTrRays - 1) / kTrRays;
-  int sms = 0; DDF_CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, 0));
-  const unsigned grid = (unsigned)(tiles < sms ? tiles : sms);
-  train_fwd_bwd_kernel<<<grid, kTrThreads, T->smem_bytes, st>>>(p);
+  const unsigned grid = (unsigned)(tiles < T->sms ? tiles : T->sms);
+  if (T->prm.arithmetic == DDF_TRAIN_BF16X3) {
+    if (n > T->ws_rays) {                                      // grow the feature workspace (synchronises; rare)
+      DDF_CUDA_TRY(cudaDeviceSynchronize());
+      cudaFree(T->ws_feat); cudaFree(T->ws_dfeat); T->ws_feat = T->ws_dfeat = nullptr; T->ws_rays = 0;
+      const size_t bytes = (size_t)n * train_tc_feat_pitch() * 4;
+      DDF_CUDA_TRY(cudaMalloc(&T->ws_feat, bytes));
+      DDF_CUDA_TRY(cudaMalloc(&T->ws_dfeat, bytes));
+      T->ws_rays = n;
+    }
+    p.feat = T->ws_feat; p.dfeat = T->ws_dfeat; p.slab = T->ws_slab;
+    train_tc_launch(p, grid, st);                              // its first kernel clears the loss
+  } else {
+    DDF_CUDA_TRY(cudaMemsetAsync(T->loss_dev, 0, 4, st));
+    train_fwd_bwd_kernel<<<grid, kTrThreads, T->smem_bytes, st>>>(p);
+  }
   DDF_CUDA_TRY(cudaGetLastError());
   return DDF_OK;
 }

@@ -1,0 +1,76 @@
+// ddf_train.cuh - what the two training kernels share (ddf_train.cu: fp32 CUDA cores,
+// ddf_train_tc.cu: split-bf16 tensor cores): the parameter block, the trainer object, the corner rule.
+#pragma once
+#include "ddf_common.cuh"
+
+namespace ddf {
+
+constexpr int kTrRays = 128;            // rays per CTA
+constexpr int kTrThreads = 256;         // two threads per ray
+constexpr int kTrPitch = 129;
+constexpr int kTrW = 64;
+constexpr int kTrMaxLevels = 16;
+
+struct TrLevel { float scale; uint32_t verts; uint32_t offset; uint32_t hashed; };
+
+struct TrParams {
+  TrLevel lv[kTrMaxLevels];
+  const float* table; const float* mlp;          // fp32 master copies
+  float* g_table; float* g_mlp; float* loss;
+  const float* o; const float* d; const float* t; const uint8_t* hit;
+  int64_t n;
+  float bmin[3], den[3];
+  float dist_clamp, ce_weight;
+  uint32_t tmask;
+  int n_levels, Ld, n_hidden, E, NF;
+  int w_off[3], b_off[3];                        // blob offsets of layer l (l = n_hidden: head)
+  float* feat; float* dfeat; float* slab;        // tensor-core path: level features / their gradients [n][32], per-CTA dW
+};
+
+struct Trainer {
+  ddf_hashgrid_layout lay;
+  ddf_train_params prm;
+  int64_t entries, n_table, n_mlp, step;
+  float *p_table, *p_mlp, *m, *v, *g;            // m, v, g hold table values first, then the MLP
+  float* loss_dev;
+  TrParams base;
+  size_t smem_bytes;
+  float *ws_feat, *ws_dfeat, *ws_slab;           // tensor-core path workspace; ws_feat / ws_dfeat hold ws_rays rays
+  int64_t ws_rays;
+  int sms;
+};
+
+// corner indices (into the table, in float2 units) and weights of one level
+__device__ __forceinline__ void tr_corners(const TrLevel& lv, uint32_t tmask, const float x01[3], uint32_t idx[8], float wt[8]) {
+  uint32_t c0[3]; float w1[3];
+  #pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    const float pos = __fmul_rn(x01[a], lv.scale);
+    const float fl = fminf(floorf(pos), lv.scale - 1.0f);
+    c0[a] = (uint32_t)fl; w1[a] = pos - fl;
+  }
+  uint32_t kx[2], ky[2], kz[2];
+  if (lv.hashed) {
+    kx[0] = c0[0]; kx[1] = c0[0] + 1u;
+    ky[0] = c0[1] * 2654435761u; ky[1] = (c0[1] + 1u) * 2654435761u;
+    kz[0] = c0[2] * 805459861u;  kz[1] = (c0[2] + 1u) * 805459861u;
+  } else {
+    kx[0] = c0[0]; kx[1] = c0[0] + 1u;
+    ky[0] = c0[1] * lv.verts; ky[1] = ky[0] + lv.verts;
+    kz[0] = c0[2] * lv.verts * lv.verts; kz[1] = kz[0] + lv.verts * lv.verts;
+  }
+  #pragma unroll
+  for (int c = 0; c < 8; ++c) {
+    const uint32_t a = kx[c & 1], b = ky[(c >> 1) & 1], e = kz[c >> 2];
+    idx[c] = lv.offset + (lv.hashed ? ((a ^ b ^ e) & tmask) : (a + b + e));
+    wt[c] = ((c & 1) ? w1[0] : 1.0f - w1[0]) * (((c >> 1) & 1) ? w1[1] : 1.0f - w1[1]) * ((c >> 2) ? w1[2] : 1.0f - w1[2]);
+  }
+}
+
+// ddf_train_tc.cu
+size_t train_tc_slab_floats();
+size_t train_tc_feat_pitch();
+cudaError_t train_tc_prepare();
+void train_tc_launch(const TrParams& p, unsigned grid, cudaStream_t st);
+
+}  // namespace ddf

@@ -137,7 +137,7 @@ def test_trainer_and_wavefront_argument_errors_without_gpu(libddf):
     any CUDA call"""
     from ddf_inputs import HashLayout, layout_hash_paper
     from paper_2606_00817_b200 import DdfTrainParams, make_train_params, make_hashgrid_layout, DdfScene
-    assert C.sizeof(DdfTrainParams) == 36
+    assert C.sizeof(DdfTrainParams) == 40
     h = C.c_void_p(0)
     w = np.zeros(16, np.float32); wp = w.ctypes.data_as(C.c_void_p)
     L = make_hashgrid_layout(layout_hash_paper()); P = make_train_params()
@@ -146,6 +146,7 @@ def test_trainer_and_wavefront_argument_errors_without_gpu(libddf):
     assert libddf.ddf_trainer_create(wp, wp, C.byref(L), C.byref(bad), C.byref(h)) == -2
     assert libddf.ddf_trainer_create(wp, wp, C.byref(L), C.byref(make_train_params(lr0=-1.0)), C.byref(h)) == -1
     assert libddf.ddf_trainer_create(wp, wp, C.byref(L), C.byref(make_train_params(beta2=1.0)), C.byref(h)) == -1
+    assert libddf.ddf_trainer_create(wp, wp, C.byref(L), C.byref(make_train_params(arithmetic=2)), C.byref(h)) == -1
     f16 = make_hashgrid_layout(HashLayout(table_dtype=2))                 # training wants fp32 master copies
     assert libddf.ddf_trainer_create(wp, wp, C.byref(f16), C.byref(P), C.byref(h)) == -2
     deep = make_hashgrid_layout(HashLayout(n_hidden=3))

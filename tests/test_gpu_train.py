@@ -1,7 +1,10 @@
 """Training the hash-grid field on the GPU against oracle/ddf_hash_oracle.c:
 loss and gradients of one batch, Adam steps, the batch generator, and a short run whose loss falls.
-fp32 arithmetic with atomic accumulation on the GPU vs fp64 in the oracle: gradients must agree to
-2e-4 of their scale, parameters after k Adam steps to a few lr * 1e-2."""
+Both arithmetics of include/ddf.h run every test against the fp64 oracle.  DDF_TRAIN_FP32 (CUDA
+cores, atomic accumulation): gradients agree to 2e-4 of their scale.  DDF_TRAIN_BF16X3 (tensor cores,
+every operand split into two bf16 terms, lo x lo dropped): a product carries ~2^-16 relative error, far
+inside the same bound, so both are held to it.  Parameters after k Adam steps
+agree to a few lr * 1e-2 either way."""
 import numpy as np
 import pytest
 import torch
@@ -29,37 +32,75 @@ def _batch(n, seed=3):
     return (o * 1.5).astype(np.float32), d, rng.uniform(0.2, 3.0, n).astype(np.float32), (rng.uniform(size=n) < 0.6).astype(np.uint8)
 
 
+ARITH = [pytest.param(1, id="fp32"), pytest.param(0, id="bf16x3")]
+LOSS_TOL = {1: 2e-5, 0: 2e-5}
+GRAD_TOL = {1: 2e-4, 0: 2e-4}
+
+
+@pytest.mark.parametrize("arith", ARITH)
 @pytest.mark.parametrize("kw", [dict(n_levels=4, log2_table=10, base_res=4, growth=2.0, n_freq_dir=2, n_hidden=2),
                                 dict(n_levels=6, log2_table=12, n_freq_dir=4, n_hidden=1),
                                 dict()])
-def test_loss_and_gradients_match_oracle(ddf, orc, kw):
+def test_loss_and_gradients_match_oracle(ddf, orc, kw, arith):
     lay = HashLayout(**kw)
     n_ent = ddf.ddf_hashgrid_table_entries(lay)
     table = make_hash_table(lay, n_ent, scale=0.5); mlp = make_hash_mlp(lay, bias_scale=0.2)
     n = 1000 if kw else 300                                  # the paper-size table: fewer rays, the oracle's gradient is dense
     o, d, t, hit = _batch(n)
-    tr = ddf.ddf_trainer_create(table, mlp, lay, ddf.make_train_params(dist_clamp=2.0))
+    tr = ddf.ddf_trainer_create(table, mlp, lay, ddf.make_train_params(dist_clamp=2.0, arithmetic=arith))
     loss = torch.zeros(1, device="cuda"); gt = torch.empty(2 * n_ent, device="cuda"); gm = torch.empty(len(mlp), device="cuda")
     ddf.ddf_trainer_loss_grads(tr, _cuda(o), _cuda(d), _cuda(t), _cuda(hit), n, loss, gt, gm)
     torch.cuda.synchronize()
     rl, rgt, rgm = orc.hash_loss_grads(lay, table, mlp, o, d, t, hit, orc.train_params(dist_clamp=2.0))
-    assert abs(float(loss) - rl) < 2e-5 * max(1.0, abs(rl))
+    print("arith", arith, "loss err", abs(float(loss) - rl) / max(1.0, abs(rl)))
+    assert abs(float(loss) - rl) < LOSS_TOL[arith] * max(1.0, abs(rl))
     for g, r, what in ((gm.cpu().numpy(), rgm, "mlp"), (gt.cpu().numpy(), rgt, "table")):
         scale = np.abs(r).max()
-        assert scale > 0 and np.abs(g - r).max() <= 2e-4 * scale + 1e-9, (what, np.abs(g - r).max(), scale)
+        print("arith", arith, what, "max err / scale", np.abs(g - r).max() / scale, "rms err / rms", np.sqrt(((g - r) ** 2).mean() / (r ** 2).mean()))
+        assert scale > 0 and np.abs(g - r).max() <= GRAD_TOL[arith] * scale + 1e-9, (what, np.abs(g - r).max(), scale)
         assert np.array_equal(g == 0, r == 0) or what == "mlp"       # untouched table entries stay exactly zero
     # a second call gives the same answer: the accumulator was left clean
     ddf.ddf_trainer_loss_grads(tr, _cuda(o), _cuda(d), _cuda(t), _cuda(hit), n, loss, gt, gm)
-    assert np.abs(gm.cpu().numpy() - rgm).max() <= 2e-4 * np.abs(rgm).max()
+    assert np.abs(gm.cpu().numpy() - rgm).max() <= GRAD_TOL[arith] * np.abs(rgm).max()
     ddf.ddf_trainer_destroy(tr)
 
 
-def test_adam_steps_match_oracle(ddf, orc):
+@pytest.mark.parametrize("arith", ARITH)
+def test_more_tiles_than_sms_ragged_tail_and_a_growing_batch(ddf, orc, arith):
+    """40,001 rays = 313 tiles of 128 on 148 SMs: every CTA walks several tiles (the tensor-core path keeps its
+    weight-gradient accumulator in tensor memory across them) and the last tile has one ray; the same trainer
+    first sees a small batch, so its feature workspace has to grow."""
+    lay = HashLayout(n_levels=5, log2_table=11, base_res=4, growth=1.7, n_freq_dir=3, n_hidden=2)
+    n_ent = ddf.ddf_hashgrid_table_entries(lay)
+    table = make_hash_table(lay, n_ent, scale=0.5); mlp = make_hash_mlp(lay, bias_scale=0.2)
+    tr = ddf.ddf_trainer_create(table, mlp, lay, ddf.make_train_params(dist_clamp=2.0, arithmetic=arith))
+    P = orc.train_params(dist_clamp=2.0)
+    for n in (130, 40001):
+        o, d, t, hit = _batch(n + 600, seed=n)
+        # The loss has no gradient where a hidden pre-activation is 0, and a forward pass rounded at 2^-17
+        # (bf16x3) or 2^-24 (fp32) instead of fp64 puts a ray that close to a kink on the other side of it
+        # (DESIGN.md reading T7).  Among 40,000 rays x 128 units a few always are: keep the rays whose every
+        # pre-activation clears 1e-4 (about 1 % go) and compare the gradients of that batch.
+        keep = np.nonzero(orc.hash_relu_margin(lay, table, mlp, o, d) > 1e-4)[0][:n]
+        assert len(keep) == n
+        o, d, t, hit = (np.ascontiguousarray(a[keep]) for a in (o, d, t, hit))
+        loss = torch.zeros(1, device="cuda"); gt = torch.empty(2 * n_ent, device="cuda"); gm = torch.empty(len(mlp), device="cuda")
+        ddf.ddf_trainer_loss_grads(tr, _cuda(o), _cuda(d), _cuda(t), _cuda(hit), n, loss, gt, gm)
+        torch.cuda.synchronize()
+        rl, rgt, rgm = orc.hash_loss_grads(lay, table, mlp, o, d, t, hit, P)
+        assert abs(float(loss) - rl) < 5e-5 * max(1.0, abs(rl))                 # 313 atomic partial sums in fp32
+        for g, r in ((gm.cpu().numpy(), rgm), (gt.cpu().numpy(), rgt)):
+            assert np.abs(g - r).max() <= GRAD_TOL[arith] * np.abs(r).max() + 1e-9, (n, np.abs(g - r).max() / np.abs(r).max())
+    ddf.ddf_trainer_destroy(tr)
+
+
+@pytest.mark.parametrize("arith", ARITH)
+def test_adam_steps_match_oracle(ddf, orc, arith):
     lay = HashLayout(n_levels=4, log2_table=10, base_res=4, growth=2.0, n_freq_dir=2, n_hidden=2)
     n_ent = ddf.ddf_hashgrid_table_entries(lay)
     table = make_hash_table(lay, n_ent, scale=0.5); mlp = make_hash_mlp(lay, bias_scale=0.2)
     kwargs = dict(lr0=1e-2, total_steps=10, dist_clamp=2.0, adam_eps=1e-8)
-    tr = ddf.ddf_trainer_create(table, mlp, lay, ddf.make_train_params(**kwargs))
+    tr = ddf.ddf_trainer_create(table, mlp, lay, ddf.make_train_params(arithmetic=arith, **kwargs))
     P = orc.train_params(**kwargs)
     rt, rm = table.copy(), mlp.copy()
     mt, vt, mm, vm = np.zeros(len(rt)), np.zeros(len(rt)), np.zeros(len(rm)), np.zeros(len(rm))
@@ -114,11 +155,12 @@ def test_supervision_and_batch_generator(ddf, orc):
     assert 0.3 < hh.mean() < 0.95
 
 
-def test_short_training_run_reduces_the_loss_and_exports_a_usable_field(ddf, orc):
+@pytest.mark.parametrize("arith", ARITH)
+def test_short_training_run_reduces_the_loss_and_exports_a_usable_field(ddf, orc, arith):
     lay = layout_hash_paper()
     n_ent = ddf.ddf_hashgrid_table_entries(lay)
     table = make_hash_table(lay, n_ent, scale=1e-4); mlp = make_hash_mlp(lay)
-    tr = ddf.ddf_trainer_create(table, mlp, lay, ddf.make_train_params(total_steps=1500))
+    tr = ddf.ddf_trainer_create(table, mlp, lay, ddf.make_train_params(total_steps=1500, arithmetic=arith))
     sc = orc.TRAIN_SCENE
     scene = ddf.DdfScene(sc["sphere_c"], sc["sphere_r"], sc["bmin"], sc["bmax"])
     B = 16384
@@ -141,5 +183,6 @@ def test_short_training_run_reduces_the_loss_and_exports_a_usable_field(ddf, orc
     agree = ((vis > 0.5) == (hit > 0)).float().mean().item()
     hh = hit > 0
     err = (dist - t).abs()[hh].median().item()
+    print("arith", arith, "agree", agree, "median err", err, "loss", l[:3], l[-3:])
     assert agree > 0.88 and err < 0.06, (agree, err)
     ddf.ddf_destroy(m)
