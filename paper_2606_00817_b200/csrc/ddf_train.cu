@@ -199,17 +199,16 @@ __global__ void __launch_bounds__(kTrThreads, 1) train_fwd_bwd_kernel(const __gr
   if ((t & 31) == 0 && p.loss) atomicAdd(p.loss, block_loss / (float)p.n);
 }
 
-// dense Adam (reading T3) over n parameters; clears the gradient
-__global__ void adam_kernel(float* __restrict__ prm, float* __restrict__ m, float* __restrict__ v, float* __restrict__ g,
-                            int64_t n, float lr, float b1, float b2, float eps, float c1, float c2) {
-  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+// dense Adam (reading T3) over one slice of n parameters; clears the gradient
+__device__ __forceinline__ void adam_slice(float* __restrict__ prm, float* __restrict__ m, float* __restrict__ v, float* __restrict__ g,
+                                           int64_t n, int64_t first, int64_t stride, float lr, float b1, float b2, float eps, float c1, float c2) {
   const bool aligned = ((reinterpret_cast<uintptr_t>(prm) | reinterpret_cast<uintptr_t>(m) | reinterpret_cast<uintptr_t>(v) |
                          reinterpret_cast<uintptr_t>(g)) & 15) == 0;
   const int64_t n4 = aligned ? (n >> 2) : 0;                  // the MLP slice of m / v / g may start on an 8-byte boundary
   // The moments are touched once per step: stream them (evict-first), which leaves more of the parameters and of
   // the gradient accumulator - what the next forward / backward pass gathers from and scatters to - in L2.
   // (Explicit evict-last policies on those two made no further difference: DESIGN.md 13.)
-  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n4; i += stride) {
+  for (int64_t i = first; i < n4; i += stride) {
     float4 gi = reinterpret_cast<float4*>(g)[i], mi = __ldcs(reinterpret_cast<float4*>(m) + i), vi = __ldcs(reinterpret_cast<float4*>(v) + i),
            pi = reinterpret_cast<float4*>(prm)[i];
     #define ADAM1(c) { mi.c = b1 * mi.c + (1.0f - b1) * gi.c; vi.c = b2 * vi.c + (1.0f - b2) * gi.c * gi.c; \
@@ -219,13 +218,26 @@ __global__ void adam_kernel(float* __restrict__ prm, float* __restrict__ m, floa
     __stcs(reinterpret_cast<float4*>(m) + i, mi); __stcs(reinterpret_cast<float4*>(v) + i, vi); reinterpret_cast<float4*>(prm)[i] = pi;
     if (gi.x != 0.0f || gi.y != 0.0f || gi.z != 0.0f || gi.w != 0.0f) reinterpret_cast<float4*>(g)[i] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
   }
-  for (int64_t i = (n4 << 2) + (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+  for (int64_t i = (n4 << 2) + first; i < n; i += stride) {
     const float gi = g[i];
     const float mi = b1 * m[i] + (1.0f - b1) * gi;
     const float vi = b2 * v[i] + (1.0f - b2) * gi * gi;
     m[i] = mi; v[i] = vi; g[i] = 0.0f;
     prm[i] -= lr * (mi / c1) / (sqrtf(vi / c2) + eps);
   }
+}
+
+// the first mlp_blocks blocks update the MLP (its moments and gradient follow the table's in m, v, g), the rest the table
+__global__ void adam_kernel(float* __restrict__ p_table, float* __restrict__ p_mlp, float* __restrict__ m, float* __restrict__ v,
+                            float* __restrict__ g, int64_t n_table, int64_t n_mlp, int mlp_blocks,
+                            float lr, float b1, float b2, float eps, float c1, float c2) {
+  pdl_wait();                                                  // the gradients are the scatter kernel's output
+  if ((int)blockIdx.x < mlp_blocks)
+    adam_slice(p_mlp, m + n_table, v + n_table, g + n_table, n_mlp, (int64_t)blockIdx.x * blockDim.x + threadIdx.x,
+               (int64_t)mlp_blocks * blockDim.x, lr, b1, b2, eps, c1, c2);
+  else
+    adam_slice(p_table, m, v, g, n_table, (int64_t)(blockIdx.x - mlp_blocks) * blockDim.x + threadIdx.x,
+               (int64_t)(gridDim.x - mlp_blocks) * blockDim.x, lr, b1, b2, eps, c1, c2);
 }
 
 // ------------------------------------------------------------------------------------------ supervision
@@ -449,7 +461,7 @@ static int tr_launch_grads(Trainer* T, const float* o, const float* d, const flo
       T->ws_rays = n;
     }
     p.feat = T->ws_feat; p.dfeat = T->ws_dfeat; p.slab = T->ws_slab;
-    train_tc_launch(p, grid, st);                              // its first kernel clears the loss
+    DDF_CUDA_TRY(train_tc_launch(p, grid, st));                // its first kernel clears the loss
   } else {
     DDF_CUDA_TRY(cudaMemsetAsync(T->loss_dev, 0, 4, st));
     train_fwd_bwd_kernel<<<grid, kTrThreads, T->smem_bytes, st>>>(p);
@@ -489,9 +501,8 @@ extern "C" int ddf_trainer_step(ddf_trainer* trainer, const float* o, const floa
   const double lr = (double)P.lr0 * (f + (1.0 - f) * 0.5 * (1.0 + cos(3.14159265358979323846 * s0 / (double)P.total_steps)));
   const int64_t s1 = T->step + 1;
   const double c1 = 1.0 - pow((double)P.beta1, (double)s1), c2 = 1.0 - pow((double)P.beta2, (double)s1);
-  adam_kernel<<<148 * 8, 256, 0, st>>>(T->p_table, T->m, T->v, T->g, T->n_table, (float)lr, P.beta1, P.beta2, P.adam_eps, (float)c1, (float)c2);
-  adam_kernel<<<8, 256, 0, st>>>(T->p_mlp, T->m + T->n_table, T->v + T->n_table, T->g + T->n_table, T->n_mlp, (float)lr, P.beta1, P.beta2, P.adam_eps, (float)c1, (float)c2);
-  DDF_CUDA_TRY(cudaGetLastError());
+  DDF_CUDA_TRY(launch_pdl(adam_kernel, (unsigned)(T->sms * 8 + 8), 256u, 0, st, T->p_table, T->p_mlp, T->m, T->v, T->g, T->n_table, T->n_mlp, 8,
+                          (float)lr, P.beta1, P.beta2, P.adam_eps, (float)c1, (float)c2));
   T->step = s1;
   return DDF_OK;
 }

@@ -2,6 +2,7 @@
 // ddf_train_tc.cu: split-bf16 tensor cores): the parameter block, the trainer object, the corner rule.
 #pragma once
 #include "ddf_common.cuh"
+#include <utility>
 
 namespace ddf {
 
@@ -67,10 +68,28 @@ __device__ __forceinline__ void tr_corners(const TrLevel& lv, uint32_t tmask, co
   }
 }
 
+// Programmatic dependent launch: a kernel launched with launch_pdl may be scheduled while its predecessor in
+// the stream is still running (as soon as every CTA of the predecessor has executed pdl_launch_dependents or
+// exited); it must execute pdl_wait before it touches anything the predecessor writes.  pdl_wait returns when
+// the predecessor grid has completed and its writes are visible.  Used along the chain gather -> MLP ->
+// scatter -> Adam, so that launch latencies and the MLP kernel's prologue overlap the kernel before.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_pdl(void (*kernel)(KArgs...), unsigned grid, unsigned block, size_t smem, cudaStream_t st, Args&&... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(grid); cfg.blockDim = dim3(block); cfg.dynamicSmemBytes = smem; cfg.stream = st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at; cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, kernel, std::forward<Args>(args)...);
+}
+
 // ddf_train_tc.cu
 size_t train_tc_slab_floats();
 size_t train_tc_feat_pitch();
 cudaError_t train_tc_prepare();
-void train_tc_launch(const TrParams& p, unsigned grid, cudaStream_t st);
+cudaError_t train_tc_launch(const TrParams& p, unsigned grid, cudaStream_t st);
 
 }  // namespace ddf

@@ -122,6 +122,8 @@ __device__ __forceinline__ void mma_x3(uint32_t d, uint32_t a_hi, uint32_t a_lo,
 
 // one thread per (ray, level): feat[ray][2 l .. 2 l + 1] = the interpolated features of that level
 __global__ void __launch_bounds__(256) tc_gather_kernel(const __grid_constant__ TrParams p) {
+  pdl_wait();                                                  // the table is the previous step's Adam output
+  pdl_launch_dependents();
   const int L = p.n_levels;
   const int64_t idx = (int64_t)blockIdx.x * 256 + threadIdx.x;
   if (idx == 0 && p.loss) *p.loss = 0.0f;
@@ -147,6 +149,8 @@ __global__ void __launch_bounds__(256) tc_gather_kernel(const __grid_constant__ 
 // the 8 float2 atomics of that level's gradient
 __global__ void __launch_bounds__(256) tc_scatter_kernel(const __grid_constant__ TrParams p, int n_slabs) {
   constexpr int kHead = kReduceBlocks * kSlabSplit;
+  pdl_wait();
+  pdl_launch_dependents();
   if ((int)blockIdx.x < kHead) {
     const int part = (int)blockIdx.x / kReduceBlocks;
     const int e = ((int)blockIdx.x - part * kReduceBlocks) * 256 + threadIdx.x;
@@ -216,6 +220,10 @@ __global__ void __launch_bounds__(kTrThreads, 1) tc_mlp_kernel(const __grid_cons
   const uint32_t idF = ptx::idesc_bf16_f32_major(128, 64, 0, 0), idB = ptx::idesc_bf16_f32_major(128, 64, 0, 1),
                  idW = ptx::idesc_bf16_f32_major(128, 64 * H, 1, 1);
   uint32_t phase = 0;
+  // everything above read only the MLP parameters (final since the gather kernel started: it waited for the
+  // Adam pass before it); what follows reads the gather kernel's features
+  pdl_wait();
+  pdl_launch_dependents();
 
   float block_loss = 0.0f;
   bool first_tile = true;
@@ -423,11 +431,12 @@ cudaError_t train_tc_prepare() {
   return cudaFuncSetAttribute(tc_mlp_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
 }
 // p.feat / p.dfeat: n x 32 floats each; p.slab: grid x train_tc_slab_floats()
-void train_tc_launch(const TrParams& p, unsigned grid, cudaStream_t st) {
+cudaError_t train_tc_launch(const TrParams& p, unsigned grid, cudaStream_t st) {
   const unsigned pair_blocks = (unsigned)((p.n * p.n_levels + 255) / 256);
-  tc_gather_kernel<<<pair_blocks, 256, 0, st>>>(p);
-  tc_mlp_kernel<<<grid, kTrThreads, kSmemBytes, st>>>(p);
-  tc_scatter_kernel<<<pair_blocks + kReduceBlocks * kSlabSplit, 256, 0, st>>>(p, (int)grid);
+  cudaError_t e;
+  if ((e = launch_pdl(tc_gather_kernel, pair_blocks, 256, 0, st, p)) != cudaSuccess) return e;
+  if ((e = launch_pdl(tc_mlp_kernel, grid, kTrThreads, kSmemBytes, st, p)) != cudaSuccess) return e;
+  return launch_pdl(tc_scatter_kernel, pair_blocks + kReduceBlocks * kSlabSplit, 256, 0, st, p, (int)grid);
 }
 
 }  // namespace ddf
