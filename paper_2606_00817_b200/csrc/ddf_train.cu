@@ -200,8 +200,10 @@ __global__ void __launch_bounds__(kTrThreads, 1) train_fwd_bwd_kernel(const __gr
 }
 
 // dense Adam (reading T3) over one slice of n parameters; clears the gradient
+// rep: kTrRep copies of g[0 .. 4 rep4) that hold part of the gradient (tensor-core path); folded in and cleared here
 __device__ __forceinline__ void adam_slice(float* __restrict__ prm, float* __restrict__ m, float* __restrict__ v, float* __restrict__ g,
-                                           int64_t n, int64_t first, int64_t stride, float lr, float b1, float b2, float eps, float c1, float c2) {
+                                           int64_t n, int64_t first, int64_t stride, float lr, float b1, float b2, float eps, float c1, float c2,
+                                           float* __restrict__ rep = nullptr, int64_t rep4 = 0) {
   const bool aligned = ((reinterpret_cast<uintptr_t>(prm) | reinterpret_cast<uintptr_t>(m) | reinterpret_cast<uintptr_t>(v) |
                          reinterpret_cast<uintptr_t>(g)) & 15) == 0;
   const int64_t n4 = aligned ? (n >> 2) : 0;                  // the MLP slice of m / v / g may start on an 8-byte boundary
@@ -211,6 +213,14 @@ __device__ __forceinline__ void adam_slice(float* __restrict__ prm, float* __res
   for (int64_t i = first; i < n4; i += stride) {
     float4 gi = reinterpret_cast<float4*>(g)[i], mi = __ldcs(reinterpret_cast<float4*>(m) + i), vi = __ldcs(reinterpret_cast<float4*>(v) + i),
            pi = reinterpret_cast<float4*>(prm)[i];
+    if (i < rep4) {
+      #pragma unroll
+      for (int k = 0; k < kTrRep; ++k) {
+        float4* r = reinterpret_cast<float4*>(rep) + k * rep4 + i;
+        const float4 q = *r;
+        if (q.x != 0.0f || q.y != 0.0f || q.z != 0.0f || q.w != 0.0f) { gi.x += q.x; gi.y += q.y; gi.z += q.z; gi.w += q.w; *r = make_float4(0.0f, 0.0f, 0.0f, 0.0f); }
+      }
+    }
     #define ADAM1(c) { mi.c = b1 * mi.c + (1.0f - b1) * gi.c; vi.c = b2 * vi.c + (1.0f - b2) * gi.c * gi.c; \
                        pi.c -= lr * (mi.c / c1) / (sqrtf(vi.c / c2) + eps); }
     ADAM1(x) ADAM1(y) ADAM1(z) ADAM1(w)
@@ -230,14 +240,29 @@ __device__ __forceinline__ void adam_slice(float* __restrict__ prm, float* __res
 // the first mlp_blocks blocks update the MLP (its moments and gradient follow the table's in m, v, g), the rest the table
 __global__ void adam_kernel(float* __restrict__ p_table, float* __restrict__ p_mlp, float* __restrict__ m, float* __restrict__ v,
                             float* __restrict__ g, int64_t n_table, int64_t n_mlp, int mlp_blocks,
-                            float lr, float b1, float b2, float eps, float c1, float c2) {
+                            float lr, float b1, float b2, float eps, float c1, float c2, float* __restrict__ rep, int64_t rep4) {
   pdl_wait();                                                  // the gradients are the scatter kernel's output
   if ((int)blockIdx.x < mlp_blocks)
     adam_slice(p_mlp, m + n_table, v + n_table, g + n_table, n_mlp, (int64_t)blockIdx.x * blockDim.x + threadIdx.x,
                (int64_t)mlp_blocks * blockDim.x, lr, b1, b2, eps, c1, c2);
   else
     adam_slice(p_table, m, v, g, n_table, (int64_t)(blockIdx.x - mlp_blocks) * blockDim.x + threadIdx.x,
-               (int64_t)(gridDim.x - mlp_blocks) * blockDim.x, lr, b1, b2, eps, c1, c2);
+               (int64_t)(gridDim.x - mlp_blocks) * blockDim.x, lr, b1, b2, eps, c1, c2, rep, rep4);
+}
+
+// the same fold for ddf_trainer_loss_grads, which reads the gradient without an update
+__global__ void fold_rep_kernel(float* __restrict__ g, float* __restrict__ rep, int64_t rep4) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= rep4) return;
+  float4 gi = reinterpret_cast<float4*>(g)[i];
+  #pragma unroll
+  for (int k = 0; k < kTrRep; ++k) {
+    float4* r = reinterpret_cast<float4*>(rep) + k * rep4 + i;
+    const float4 q = *r;
+    gi.x += q.x; gi.y += q.y; gi.z += q.z; gi.w += q.w;
+    *r = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+  }
+  reinterpret_cast<float4*>(g)[i] = gi;
 }
 
 // ------------------------------------------------------------------------------------------ supervision
@@ -368,7 +393,7 @@ static int tr_check(const ddf_hashgrid_layout* L, const ddf_train_params* P) {
 static void tr_free(Trainer* T) {
   if (!T) return;
   cudaFree(T->p_table); cudaFree(T->p_mlp); cudaFree(T->m); cudaFree(T->v); cudaFree(T->g); cudaFree(T->loss_dev);
-  cudaFree(T->ws_feat); cudaFree(T->ws_dfeat); cudaFree(T->ws_slab);
+  cudaFree(T->ws_feat); cudaFree(T->ws_dfeat); cudaFree(T->ws_slab); cudaFree(T->ws_rep);
   (void)cudaGetLastError();
   delete T;
 }
@@ -418,6 +443,21 @@ extern "C" int ddf_trainer_create(const float* table, const float* mlp, const dd
       p.lv[l].scale = (float)N; p.lv[l].verts = (uint32_t)V; p.lv[l].hashed = dense ? 0u : 1u; p.lv[l].offset = (uint32_t)o2;
       o2 += dense ? V * V * V : Tn;
     }
+  }
+  if (params->arithmetic == DDF_TRAIN_BF16X3) {                // coarse levels: private gradient copies (ddf_train_tc.cu)
+    int64_t pre = 0; int lv = 0;
+    for (uint32_t l = 0; l < L.n_levels; ++l) {
+      const int64_t ent = (l + 1 < L.n_levels ? (int64_t)p.lv[l + 1].offset : entries) - (int64_t)p.lv[l].offset;
+      if (ent > kTrRepLevelMax) break;
+      if (((pre + ent) & 1) == 0) { p.rep_entries = (uint32_t)(pre + ent); p.rep_levels = (int)l + 1; }   // whole float4s only
+      pre += ent; lv = (int)l + 1;
+    }
+    (void)lv;
+    if (p.rep_entries) {
+      const size_t bytes = (size_t)kTrRep * p.rep_entries * 2 * 4;
+      if ((e = cudaMalloc(&T->ws_rep, bytes)) != cudaSuccess || (e = cudaMemset(T->ws_rep, 0, bytes)) != cudaSuccess) return fail(e);
+    }
+    p.rep = T->ws_rep;
   }
   p.table = T->p_table; p.mlp = T->p_mlp; p.g_table = T->g; p.g_mlp = T->g + T->n_table; p.loss = T->loss_dev;
   for (int a = 0; a < 3; ++a) { p.bmin[a] = L.box_min[a]; p.den[a] = L.box_max[a] - L.box_min[a]; }
@@ -479,6 +519,11 @@ extern "C" int ddf_trainer_loss_grads(ddf_trainer* trainer, const float* o, cons
   const size_t total = (size_t)(T->n_table + T->n_mlp);
   int rc = tr_launch_grads(T, o, d, t, hit, n, st);
   if (rc != DDF_OK) return rc;
+  if (T->base.rep_entries) {
+    const int64_t rep4 = (int64_t)T->base.rep_entries / 2;
+    fold_rep_kernel<<<(unsigned)((rep4 + 255) / 256), 256, 0, st>>>(T->g, T->ws_rep, rep4);
+    DDF_CUDA_TRY(cudaGetLastError());
+  }
   if (loss) DDF_CUDA_TRY(cudaMemcpyAsync(loss, T->loss_dev, 4, cudaMemcpyDeviceToDevice, st));
   if (grad_table) DDF_CUDA_TRY(cudaMemcpyAsync(grad_table, T->g, (size_t)T->n_table * 4, cudaMemcpyDeviceToDevice, st));
   if (grad_mlp) DDF_CUDA_TRY(cudaMemcpyAsync(grad_mlp, T->g + T->n_table, (size_t)T->n_mlp * 4, cudaMemcpyDeviceToDevice, st));
@@ -502,7 +547,7 @@ extern "C" int ddf_trainer_step(ddf_trainer* trainer, const float* o, const floa
   const int64_t s1 = T->step + 1;
   const double c1 = 1.0 - pow((double)P.beta1, (double)s1), c2 = 1.0 - pow((double)P.beta2, (double)s1);
   DDF_CUDA_TRY(launch_pdl(adam_kernel, (unsigned)(T->sms * 8 + 8), 256u, 0, st, T->p_table, T->p_mlp, T->m, T->v, T->g, T->n_table, T->n_mlp, 8,
-                          (float)lr, P.beta1, P.beta2, P.adam_eps, (float)c1, (float)c2));
+                          (float)lr, P.beta1, P.beta2, P.adam_eps, (float)c1, (float)c2, T->ws_rep, (int64_t)T->base.rep_entries / 2));
   T->step = s1;
   return DDF_OK;
 }

@@ -11,6 +11,8 @@ constexpr int kTrThreads = 256;         // two threads per ray
 constexpr int kTrPitch = 129;
 constexpr int kTrW = 64;
 constexpr int kTrMaxLevels = 16;
+constexpr int kTrRep = 8;               // copies of the coarse levels' gradient accumulator (tensor-core path)
+constexpr int64_t kTrRepLevelMax = 32768;   // levels with at most this many entries are replicated
 
 struct TrLevel { float scale; uint32_t verts; uint32_t offset; uint32_t hashed; };
 
@@ -26,6 +28,7 @@ struct TrParams {
   int n_levels, Ld, n_hidden, E, NF;
   int w_off[3], b_off[3];                        // blob offsets of layer l (l = n_hidden: head)
   float* feat; float* dfeat; float* slab;        // tensor-core path: level features / their gradients [n][32], per-CTA dW
+  float* rep; uint32_t rep_entries; int rep_levels;   // kTrRep private copies of the gradient of the first rep_levels levels (rep_entries entries)
 };
 
 struct Trainer {
@@ -36,7 +39,7 @@ struct Trainer {
   float* loss_dev;
   TrParams base;
   size_t smem_bytes;
-  float *ws_feat, *ws_dfeat, *ws_slab;           // tensor-core path workspace; ws_feat / ws_dfeat hold ws_rays rays
+  float *ws_feat, *ws_dfeat, *ws_slab, *ws_rep;  // tensor-core path workspace; ws_feat / ws_dfeat hold ws_rays rays
   int64_t ws_rays;
   int sms;
 };

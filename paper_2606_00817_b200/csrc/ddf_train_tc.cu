@@ -178,8 +178,13 @@ __global__ void __launch_bounds__(256) tc_scatter_kernel(const __grid_constant__
   }
   uint32_t ix[8]; float wt[8];
   tr_corners(p.lv[l], p.tmask, x01, ix, wt);
+  // The coarsest levels have few entries (17^3, 25^3 for the paper's grid) and every ray of the batch lands on
+  // them: 8-27 atomics per address.  They go to one of kTrRep private copies, chosen by the ray; the Adam pass
+  // (or fold_rep_kernel) adds the copies up.
+  float2* dst = reinterpret_cast<float2*>(p.g_table);
+  if (l < p.rep_levels) dst = reinterpret_cast<float2*>(p.rep) + (size_t)(ray & (kTrRep - 1)) * p.rep_entries;
   #pragma unroll
-  for (int c = 0; c < 8; ++c) atomicAdd(reinterpret_cast<float2*>(p.g_table) + ix[c], make_float2(wt[c] * g.x, wt[c] * g.y));
+  for (int c = 0; c < 8; ++c) atomicAdd(dst + ix[c], make_float2(wt[c] * g.x, wt[c] * g.y));
 }
 
 __global__ void __launch_bounds__(kTrThreads, 1) tc_mlp_kernel(const __grid_constant__ TrParams p) {
