@@ -218,9 +218,14 @@ int  ddf_query_shadowed(ddf_model* model, const float* o, const float* d, int64_
  * shifted points.  Readings T1-T6:
  *   per ray  l = hit * min(|softplus(z0) - t|, dist_clamp) + ce_weight * CE(sigmoid(z1), hit),
  *   loss = mean over the batch; Adam as published, bias-corrected, dense over every parameter;
- *   lr(s) = lr0 (f + (1-f)(1 + cos(pi min(s,S)/S))/2);  fp32 master parameters and arithmetic.
+ *   lr(s) = lr0 (f + (1-f)(1 + cos(pi min(s,S)/S))/2);  fp32 master parameters; the arithmetic of the
+ *   hidden layers' products is ddf_train_params.arithmetic.
  * The trainer owns fp32 copies of the table and the MLP (+ Adam moments and a gradient buffer:
- * 4 x the field size).  This build trains n_features == 2, width == 64, n_hidden <= 2. */
+ * 4 x the field size) and, for DDF_TRAIN_BF16X3, a workspace of 256 bytes per ray of the largest
+ * batch seen (it grows, synchronising the device, when a larger batch arrives).  This build trains
+ * n_features == 2, width == 64, n_hidden <= 2.  A step is 4 kernels (gather, MLP, scatter, Adam)
+ * chained on `stream` by programmatic dependent launch; like every call here it is ordered after
+ * the work already in `stream` and needs no synchronisation. */
 typedef struct ddf_train_params {
   uint32_t struct_size;        /* sizeof(ddf_train_params) */
   float lr0, lr_final_frac; int32_t total_steps;
