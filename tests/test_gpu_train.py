@@ -125,6 +125,42 @@ def test_adam_steps_match_oracle(ddf, orc, arith):
     ddf.ddf_trainer_destroy(tr)
 
 
+@pytest.mark.parametrize("arith", ARITH)
+def test_steps_on_a_side_stream_follow_the_work_already_in_it(ddf, orc, arith):
+    """The kernels of a step are chained by programmatic dependent launch: each may be scheduled before its
+    predecessor has finished and waits where it first needs it.  Batches are generated and consumed back to
+    back on a side stream, with no synchronisation, into ONE set of buffers that the next generator call
+    overwrites; the result must be the run that synchronises after every call."""
+    lay = HashLayout(n_levels=6, log2_table=12, n_freq_dir=4, n_hidden=2)
+    n_ent = ddf.ddf_hashgrid_table_entries(lay)
+    table = make_hash_table(lay, n_ent, scale=0.5); mlp = make_hash_mlp(lay, bias_scale=0.2)
+    sc = orc.TRAIN_SCENE
+    scene = ddf.DdfScene(sc["sphere_c"], sc["sphere_r"], sc["bmin"], sc["bmax"])
+    B, steps = 5000, 12
+    out = []
+    for mode in ("async", "sync"):
+        tr = ddf.ddf_trainer_create(table, mlp, lay, ddf.make_train_params(total_steps=steps, lr0=1e-3, arithmetic=arith))
+        st = torch.cuda.Stream()
+        o = torch.empty((B, 3), device="cuda"); d = torch.empty((B, 3), device="cuda")
+        t = torch.empty(B, device="cuda"); hit = torch.empty(B, dtype=torch.uint8, device="cuda")
+        losses = torch.zeros(steps, device="cuda")
+        torch.cuda.synchronize()
+        for s in range(steps):
+            ddf.ddf_gen_train_batch(scene, MASTER_SEED, STREAMS["train_rays"], s, B, 2.0, o, d, t, hit, stream=st.cuda_stream)
+            if mode == "sync": torch.cuda.synchronize()
+            ddf.ddf_trainer_step(tr, o, d, t, hit, B, losses[s:s + 1], stream=st.cuda_stream)
+            if mode == "sync": torch.cuda.synchronize()
+        torch.cuda.synchronize()
+        tt, mm = ddf.ddf_trainer_export(tr, 2 * n_ent, len(mlp))
+        out.append((losses.cpu().numpy(), tt, mm))
+        ddf.ddf_trainer_destroy(tr)
+    (la, ta, ma), (ls, ts, ms) = out
+    assert np.isfinite(la).all() and np.allclose(la, ls, rtol=2e-4, atol=1e-6), (la, ls)
+    # atomics reorder the sums, Adam divides by sqrt(v): compare in units of the total step budget (12 x lr)
+    assert np.abs(ma - ms).max() < 0.05 * steps * 1e-3 and np.abs(ta - ts).max() < 0.05 * steps * 1e-3
+    assert np.abs(ma - ms).mean() < 1e-5 and np.abs(ta - ts).mean() < 1e-5
+
+
 def test_supervision_and_batch_generator(ddf, orc):
     sc = orc.TRAIN_SCENE
     scene = ddf.DdfScene(sc["sphere_c"], sc["sphere_r"], sc["bmin"], sc["bmax"])
