@@ -309,6 +309,8 @@ __device__ __forceinline__ void tr_dir_from_u(float u1, float u2, float out[3]) 
 
 __global__ void gen_train_batch_kernel(ddf_scene sc, uint64_t key, int64_t step, int64_t n, float sample_half,
                                        float* __restrict__ o, float* __restrict__ d, float* __restrict__ t, uint8_t* __restrict__ hit) {
+  pdl_wait();                                                  // the buffers may still be read by the step before
+  pdl_launch_dependents();
   const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (k >= n) return;
   const uint64_t base = ((uint64_t)step * (uint64_t)n + (uint64_t)k) * 16ull;
@@ -370,8 +372,7 @@ extern "C" int ddf_gen_train_batch(const ddf_scene* scene, uint64_t seed, uint64
   if (n == 0) return DDF_OK;
   if (!o || !d || !t || !hit) return DDF_E_INVALID_ARG;
   const uint64_t key = tr_mix64(tr_mix64(seed) ^ rng_stream);
-  gen_train_batch_kernel<<<(unsigned)((n + 255) / 256), 256, 0, (cudaStream_t)stream>>>(*scene, key, step, n, sample_half, o, d, t, hit);
-  DDF_CUDA_TRY(cudaGetLastError());
+  DDF_CUDA_TRY(launch_pdl(gen_train_batch_kernel, (unsigned)((n + 255) / 256), 256u, 0, (cudaStream_t)stream, *scene, key, step, n, sample_half, o, d, t, hit));
   return DDF_OK;
 }
 
