@@ -138,9 +138,21 @@ __global__ void __launch_bounds__(256) tc_gather_kernel(const __grid_constant__ 
   }
   uint32_t ix[8]; float wt[8];
   tr_corners(p.lv[l], p.tmask, x01, ix, wt);
+  // The two x-neighbours of a cell edge are entries i and i ^ 1 half of the time (always when x is even on a
+  // hashed level: the hash is an XOR with x): then they are one aligned 16-byte access instead of two 8-byte ones.
   float f0 = 0.0f, f1 = 0.0f;
   #pragma unroll
-  for (int c = 0; c < 8; ++c) { const float2 v = __ldg(reinterpret_cast<const float2*>(p.table) + ix[c]); f0 = fmaf(wt[c], v.x, f0); f1 = fmaf(wt[c], v.y, f1); }
+  for (int c = 0; c < 8; c += 2) {
+    if ((ix[c] ^ ix[c + 1]) == 1u) {
+      const float4 v = __ldg(reinterpret_cast<const float4*>(p.table) + (ix[c] >> 1));
+      const bool sw = ix[c] & 1u;                              // corner c is the odd entry
+      const float wa = sw ? wt[c + 1] : wt[c], wb = sw ? wt[c] : wt[c + 1];
+      f0 = fmaf(wa, v.x, f0); f1 = fmaf(wa, v.y, f1); f0 = fmaf(wb, v.z, f0); f1 = fmaf(wb, v.w, f1);
+    } else {
+      const float2 v0 = __ldg(reinterpret_cast<const float2*>(p.table) + ix[c]), v1 = __ldg(reinterpret_cast<const float2*>(p.table) + ix[c + 1]);
+      f0 = fmaf(wt[c], v0.x, f0); f1 = fmaf(wt[c], v0.y, f1); f0 = fmaf(wt[c + 1], v1.x, f0); f1 = fmaf(wt[c + 1], v1.y, f1);
+    }
+  }
   *reinterpret_cast<float2*>(p.feat + ray * kFeatPitch + 2 * l) = make_float2(f0, f1);
 }
 
@@ -184,7 +196,16 @@ __global__ void __launch_bounds__(256) tc_scatter_kernel(const __grid_constant__
   float2* dst = reinterpret_cast<float2*>(p.g_table);
   if (l < p.rep_levels) dst = reinterpret_cast<float2*>(p.rep) + (size_t)(ray & (kTrRep - 1)) * p.rep_entries;
   #pragma unroll
-  for (int c = 0; c < 8; ++c) atomicAdd(dst + ix[c], make_float2(wt[c] * g.x, wt[c] * g.y));
+  for (int c = 0; c < 8; c += 2) {
+    if ((ix[c] ^ ix[c + 1]) == 1u) {                           // entries i, i ^ 1: one 16-byte atomic (see the gather)
+      const bool sw = ix[c] & 1u;
+      const float wa = sw ? wt[c + 1] : wt[c], wb = sw ? wt[c] : wt[c + 1];
+      atomicAdd(reinterpret_cast<float4*>(dst) + (ix[c] >> 1), make_float4(wa * g.x, wa * g.y, wb * g.x, wb * g.y));
+    } else {
+      atomicAdd(dst + ix[c], make_float2(wt[c] * g.x, wt[c] * g.y));
+      atomicAdd(dst + ix[c + 1], make_float2(wt[c + 1] * g.x, wt[c + 1] * g.y));
+    }
+  }
 }
 
 __global__ void __launch_bounds__(kTrThreads, 1) tc_mlp_kernel(const __grid_constant__ TrParams p) {
