@@ -463,6 +463,12 @@ def run_wavefront(ddf, torch):
         k = int(cnt.item())
         out[name] = {"ms": ms, "shadow_rays": k, "lit_fraction_of_hits": float(lit.sum().item()) / max(k, 1),
                      "launches": ddf.ddf_get_info(m, 1), "Mrays_s_primary_plus_secondary": (n + k) / ms / 1e3}
+        # three point lights from the same hit points (ddf_query_shadowed_lights): one primary query, three shadow queries
+        lights = [(3.0, 3.0, 3.0), (-3.0, 2.0, 1.0), (0.5, -4.0, 2.5)]
+        ms3 = _time_ms(torch, lambda: ddf.ddf_query_shadowed_lights(m, o, d, n, lights, 1e-3, dist, vis, lit, cnt), reps=5)
+        k3 = int(cnt.item())
+        out[name]["three_lights"] = {"ms": ms3, "shadow_rays": k3, "launches": ddf.ddf_get_info(m, 1),
+                                     "Mrays_s_primary_plus_secondary": (n + k3) / ms3 / 1e3}
         ddf.ddf_destroy(m)
     return out
 

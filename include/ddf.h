@@ -210,6 +210,15 @@ int  ddf_gen_shadow_from_hits(ddf_model* model, const float* o, const float* d, 
 int  ddf_query_shadowed(ddf_model* model, const float* o, const float* d, int64_t n,
                         const float light[3], float eps, float* out_dist, float* out_vis,
                         uint8_t* out_lit, int64_t* out_count, void* stream);
+/* The same loop for several point lights (PAPER.md:80 evaluates f "toward the light"; a scene has
+ * more than one): lights [host] float[n_lights][3], 1 <= n_lights <= 8.  The primary query and the
+ * ranking of the hits run once; every light then gets its own shadow rays from the same hit points,
+ * its own second query and bit j of out_lit_mask[i] (1 = ray i hit and light j is not occluded).
+ * out_count receives the number of shadow rays traced, hits x n_lights.  With n_lights == 1 this is
+ * ddf_query_shadowed bit for bit. */
+int  ddf_query_shadowed_lights(ddf_model* model, const float* o, const float* d, int64_t n,
+                               const float* lights, int n_lights, float eps, float* out_dist,
+                               float* out_vis, uint8_t* out_lit_mask, int64_t* out_count, void* stream);
 
 /* ---------------------------------------------------------------- training the hash-grid field
  * PAPER.md:70 / 86: "an L1 term on distance, clamped at the box scale, plus a cross-entropy term

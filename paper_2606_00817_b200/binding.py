@@ -16,7 +16,7 @@ EXPORTED_SYMBOLS = [
     "ddf_get_info", "ddf_query", "ddf_query_host", "ddf_query_logits", "ddf_camera_from_seed",
     "ddf_gen_camera", "ddf_gen_sphere_points", "ddf_gen_shadow", "ddf_gen_gbuffer", "ddf_gen_ao",
     "ddf_ao_reduce", "ddf_query_ao", "ddf_shadow_test", "sdf_sphere_trace",
-    "ddf_hashgrid_table_entries", "ddf_create_hashgrid", "ddf_gen_shadow_from_hits", "ddf_query_shadowed",
+    "ddf_hashgrid_table_entries", "ddf_create_hashgrid", "ddf_gen_shadow_from_hits", "ddf_query_shadowed", "ddf_query_shadowed_lights",
     "ddf_trainer_create", "ddf_trainer_destroy", "ddf_trainer_step", "ddf_trainer_loss_grads", "ddf_trainer_export",
     "ddf_trainer_steps", "ddf_scene_raycast", "ddf_gen_train_batch", "ddf_query_camera",
 ]
@@ -287,6 +287,14 @@ def ddf_query_shadowed(model, o, d, n, light, eps, out_dist, out_vis, out_lit, o
     _check(lib().ddf_query_shadowed(model.handle, _dev(o), _dev(d), C.c_int64(n), li, C.c_float(eps), _dev(out_dist),
                                     _dev(out_vis), _dev(out_lit, torch.uint8), _dev(out_count, torch.int64),
                                     _stream(stream)), "ddf_query_shadowed")
+
+
+def ddf_query_shadowed_lights(model, o, d, n, lights, eps, out_dist, out_vis, out_lit_mask, out_count=None, stream=None):
+    flat = [float(x) for l in lights for x in l]
+    li = (C.c_float * len(flat))(*flat)
+    _check(lib().ddf_query_shadowed_lights(model.handle, _dev(o), _dev(d), C.c_int64(n), li, C.c_int(len(flat) // 3), C.c_float(eps),
+                                           _dev(out_dist), _dev(out_vis), _dev(out_lit_mask, torch.uint8),
+                                           _dev(out_count, torch.int64), _stream(stream)), "ddf_query_shadowed_lights")
 
 
 # ------------------------------------------------------------------ training

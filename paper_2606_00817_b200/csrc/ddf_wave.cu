@@ -77,13 +77,17 @@ __global__ void wave_scatter_kernel(const float* __restrict__ o, const float* __
   index[k] = (int32_t)i;
 }
 
-// lit[index[k]] = not occluded, for k < *count (lit was zeroed before: primary misses stay 0)
+// bit `bit` of lit[index[k]] = light not occluded, for k < *count (lit was zeroed before: primary misses stay 0;
+// every k owns its own byte, and the lights run one after the other in the stream); the last light also
+// reports the number of shadow rays traced, *count x n_lights
 __global__ void wave_lit_kernel(const float* __restrict__ vis2, const float* __restrict__ dist2,
                                 const float* __restrict__ tmax, const int32_t* __restrict__ index,
-                                const int64_t* __restrict__ count, uint8_t* __restrict__ lit) {
+                                const int64_t* __restrict__ count, uint8_t* __restrict__ lit, int bit,
+                                int64_t* __restrict__ out_count, int n_lights) {
   const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (k == 0 && out_count) *out_count = *count * n_lights;
   if (k >= *count) return;
-  lit[index[k]] = (vis2[k] > 0.5f && dist2[k] < tmax[k]) ? 0 : 1;
+  if (!(vis2[k] > 0.5f && dist2[k] < tmax[k])) lit[index[k]] |= (uint8_t)(1u << bit);
 }
 
 struct WaveWs { int32_t* block_counts; float *o2, *d2, *tmax, *dist2, *vis2; int32_t* index; int64_t* count; };
@@ -113,12 +117,18 @@ static int wave_ws(Model* m, int64_t n, bool full, WaveWs* w) {
   return DDF_OK;
 }
 
-static int wave_compact(Model* m, const WaveWs& w, const float* o, const float* d, const float* dist, const float* vis,
-                        int64_t n, const float light[3], float eps, float* o2, float* d2, float* tmax, int32_t* index,
-                        int64_t* count, cudaStream_t st) {
+// count + scan once per primary batch, then one scatter per light
+static int wave_count(const WaveWs& w, const float* vis, int64_t n, int64_t* count, cudaStream_t st) {
   const unsigned nb = (unsigned)((n + kWaveBlock - 1) / kWaveBlock);
   wave_count_kernel<<<nb, kWaveBlock, 0, st>>>(vis, n, w.block_counts);
   wave_scan_kernel<<<1, 1024, 0, st>>>(w.block_counts, (int64_t)nb, count);
+  DDF_CUDA_TRY(cudaGetLastError());
+  return DDF_OK;
+}
+static int wave_scatter(const WaveWs& w, const float* o, const float* d, const float* dist, const float* vis,
+                        int64_t n, const float light[3], float eps, float* o2, float* d2, float* tmax, int32_t* index,
+                        cudaStream_t st) {
+  const unsigned nb = (unsigned)((n + kWaveBlock - 1) / kWaveBlock);
   wave_scatter_kernel<<<nb, kWaveBlock, 0, st>>>(o, d, dist, vis, n, light[0], light[1], light[2], eps,
                                                 w.block_counts, o2, d2, tmax, index);
   DDF_CUDA_TRY(cudaGetLastError());
@@ -141,45 +151,59 @@ extern "C" int ddf_gen_shadow_from_hits(ddf_model* model, const float* o, const 
   WaveWs w;
   int rc = wave_ws(m, n, false, &w);
   if (rc != DDF_OK) return rc;
-  rc = wave_compact(m, w, o, d, dist, vis, n, light, eps, o2, d2, tmax, index, count, st);
+  if ((rc = wave_count(w, vis, n, count, st)) != DDF_OK) return rc;
+  rc = wave_scatter(w, o, d, dist, vis, n, light, eps, o2, d2, tmax, index, st);
   m->last_launches = 3;
   return rc;
 }
 
-extern "C" int ddf_query_shadowed(ddf_model* model, const float* o, const float* d, int64_t n,
-                                  const float light[3], float eps, float* out_dist, float* out_vis,
-                                  uint8_t* out_lit, int64_t* out_count, void* stream) {
-  if (!model || !light || n < 0 || n > 0x7fffffff) return DDF_E_INVALID_ARG;
+extern "C" int ddf_query_shadowed_lights(ddf_model* model, const float* o, const float* d, int64_t n,
+                                         const float* lights, int n_lights, float eps, float* out_dist,
+                                         float* out_vis, uint8_t* out_lit_mask, int64_t* out_count, void* stream) {
+  if (!model || !lights || n < 0 || n > 0x7fffffff || n_lights < 1 || n_lights > 8) return DDF_E_INVALID_ARG;
   Model* m = reinterpret_cast<Model*>(model);
   if (m->lay.input_kind != 0 || m->lay.n_out != 2) return DDF_E_INVALID_ARG;
   cudaStream_t st = (cudaStream_t)stream;
   if (n == 0) { if (out_count) DDF_CUDA_TRY(cudaMemsetAsync(out_count, 0, 8, st)); m->last_launches = 0; return DDF_OK; }
-  if (!o || !d || !out_dist || !out_vis || !out_lit) return DDF_E_INVALID_ARG;
+  if (!o || !d || !out_dist || !out_vis || !out_lit_mask) return DDF_E_INVALID_ARG;
   WaveWs w;
   int rc = wave_ws(m, n, true, &w);
   if (rc != DDF_OK) return rc;
   // 1. primary rays
   if ((rc = ddf_query(model, o, d, n, out_dist, out_vis, stream)) != DDF_OK) return rc;
   int launches = m->last_launches;
-  // 2. hit points -> compacted shadow rays
-  if ((rc = wave_compact(m, w, o, d, out_dist, out_vis, n, light, eps, w.o2, w.d2, w.tmax, w.index, w.count, st)) != DDF_OK) return rc;
-  launches += 3;
-  DDF_CUDA_TRY(cudaMemsetAsync(out_lit, 0, (size_t)n, st));
-  // 3. second query on the compacted batch; the fused paths read its size on the device
-  if (has_fused_path(m)) rc = fused_forward(m, w.o2, w.d2, n, w.count, 0, w.dist2, w.vis2, 0, 0.0f, st);
-  else {
-    int64_t live = 0;                                    // the SIMT path sizes its grids on the host
-    DDF_CUDA_TRY(cudaMemcpyAsync(&live, w.count, 8, cudaMemcpyDeviceToHost, st));
-    DDF_CUDA_TRY(cudaStreamSynchronize(st));
-    rc = live > 0 ? simt_forward(m, w.o2, w.d2, live, 0, w.dist2, w.vis2, st) : DDF_OK;
-    if (live == 0) m->last_launches = 0;
+  // 2. where the hits go in the compacted batch (the same for every light)
+  if ((rc = wave_count(w, out_vis, n, w.count, st)) != DDF_OK) return rc;
+  launches += 2;
+  DDF_CUDA_TRY(cudaMemsetAsync(out_lit_mask, 0, (size_t)n, st));
+  int64_t live = -1;
+  for (int j = 0; j < n_lights; ++j) {
+    // 3. shadow rays toward light j, 4. second query; the fused paths read the batch size on the device
+    if ((rc = wave_scatter(w, o, d, out_dist, out_vis, n, lights + 3 * j, eps, w.o2, w.d2, w.tmax, w.index, st)) != DDF_OK) return rc;
+    if (has_fused_path(m)) rc = fused_forward(m, w.o2, w.d2, n, w.count, 0, w.dist2, w.vis2, 0, 0.0f, st);
+    else {
+      if (live < 0) {                                      // the SIMT path sizes its grids on the host
+        DDF_CUDA_TRY(cudaMemcpyAsync(&live, w.count, 8, cudaMemcpyDeviceToHost, st));
+        DDF_CUDA_TRY(cudaStreamSynchronize(st));
+      }
+      rc = live > 0 ? simt_forward(m, w.o2, w.d2, live, 0, w.dist2, w.vis2, st) : DDF_OK;
+      if (live == 0) m->last_launches = 0;
+    }
+    if (rc != DDF_OK) return rc;
+    launches += 1 + m->last_launches;
+    // 5. shadow decision for light j, scattered back to bit j of the primary rays
+    wave_lit_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(w.vis2, w.dist2, w.tmax, w.index, w.count, out_lit_mask, j,
+                                                                 j == n_lights - 1 ? out_count : nullptr, n_lights);
+    DDF_CUDA_TRY(cudaGetLastError());
+    launches += 1;
   }
-  if (rc != DDF_OK) return rc;
-  launches += m->last_launches;
-  // 4. shadow decision, scattered back to the primary rays
-  wave_lit_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(w.vis2, w.dist2, w.tmax, w.index, w.count, out_lit);
-  DDF_CUDA_TRY(cudaGetLastError());
-  if (out_count) DDF_CUDA_TRY(cudaMemcpyAsync(out_count, w.count, 8, cudaMemcpyDeviceToDevice, st));
-  m->last_launches = launches + 1;
+  m->last_launches = launches;
   return DDF_OK;
+}
+
+extern "C" int ddf_query_shadowed(ddf_model* model, const float* o, const float* d, int64_t n,
+                                  const float light[3], float eps, float* out_dist, float* out_vis,
+                                  uint8_t* out_lit, int64_t* out_count, void* stream) {
+  if (!light) return DDF_E_INVALID_ARG;
+  return ddf_query_shadowed_lights(model, o, d, n, light, 1, eps, out_dist, out_vis, out_lit, out_count, stream);
 }

@@ -159,4 +159,5 @@ def test_trainer_and_wavefront_argument_errors_without_gpu(libddf):
     assert libddf.ddf_gen_train_batch(C.byref(sc), C.c_uint64(1), C.c_uint64(1), C.c_int64(-1), C.c_int64(4), C.c_float(2.0), None, None, None, None, None) == -1
     li = (C.c_float * 3)(1, 2, 3)
     assert libddf.ddf_query_shadowed(None, None, None, C.c_int64(4), li, C.c_float(1e-3), None, None, None, None, None) == -1
+    assert libddf.ddf_query_shadowed_lights(None, None, None, C.c_int64(4), li, C.c_int(1), C.c_float(1e-3), None, None, None, None, None) == -1
     assert libddf.ddf_gen_shadow_from_hits(None, None, None, None, None, C.c_int64(4), li, C.c_float(1e-3), None, None, None, None, None, None) == -1

@@ -110,6 +110,26 @@ def test_gpu_wavefront_against_twin(orc):
         ref = ~((xi2 > 0.5) & (t2 < rt[sel]))
         got = lit.cpu().numpy()[ridx[sel]].astype(bool)
         assert np.array_equal(got[safe], ref[safe]) and safe.mean() > 0.5, name
+        # several lights: bit j of the mask is the single-light answer for light j (verified above for the first),
+        # the primary results are the same, every hit is traced once per light
+        lights = [light, (-3.0, 2.0, 1.0), (0.5, -4.0, 2.5)]
+        mask = torch.full((n,), 0xAA, dtype=torch.uint8, device="cuda"); c3 = torch.zeros(1, dtype=torch.int64, device="cuda")
+        dm = torch.empty(n, device="cuda"); vm = torch.empty(n, device="cuda")
+        ddf.ddf_query_shadowed_lights(m, o, d, n, lights, 1e-3, dm, vm, mask, c3)
+        assert int(c3.item()) == 3 * k and torch.equal(dm, dist) and torch.equal(vm, vis)
+        assert int(mask.max().item()) < 8
+        for j, lj in enumerate(lights):
+            one = torch.empty(n, dtype=torch.uint8, device="cuda")
+            ddf.ddf_query_shadowed(m, o, d, n, lj, 1e-3, dist, vis, one, None)
+            assert torch.equal((mask >> j) & 1, one), (name, j)
+            if j:                                            # the other lights against the oracle too, on a sample
+                qo2, qd2, qt, qidx = orc.gen_shadow_from_hits(o.cpu().numpy(), d.cpu().numpy(), dist.cpu().numpy(), vis.cpu().numpy(), lj, 1e-3)
+                z, t2, xi2 = oracle_fwd(orc, qo2[sel], qd2[sel])
+                safe = (np.abs(xi2 - 0.5) > 1e-2) & (np.abs(t2 - qt[sel]) > 1e-2 * (1 + np.abs(t2)))
+                ref = ~((xi2 > 0.5) & (t2 < qt[sel]))
+                got = one.cpu().numpy()[qidx[sel]].astype(bool)
+                assert np.array_equal(got[safe], ref[safe]) and safe.mean() > 0.5, (name, j)
+        assert len(set(int(x) for x in mask.unique().cpu())) > 2          # the lights disagree somewhere
         # n = 0 and determinism
         ddf.ddf_query_shadowed(m, o, d, 0, light, 1e-3, dist, vis, lit, cnt)
         assert int(cnt.item()) == 0
