@@ -24,14 +24,18 @@
  *  - All work is enqueued on `stream` (a cudaStream_t passed as void*; NULL = default stream);
  *    no call synchronises the stream except ddf_create / ddf_destroy / ddf_trainer_create /
  *    ddf_trainer_export / the *_host variants, and - only for models served by the CUDA-core path -
- *    sdf_sphere_trace with early_exit and ddf_query_shadowed (their grids are sized on the host).
+ *    sdf_sphere_trace with early_exit and ddf_query_shadowed[_lights] (their grids are sized on the host).
  *    Results are valid once the stream reaches the point after the call.
  *  - n == 0 is DDF_OK and a no-op; n < 0 or a NULL pointer with n > 0 is DDF_E_INVALID_ARG.
  *  - Results are a pure function of (weights, ray): independent of n and of the ray's position
  *    in the batch, bit-reproducible run to run (training steps accumulate gradients with atomics
  *    and are reproducible to rounding only).  Directions must be unit length (not checked).
  *  - A model (and a trainer) owns device workspaces that its calls reuse: use one model from one
- *    stream / host thread at a time; different models are independent.
+ *    stream / host thread at a time; different models are independent.  A workspace is allocated
+ *    (or grown: a synchronising cudaFree / cudaMalloc) the first time a call needs it for a batch
+ *    that large; after that the call issues only stream-ordered work, so it can be recorded by
+ *    stream capture and replayed as a CUDA graph (ddf_trainer_step bakes that step's learning
+ *    rate into the capture; ddf_trainer_loss_grads and every query are replayable as they are).
  *  - There is no CPU fallback: without a CUDA device of compute capability 10.x the calls
  *    return DDF_E_UNSUPPORTED / DDF_E_CUDA.
  */
