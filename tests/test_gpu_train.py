@@ -66,6 +66,30 @@ def test_loss_and_gradients_match_oracle(ddf, orc, kw, arith):
 
 
 @pytest.mark.parametrize("arith", ARITH)
+@pytest.mark.parametrize("kw,n", [(dict(n_levels=1, log2_table=14, n_freq_dir=0, n_hidden=1), 1),
+                                  (dict(n_levels=1, log2_table=14, n_freq_dir=0, n_hidden=2), 129),
+                                  (dict(n_levels=16, log2_table=9, base_res=2, growth=1.3, n_freq_dir=4, n_hidden=2), 127),
+                                  (dict(n_levels=3, log2_table=19, base_res=16, growth=1.5, n_freq_dir=1, n_hidden=1), 128)])
+def test_degenerate_layouts_and_batches(ddf, orc, arith, kw, n):
+    """one ray; one level with an odd entry count (no replicated accumulator) and no direction bands (a 5-wide
+    input); 16 tiny levels that are all replicated; batches of T - 1, T, T + 1 rays"""
+    lay = HashLayout(**kw)
+    n_ent = ddf.ddf_hashgrid_table_entries(lay)
+    table = make_hash_table(lay, n_ent, scale=0.5); mlp = make_hash_mlp(lay, bias_scale=0.2)
+    o, d, t, hit = _batch(n, seed=n)
+    tr = ddf.ddf_trainer_create(table, mlp, lay, ddf.make_train_params(dist_clamp=2.0, arithmetic=arith))
+    loss = torch.zeros(1, device="cuda"); gt = torch.empty(2 * n_ent, device="cuda"); gm = torch.empty(len(mlp), device="cuda")
+    ddf.ddf_trainer_loss_grads(tr, _cuda(o), _cuda(d), _cuda(t), _cuda(hit), n, loss, gt, gm)
+    torch.cuda.synchronize()
+    rl, rgt, rgm = orc.hash_loss_grads(lay, table, mlp, o, d, t, hit, orc.train_params(dist_clamp=2.0))
+    assert abs(float(loss) - rl) < LOSS_TOL[arith] * max(1.0, abs(rl))
+    for g, r in ((gm.cpu().numpy(), rgm), (gt.cpu().numpy(), rgt)):
+        assert np.isfinite(g).all() and np.abs(g - r).max() <= GRAD_TOL[arith] * np.abs(r).max() + 1e-9
+    assert np.array_equal(gt.cpu().numpy() == 0, rgt == 0)
+    ddf.ddf_trainer_destroy(tr)
+
+
+@pytest.mark.parametrize("arith", ARITH)
 def test_more_tiles_than_sms_ragged_tail_and_a_growing_batch(ddf, orc, arith):
     """40,001 rays = 313 tiles of 128 on 148 SMs: every CTA walks several tiles (the tensor-core path keeps its
     weight-gradient accumulator in tensor memory across them) and the last tile has one ray; the same trainer
