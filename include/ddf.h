@@ -236,9 +236,10 @@ int  ddf_query_shadowed_lights(ddf_model* model, const float* o, const float* d,
  * The trainer owns fp32 copies of the table and the MLP (+ Adam moments and a gradient buffer:
  * 4 x the field size) and, for DDF_TRAIN_BF16X3, a workspace of 256 bytes per ray of the largest
  * batch seen (it grows, synchronising the device, when a larger batch arrives).  This build trains
- * n_features == 2, width == 64, n_hidden <= 2.  A step is 4 kernels (gather, MLP, scatter, Adam)
- * chained on `stream` by programmatic dependent launch; like every call here it is ordered after
- * the work already in `stream` and needs no synchronisation. */
+ * n_features == 2, width == 64, n_hidden <= 2.  A step is 4 kernels (gather, MLP, scatter, Adam),
+ * the first three (and ddf_gen_train_batch) chained on `stream` by programmatic dependent launch;
+ * like every call here it is ordered after the work already in `stream` and needs no
+ * synchronisation. */
 typedef struct ddf_train_params {
   uint32_t struct_size;        /* sizeof(ddf_train_params) */
   float lr0, lr_final_frac; int32_t total_steps;
