@@ -95,7 +95,14 @@ int  ddf_last_cuda_error(void);                           /* cudaError_t of the 
  * kernel; any other width up to 2048 is zero-padded at create to the next such width (padded units
  * have zero weights and bias, so every result is unchanged); everything else: the CUDA-core path. */
 /* kernel selection: 0 = automatic (tcgen05 path when the layout allows, else the SIMT path),
- * 1 = force the SIMT path, 2 = force the tcgen05 path (DDF_E_UNSUPPORTED if it cannot run). */
+ * 1 = force the SIMT path, 2 = force the tcgen05 path (DDF_E_UNSUPPORTED if it cannot run).
+ * The persistent tcgen05 kernel answers a batch in one launch; a batch of at most 40 of its 256-ray
+ * tiles (n <= 10,240) is instead answered as n_hidden + 2 launches chained by programmatic dependent
+ * launch - encoding, one launch per hidden layer with the layer's output columns split over the
+ * CTA pairs, heads - which keeps the whole chip busy on a small batch (2.2x faster at n <= 3,072).
+ * Both return the same bits.  3 = tcgen05 path, always the single persistent launch; 4 = tcgen05
+ * path, column-split whenever the batch fits the split scratch (n <= 18,944), else persistent.
+ * 3 and 4 are DDF_E_UNSUPPORTED for models the persistent kernel does not serve. */
 int  ddf_set_path(ddf_model* model, int path);
 /* which = 0: 1 if the tcgen05 path serves this model, else 0; 1: kernels launched by the
  * last query call on this model; 2: E (encoded input width); 3: rays per tile of the path. */

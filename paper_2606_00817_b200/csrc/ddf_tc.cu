@@ -65,6 +65,7 @@ struct TcPlan {
   int cg;
   int grid;
   __nv_bfloat16 *x0, *x1, *g;
+  float2* zpart;                     // column-split path: head partials [rows][n_chunks][2 halves]
   uint32_t* dbg_host; uint32_t* dbg_dev;
   TcParams base;
 };
@@ -261,6 +262,7 @@ __global__ void __launch_bounds__(kThreads, 1) ddf_tc_kernel(const __grid_consta
           wait_bar<CG == 2>(tfull_bar(buf), use & 1u, p.dbg, 0x600 + buf);
           ptx::tc_fence_after();
           const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + buf * kChunkN + h * 128;
+          float pc0 = 0.0f, pc1 = 0.0f;           // this chunk's share of the head dot products
           #pragma unroll 1
           for (int box = 0; box < 2; ++box) {
             uint32_t r[64];
@@ -310,20 +312,23 @@ __global__ void __launch_bounds__(kThreads, 1) ddf_tc_kernel(const __grid_consta
               #pragma unroll
               for (int i = 0; i < 16; ++i) {
                 float4 ww = __ldg(w0 + i);
-                z0 = fmaf(__uint_as_float(r[4 * i + 0]), ww.x, z0); z0 = fmaf(__uint_as_float(r[4 * i + 1]), ww.y, z0);
-                z0 = fmaf(__uint_as_float(r[4 * i + 2]), ww.z, z0); z0 = fmaf(__uint_as_float(r[4 * i + 3]), ww.w, z0);
+                pc0 = fmaf(__uint_as_float(r[4 * i + 0]), ww.x, pc0); pc0 = fmaf(__uint_as_float(r[4 * i + 1]), ww.y, pc0);
+                pc0 = fmaf(__uint_as_float(r[4 * i + 2]), ww.z, pc0); pc0 = fmaf(__uint_as_float(r[4 * i + 3]), ww.w, pc0);
               }
               if (p.n_out == 2) {
                 const float4* w1 = reinterpret_cast<const float4*>(p.head_w + p.width + col);
                 #pragma unroll
                 for (int i = 0; i < 16; ++i) {
                   float4 ww = __ldg(w1 + i);
-                  z1 = fmaf(__uint_as_float(r[4 * i + 0]), ww.x, z1); z1 = fmaf(__uint_as_float(r[4 * i + 1]), ww.y, z1);
-                  z1 = fmaf(__uint_as_float(r[4 * i + 2]), ww.z, z1); z1 = fmaf(__uint_as_float(r[4 * i + 3]), ww.w, z1);
+                  pc1 = fmaf(__uint_as_float(r[4 * i + 0]), ww.x, pc1); pc1 = fmaf(__uint_as_float(r[4 * i + 1]), ww.y, pc1);
+                  pc1 = fmaf(__uint_as_float(r[4 * i + 2]), ww.z, pc1); pc1 = fmaf(__uint_as_float(r[4 * i + 3]), ww.w, pc1);
                 }
               }
             }
           }
+          // chunk partials are summed in chunk order: the column-split path (below) adds the same
+          // partials in the same order, so both give the same bits
+          if (l == last_layer) { z0 += pc0; z1 += pc1; }
           if (l < last_layer && lane == 0) {
             ptx::bulk_wait<0>();                  // this warp's part of chunk c is in global memory
             ptx::mbar_arrive(act_bar(c));
@@ -396,6 +401,285 @@ __global__ void __launch_bounds__(kThreads, 1) ddf_tc_kernel(const __grid_consta
   if (warp == 2) ptx::tmem_dealloc<CG>(tmem_base, 512);
 }
 
+// ------------------------------------------------------------------------------------------
+// Column-split path for small batches.  With fewer ray tiles than CTA pairs the persistent kernel
+// above leaves most of the chip idle (a tile walks all layers on one pair: ~0.35 ms whatever n).
+// Here a layer is one launch and the work item is (ray tile, 256-column output chunk), so a batch
+// of t tiles keeps min(74, t * n_chunks) pairs busy; activations go through the same scratch
+// (rows indexed by ray, not by CTA) and the launch boundary is the layer hand-off.  The chain
+//   encode -> layer 0 .. layer n_hidden-1 -> finish
+// is linked by programmatic dependent launch, so each prologue (barrier init, TMEM allocation,
+// descriptor prefetch) overlaps the launch before.  Every accumulator is produced by the same MMA
+// sequence as in the persistent kernel and the head partials are added in the same order:
+// both paths return the same bits (tests/test_gpu_contract.py).
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
+// gamma(o, d) of every row of the batch's tiles (rows >= n: zero), one thread per row
+__global__ void __launch_bounds__(128) ddf_tc_split_encode_kernel(const __grid_constant__ TcParams p) {
+  pdl_launch_dependents();
+  const int64_t n = p.n_dev ? *p.n_dev : p.n;
+  const int64_t rows = (n + 2 * kTileM - 1) / (2 * kTileM) * (2 * kTileM);
+  const int64_t grow = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (grow >= rows) return;
+  __align__(16) __nv_bfloat16 enc[256];
+  #pragma unroll 1
+  for (int k = 0; k < p.E_pad; ++k) enc[k] = __float2bfloat16_rn(0.0f);
+  if (grow < n) {
+    float v[3] = { p.o[3 * grow], p.o[3 * grow + 1], p.o[3 * grow + 2] };
+    encode_vec_bf16(v, p.Lo, enc);
+    if (p.input_kind == 0) {
+      float w[3] = { p.d[3 * grow], p.d[3 * grow + 1], p.d[3 * grow + 2] };
+      encode_vec_bf16(w, p.Ld, enc + 3 + 6 * p.Lo);
+    }
+  }
+  uint4* dst = reinterpret_cast<uint4*>(p.gp + (size_t)grow * p.E_pad);
+  const uint4* src = reinterpret_cast<const uint4*>(enc);
+  #pragma unroll 1
+  for (int k = 0; k < p.E_pad / 8; ++k) dst[k] = src[k];
+}
+
+// one hidden layer: item = (tile, chunk), tile = 256 rays of a CTA pair, chunk = 256 output columns
+__global__ void __launch_bounds__(kThreads, 1) ddf_tc_split_layer_kernel(const __grid_constant__ TcParams p, const int l,
+                                                                          float2* __restrict__ zpart) {
+  constexpr int CG = 2;
+  using Cfg = TcCfg<CG>;
+  constexpr int S = Cfg::kStages;
+  extern __shared__ uint8_t smem_raw[];
+  const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
+  const uint32_t stg_base = smem_base + S * Cfg::kStageBytes;
+  const uint32_t bar_base = stg_base + 8u * 4096u;
+  auto full_bar   = [&](int s) { return bar_base + 8u * s; };
+  auto empty_bar  = [&](int s) { return bar_base + 8u * (8 + s); };
+  auto tfull_bar  = [&](int b) { return bar_base + 8u * (16 + b); };
+  auto tempty_bar = [&](int b) { return bar_base + 8u * (18 + b); };
+  const uint32_t tmem_slot = bar_base + 8u * 32;
+  auto a_smem = [&](int s) { return smem_base + s * Cfg::kStageBytes; };
+  auto b_smem = [&](int s) { return smem_base + s * Cfg::kStageBytes + kABytes; };
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const uint32_t rank = ptx::cluster_ctarank();
+  const bool leader = (rank == 0);
+  const int pid = blockIdx.x / CG, num_pairs = gridDim.x / CG;
+  const int last_layer = p.n_hidden - 1;
+
+  if (threadIdx.x == 0) {
+    pdl_launch_dependents();
+    for (int s = 0; s < S; ++s) { ptx::mbar_init(full_bar(s), 1); ptx::mbar_init(empty_bar(s), 1); }
+    for (int b = 0; b < 2; ++b) { ptx::mbar_init(tfull_bar(b), 1); ptx::mbar_init(tempty_bar(b), 8 * CG); }
+    ptx::fence_mbar_init();
+  }
+  if (warp == 0 && lane == 0) {
+    ptx::prefetch_tmap(&p.w[l]); ptx::prefetch_tmap(&p.g);
+    ptx::prefetch_tmap(((l - 1) & 1) ? &p.x1 : &p.x0); ptx::prefetch_tmap((l & 1) ? &p.xs1 : &p.xs0);
+  }
+  if (warp == 2) { ptx::tmem_alloc<CG>(tmem_slot, 512); ptx::tmem_relinquish<CG>(); }
+  ptx::tc_fence_before();
+  ptx::cluster_sync();
+  ptx::tc_fence_after();
+  uint32_t tmem_base;
+  asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
+  // n_dev (if any) was written before the chain's first, ordinary launch: safe to read before the wait
+  const int64_t n = p.n_dev ? *p.n_dev : p.n;
+  const int64_t tile_rays = (int64_t)kTileM * CG;
+  const int64_t num_tiles = (n + tile_rays - 1) / tile_rays;
+  const int64_t items = num_tiles * p.n_chunks;
+  const int nk0 = p.nkb0[l], nk1 = p.nkb1[l], nk = nk0 + nk1;
+
+  if (warp == 0) {
+    // ================================================================ TMA producer
+    // The weights do not depend on the launch before: the first item's first S weight blocks are
+    // requested before the dependency wait, the activations after it.
+    const CUtensorMap* amap = (l == 0) ? &p.g : (((l - 1) & 1) ? &p.x1 : &p.x0);
+    const int pre = (pid < items) ? (nk < S ? nk : S) : 0;
+    if (pre > 0 && ptx::elect_one()) {
+      const int brow = (int)(pid % p.n_chunks) * kChunkN + (int)rank * 128;
+      for (int kb = 0; kb < pre; ++kb) {
+        if (leader) ptx::mbar_arrive_expect_tx(full_bar(kb), 2u * Cfg::kStageBytes);
+        ptx::tma_load_2d_cg2(b_smem(kb), &p.w[l], ptx::mapa(full_bar(kb), 0), kb * kKBlock, brow);
+      }
+    }
+    __syncwarp();
+    pdl_wait();                        // everything below reads or overwrites what the launch before produced
+    ptx::fence_proxy_async();          // ... some of it written through the generic proxy (gamma) and read by TMA
+    uint32_t it = 0;
+    for (int64_t item = pid; item < items; item += num_pairs) {
+      const int tile = (int)(item / p.n_chunks), c = (int)(item - (int64_t)tile * p.n_chunks);
+      const int a_row = tile * (int)tile_rays + (int)rank * kTileM;
+      const int brow = c * kChunkN + (int)rank * 128;
+      for (int kb = 0; kb < nk; ++kb, ++it) {
+        const int s = it % S; const uint32_t ph = (it / S) & 1u;
+        const bool early = it < (uint32_t)pre;             // stage armed and its weights requested above
+        if (!early) wait_bar<true>(empty_bar(s), ph ^ 1u, p.dbg, 0x1300 + s);
+        if (ptx::elect_one()) {
+          if (leader && !early) ptx::mbar_arrive_expect_tx(full_bar(s), 2u * Cfg::kStageBytes);
+          const uint32_t fb = ptx::mapa(full_bar(s), 0);
+          if (kb < nk0) ptx::tma_load_2d_cg2(a_smem(s), amap, fb, kb * kKBlock, a_row);
+          else          ptx::tma_load_2d_cg2(a_smem(s), &p.g, fb, (kb - nk0) * kKBlock, a_row);
+          if (!early) ptx::tma_load_2d_cg2(b_smem(s), &p.w[l], fb, kb * kKBlock, brow);
+        }
+        __syncwarp();
+      }
+    }
+  } else if (warp == 1) {
+    // ================================================================ MMA issuer (same instruction sequence per accumulator as ddf_tc_kernel)
+    pdl_wait();
+    if (leader) {
+      constexpr uint32_t idesc = ptx::idesc_bf16_f32(128 * CG, kChunkN);
+      uint32_t it = 0, cc = 0;
+      for (int64_t item = pid; item < items; item += num_pairs, ++cc) {
+        const uint32_t buf = cc & 1u, use = cc >> 1;
+        wait_bar<true>(tempty_bar(buf), (use & 1u) ^ 1u, p.dbg, 0x1400 + buf);
+        ptx::tc_fence_after();
+        const uint32_t d_tmem = tmem_base + buf * kChunkN;
+        for (int kb = 0; kb < nk; ++kb, ++it) {
+          const int s = it % S; const uint32_t ph = (it / S) & 1u;
+          wait_bar<true>(full_bar(s), ph, p.dbg, 0x1500 + s);
+          ptx::tc_fence_after();
+          const bool g_last = (l == 0) ? (kb == nk0 - 1) : (kb == nk - 1 && nk1 > 0);
+          const int nk16 = g_last ? p.g_last_nk16 : 4;
+          const uint64_t adesc = ptx::smem_desc_k_sw128(a_smem(s));
+          const uint64_t bdesc = ptx::smem_desc_k_sw128(b_smem(s));
+          if (ptx::elect_one()) {
+            if (nk16 == 4) {
+              ptx::umma_bf16<CG>(d_tmem, adesc, bdesc, idesc, (uint32_t)(kb != 0));
+              ptx::umma_bf16<CG>(d_tmem, adesc + 2u, bdesc + 2u, idesc, 1u);
+              ptx::umma_bf16<CG>(d_tmem, adesc + 4u, bdesc + 4u, idesc, 1u);
+              ptx::umma_bf16<CG>(d_tmem, adesc + 6u, bdesc + 6u, idesc, 1u);
+            } else {
+              for (int k = 0; k < nk16; ++k)
+                ptx::umma_bf16<CG>(d_tmem, adesc + 2u * k, bdesc + 2u * k, idesc, (uint32_t)((kb | k) != 0));
+            }
+            ptx::umma_commit<CG>(empty_bar(s));
+            if (kb == nk - 1) ptx::umma_commit<CG>(tfull_bar(buf));
+          }
+          __syncwarp();
+        }
+      }
+    }
+  } else if (warp >= 4) {
+    // ================================================================ epilogue (8 warps), as in ddf_tc_kernel
+    const int q = warp & 3, h = (warp - 4) >> 2;
+    const int row = q * 32 + lane;
+    const uint32_t stage = stg_base + (uint32_t)(warp - 4) * 4096u;
+    const uint32_t tempty_remote = ptx::mapa(tempty_bar(0), 0);
+    const CUtensorMap* smap = (l & 1) ? &p.xs1 : &p.xs0;
+    const float* bias = p.bias + p.b_off[l];
+    uint32_t cc = 0;
+    pdl_wait();
+    for (int64_t item = pid; item < items; item += num_pairs, ++cc) {
+      const int tile = (int)(item / p.n_chunks), c = (int)(item - (int64_t)tile * p.n_chunks);
+      const int t_row = tile * (int)tile_rays + (int)rank * kTileM;
+      const uint32_t buf = cc & 1u, use = cc >> 1;
+      wait_bar<true>(tfull_bar(buf), use & 1u, p.dbg, 0x1600 + buf);
+      ptx::tc_fence_after();
+      const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + buf * kChunkN + h * 128;
+      float pc0 = 0.0f, pc1 = 0.0f;
+      #pragma unroll 1
+      for (int box = 0; box < 2; ++box) {
+        uint32_t r[64];
+        ptx::tmem_ld32(taddr + box * 64, *reinterpret_cast<uint32_t(*)[32]>(&r[0]));
+        ptx::tmem_ld32(taddr + box * 64 + 32, *reinterpret_cast<uint32_t(*)[32]>(&r[32]));
+        ptx::tmem_ld_wait();
+        if (box == 1) {
+          ptx::tc_fence_before();
+          __syncwarp();
+          if (lane == 0) ptx::mbar_arrive_cluster(tempty_remote + 8u * buf);
+        }
+        const int col = c * kChunkN + h * 128 + box * 64;
+        const float4* b4 = reinterpret_cast<const float4*>(bias + col);
+        #pragma unroll
+        for (int i = 0; i < 16; ++i) {
+          float4 bb = __ldg(b4 + i);
+          r[4 * i + 0] = __float_as_uint(fmaxf(__uint_as_float(r[4 * i + 0]) + bb.x, 0.0f));
+          r[4 * i + 1] = __float_as_uint(fmaxf(__uint_as_float(r[4 * i + 1]) + bb.y, 0.0f));
+          r[4 * i + 2] = __float_as_uint(fmaxf(__uint_as_float(r[4 * i + 2]) + bb.z, 0.0f));
+          r[4 * i + 3] = __float_as_uint(fmaxf(__uint_as_float(r[4 * i + 3]) + bb.w, 0.0f));
+        }
+        if (l < last_layer) {
+          if (lane == 0) ptx::bulk_wait_read<0>();
+          __syncwarp();
+          #pragma unroll
+          for (int j = 0; j < 8; ++j) {
+            uint4 pk;
+            __nv_bfloat162 t0 = __floats2bfloat162_rn(__uint_as_float(r[8 * j + 0]), __uint_as_float(r[8 * j + 1]));
+            __nv_bfloat162 t1 = __floats2bfloat162_rn(__uint_as_float(r[8 * j + 2]), __uint_as_float(r[8 * j + 3]));
+            __nv_bfloat162 t2 = __floats2bfloat162_rn(__uint_as_float(r[8 * j + 4]), __uint_as_float(r[8 * j + 5]));
+            __nv_bfloat162 t3 = __floats2bfloat162_rn(__uint_as_float(r[8 * j + 6]), __uint_as_float(r[8 * j + 7]));
+            pk.x = *reinterpret_cast<uint32_t*>(&t0); pk.y = *reinterpret_cast<uint32_t*>(&t1);
+            pk.z = *reinterpret_cast<uint32_t*>(&t2); pk.w = *reinterpret_cast<uint32_t*>(&t3);
+            ptx::st_shared_v4(stage + (uint32_t)lane * 128u + (uint32_t)((j ^ (lane & 7)) << 4), pk);
+          }
+          ptx::fence_proxy_async_smem();
+          __syncwarp();
+          if (lane == 0) {
+            ptx::tma_store_2d(smap, stage, col, t_row + q * 32);
+            ptx::bulk_commit();
+          }
+        } else {
+          const float4* w0 = reinterpret_cast<const float4*>(p.head_w + col);
+          #pragma unroll
+          for (int i = 0; i < 16; ++i) {
+            float4 ww = __ldg(w0 + i);
+            pc0 = fmaf(__uint_as_float(r[4 * i + 0]), ww.x, pc0); pc0 = fmaf(__uint_as_float(r[4 * i + 1]), ww.y, pc0);
+            pc0 = fmaf(__uint_as_float(r[4 * i + 2]), ww.z, pc0); pc0 = fmaf(__uint_as_float(r[4 * i + 3]), ww.w, pc0);
+          }
+          if (p.n_out == 2) {
+            const float4* w1 = reinterpret_cast<const float4*>(p.head_w + p.width + col);
+            #pragma unroll
+            for (int i = 0; i < 16; ++i) {
+              float4 ww = __ldg(w1 + i);
+              pc1 = fmaf(__uint_as_float(r[4 * i + 0]), ww.x, pc1); pc1 = fmaf(__uint_as_float(r[4 * i + 1]), ww.y, pc1);
+              pc1 = fmaf(__uint_as_float(r[4 * i + 2]), ww.z, pc1); pc1 = fmaf(__uint_as_float(r[4 * i + 3]), ww.w, pc1);
+            }
+          }
+        }
+      }
+      if (l == last_layer) zpart[((size_t)(t_row + row) * p.n_chunks + c) * 2 + h] = make_float2(pc0, pc1);
+    }
+    if (lane == 0) ptx::bulk_wait_read<0>();     // the staging boxes must outlive the bulk stores that read them
+  } else {
+    pdl_wait();
+  }
+
+  ptx::tc_fence_before();
+  ptx::cluster_sync();
+  if (warp == 2) ptx::tmem_dealloc<CG>(tmem_base, 512);
+}
+
+// heads from the chunk partials, added in the order ddf_tc_kernel adds them; one thread per ray
+__global__ void __launch_bounds__(128) ddf_tc_split_finish_kernel(const __grid_constant__ TcParams p, const float2* __restrict__ zpart) {
+  pdl_wait();
+  const int64_t n = p.n_dev ? *p.n_dev : p.n;
+  const int64_t rows = (n + 2 * kTileM - 1) / (2 * kTileM) * (2 * kTileM);
+  const int64_t grow = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (grow >= rows) return;                      // whole warps: rows is a multiple of 256
+  const int lane = threadIdx.x & 31;
+  const bool valid = grow < n;
+  float z0 = 0.0f, z1 = 0.0f, y0 = 0.0f, y1 = 0.0f;
+  for (int c = 0; c < p.n_chunks; ++c) {
+    const float2 a = zpart[((size_t)grow * p.n_chunks + c) * 2 + 0];
+    const float2 b = zpart[((size_t)grow * p.n_chunks + c) * 2 + 1];
+    z0 += a.x; z1 += a.y; y0 += b.x; y1 += b.y;
+  }
+  z0 = (z0 + y0) + p.bias[p.b_off[p.n_hidden]];
+  if (p.n_out == 2) z1 = (z1 + y1) + p.bias[p.b_off[p.n_hidden] + 1];
+  if (p.mode_out == 1) {
+    if (valid) { p.out0[grow * p.n_out] = z0; if (p.n_out == 2) p.out0[grow * p.n_out + 1] = z1; }
+  } else if (p.mode_out == 0) {
+    if (valid) {
+      if (p.n_out == 2) { p.out0[grow] = softplus_f(z0); if (p.out1) p.out1[grow] = sigmoid_f(z1); }
+      else p.out0[grow] = z0;
+    }
+  } else {
+    const bool hit = valid && (sigmoid_f(z1) > 0.5f) && (softplus_f(z0) < p.ao_radius);
+    const uint32_t m = __ballot_sync(0xffffffffu, hit);
+    const int g0 = (lane / p.spp) * p.spp;
+    const uint32_t bits = (p.spp == 32) ? m : ((m >> g0) & ((1u << p.spp) - 1u));
+    if (valid && (lane % p.spp) == 0) p.out0[grow / p.spp] = 1.0f - (float)__popc(bits) / (float)p.spp;
+  }
+}
+
 // ------------------------------------------------------------------------------------------ host
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
@@ -430,7 +714,7 @@ static int make_map(CUtensorMap* out, void* base, uint64_t cols, uint64_t rows, 
 
 void tc_plan_destroy(Model* m) {
   if (!m->tc) return;
-  cudaFree(m->tc->x0); cudaFree(m->tc->x1); cudaFree(m->tc->g);
+  cudaFree(m->tc->x0); cudaFree(m->tc->x1); cudaFree(m->tc->g); cudaFree(m->tc->zpart);
   if (m->tc->dbg_host) cudaFreeHost(m->tc->dbg_host);
   delete m->tc;
   m->tc = nullptr;
@@ -456,6 +740,7 @@ int tc_plan_create(Model* m) {
   DDF_CUDA_TRY(cudaMemset(t->x0, 0, rows * L.width * 2));
   DDF_CUDA_TRY(cudaMemset(t->x1, 0, rows * L.width * 2));
   DDF_CUDA_TRY(cudaMemset(t->g, 0, rows * 2 * m->E_pad * 2));
+  DDF_CUDA_TRY(cudaMalloc(&t->zpart, rows * (L.width / kChunkN) * 2 * sizeof(float2)));
   DDF_CUDA_TRY(cudaHostAlloc(&t->dbg_host, 64, cudaHostAllocMapped));
   memset(t->dbg_host, 0, 64);
   DDF_CUDA_TRY(cudaHostGetDevicePointer((void**)&t->dbg_dev, t->dbg_host, 0));
@@ -484,6 +769,39 @@ int tc_plan_create(Model* m) {
   p.g_last_nk16 = (m->E - (m->E_pad - kKBlock) + 15) / 16;
   DDF_CUDA_TRY(cudaFuncSetAttribute(ddf_tc_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, TcCfg<1>::kSmemBytes));
   DDF_CUDA_TRY(cudaFuncSetAttribute(ddf_tc_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, TcCfg<2>::kSmemBytes));
+  DDF_CUDA_TRY(cudaFuncSetAttribute(ddf_tc_split_layer_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TcCfg<2>::kSmemBytes));
+  return DDF_OK;
+}
+
+// Batches of at most this many 256-ray tiles take the column-split path when the choice is automatic
+// (measured on one B200: the split path wins below ~2^14 rays).
+constexpr int kSplitAutoTiles = 40;
+
+// encode -> one launch per hidden layer -> finish, chained by programmatic dependent launch
+static int tc_forward_split(Model* m, const TcParams& p, int64_t tiles, cudaStream_t st) {
+  TcPlan* t = m->tc;
+  const int n_chunks = p.n_chunks;
+  int64_t pairs = tiles * n_chunks;
+  if (pairs > t->grid / 2) pairs = t->grid / 2;
+  cudaLaunchAttribute attr[2];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  attr[1].id = cudaLaunchAttributeClusterDimension;
+  attr[1].val.clusterDim.x = 2; attr[1].val.clusterDim.y = 1; attr[1].val.clusterDim.z = 1;
+  cudaLaunchConfig_t cfg;
+  memset(&cfg, 0, sizeof(cfg));
+  cfg.stream = st;
+  // the first launch of the chain is an ordinary one: it waits for everything queued before it
+  cfg.gridDim = dim3((unsigned)(tiles * 2)); cfg.blockDim = dim3(128);
+  DDF_CUDA_TRY(cudaLaunchKernelEx(&cfg, ddf_tc_split_encode_kernel, p));
+  cfg.gridDim = dim3((unsigned)(pairs * 2)); cfg.blockDim = dim3(kThreads);
+  cfg.dynamicSmemBytes = TcCfg<2>::kSmemBytes; cfg.attrs = attr; cfg.numAttrs = 2;
+  for (int l = 0; l < p.n_hidden; ++l)
+    DDF_CUDA_TRY(cudaLaunchKernelEx(&cfg, ddf_tc_split_layer_kernel, p, l, t->zpart));
+  cfg.gridDim = dim3((unsigned)(tiles * 2)); cfg.blockDim = dim3(128);
+  cfg.dynamicSmemBytes = 0; cfg.numAttrs = 1;
+  DDF_CUDA_TRY(cudaLaunchKernelEx(&cfg, ddf_tc_split_finish_kernel, p, (const float2*)t->zpart));
+  m->last_launches = p.n_hidden + 2;
   return DDF_OK;
 }
 
@@ -497,6 +815,9 @@ int tc_forward(Model* m, const float* o, const float* d, int64_t n, const int64_
   p.out0 = out0; p.out1 = out1; p.mode_out = mode_out; p.spp = spp > 0 ? spp : 1; p.ao_radius = ao_radius;
   const int64_t tile_rays = (int64_t)kTileM * t->cg;
   int64_t tiles = (n + tile_rays - 1) / tile_rays;
+  // small batches: split the output columns of a layer over the CTA pairs (ddf_set_path 3 / 4 pin the choice)
+  const int64_t split_max = (t->cg != 2 || m->path == 3) ? 0 : (m->path == 4 ? t->grid / 2 : kSplitAutoTiles);
+  if (tiles <= split_max) return tc_forward_split(m, p, tiles, st);
   int grid = t->grid;
   if (tiles * t->cg < grid) grid = (int)tiles * t->cg;   // n_dev can only shrink n
   cudaLaunchConfig_t cfg;

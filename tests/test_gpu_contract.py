@@ -181,6 +181,65 @@ def test_edge_sizes_permutation_determinism(ddf, c1):
     assert torch.equal(outu, full_d[:1001])
 
 
+def test_column_split_path_is_bit_identical_to_the_persistent_kernel(ddf, c1, sdf):
+    """Batches of at most 40 tiles are answered one launch per layer with a layer's output columns
+    split over the CTA pairs (ddf_set_path 4 forces it up to 74 tiles, 3 forbids it): heads, logits,
+    the AO reduction and the sphere tracer's device-side ray count must give the persistent kernel's bits."""
+    lay, m = c1
+    N = 256 * 74 + 300
+    o, d = random_rays(N, seed=21)
+    od, dd = _cuda(o), _cuda(d)
+
+    def run(path, n, mode):
+        ddf.ddf_set_path(m, path)
+        if mode == "heads":
+            out = torch.full((2, n + 8), -7.0, device="cuda")
+            ddf.ddf_query(m, od, dd, n, out[0], out[1])
+        elif mode == "logits":
+            out = torch.full((n + 8, 2), -7.0, device="cuda")
+            ddf.ddf_query_logits(m, od, dd, n, out)
+        else:
+            out = torch.full((n // 16 + 8,), -7.0, device="cuda")
+            ddf.ddf_query_ao(m, od, dd, n // 16, 16, 0.7, out)
+        torch.cuda.synchronize()
+        return out, ddf.ddf_get_info(m, 1)
+
+    try:
+        for n in (1, 255, 256, 257, 1000, 4099, 40 * 256, 40 * 256 + 16, 74 * 256):
+            for mode in ("heads", "logits", "ao"):
+                if mode == "ao" and n < 16:
+                    continue
+                a, la = run(3, n, mode)
+                b, lb = run(4, n, mode)
+                c, lc = run(0, n, mode)
+                assert la == 1 and lb == lay.n_hidden + 2, (n, mode, la, lb)
+                assert lc == (lb if n <= 40 * 256 else la), (n, mode, lc)        # the automatic choice
+                assert torch.equal(a, b) and torch.equal(a, c), (n, mode)
+                assert bool(torch.isfinite(a).all())                             # includes the -7 guard past n
+                if mode == "heads":
+                    assert bool((a[:, n:] == -7.0).all()) and bool((a[:, :n] != -7.0).all())
+        # more tiles than the scratch has rows for: path 4 falls back to the persistent kernel
+        a, la = run(4, N, "heads")
+        assert la == 1
+    finally:
+        ddf.ddf_set_path(m, 0)
+    # sphere tracer (device-side live-ray count, early exit) on a batch small enough to be split
+    slay, sblob, sm = sdf
+    oo, ddd = random_rays(3000, seed=22)
+    oo = (oo * 2.5 / np.linalg.norm(oo, axis=1, keepdims=True)).astype(np.float32)
+    ddd = (-oo / np.linalg.norm(oo, axis=1, keepdims=True)).astype(np.float32)
+    res = []
+    try:
+        for path in (3, 4):
+            ddf.ddf_set_path(sm, path)
+            res.append(_trace(ddf, sm, oo, ddd, ddf.SdfTraceParams(32, 1e-3, 6.0, 1.0, 0.05, 1)))
+    finally:
+        ddf.ddf_set_path(sm, 0)
+    for x, y in zip(res[0], res[1]):
+        assert np.array_equal(x, y)
+    assert res[0][3] > 3000                                                      # more than one step was taken
+
+
 def test_bad_arguments(ddf, c1):
     lay, m = c1
     from paper_2606_00817_b200.binding import lib, _stream
@@ -218,7 +277,9 @@ def test_simt_and_tcgen05_paths_agree(ddf, orc, lay):
     o, d = random_rays(2000, seed=5)
     if lay.input_kind == 1:
         d = None
-    ddf.ddf_set_path(m, 2); z_tc = _logits(ddf, m, o, d); assert ddf.ddf_get_info(m, 1) == 1
+    ddf.ddf_set_path(m, 2); z_tc = _logits(ddf, m, o, d)
+    # one fused launch, or (wide kernel, a batch this small) encode + one launch per layer + heads
+    assert ddf.ddf_get_info(m, 1) == (lay.n_hidden + 2 if ddf.ddf_get_info(m, 3) == 256 else 1)
     ddf.ddf_set_path(m, 1); z_si = _logits(ddf, m, o, d); assert ddf.ddf_get_info(m, 1) > 1
     zq, _, _ = orc.forward(lay, blob, o, d, mode=1)
     ze, _, _ = orc.forward(lay, blob, o, d, mode=0)
