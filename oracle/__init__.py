@@ -78,6 +78,7 @@ def lib():
         _lib.orc_hash_mlp_params.restype = C.c_int64
         _lib.orc_hash_index.restype = C.c_int64
         _lib.orc_gen_shadow_from_hits.restype = C.c_int64
+        _lib.orc_hit_normals.restype = C.c_int64
         _lib.orc_hash_loss_grads.restype = C.c_double
         _lib.orc_lr_at.restype = C.c_double
         _lib.orc_solid_scene_raycast.restype = C.c_double
@@ -377,6 +378,16 @@ def shadow_lit(vis2, dist2, tmax, index, n):
     lit = np.empty(n, np.uint8)
     lib().orc_shadow_lit(_p(vis2), _p(dist2), _p(tmax), _p(index), C.c_int64(len(index)), C.c_int64(n), _p(lit))
     return lit
+
+
+def hit_normals(o, d, dist, vis, width, height):
+    """Returns (p, nrm, index) of the hits of a width x height primary batch (reading W5)."""
+    o, d, dist, vis = _f32(o), _f32(d), _f32(dist), _f32(vis)
+    n = width * height
+    assert o.shape[0] == n
+    p = np.empty((n, 3), np.float32); nrm = np.empty((n, 3), np.float32); index = np.empty(n, np.int32)
+    k = lib().orc_hit_normals(_p(o), _p(d), _p(dist), _p(vis), C.c_int(width), C.c_int(height), _p(p), _p(nrm), _p(index))
+    return p[:k].copy(), nrm[:k].copy(), index[:k].copy()
 
 
 # ------------------------------------------------------------------ training (ddf_hash_oracle.h, T1-T5)

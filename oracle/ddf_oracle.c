@@ -465,3 +465,51 @@ void orc_shadow_lit(const float* vis2, const float* dist2, const float* tmax, co
   for (int64_t k = 0; k < count; ++k)                     /* occluded within the distance to the light */
     lit[index[k]] = (vis2[k] > 0.5f && dist2[k] < tmax[k]) ? 0 : 1;
 }
+
+/* reading W5: normal from the hit-point image */
+static int pick_neighbour(const float* dist, const float* vis, int64_t i, int64_t step, int has_f, int has_b) {
+  const int f = has_f && vis[i + step] > 0.5f, b = has_b && vis[i - step] > 0.5f;
+  if (f && b) {
+    const float df = fabsf(dist[i + step] - dist[i]), db = fabsf(dist[i - step] - dist[i]);   /* fp32 */
+    return df <= db ? +1 : -1;
+  }
+  return f ? +1 : (b ? -1 : 0);
+}
+
+int64_t orc_hit_normals(const float* o, const float* d, const float* dist, const float* vis,
+                        int width, int height, float* p, float* nrm, int32_t* index) {
+  int64_t k = 0;
+  for (int y = 0; y < height; ++y)
+    for (int x = 0; x < width; ++x) {
+      const int64_t i = (int64_t)y * width + x;
+      if (!(vis[i] > 0.5f)) continue;
+      double P[3], du[3], dv[3], n[3];
+      for (int a = 0; a < 3; ++a) P[a] = (double)o[3 * i + a] + (double)dist[i] * (double)d[3 * i + a];
+      const int su = pick_neighbour(dist, vis, i, 1, x + 1 < width, x >= 1);
+      const int sv = pick_neighbour(dist, vis, i, width, y + 1 < height, y >= 1);
+      int ok = su != 0 && sv != 0;
+      if (ok) {
+        const int64_t ju = i + su, jv = i + (int64_t)sv * width;
+        for (int a = 0; a < 3; ++a) {
+          const double Pu = (double)o[3 * ju + a] + (double)dist[ju] * (double)d[3 * ju + a];
+          const double Pv = (double)o[3 * jv + a] + (double)dist[jv] * (double)d[3 * jv + a];
+          du[a] = su * (Pu - P[a]);
+          dv[a] = sv * (Pv - P[a]);
+        }
+        n[0] = du[1] * dv[2] - du[2] * dv[1];
+        n[1] = du[2] * dv[0] - du[0] * dv[2];
+        n[2] = du[0] * dv[1] - du[1] * dv[0];
+        const double len = sqrt(n[0] * n[0] + n[1] * n[1] + n[2] * n[2]);
+        if (len > 0.0 && len < INFINITY) {
+          double dot = 0.0;
+          for (int a = 0; a < 3; ++a) { n[a] /= len; dot += n[a] * (double)d[3 * i + a]; }
+          if (dot > 0.0) for (int a = 0; a < 3; ++a) n[a] = -n[a];
+        } else ok = 0;
+      }
+      if (!ok) for (int a = 0; a < 3; ++a) n[a] = -(double)d[3 * i + a];
+      for (int a = 0; a < 3; ++a) { p[3 * k + a] = (float)P[a]; nrm[3 * k + a] = (float)n[a]; }
+      index[k] = (int32_t)i;
+      ++k;
+    }
+  return k;
+}

@@ -86,6 +86,18 @@ int64_t orc_gen_shadow_from_hits(const float* o, const float* d, const float* di
 void orc_shadow_lit(const float* vis2, const float* dist2, const float* tmax, const int32_t* index,
                     int64_t count, int64_t n, uint8_t* lit);
 
+/* ---- normals of the field's own hits (reading W5; "offset it slightly
+ * along its normal": the field returns no normal, so it is estimated from the hit-point image) ----
+ * The primary batch is a width x height image, ray i = y * width + x.  For every i with vis[i] > 0.5,
+ * in increasing i: P_i = o_i + dist_i d_i; along x the difference is taken toward the neighbour that
+ * also hit (both hit: the one with the smaller |dist_j - dist_i| in fp32, forward on ties): forward
+ * P_{i+1} - P_i, backward P_i - P_{i-1}; along y likewise with +-width.  n = normalise(du x dv), turned
+ * so that n . d_i <= 0; if an axis has no hit neighbour, or the product vanishes, n = -d_i.
+ * Writes the compacted p, nrm [count][3] and index [count]; returns count.  fp64 but for the stated
+ * fp32 comparison. */
+int64_t orc_hit_normals(const float* o, const float* d, const float* dist, const float* vis,
+                        int width, int height, float* p, float* nrm, int32_t* index);
+
 /* ---- sphere tracing of s(p) = (|p| - base_radius) + alpha * MLP(p)  (readings A19, A20) ----
  * Ray state (t, p, s) is carried in fp32 exactly as the kernel carries it; the MLP itself is
  * evaluated by orc_forward in `mode`.  trace_p/trace_s (may be NULL) receive, for every ray,

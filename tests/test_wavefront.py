@@ -37,6 +37,81 @@ def test_twin_on_an_analytic_sphere(orc):
     assert lit[np.nonzero(vis < 0.5)[0]].sum() == 0                                 # primary misses are never lit
 
 
+def _plane_t(o, d, z0):
+    """distance of rays to the plane z = z0 (inf where they do not reach it)"""
+    with np.errstate(divide="ignore", invalid="ignore"):
+        t = (z0 - o[:, 2].astype(np.float64)) / d[:, 2].astype(np.float64)
+    return np.where(np.isfinite(t) & (t > 0), t, np.inf)
+
+
+def test_hit_normals_on_exact_fields(orc):
+    """Reading W5 against geometry.  Exact plane field: every normal is the plane's, facing the camera.
+    Exact sphere field: normals are P / |P| up to the finite-difference error of one pixel.
+    Sphere in front of a plane: plane pixels beside the silhouette keep the plane normal, because the
+    difference goes to the neighbour with the smaller distance jump (an always-forward rule fails)."""
+    W, H = 96, 80
+    ocam = orc.make_camera((0.3, -0.4, 2.5))
+    o, d = orc.gen_camera(ocam, W, H)
+    tp = _plane_t(o, d, -1.0)
+    assert np.all(np.isfinite(tp))
+    vis = np.ones(W * H, np.float32)
+    p, nrm, idx = orc.hit_normals(o, d, tp.astype(np.float32), vis, W, H)
+    assert np.array_equal(idx, np.arange(W * H))
+    assert np.allclose(p[:, 2], -1.0, atol=1e-5)
+    assert np.allclose(nrm, np.array([0.0, 0.0, 1.0])[None, :], atol=2e-3)          # fp32 distances: ~1e-7 / pixel footprint
+    # sphere alone
+    ts = np.array([orc.ray_sphere(o[i], d[i], (0, 0, 0), 1.0) for i in range(W * H)])
+    vis = (ts > 0).astype(np.float32); dist = np.where(ts > 0, ts, 0.0).astype(np.float32)
+    p, nrm, idx = orc.hit_normals(o, d, dist, vis, W, H)
+    assert np.array_equal(idx, np.nonzero(vis > 0.5)[0]) and 0 < len(idx) < W * H
+    assert np.allclose(np.linalg.norm(nrm, axis=1), 1.0, atol=1e-6)
+    assert np.all(np.einsum("ij,ij->i", nrm, d[idx]) <= 1e-6)                       # faces the camera
+    true_n = p / np.linalg.norm(p, axis=1, keepdims=True)
+    front = -np.einsum("ij,ij->i", true_n, d[idx]) > 0.4                            # away from the silhouette
+    cosang = np.einsum("ij,ij->i", nrm, true_n)[front]
+    assert front.sum() > 500 and np.degrees(np.arccos(np.clip(cosang, -1, 1))).max() < 2.5
+    # sphere in front of the plane
+    both = np.minimum(np.where(ts > 0, ts, np.inf), tp)
+    on_plane = ~(ts > 0)
+    p, nrm, idx = orc.hit_normals(o, d, both.astype(np.float32), np.ones(W * H, np.float32), W, H)
+    img = nrm.reshape(H, W, 3); pl = on_plane.reshape(H, W)
+    nb_x = np.zeros_like(pl); nb_x[:, 1:] |= pl[:, :-1]; nb_x[:, :-1] |= pl[:, 1:]  # a plane neighbour on each axis
+    nb_y = np.zeros_like(pl); nb_y[1:, :] |= pl[:-1, :]; nb_y[:-1, :] |= pl[1:, :]
+    sel = pl & nb_x & nb_y
+    beside = sel.copy(); beside[:, :-1] &= ~pl[:, 1:]                               # forward x-neighbour is on the sphere
+    assert beside[:, :-1].sum() > 10
+    assert np.allclose(img[sel], np.array([0.0, 0.0, 1.0])[None, :], atol=2e-3)
+
+
+def test_hit_normals_hand_cases(orc):
+    """Ties go forward, an axis without a hit neighbour falls back to -d, misses are skipped."""
+    a = 0.25
+    xs, ys = np.meshgrid(np.arange(3.0), np.arange(3.0))                            # 3 x 3 parallel rays along +z
+    o = np.stack([xs.ravel(), ys.ravel(), np.zeros(9)], 1).astype(np.float32)
+    d = np.tile(np.array([0.0, 0.0, 1.0], np.float32), (9, 1))
+    dist = (1.0 + a * np.abs(xs.ravel() - 1.0)).astype(np.float32)                  # a V-shaped valley along x = 1
+    vis = np.ones(9, np.float32)
+    p, nrm, idx = orc.hit_normals(o, d, dist, vis, 3, 3)
+    s = math.sqrt(1 + a * a)
+    # centre pixel: |dt| ties, forward: du = (1, 0, a), dv = (0, 1, 0): du x dv = (-a, 0, 1), turned against d
+    assert np.allclose(nrm[4], [a / s, 0.0, -1.0 / s], atol=1e-6)
+    # left column has only a forward x-neighbour: du = (1, 0, -a) -> (a, 0, 1) -> turned: (-a, 0, -1) / s
+    assert np.allclose(nrm[3], [-a / s, 0.0, -1.0 / s], atol=1e-6)
+    # an isolated hit and a one-row image: no y-neighbour -> -d
+    vis1 = np.zeros(9, np.float32); vis1[4] = 1.0
+    p, nrm, idx = orc.hit_normals(o, d, dist, vis1, 3, 3)
+    assert list(idx) == [4] and np.allclose(nrm[0], [0, 0, -1]) and np.allclose(p[0], [1, 1, 1])
+    p, nrm, idx = orc.hit_normals(o[:3], d[:3], dist[:3], vis[:3], 3, 1)
+    assert len(idx) == 3 and np.allclose(nrm, [[0, 0, -1]] * 3)
+    # the smaller jump wins: make the forward neighbour of the centre far away
+    dist2 = dist.copy(); dist2[5] = 5.0
+    p, nrm, idx = orc.hit_normals(o, d, dist2, vis, 3, 3)
+    assert np.allclose(nrm[4], [-a / s, 0.0, -1.0 / s], atol=1e-6)                  # backward: du = (1, 0, -a)
+    # threshold: vis exactly 0.5 is a miss
+    vis2 = vis.copy(); vis2[0] = 0.5
+    assert 0 not in orc.hit_normals(o, d, dist, vis2, 3, 3)[2]
+
+
 def test_twin_threshold_and_order(orc):
     o = np.zeros((6, 3), np.float32); d = np.tile(np.array([[0, 0, 1]], np.float32), (6, 1))
     dist = np.arange(1, 7, dtype=np.float32)
