@@ -231,6 +231,35 @@ int  ddf_query_shadowed_lights(ddf_model* model, const float* o, const float* d,
                                const float* lights, int n_lights, float eps, float* out_dist,
                                float* out_vis, uint8_t* out_lit_mask, int64_t* out_count, void* stream);
 
+/* Ambient occlusion at the field's OWN hits (AO "along a set of hemisphere directions"
+ * from a surface point "offset slightly along its normal"; the field as the renderer's
+ * secondary-ray oracle, "no mesh in the pipeline").  The field returns no normal, so it is estimated
+ * from the hit-point image of the primary batch (reading W5): the batch is a
+ * width x height image, ray i = y * width + x; for every i with vis[i] > 0.5, P_i = o_i + dist_i d_i;
+ * along x the difference goes to the neighbour that also hit (both hit: the one with the smaller
+ * |dist_j - dist_i|, forward on ties), forward P_{i+1} - P_i, backward P_i - P_{i-1}; along y likewise
+ * with +-width; n = normalise(du x dv) turned so that n . d_i <= 0; n = -d_i if an axis has no hit
+ * neighbour or the product vanishes.
+ * ddf_gen_ao_from_hits: stable compaction of the hits in increasing i: p_c, nrm_c [n][3], index [n]
+ * (all must hold n = width * height entries), *count (int64 [device]) the number of hits; when o2 / d2
+ * (both or neither; [n * spp][3]) are given they receive spp cosine-weighted rays per hit from
+ * p_c + eps * nrm_c, exactly ddf_gen_ao(p_c, nrm_c, count, ...) with the count read on the device.
+ * All pointers [device]; asynchronous on `stream`; uses a workspace owned by `model`. */
+int  ddf_gen_ao_from_hits(ddf_model* model, const float* o, const float* d, const float* dist,
+                          const float* vis, int width, int height, int spp, uint64_t seed,
+                          uint64_t rng_stream, float eps, float* p_c, float* nrm_c, int32_t* index,
+                          float* o2, float* d2, int64_t* count, void* stream);
+/* The whole loop in one call: primary query -> hit points and normals -> compacted AO rays -> second
+ * query with the 16 -> 1 reduce fused (batch size read on the device on the tcgen05 and hash-grid paths
+ * when spp divides 32; otherwise one host read of the count) -> out_ao[i] = 1 - mean over the spp rays of
+ * (vis2 > 0.5 and dist2 < ao_radius) where ray i hit, 1 where it missed.  out_dist / out_vis [n] receive
+ * the primary results, out_nrm ([n][3], may be NULL) the normal per pixel (0 where the ray missed),
+ * out_count (int64 [device], may be NULL) the number of AO rays traced, hits x spp. */
+int  ddf_query_ao_wavefront(ddf_model* model, const float* o, const float* d, int width, int height,
+                            int spp, uint64_t seed, uint64_t rng_stream, float eps, float ao_radius,
+                            float* out_dist, float* out_vis, float* out_nrm, float* out_ao,
+                            int64_t* out_count, void* stream);
+
 /* ---------------------------------------------------------------- training the hash-grid field
  * PAPER.md:70 / 86: "an L1 term on distance, clamped at the box scale, plus a cross-entropy term
  * on the hit weighted at 0.3"; "Adam for 30,000 steps, a batch of 16,384 rays, and a learning rate

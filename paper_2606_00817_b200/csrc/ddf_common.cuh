@@ -101,6 +101,10 @@ void narrow_plan_destroy(Model* m);
 int narrow_forward(Model* m, const float* o, const float* d, int64_t n, const int64_t* n_dev, int mode_out,
                    float* out0, float* out1, int spp, float ao_radius, cudaStream_t st);
 
+// ---- generators (ddf_gen.cu): AO rays about (p, nrm); n_pts_dev (device) overrides n_pts when non-null
+int gen_ao_launch(const float* p, const float* nrm, int64_t n_pts, const int64_t* n_pts_dev, int spp, uint64_t seed,
+                  uint64_t rng_stream, float eps, float* o, float* d, cudaStream_t st);
+
 // one dispatch for every fused path: tcgen05 wide, tcgen05 narrow, hash grid (n_dev: device-side count or null)
 inline bool has_fused_path(const Model* m) { return m->hg || ((m->tc || m->nw) && m->path != 1); }
 inline int fused_forward(Model* m, const float* o, const float* d, int64_t n, const int64_t* n_dev, int mode_out,

@@ -90,9 +90,12 @@ __global__ void gen_gbuffer_kernel(CamFrame c, ddf_scene sc, int width, int heig
 }
 
 // AO rays: one thread per ray (pixel-major, spp consecutive rays per point).
-__global__ void gen_ao_kernel(const float* __restrict__ p, const float* __restrict__ nrm, int64_t n_pts, int spp,
+// n_pts_dev (device, optional) overrides n_pts; it can only be smaller.
+__global__ void gen_ao_kernel(const float* __restrict__ p, const float* __restrict__ nrm, int64_t n_pts,
+                              const int64_t* __restrict__ n_pts_dev, int spp,
                               uint64_t key, float eps, float* __restrict__ o, float* __restrict__ d) {
   int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (n_pts_dev) n_pts = *n_pts_dev;
   if (k >= n_pts * spp) return;
   int64_t i = k / spp;
   float n[3] = { nrm[3 * i], nrm[3 * i + 1], nrm[3 * i + 2] };
@@ -142,6 +145,13 @@ __global__ void shadow_test_kernel(const float* __restrict__ vis, const float* _
 }
 
 static inline unsigned blocks_for(int64_t n, int t) { return (unsigned)((n + t - 1) / t); }
+
+int gen_ao_launch(const float* p, const float* nrm, int64_t n_pts, const int64_t* n_pts_dev, int spp, uint64_t seed,
+                  uint64_t rng_stream, float eps, float* o, float* d, cudaStream_t st) {
+  gen_ao_kernel<<<blocks_for(n_pts * spp, 256), 256, 0, st>>>(p, nrm, n_pts, n_pts_dev, spp, host_key(seed, rng_stream), eps, o, d);
+  DDF_CUDA_TRY(cudaGetLastError());
+  return DDF_OK;
+}
 
 }  // namespace ddf
 
@@ -205,9 +215,7 @@ extern "C" int ddf_gen_ao(const float* p, const float* nrm, int64_t n_pts, int s
   if (n_pts < 0 || spp <= 0) return DDF_E_INVALID_ARG;
   if (n_pts == 0) return DDF_OK;
   if (!p || !nrm || !o || !d) return DDF_E_INVALID_ARG;
-  gen_ao_kernel<<<blocks_for(n_pts * spp, 256), 256, 0, (cudaStream_t)stream>>>(p, nrm, n_pts, spp, host_key(seed, rng_stream), eps, o, d);
-  DDF_CUDA_TRY(cudaGetLastError());
-  return DDF_OK;
+  return gen_ao_launch(p, nrm, n_pts, nullptr, spp, seed, rng_stream, eps, o, d, (cudaStream_t)stream);
 }
 
 extern "C" int ddf_ao_reduce(const float* vis, const float* dist, int64_t n_pts, int spp, float ao_radius,

@@ -240,3 +240,116 @@ def test_gpu_compaction_edge_cases(orc):
             p = o[want.long()] + (dist[want.long()] - 1e-2)[:, None] * d[want.long()]
             assert torch.allclose(o2[:k], p, atol=1e-6)
     ddf.ddf_destroy(m)
+
+
+@pytest.mark.gpu
+def test_gpu_hit_normals_on_an_exact_sphere_field(orc):
+    """ddf_gen_ao_from_hits fed the exact field of a unit sphere in front of a plane: the compacted index is
+    the oracle's, hit points and normals agree with it (smooth data: no sign or neighbour ambiguity), and the
+    rays are the oracle's generator run on them."""
+    import torch
+    import paper_2606_00817_b200 as ddf
+    from ddf_inputs import layout_c0
+    ddf.build()
+    m = ddf.ddf_create(make_weights(layout_c0()), layout_c0())
+    for (W, H) in [(96, 80), (257, 3), (1, 1), (5, 1), (1, 300)]:
+        ocam = orc.make_camera((0.3, -0.4, 2.5))
+        o, d = orc.gen_camera(ocam, W, H)
+        ts = np.array([orc.ray_sphere(o[i], d[i], (0, 0, 0), 1.0) for i in range(W * H)])
+        tp = _plane_t(o, d, -1.0)
+        dist = np.minimum(np.where(ts > 0, ts, np.inf), tp).astype(np.float32)
+        vis = np.ones(W * H, np.float32); vis[::7] = 0.0                                # holes: one-sided differences
+        rp, rn, ridx = orc.hit_normals(o, d, dist, vis, W, H)
+        n = W * H; spp = 4
+        og, dg, tg, vg = (torch.from_numpy(x).cuda() for x in (o, d, dist, vis))
+        p_c = torch.empty((n, 3), device="cuda"); n_c = torch.empty((n, 3), device="cuda")
+        idx = torch.full((n,), -1, dtype=torch.int32, device="cuda"); cnt = torch.full((1,), -5, dtype=torch.int64, device="cuda")
+        o2 = torch.full((n * spp, 3), float("nan"), device="cuda"); d2 = torch.full((n * spp, 3), float("nan"), device="cuda")
+        ddf.ddf_gen_ao_from_hits(m, og, dg, tg, vg, W, H, spp, MASTER_SEED, STREAMS["ao_samples"], 1e-3, p_c, n_c, idx, o2, d2, cnt)
+        torch.cuda.synchronize()
+        k = int(cnt.item())
+        assert k == len(ridx) and np.array_equal(idx[:k].cpu().numpy(), ridx) and bool((idx[k:] == -1).all()), (W, H)
+        assert np.allclose(p_c[:k].cpu().numpy(), rp, atol=2e-6)
+        # fp32 differences of neighbouring hit points: 1e-7 against a pixel footprint of ~1e-2 .. 3e-2
+        assert np.allclose(n_c[:k].cpu().numpy(), rn, atol=5e-4), (W, H, np.abs(n_c[:k].cpu().numpy() - rn).max())
+        ro2, rd2 = orc.gen_ao(p_c[:k].cpu().numpy(), n_c[:k].cpu().numpy(), spp, MASTER_SEED, STREAMS["ao_samples"], 1e-3)
+        assert np.allclose(o2[:k * spp].cpu().numpy(), ro2, atol=1e-5) and np.allclose(d2[:k * spp].cpu().numpy(), rd2, atol=2e-5)
+        assert bool(torch.isnan(o2[k * spp:]).all())                                     # nothing past the count
+        # normals only
+        ddf.ddf_gen_ao_from_hits(m, og, dg, tg, vg, W, H, spp, 0, 0, 1e-3, p_c, n_c, idx, None, None, cnt)
+        assert int(cnt.item()) == k and ddf.ddf_get_info(m, 1) == 3
+    # no hits at all, empty image
+    z = torch.zeros(64, device="cuda")
+    ddf.ddf_gen_ao_from_hits(m, og[:64].contiguous(), dg[:64].contiguous(), tg[:64].contiguous(), z, 8, 8, 4, 1, 2, 1e-3,
+                             p_c, n_c, idx, o2, d2, cnt)
+    assert int(cnt.item()) == 0
+    cnt.fill_(9)
+    ddf.ddf_gen_ao_from_hits(m, None, None, None, None, 0, 5, 4, 1, 2, 1e-3, None, None, None, None, None, cnt)
+    assert int(cnt.item()) == 0
+    ddf.ddf_destroy(m)
+
+
+@pytest.mark.gpu
+def test_gpu_ao_wavefront_against_twin(orc):
+    """ddf_query_ao_wavefront: primary results are ddf_query's; hits, hit points, normals and rays follow the twin
+    on the GPU's own primary results; the AO image is the decision rule applied to a plain second query of the
+    compacted rays (bit for bit) and agrees with the oracle evaluated end to end on sampled pixels."""
+    import torch
+    import paper_2606_00817_b200 as ddf
+    ddf.build()
+    cam = ddf.ddf_camera_from_seed(MASTER_SEED, STREAMS["camera_pos"], 2.5)
+    for name, m, oracle_fwd in _models(ddf):
+        for (W, H, spp, radius) in [(256, 192, 16, 1.5), (61, 47, 5, float("inf"))]:   # fused reduce / host-counted path
+            n = W * H
+            o = torch.empty((n, 3), device="cuda"); d = torch.empty((n, 3), device="cuda")
+            ddf.ddf_gen_camera(cam, W, H, o, d)
+            o += torch.from_numpy(random_rays(n)[0]).cuda() * 0.4
+            dist = torch.empty(n, device="cuda"); vis = torch.empty(n, device="cuda"); nrm = torch.full((n, 3), 9.0, device="cuda")
+            ao = torch.full((n,), float("nan"), device="cuda"); cnt = torch.zeros(1, dtype=torch.int64, device="cuda")
+            seed, stream = MASTER_SEED, STREAMS["ao_samples"]
+            ddf.ddf_query_ao_wavefront(m, o, d, W, H, spp, seed, stream, 1e-3, radius, dist, vis, nrm, ao, cnt)
+            torch.cuda.synchronize()
+            d1 = torch.empty(n, device="cuda"); v1 = torch.empty(n, device="cuda")
+            ddf.ddf_query(m, o, d, n, d1, v1)
+            assert torch.equal(d1, dist) and torch.equal(v1, vis)
+            k = int((vis > 0.5).sum().item())
+            assert int(cnt.item()) == k * spp and 0 < k < n, (name, k)
+            # the twin on the GPU's primary results
+            on, dn, tn, vn = o.cpu().numpy(), d.cpu().numpy(), dist.cpu().numpy(), vis.cpu().numpy()
+            rp, rn, ridx = orc.hit_normals(on, dn, tn, vn, W, H)
+            p_c = torch.empty((n, 3), device="cuda"); n_c = torch.empty((n, 3), device="cuda"); idx = torch.empty(n, dtype=torch.int32, device="cuda")
+            o2 = torch.empty((n * spp, 3), device="cuda"); d2 = torch.empty((n * spp, 3), device="cuda"); c2 = torch.zeros(1, dtype=torch.int64, device="cuda")
+            ddf.ddf_gen_ao_from_hits(m, o, d, dist, vis, W, H, spp, seed, stream, 1e-3, p_c, n_c, idx, o2, d2, c2)
+            assert int(c2.item()) == k and np.array_equal(idx[:k].cpu().numpy(), ridx)
+            assert np.allclose(p_c[:k].cpu().numpy(), rp, atol=4e-6)
+            ng = n_c[:k].cpu().numpy()
+            grazing = np.abs(np.einsum("ij,ij->i", rn, dn[ridx])) < 1e-3                 # the turn against the ray may flip
+            err = np.minimum(np.abs(ng - rn).max(1), np.where(grazing, np.abs(ng + rn).max(1), np.inf))
+            assert (err < 1e-3).mean() > 0.999 and grazing.mean() < 0.01, (name, err.max())
+            assert np.allclose(np.linalg.norm(ng, axis=1), 1.0, atol=1e-5)
+            img = nrm.cpu().numpy()
+            assert np.array_equal(img[ridx], ng) and not img[vn <= 0.5].any()             # per-pixel copy, 0 on misses
+            ro2, rd2 = orc.gen_ao(p_c[:k].cpu().numpy(), ng, spp, seed, stream, 1e-3)
+            assert np.allclose(o2[:k * spp].cpu().numpy(), ro2, atol=1e-5) and np.allclose(d2[:k * spp].cpu().numpy(), rd2, atol=2e-5)
+            # AO = the rule on a plain second query of those rays, scattered back; misses = 1
+            dist2 = torch.empty(k * spp, device="cuda"); vis2 = torch.empty(k * spp, device="cuda")
+            ddf.ddf_query(m, o2[:k * spp].contiguous(), d2[:k * spp].contiguous(), k * spp, dist2, vis2)
+            want = np.ones(n, np.float32)
+            want[ridx] = orc.ao_reduce(vis2.cpu().numpy(), dist2.cpu().numpy(), spp, radius)
+            if spp & (spp - 1) == 0: assert np.array_equal(ao.cpu().numpy(), want), (name, W, spp)
+            else: assert np.allclose(ao.cpu().numpy(), want, atol=1e-6, rtol=0), (name, W, spp)   # hits / spp rounds in fp32 on the GPU, fp64 in the oracle
+            assert 0.0 < want[ridx].mean() < 1.0
+            # the oracle end to end on sampled pixels
+            sel = np.arange(0, k, max(1, k // 100))[:100]
+            rows = (sel[:, None] * spp + np.arange(spp)[None, :]).reshape(-1)
+            z, t2, xi2 = oracle_fwd(orc, ro2[rows], rd2[rows])
+            ref = orc.ao_reduce(xi2.astype(np.float32), t2.astype(np.float32), spp, radius)
+            near = ((np.abs(xi2 - 0.5) < 1e-2) | (np.abs(t2 - radius) < 1e-2 * (1 + np.abs(t2)))).reshape(-1, spp).sum(1)
+            assert np.all(np.abs(want[ridx[sel]] - ref) <= near / spp + 1e-6), name
+            # determinism
+            ao_b = torch.empty(n, device="cuda")
+            ddf.ddf_query_ao_wavefront(m, o, d, W, H, spp, seed, stream, 1e-3, radius, dist, vis, None, ao_b, None)
+            assert torch.equal(ao_b, ao)
+        ddf.ddf_query_ao_wavefront(m, o, d, 0, 7, 4, 1, 2, 1e-3, 1.0, dist, vis, None, ao, cnt)
+        assert int(cnt.item()) == 0
+        ddf.ddf_destroy(m)
