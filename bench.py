@@ -471,6 +471,14 @@ def run_wavefront(ddf, torch):
         k3 = int(cnt.item())
         out[name]["three_lights"] = {"ms": ms3, "shadow_rays": k3, "launches": ddf.ddf_get_info(m, 1),
                                      "Mrays_s_primary_plus_secondary": (n + k3) / ms3 / 1e3}
+        # ambient occlusion at the field's own hits (ddf_query_ao_wavefront): normals from the hit-point image,
+        # 16 cosine-weighted rays per hit, fused reduce; 1024 x 1024 primary rays
+        ao = torch.empty(n, device="cuda")
+        msa = _time_ms(torch, lambda: ddf.ddf_query_ao_wavefront(m, o, d, 1024, 1024, 16, MASTER_SEED, STREAMS["ao_samples"], 1e-3,
+                                                                 float("inf"), dist, vis, None, ao, cnt), reps=3)
+        ka = int(cnt.item())
+        out[name]["ao_16spp"] = {"ms": msa, "ao_rays": ka, "mean_ao_of_hits": float(ao[vis > 0.5].mean().item()),
+                                 "launches": ddf.ddf_get_info(m, 1), "Mrays_s_primary_plus_secondary": (n + ka) / msa / 1e3}
         ddf.ddf_destroy(m)
     return out
 

@@ -64,6 +64,37 @@ def test_wavefront_call_replays_from_a_graph(ddf, kind):
     ddf.ddf_destroy(m)
 
 
+@pytest.mark.parametrize("kind", ["hash", "dense"])
+def test_ao_wavefront_call_replays_from_a_graph(ddf, kind):
+    """ddf_query_ao_wavefront with the fused reduce never reads the hit count on the host: capturable"""
+    if kind == "hash":
+        hl = layout_hash_paper(); mlp = make_hash_mlp(hl).copy(); mlp[-1] = 1.0
+        m = ddf.ddf_create_hashgrid(make_hash_table(hl, ddf.ddf_hashgrid_table_entries(hl)), mlp, hl)
+        W, H = 250, 200
+    else:
+        lay = layout_c1(); blob = make_weights(lay).copy(); blob[-1] = 0x3F80
+        m = ddf.ddf_create(blob, lay)
+        W, H = 100, 50
+    n = W * H
+    o_np, d_np = random_rays(n)
+    o = torch.from_numpy(o_np).cuda(); d = torch.from_numpy(d_np).cuda()
+    dist = torch.empty(n, device="cuda"); vis = torch.empty(n, device="cuda"); nrm = torch.empty((n, 3), device="cuda")
+    ao = torch.empty(n, device="cuda"); cnt = torch.zeros(1, dtype=torch.int64, device="cuda")
+    call = lambda st=None: ddf.ddf_query_ao_wavefront(m, o, d, W, H, 16, 11, 3, 1e-3, 2.0, dist, vis, nrm, ao, cnt, stream=st)
+    call()                                                                                # eager: creates the workspaces
+    torch.cuda.synchronize()
+    g = _capture(lambda st: call(st))
+    o.copy_(o.flip(0).contiguous()); d.copy_(d.flip(0).contiguous())                      # new inputs in the same buffers
+    call(); torch.cuda.synchronize()
+    want = (dist.clone(), vis.clone(), nrm.clone(), ao.clone(), int(cnt.item()))
+    assert 0 < want[4] < 16 * n
+    dist.zero_(); vis.zero_(); nrm.zero_(); ao.zero_(); cnt.zero_()
+    g.replay(); torch.cuda.synchronize()
+    assert torch.equal(dist, want[0]) and torch.equal(vis, want[1]) and torch.equal(nrm, want[2]) and torch.equal(ao, want[3])
+    assert int(cnt.item()) == want[4]
+    ddf.ddf_destroy(m)
+
+
 def test_training_pass_replays_from_a_graph(ddf, orc):
     """loss + gradients of one batch (gather -> tcgen05 MLP -> scatter, chained by programmatic dependent
     launch, then the fold and the copies out) captured and replayed on a new batch, against the oracle."""
