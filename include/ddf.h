@@ -259,6 +259,16 @@ int  ddf_query_ao_wavefront(ddf_model* model, const float* o, const float* d, in
                             int spp, uint64_t seed, uint64_t rng_stream, float eps, float ao_radius,
                             float* out_dist, float* out_vis, float* out_nrm, float* out_ao,
                             int64_t* out_count, void* stream);
+/* Shadows and ambient occlusion of one frame from ONE primary query (PAPER.md:155 / Table VI: the field as
+ * the renderer's secondary-ray oracle for exactly these two effects): ddf_query, then the shadow loop of
+ * ddf_query_shadowed_lights (n_lights = 0: skipped, out_lit_mask may be NULL) and the AO loop of
+ * ddf_query_ao_wavefront (spp = 0: skipped, out_ao / out_nrm may be NULL) on the same primary results;
+ * every output is bit for bit what those two calls return.  out_counts (int64[2] [device], may be NULL)
+ * receives {shadow rays traced, AO rays traced}. */
+int  ddf_query_shaded(ddf_model* model, const float* o, const float* d, int width, int height,
+                      const float* lights, int n_lights, int spp, uint64_t seed, uint64_t rng_stream,
+                      float eps, float ao_radius, float* out_dist, float* out_vis, uint8_t* out_lit_mask,
+                      float* out_nrm, float* out_ao, int64_t* out_counts, void* stream);
 
 /* ---------------------------------------------------------------- training the hash-grid field
  * PAPER.md:70 / 86: "an L1 term on distance, clamped at the box scale, plus a cross-entropy term

@@ -17,7 +17,7 @@ EXPORTED_SYMBOLS = [
     "ddf_gen_camera", "ddf_gen_sphere_points", "ddf_gen_shadow", "ddf_gen_gbuffer", "ddf_gen_ao",
     "ddf_ao_reduce", "ddf_query_ao", "ddf_shadow_test", "sdf_sphere_trace",
     "ddf_hashgrid_table_entries", "ddf_create_hashgrid", "ddf_gen_shadow_from_hits", "ddf_query_shadowed", "ddf_query_shadowed_lights",
-    "ddf_gen_ao_from_hits", "ddf_query_ao_wavefront",
+    "ddf_gen_ao_from_hits", "ddf_query_ao_wavefront", "ddf_query_shaded",
     "ddf_trainer_create", "ddf_trainer_destroy", "ddf_trainer_step", "ddf_trainer_loss_grads", "ddf_trainer_export",
     "ddf_trainer_steps", "ddf_scene_raycast", "ddf_gen_train_batch", "ddf_query_camera",
 ]
@@ -312,6 +312,16 @@ def ddf_query_ao_wavefront(model, o, d, width, height, spp, seed, rng_stream, ep
                                         C.c_uint64(int(seed)), C.c_uint64(int(rng_stream)), C.c_float(eps),
                                         C.c_float(ao_radius), _dev(out_dist), _dev(out_vis), _dev(out_nrm), _dev(out_ao),
                                         _dev(out_count, torch.int64), _stream(stream)), "ddf_query_ao_wavefront")
+
+
+def ddf_query_shaded(model, o, d, width, height, lights, spp, seed, rng_stream, eps, ao_radius, out_dist, out_vis, out_lit_mask,
+                     out_nrm, out_ao, out_counts=None, stream=None):
+    flat = [float(x) for l in lights for x in l]
+    li = (C.c_float * max(len(flat), 1))(*flat)
+    _check(lib().ddf_query_shaded(model.handle, _dev(o), _dev(d), C.c_int(width), C.c_int(height), li, C.c_int(len(flat) // 3),
+                                  C.c_int(spp), C.c_uint64(int(seed)), C.c_uint64(int(rng_stream)), C.c_float(eps),
+                                  C.c_float(ao_radius), _dev(out_dist), _dev(out_vis), _dev(out_lit_mask, torch.uint8),
+                                  _dev(out_nrm), _dev(out_ao), _dev(out_counts, torch.int64), _stream(stream)), "ddf_query_shaded")
 
 
 # ------------------------------------------------------------------ training

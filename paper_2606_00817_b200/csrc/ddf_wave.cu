@@ -241,9 +241,10 @@ extern "C" int ddf_gen_shadow_from_hits(ddf_model* model, const float* o, const 
   return rc;
 }
 
-extern "C" int ddf_query_shadowed_lights(ddf_model* model, const float* o, const float* d, int64_t n,
-                                         const float* lights, int n_lights, float eps, float* out_dist,
-                                         float* out_vis, uint8_t* out_lit_mask, int64_t* out_count, void* stream) {
+// do_primary = false: out_dist / out_vis already hold the primary results (ddf_query_shaded)
+static int shadowed_lights_impl(ddf_model* model, const float* o, const float* d, int64_t n,
+                                const float* lights, int n_lights, float eps, float* out_dist,
+                                float* out_vis, uint8_t* out_lit_mask, int64_t* out_count, void* stream, bool do_primary) {
   if (!model || !lights || n < 0 || n > 0x7fffffff || n_lights < 1 || n_lights > 8) return DDF_E_INVALID_ARG;
   Model* m = reinterpret_cast<Model*>(model);
   if (m->lay.input_kind != 0 || m->lay.n_out != 2) return DDF_E_INVALID_ARG;
@@ -254,8 +255,11 @@ extern "C" int ddf_query_shadowed_lights(ddf_model* model, const float* o, const
   int rc = wave_ws(m, n, true, &w);
   if (rc != DDF_OK) return rc;
   // 1. primary rays
-  if ((rc = ddf_query(model, o, d, n, out_dist, out_vis, stream)) != DDF_OK) return rc;
-  int launches = m->last_launches;
+  int launches = 0;
+  if (do_primary) {
+    if ((rc = ddf_query(model, o, d, n, out_dist, out_vis, stream)) != DDF_OK) return rc;
+    launches = m->last_launches;
+  }
   // 2. where the hits go in the compacted batch (the same for every light)
   if ((rc = wave_count(w, out_vis, n, w.count, st)) != DDF_OK) return rc;
   launches += 2;
@@ -283,6 +287,12 @@ extern "C" int ddf_query_shadowed_lights(ddf_model* model, const float* o, const
   }
   m->last_launches = launches;
   return DDF_OK;
+}
+
+extern "C" int ddf_query_shadowed_lights(ddf_model* model, const float* o, const float* d, int64_t n,
+                                         const float* lights, int n_lights, float eps, float* out_dist,
+                                         float* out_vis, uint8_t* out_lit_mask, int64_t* out_count, void* stream) {
+  return shadowed_lights_impl(model, o, d, n, lights, n_lights, eps, out_dist, out_vis, out_lit_mask, out_count, stream, true);
 }
 
 extern "C" int ddf_query_shadowed(ddf_model* model, const float* o, const float* d, int64_t n,
@@ -362,10 +372,10 @@ extern "C" int ddf_gen_ao_from_hits(ddf_model* model, const float* o, const floa
                       o2, d2, count, nullptr, st);
 }
 
-extern "C" int ddf_query_ao_wavefront(ddf_model* model, const float* o, const float* d, int width, int height,
-                                      int spp, uint64_t seed, uint64_t rng_stream, float eps, float ao_radius,
-                                      float* out_dist, float* out_vis, float* out_nrm, float* out_ao,
-                                      int64_t* out_count, void* stream) {
+static int ao_wavefront_impl(ddf_model* model, const float* o, const float* d, int width, int height,
+                             int spp, uint64_t seed, uint64_t rng_stream, float eps, float ao_radius,
+                             float* out_dist, float* out_vis, float* out_nrm, float* out_ao,
+                             int64_t* out_count, void* stream, bool do_primary) {
   if (!model || width < 0 || height < 0 || spp <= 0 || (int64_t)width * height > 0x7fffffff) return DDF_E_INVALID_ARG;
   Model* m = reinterpret_cast<Model*>(model);
   if (m->lay.input_kind != 0 || m->lay.n_out != 2) return DDF_E_INVALID_ARG;
@@ -377,8 +387,11 @@ extern "C" int ddf_query_ao_wavefront(ddf_model* model, const float* o, const fl
   int rc = wave_ao_ws(m, n, spp, true, &w);
   if (rc != DDF_OK) return rc;
   // 1. primary rays
-  if ((rc = ddf_query(model, o, d, n, out_dist, out_vis, stream)) != DDF_OK) return rc;
-  int launches = m->last_launches;
+  int launches = 0;
+  if (do_primary) {
+    if ((rc = ddf_query(model, o, d, n, out_dist, out_vis, stream)) != DDF_OK) return rc;
+    launches = m->last_launches;
+  }
   // 2. hit points, normals from the hit-point image, spp rays about each normal (compacted, size on the device)
   if ((rc = wave_ao_rays(m, w, o, d, out_dist, out_vis, width, height, spp, seed, rng_stream, eps, w.p_c, w.n_c, w.index,
                          out_nrm, w.o2, w.d2, w.count, w.count_rays, st)) != DDF_OK) return rc;
@@ -399,5 +412,45 @@ extern "C" int ddf_query_ao_wavefront(ddf_model* model, const float* o, const fl
   wave_ao_scatter_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(out_vis, n, w.ao_c, w.index, w.count, out_ao, out_count, spp);
   DDF_CUDA_TRY(cudaGetLastError());
   m->last_launches = launches + 1;
+  return DDF_OK;
+}
+
+extern "C" int ddf_query_ao_wavefront(ddf_model* model, const float* o, const float* d, int width, int height,
+                                      int spp, uint64_t seed, uint64_t rng_stream, float eps, float ao_radius,
+                                      float* out_dist, float* out_vis, float* out_nrm, float* out_ao,
+                                      int64_t* out_count, void* stream) {
+  return ao_wavefront_impl(model, o, d, width, height, spp, seed, rng_stream, eps, ao_radius, out_dist, out_vis, out_nrm,
+                           out_ao, out_count, stream, true);
+}
+
+// shadows and ambient occlusion of one frame from ONE primary query (the field as the renderer's
+// secondary-ray oracle; its Table VI reports exactly these two effects)
+extern "C" int ddf_query_shaded(ddf_model* model, const float* o, const float* d, int width, int height,
+                                const float* lights, int n_lights, int spp, uint64_t seed, uint64_t rng_stream,
+                                float eps, float ao_radius, float* out_dist, float* out_vis, uint8_t* out_lit_mask,
+                                float* out_nrm, float* out_ao, int64_t* out_counts, void* stream) {
+  if (!model || width < 0 || height < 0 || (int64_t)width * height > 0x7fffffff || n_lights < 0 || n_lights > 8 || spp < 0)
+    return DDF_E_INVALID_ARG;
+  if ((n_lights > 0 && (!lights || !out_lit_mask)) || (spp > 0 && !out_ao)) return DDF_E_INVALID_ARG;
+  Model* m = reinterpret_cast<Model*>(model);
+  if (m->lay.input_kind != 0 || m->lay.n_out != 2) return DDF_E_INVALID_ARG;
+  cudaStream_t st = (cudaStream_t)stream;
+  const int64_t n = (int64_t)width * height;
+  if (out_counts) DDF_CUDA_TRY(cudaMemsetAsync(out_counts, 0, 16, st));
+  if (n == 0) { m->last_launches = 0; return DDF_OK; }
+  if (!o || !d || !out_dist || !out_vis) return DDF_E_INVALID_ARG;
+  int rc = ddf_query(model, o, d, n, out_dist, out_vis, stream);
+  if (rc != DDF_OK) return rc;
+  int launches = m->last_launches;
+  if (n_lights > 0) {
+    if ((rc = shadowed_lights_impl(model, o, d, n, lights, n_lights, eps, out_dist, out_vis, out_lit_mask, out_counts, stream, false)) != DDF_OK) return rc;
+    launches += m->last_launches;
+  }
+  if (spp > 0) {
+    if ((rc = ao_wavefront_impl(model, o, d, width, height, spp, seed, rng_stream, eps, ao_radius, out_dist, out_vis, out_nrm,
+                                out_ao, out_counts ? out_counts + 1 : nullptr, stream, false)) != DDF_OK) return rc;
+    launches += m->last_launches;
+  }
+  m->last_launches = launches;
   return DDF_OK;
 }

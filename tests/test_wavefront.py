@@ -353,3 +353,47 @@ def test_gpu_ao_wavefront_against_twin(orc):
         ddf.ddf_query_ao_wavefront(m, o, d, 0, 7, 4, 1, 2, 1e-3, 1.0, dist, vis, None, ao, cnt)
         assert int(cnt.item()) == 0
         ddf.ddf_destroy(m)
+
+
+@pytest.mark.gpu
+def test_gpu_shaded_frame_is_the_two_loops_on_one_primary_query(orc):
+    """ddf_query_shaded = ddf_query + the shadow loop + the AO loop on the same primary results: every output
+    bit for bit what ddf_query_shadowed_lights and ddf_query_ao_wavefront return, one primary query fewer."""
+    import torch
+    import paper_2606_00817_b200 as ddf
+    ddf.build()
+    cam = ddf.ddf_camera_from_seed(MASTER_SEED, STREAMS["camera_pos"], 2.5)
+    W, H, spp = 200, 160, 8; n = W * H
+    lights = [(3.0, 3.0, 3.0), (-3.0, 2.0, 1.0)]
+    for name, m, _ in _models(ddf):
+        o = torch.empty((n, 3), device="cuda"); d = torch.empty((n, 3), device="cuda")
+        ddf.ddf_gen_camera(cam, W, H, o, d)
+        o += torch.from_numpy(random_rays(n)[0]).cuda() * 0.4
+        new = lambda *s, dt=torch.float32, v=0: torch.full(s, v, dtype=dt, device="cuda")
+        dist_a, vis_a, mask_a, c_a = new(n), new(n), new(n, dt=torch.uint8), new(1, dt=torch.int64)
+        ddf.ddf_query_shadowed_lights(m, o, d, n, lights, 1e-3, dist_a, vis_a, mask_a, c_a)
+        l_a = ddf.ddf_get_info(m, 1)
+        dist_b, vis_b, nrm_b, ao_b, c_b = new(n), new(n), new(n, 3), new(n), new(1, dt=torch.int64)
+        ddf.ddf_query_ao_wavefront(m, o, d, W, H, spp, 5, 6, 1e-3, 2.0, dist_b, vis_b, nrm_b, ao_b, c_b)
+        l_b = ddf.ddf_get_info(m, 1)
+        ddf.ddf_query(m, o, d, n, dist_b, vis_b)
+        l_q = ddf.ddf_get_info(m, 1)
+        dist, vis, mask, nrm, ao, cs = new(n, v=7), new(n, v=7), new(n, dt=torch.uint8, v=0xFF), new(n, 3, v=7), new(n, v=7), new(2, dt=torch.int64, v=-1)
+        ddf.ddf_query_shaded(m, o, d, W, H, lights, spp, 5, 6, 1e-3, 2.0, dist, vis, mask, nrm, ao, cs)
+        torch.cuda.synchronize()
+        assert ddf.ddf_get_info(m, 1) == l_a + l_b - l_q, name
+        assert torch.equal(dist, dist_a) and torch.equal(vis, vis_a) and torch.equal(mask, mask_a), name
+        assert torch.equal(nrm, nrm_b) and torch.equal(ao, ao_b), name
+        assert cs.tolist() == [int(c_a.item()), int(c_b.item())] and cs[0] > 0 and cs[1] > 0
+        # one loop only
+        mask2, cs2 = new(n, dt=torch.uint8, v=0xFF), new(2, dt=torch.int64, v=-1)
+        ddf.ddf_query_shaded(m, o, d, W, H, lights, 0, 0, 0, 1e-3, 2.0, dist, vis, mask2, None, None, cs2)
+        assert torch.equal(mask2, mask_a) and cs2.tolist() == [int(c_a.item()), 0]
+        ao2, cs3 = new(n, v=7), new(2, dt=torch.int64, v=-1)
+        ddf.ddf_query_shaded(m, o, d, W, H, [], spp, 5, 6, 1e-3, 2.0, dist, vis, None, None, ao2, cs3)
+        assert torch.equal(ao2, ao_b) and cs3.tolist() == [0, int(c_b.item())]
+        ddf.ddf_query_shaded(m, o, d, 0, 0, lights, spp, 5, 6, 1e-3, 2.0, dist, vis, mask, nrm, ao, cs)
+        assert cs.tolist() == [0, 0]
+        with pytest.raises(ddf.DdfError):
+            ddf.ddf_query_shaded(m, o, d, W, H, lights, spp, 5, 6, 1e-3, 2.0, dist, vis, None, nrm, ao, cs)
+        ddf.ddf_destroy(m)
