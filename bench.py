@@ -439,6 +439,34 @@ def run_training(ddf, torch, steps=30000, batch=16384, arithmetic=0):
     out["primary_hit_agreement"] = float(((pvis > 0.5) == gh).float().mean())
     out["primary_depth_mae_on_common_hits"] = float((pdist - gt_t).abs()[gh & (pvis > 0.5)].mean())
     out["view"] = "512x512 pinhole at radius 2.5, %d of %d pixels hit" % (k, n)
+    # the same frame with NO analytic G-buffer ("no mesh in the pipeline"): hit points and normals from
+    # the field's own primary answers, shadow + AO rays from there (ddf_query_shaded), judged against the scene
+    lit = torch.empty(n, dtype=torch.uint8, device="cuda"); nrm = torch.empty((n, 3), device="cuda")
+    aow = torch.empty(n, device="cuda"); cs = torch.zeros(2, dtype=torch.int64, device="cuda")
+    eps_w = 2e-2
+    ddf.ddf_query_shaded(m, po, pd, W, H, [(3.0, 3.0, 3.0)], spp, MASTER_SEED, STREAMS["ao_samples"], eps_w, float("inf"),
+                         pdist, pvis, lit, nrm, aow, cs)
+    both = gh & (pvis > 0.5)
+    gn_img = torch.zeros((n, 3), device="cuda"); gn_img[pix] = gn
+    ang = torch.rad2deg(torch.acos((nrm * gn_img).sum(1)[both].clamp(-1.0, 1.0)))
+    gs_img = torch.zeros(n, dtype=torch.bool, device="cuda"); gs_img[pix] = gt_shadow
+    mf = {"eps": eps_w, "pixels_hit_by_both": int(both.sum().item()),
+          "normal_error_deg_median": float(ang.median()), "normal_error_deg_mean": float(ang.mean()),
+          "shadow_agreement": float(((lit == 0) == gs_img)[both].float().mean())}
+    # AO: the scene ray-cast along the very rays the wavefront traced (isolates the field's answers from sampling noise)
+    p_c = torch.empty((n, 3), device="cuda"); n_c = torch.empty((n, 3), device="cuda"); idx = torch.empty(n, dtype=torch.int32, device="cuda")
+    wo = torch.empty((n * spp, 3), device="cuda"); wd = torch.empty((n * spp, 3), device="cuda"); cnt = torch.zeros(1, dtype=torch.int64, device="cuda")
+    ddf.ddf_gen_ao_from_hits(m, po, pd, pdist, pvis, W, H, spp, MASTER_SEED, STREAMS["ao_samples"], eps_w, p_c, n_c, idx, wo, wd, cnt)
+    kk = int(cnt.item())
+    wt = torch.empty(kk * spp, device="cuda"); wh = torch.empty(kk * spp, dtype=torch.uint8, device="cuda")
+    ddf.ddf_scene_raycast(scene, wo[:kk * spp].contiguous(), wd[:kk * spp].contiguous(), kk * spp, wt, wh)
+    ao_scene = 1.0 - wh.view(kk, spp).float().mean(dim=1)
+    ao_field = aow[idx[:kk].long()]
+    mf["ao_mae_same_rays"] = float((ao_field - ao_scene).abs().mean())
+    ao_gt_img = torch.ones(n, device="cuda"); ao_gt_img[pix] = ao_gt
+    mf["ao_mae_vs_gbuffer_ao_other_samples"] = float((aow - ao_gt_img).abs()[both].mean())
+    mf["rays"] = {"shadow": int(cs[0].item()), "ao": int(cs[1].item())}
+    out["meshfree_frame"] = mf
     ddf.ddf_destroy(m)
     return out
 
