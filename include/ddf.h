@@ -24,7 +24,9 @@
  *  - All work is enqueued on `stream` (a cudaStream_t passed as void*; NULL = default stream);
  *    no call synchronises the stream except ddf_create / ddf_destroy / ddf_trainer_create /
  *    ddf_trainer_export / the *_host variants, and - only for models served by the CUDA-core path -
- *    sdf_sphere_trace with early_exit and ddf_query_shadowed[_lights] (their grids are sized on the host).
+ *    sdf_sphere_trace with early_exit and ddf_query_shadowed[_lights] (their grids are sized on the host),
+ *    and ddf_query_ao_wavefront / ddf_query_shaded when spp does not divide 32 or only the CUDA-core path
+ *    serves the model (one host read of the hit count; such a call cannot be captured).
  *    Results are valid once the stream reaches the point after the call.
  *  - n == 0 is DDF_OK and a no-op; n < 0 or a NULL pointer with n > 0 is DDF_E_INVALID_ARG.
  *  - Results are a pure function of (weights, ray): independent of n and of the ray's position
