@@ -101,7 +101,7 @@ int  ddf_last_cuda_error(void);                           /* cudaError_t of the 
  * The persistent tcgen05 kernel answers a batch in one launch; a batch of at most 40 of its 256-ray
  * tiles (n <= 10,240) is instead answered as n_hidden + 2 launches chained by programmatic dependent
  * launch - encoding, one launch per hidden layer with the layer's output columns split over the
- * CTA pairs, heads - which keeps the whole chip busy on a small batch (2.2x faster at n <= 3,072).
+ * CTA pairs, heads - which keeps the whole chip busy on a small batch (2.5x faster at n <= 2,048).
  * Both return the same bits.  3 = tcgen05 path, always the single persistent launch; 4 = tcgen05
  * path, column-split whenever the batch fits the split scratch (n <= 18,944), else persistent.
  * 3 and 4 are DDF_E_UNSUPPORTED for models the persistent kernel does not serve. */
