@@ -246,7 +246,8 @@ int  ddf_query_shadowed_lights(ddf_model* model, const float* o, const float* d,
  * (all must hold n = width * height entries), *count (int64 [device]) the number of hits; when o2 / d2
  * (both or neither; [n * spp][3]) are given they receive spp cosine-weighted rays per hit from
  * p_c + eps * nrm_c, exactly ddf_gen_ao(p_c, nrm_c, count, ...) with the count read on the device.
- * All pointers [device]; asynchronous on `stream`; uses a workspace owned by `model`. */
+ * All pointers [device]; asynchronous on `stream`; uses a workspace owned by `model`.
+ * width * height * spp must not exceed 2^31 - 1 (DDF_E_INVALID_ARG). */
 int  ddf_gen_ao_from_hits(ddf_model* model, const float* o, const float* d, const float* dist,
                           const float* vis, int width, int height, int spp, uint64_t seed,
                           uint64_t rng_stream, float eps, float* p_c, float* nrm_c, int32_t* index,

@@ -358,7 +358,7 @@ extern "C" int ddf_gen_ao_from_hits(ddf_model* model, const float* o, const floa
                                     const float* vis, int width, int height, int spp, uint64_t seed,
                                     uint64_t rng_stream, float eps, float* p_c, float* nrm_c, int32_t* index,
                                     float* o2, float* d2, int64_t* count, void* stream) {
-  if (!model || !count || width < 0 || height < 0 || spp <= 0 || (int64_t)width * height > 0x7fffffff) return DDF_E_INVALID_ARG;
+  if (!model || !count || width < 0 || height < 0 || spp <= 0 || (int64_t)width * height * spp > 0x7fffffff) return DDF_E_INVALID_ARG;
   if ((o2 == nullptr) != (d2 == nullptr)) return DDF_E_INVALID_ARG;
   cudaStream_t st = (cudaStream_t)stream;
   Model* m = reinterpret_cast<Model*>(model);
@@ -376,7 +376,7 @@ static int ao_wavefront_impl(ddf_model* model, const float* o, const float* d, i
                              int spp, uint64_t seed, uint64_t rng_stream, float eps, float ao_radius,
                              float* out_dist, float* out_vis, float* out_nrm, float* out_ao,
                              int64_t* out_count, void* stream, bool do_primary) {
-  if (!model || width < 0 || height < 0 || spp <= 0 || (int64_t)width * height > 0x7fffffff) return DDF_E_INVALID_ARG;
+  if (!model || width < 0 || height < 0 || spp <= 0 || (int64_t)width * height * spp > 0x7fffffff) return DDF_E_INVALID_ARG;
   Model* m = reinterpret_cast<Model*>(model);
   if (m->lay.input_kind != 0 || m->lay.n_out != 2) return DDF_E_INVALID_ARG;
   cudaStream_t st = (cudaStream_t)stream;
