@@ -92,6 +92,19 @@ def test_ao_wavefront_call_replays_from_a_graph(ddf, kind):
     g.replay(); torch.cuda.synchronize()
     assert torch.equal(dist, want[0]) and torch.equal(vis, want[1]) and torch.equal(nrm, want[2]) and torch.equal(ao, want[3])
     assert int(cnt.item()) == want[4]
+    # the whole shaded frame (shadow loop for two lights + AO loop on one primary query) replays too
+    mask = torch.empty(n, dtype=torch.uint8, device="cuda"); cs = torch.zeros(2, dtype=torch.int64, device="cuda")
+    lights = [(3.0, 3.0, 3.0), (-3.0, 2.0, 1.0)]
+    shaded = lambda st=None: ddf.ddf_query_shaded(m, o, d, W, H, lights, 16, 11, 3, 1e-3, 2.0, dist, vis, mask, nrm, ao, cs, stream=st)
+    shaded(); torch.cuda.synchronize()
+    g2 = _capture(lambda st: shaded(st))
+    o.copy_(o.flip(0).contiguous()); d.copy_(d.flip(0).contiguous())
+    shaded(); torch.cuda.synchronize()
+    want2 = (dist.clone(), vis.clone(), mask.clone(), nrm.clone(), ao.clone(), cs.clone())
+    for x in (dist, vis, mask, nrm, ao, cs): x.zero_()
+    g2.replay(); torch.cuda.synchronize()
+    for got, ref in zip((dist, vis, mask, nrm, ao, cs), want2): assert torch.equal(got, ref)
+    assert int(cs[0].item()) > 0 and int(cs[1].item()) > 0
     ddf.ddf_destroy(m)
 
 
