@@ -287,10 +287,11 @@ def run_extras(ddf, torch, model, peaks):
         m = 1 << lg
         ms = _time_ms(torch, lambda: ddf.ddf_query(model, o, d, m, dist, vis), reps=3 if lg > 20 else 7)
         sweep["2^%d" % lg] = {"ms": ms, "ns_per_ray": ms * 1e6 / m, "Mrays_s": m / ms / 1e3, "frac_peak": tf(m, ms) / peaks["burst"]}
-        if lg <= 14:      # an isolated call on an idle stream above; here the per-call time of 50 calls back to back
+        if lg <= 17:      # an isolated call on an idle stream above; here the per-call time of calls queued back to back
+            nb = 50 if lg <= 14 else 16
             def burst():
-                for _ in range(50): ddf.ddf_query(model, o, d, m, dist, vis)
-            sweep["2^%d" % lg]["ms_back_to_back"] = _time_ms(torch, burst, reps=3) / 50
+                for _ in range(nb): ddf.ddf_query(model, o, d, m, dist, vis)
+            sweep["2^%d" % lg]["ms_back_to_back"] = _time_ms(torch, burst, reps=3) / nb
     ex["sweep"] = sweep
     del o, d, dist, vis, ao
     # ---- configs[4]: sphere tracing an SDF MLP of the same width and depth on the camera rays

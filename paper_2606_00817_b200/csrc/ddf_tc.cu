@@ -837,8 +837,11 @@ int tc_forward(Model* m, const float* o, const float* d, int64_t n, const int64_
   // small batches: split the output columns of a layer over the CTA pairs (ddf_set_path 3 / 4 pin the choice)
   const int64_t split_max = (t->cg != 2 || m->path == 3) ? 0 : (m->path == 4 ? t->grid / 2 : kSplitAutoTiles);
   if (tiles <= split_max) return tc_forward_split(m, p, tiles, st);
-  int grid = t->grid;
-  if (tiles * t->cg < grid) grid = (int)tiles * t->cg;   // n_dev can only shrink n
+  // as many CTAs (pairs) as give every one the same number of tiles (+-1): the last wave of a persistent grid is
+  // otherwise part empty, and the CTAs that would idle through it only add L2 contention and power in the others
+  const int64_t units = t->grid / t->cg;
+  const int64_t waves = (tiles + units - 1) / units;
+  int grid = (int)((tiles + waves - 1) / waves) * t->cg;  // <= t->grid; n_dev can only shrink n
   cudaLaunchConfig_t cfg;
   memset(&cfg, 0, sizeof(cfg));
   cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3(kThreads); cfg.stream = st;
