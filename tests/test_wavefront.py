@@ -397,3 +397,36 @@ def test_gpu_shaded_frame_is_the_two_loops_on_one_primary_query(orc):
         with pytest.raises(ddf.DdfError):
             ddf.ddf_query_shaded(m, o, d, W, H, lights, spp, 5, 6, 1e-3, 2.0, dist, vis, None, nrm, ao, cs)
         ddf.ddf_destroy(m)
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("path", [0, 1])                 # narrow tcgen05 kernel (count stays on the device) / CUDA-core path (host-counted)
+def test_gpu_ao_wavefront_on_the_narrow_and_cuda_core_paths(orc, path):
+    import torch
+    import paper_2606_00817_b200 as ddf
+    from ddf_inputs import layout_c0
+    ddf.build()
+    m = ddf.ddf_create(make_weights(layout_c0()), layout_c0())
+    ddf.ddf_set_path(m, path)
+    W, H, spp = 64, 48, 8; n = W * H
+    cam = ddf.ddf_camera_from_seed(MASTER_SEED, STREAMS["camera_pos"], 2.5)
+    o = torch.empty((n, 3), device="cuda"); d = torch.empty((n, 3), device="cuda")
+    ddf.ddf_gen_camera(cam, W, H, o, d)
+    o += torch.from_numpy(random_rays(n)[0]).cuda() * 0.4
+    dist = torch.empty(n, device="cuda"); vis = torch.empty(n, device="cuda"); ao = torch.full((n,), float("nan"), device="cuda")
+    cnt = torch.zeros(1, dtype=torch.int64, device="cuda")
+    ddf.ddf_query_ao_wavefront(m, o, d, W, H, spp, 3, 4, 1e-3, 1.0, dist, vis, None, ao, cnt)
+    torch.cuda.synchronize()
+    k = int((vis > 0.5).sum().item())
+    assert int(cnt.item()) == k * spp and 0 < k < n
+    p_c = torch.empty((n, 3), device="cuda"); n_c = torch.empty((n, 3), device="cuda"); idx = torch.empty(n, dtype=torch.int32, device="cuda")
+    o2 = torch.empty((n * spp, 3), device="cuda"); d2 = torch.empty((n * spp, 3), device="cuda"); c2 = torch.zeros(1, dtype=torch.int64, device="cuda")
+    ddf.ddf_gen_ao_from_hits(m, o, d, dist, vis, W, H, spp, 3, 4, 1e-3, p_c, n_c, idx, o2, d2, c2)
+    rp, rn, ridx = orc.hit_normals(o.cpu().numpy(), d.cpu().numpy(), dist.cpu().numpy(), vis.cpu().numpy(), W, H)
+    assert int(c2.item()) == k and np.array_equal(idx[:k].cpu().numpy(), ridx)
+    dist2 = torch.empty(k * spp, device="cuda"); vis2 = torch.empty(k * spp, device="cuda")
+    ddf.ddf_query(m, o2[:k * spp].contiguous(), d2[:k * spp].contiguous(), k * spp, dist2, vis2)
+    want = np.ones(n, np.float32)
+    want[ridx] = orc.ao_reduce(vis2.cpu().numpy(), dist2.cpu().numpy(), spp, 1.0)
+    assert np.array_equal(ao.cpu().numpy(), want) and 0.0 < want[ridx].mean() < 1.0
+    ddf.ddf_destroy(m)
