@@ -185,15 +185,43 @@ __global__ void __launch_bounds__(kHgThreads, 5) ddf_hash_kernel(const __grid_co
       }
       #pragma unroll
       for (int i = 0; i < 16; ++i) rw[i] = pack_bf16(g[2 * i], g[2 * i + 1]);
-      // ---- hash grid on the origin (readings H1-H5)
-      float x01[3] = {0.0f, 0.0f, 0.0f};
-      if (!p.cam_mode) {
+    }
+    // ---- hash grid on the origin (readings H1-H5)
+    float x01[3] = {0.0f, 0.0f, 0.0f};
+    if (valid && !p.cam_mode) {
+      #pragma unroll
+      for (int a = 0; a < 3; ++a) {
+        const float v = __fdiv_rn(__fsub_rn(p.o[3 * ray + a], p.bmin[a]), p.den[a]);
+        x01[a] = fminf(fmaxf(v, 0.0f), 1.0f);
+      }
+    }
+    // Rays that share an origin share its level features.  When every aligned group of 16 rays of this warp
+    // does (the rays of an AO point, of a camera, of a light sample), lane j of a group computes level j once
+    // and the group exchanges the results: 8 gathers per ray instead of 128, the same function of the same
+    // point, so the same bits.  The test is warp-uniform; any other warp takes the per-ray path below.
+    static_assert(kHgMaxLevels <= 16, "one level per lane of a 16-lane group");
+    bool shared16 = false;
+    if (!p.cam_mode) {
+      const int leader = lane & ~15;
+      float xg[3];
+      bool same = true;
+      #pragma unroll
+      for (int a = 0; a < 3; ++a) {
+        xg[a] = __shfl_sync(0xffffffffu, x01[a], leader);
+        same = same && (__float_as_uint(xg[a]) == __float_as_uint(x01[a]));
+      }
+      shared16 = __all_sync(0xffffffffu, same || !valid);
+      if (shared16) {
+        const int lj = lane & 15;
+        const uint32_t f = (lj < p.n_levels) ? hg_level_feature<F16>(p.lv[lj], p.tmask, p.table, xg) : 0u;
         #pragma unroll
-        for (int a = 0; a < 3; ++a) {
-          const float v = __fdiv_rn(__fsub_rn(p.o[3 * ray + a], p.bmin[a]), p.den[a]);
-          x01[a] = fminf(fmaxf(v, 0.0f), 1.0f);
+        for (int l = 0; l < kHgMaxLevels; ++l) {
+          const uint32_t v = __shfl_sync(0xffffffffu, f, leader + l);
+          if (valid && l < p.n_levels) rw[kHgFeatCol / 2 + l] = v;
         }
       }
+    }
+    if (valid && !shared16) {
       #pragma unroll
       for (int l = 0; l < kHgMaxLevels; ++l) {
         if (l < p.n_levels) {

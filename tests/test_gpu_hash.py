@@ -205,3 +205,38 @@ def test_query_camera_is_generator_plus_query(ddf, kind):
             assert ddf.ddf_get_info(m, 1) == 1                # one launch, no generator
     ddf.ddf_query_camera(m, cam, 0, 5, d1, v1)                 # empty image: a no-op
     ddf.ddf_destroy(m)
+
+
+@pytest.mark.parametrize("table_dtype", [0, 2])
+def test_shared_origin_groups_return_the_per_ray_bits(ddf, orc, table_dtype):
+    """Warps whose aligned 16-ray groups share an origin compute each level once per group (ddf_hash.cu); the
+    same rays in an order that breaks the groups take the per-ray path.  Same function of the same point:
+    the results must be bit-identical ray by ray, whatever the group size, the tail, or the mix of warps."""
+    lay = layout_hash_paper() if table_dtype == 0 else HashLayout(table_dtype=2)
+    table, mlp, m = _field(ddf, lay)
+    g = torch.Generator(device="cuda").manual_seed(11)
+    for spp, npts in [(16, 1000), (32, 333), (8, 777), (16, 1), (48, 100)]:       # 8: groups of 16 span two origins -> per-ray path
+        n = spp * npts
+        op = (torch.rand((npts, 3), device="cuda", generator=g) * 2 - 1) * 2.9
+        o = op.repeat_interleave(spp, dim=0).contiguous()
+        d = torch.nn.functional.normalize(torch.randn((n, 3), device="cuda", generator=g), dim=1).contiguous()
+        if spp == 16 and npts == 1000:                                             # a mix: every third point's rays get their own origins
+            o.view(npts, spp, 3)[::3] += torch.rand((len(range(0, npts, 3)), spp, 3), device="cuda", generator=g) * 1e-3
+        t = torch.empty(n, device="cuda"); xi = torch.empty(n, device="cuda")
+        ddf.ddf_query(m, o, d, n, t, xi)
+        perm = torch.randperm(n, device="cuda", generator=g)
+        t2 = torch.empty(n, device="cuda"); xi2 = torch.empty(n, device="cuda")
+        ddf.ddf_query(m, o[perm].contiguous(), d[perm].contiguous(), n, t2, xi2)
+        assert torch.equal(t[perm], t2) and torch.equal(xi[perm], xi2), (spp, npts)
+        # ... and both are the oracle's field
+        k = min(n, 2000)
+        sel = torch.arange(0, n, max(1, n // k), device="cuda")[:k]
+        z, tr, xr = orc.hash_forward(lay, table, mlp, o[sel].cpu().numpy(), d[sel].cpu().numpy())
+        _check(t[sel].cpu().numpy(), xi[sel].cpu().numpy(), tr, xr, "shared origin spp=%d" % spp)
+        # fused AO reduce on the grouped batch = reducer on the per-ray answers
+        if 32 % spp == 0:
+            ao = torch.empty(npts, device="cuda"); ao2 = torch.empty(npts, device="cuda")
+            ddf.ddf_query_ao(m, o, d, npts, spp, 1.5, ao)
+            ddf.ddf_ao_reduce(xi, t, npts, spp, 1.5, ao2)
+            assert torch.equal(ao, ao2)
+    ddf.ddf_destroy(m)
