@@ -559,6 +559,11 @@ def run_hashgrid(ddf, torch, peaks):
     oa = torch.empty((na, 3), device="cuda"); da = torch.empty((na, 3), device="cuda"); ao = torch.empty(npts, device="cuda")
     ddf.ddf_gen_ao(gp, gn, npts, spp, MASTER_SEED, STREAMS["ao_samples"], 1e-3, oa, da)
     rec("ao_16.7M_fused", na, _time_ms(torch, lambda: ddf.ddf_query_ao(m, oa, da, npts, spp, float("inf"), ao), reps=5))
+    # the same AO image from the G-buffer points themselves (ddf_query_ao_points): rays generated inside the kernel
+    ao_pts = torch.empty(npts, device="cuda")
+    rec("ao_16.7M_from_points", na, _time_ms(torch, lambda: ddf.ddf_query_ao_points(m, gp, gn, npts, spp, MASTER_SEED, STREAMS["ao_samples"], 1e-3,
+                                                                                        float("inf"), ao_pts), reps=5))
+    out["ao_16.7M_from_points"]["bit_identical_to_gen_plus_query_ao"] = bool(torch.equal(ao, ao_pts))
     del oa, da
     ddf.ddf_destroy(m)
     # the same field with an fp16 table (26 MB): random origins again

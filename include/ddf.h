@@ -196,6 +196,15 @@ int  ddf_ao_reduce(const float* vis, const float* dist, int64_t n_pts, int spp, 
  * owned by the model is used and ddf_ao_reduce runs as a second launch. */
 int  ddf_query_ao(ddf_model* model, const float* o, const float* d, int64_t n_pts, int spp,
                   float ao_radius, float* ao, void* stream);
+/* The same from surface points: the spp rays of point i are ddf_gen_ao's (same seed, rng_stream, eps: ray
+ * k = i * spp + s), ao[i] as ddf_query_ao.  For a hash-grid field with spp dividing 32 the rays are generated
+ * inside the query kernel and never exist in memory (12 B of point + 12 B of normal per spp rays instead of
+ * 24 B per ray, and the spp rays of a point share one set of level look-ups); every other model generates
+ * them into a workspace owned by `model` and calls ddf_query_ao.  Bit for bit ddf_gen_ao + ddf_query_ao.
+ * p, nrm [n_pts][3] [device], ao [n_pts] [device]; n_pts * spp <= 2^31 - 1. */
+int  ddf_query_ao_points(ddf_model* model, const float* p, const float* nrm, int64_t n_pts, int spp,
+                         uint64_t seed, uint64_t rng_stream, float eps, float ao_radius, float* ao,
+                         void* stream);
 /* shadow[i] = 1 if vis > 0.5 and dist < tmax ("occluded within the distance to the light"). */
 int  ddf_shadow_test(const float* vis, const float* dist, const float* tmax, int64_t n,
                      uint8_t* shadow, void* stream);

@@ -17,7 +17,7 @@ EXPORTED_SYMBOLS = [
     "ddf_gen_camera", "ddf_gen_sphere_points", "ddf_gen_shadow", "ddf_gen_gbuffer", "ddf_gen_ao",
     "ddf_ao_reduce", "ddf_query_ao", "ddf_shadow_test", "sdf_sphere_trace",
     "ddf_hashgrid_table_entries", "ddf_create_hashgrid", "ddf_gen_shadow_from_hits", "ddf_query_shadowed", "ddf_query_shadowed_lights",
-    "ddf_gen_ao_from_hits", "ddf_query_ao_wavefront", "ddf_query_shaded",
+    "ddf_gen_ao_from_hits", "ddf_query_ao_wavefront", "ddf_query_shaded", "ddf_query_ao_points",
     "ddf_trainer_create", "ddf_trainer_destroy", "ddf_trainer_step", "ddf_trainer_loss_grads", "ddf_trainer_export",
     "ddf_trainer_steps", "ddf_scene_raycast", "ddf_gen_train_batch", "ddf_query_camera",
 ]
@@ -296,6 +296,12 @@ def ddf_query_shadowed_lights(model, o, d, n, lights, eps, out_dist, out_vis, ou
     _check(lib().ddf_query_shadowed_lights(model.handle, _dev(o), _dev(d), C.c_int64(n), li, C.c_int(len(flat) // 3), C.c_float(eps),
                                            _dev(out_dist), _dev(out_vis), _dev(out_lit_mask, torch.uint8),
                                            _dev(out_count, torch.int64), _stream(stream)), "ddf_query_shadowed_lights")
+
+
+def ddf_query_ao_points(model, p, nrm, n_pts, spp, seed, rng_stream, eps, ao_radius, ao, stream=None):
+    _check(lib().ddf_query_ao_points(model.handle, _dev(p), _dev(nrm), C.c_int64(n_pts), C.c_int(spp), C.c_uint64(int(seed)),
+                                     C.c_uint64(int(rng_stream)), C.c_float(eps), C.c_float(ao_radius), _dev(ao),
+                                     _stream(stream)), "ddf_query_ao_points")
 
 
 def ddf_gen_ao_from_hits(model, o, d, dist, vis, width, height, spp, seed, rng_stream, eps, p_c, nrm_c, index, o2, d2, count,

@@ -364,6 +364,31 @@ extern "C" int ddf_query_camera(ddf_model* model, const ddf_camera* cam, int wid
   return rc;
 }
 
+extern "C" int ddf_query_ao_points(ddf_model* model, const float* p, const float* nrm, int64_t n_pts, int spp,
+                                   uint64_t seed, uint64_t rng_stream, float eps, float ao_radius, float* ao,
+                                   void* stream) {
+  if (!model || n_pts < 0 || spp <= 0 || n_pts * spp > 0x7fffffff) return DDF_E_INVALID_ARG;
+  Model* m = reinterpret_cast<Model*>(model);
+  if (m->lay.n_out != 2 || m->lay.input_kind != 0) return DDF_E_INVALID_ARG;
+  if (n_pts == 0) { m->last_launches = 0; return DDF_OK; }
+  if (!p || !nrm || !ao) return DDF_E_INVALID_ARG;
+  cudaStream_t st = (cudaStream_t)stream;
+  if (m->hg && spp <= 32 && 32 % spp == 0)                    // the rays never exist in memory
+    return hash_forward_ao_points(m, p, nrm, n_pts, nullptr, spp, gen_key(seed, rng_stream), eps, ao_radius, ao, st);
+  const int64_t n = n_pts * spp;
+  if (n > m->cam_rows) {
+    cudaFree(m->cam_o); cudaFree(m->cam_d); m->cam_o = m->cam_d = nullptr; m->cam_rows = 0;
+    DDF_CUDA_TRY(cudaMalloc(&m->cam_o, (size_t)n * 12));
+    DDF_CUDA_TRY(cudaMalloc(&m->cam_d, (size_t)n * 12));
+    m->cam_rows = n;
+  }
+  int rc = ddf_gen_ao(p, nrm, n_pts, spp, seed, rng_stream, eps, m->cam_o, m->cam_d, stream);
+  if (rc != DDF_OK) return rc;
+  rc = ddf_query_ao(model, m->cam_o, m->cam_d, n_pts, spp, ao_radius, ao, stream);
+  if (rc == DDF_OK) m->last_launches += 1;
+  return rc;
+}
+
 extern "C" int ddf_query_ao(ddf_model* model, const float* o, const float* d, int64_t n_pts, int spp,
                             float ao_radius, float* ao, void* stream) {
   if (!model || n_pts < 0 || spp <= 0) return DDF_E_INVALID_ARG;

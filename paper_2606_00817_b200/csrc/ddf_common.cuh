@@ -94,6 +94,10 @@ int hash_forward(Model* m, const float* o, const float* d, int64_t n, const int6
                  float* out0, float* out1, int spp, float ao_radius, cudaStream_t st);
 
 int hash_forward_camera(Model* m, const ddf_camera* cam, int width, int height, float* out0, float* out1, cudaStream_t st);
+// AO of n_pts points (n_pts_dev: device-side count or null), the spp rays of a point generated in the kernel
+int hash_forward_ao_points(Model* m, const float* pts, const float* nrm, int64_t n_pts, const int64_t* n_rays_dev, int spp,
+                           uint64_t key, float eps, float ao_radius, float* ao, cudaStream_t st);
+uint64_t gen_key(uint64_t seed, uint64_t rng_stream);   // ddf_gen.cu: the generators' counter key
 
 // ---- narrow-network tcgen05 path (ddf_narrow.cu)
 int narrow_plan_create(Model* m, const uint16_t* hw_host, const float* hb_host);   // sets m->nw or leaves it null
@@ -131,6 +135,31 @@ __device__ __forceinline__ float softplus_f(float z) {
   return fmaxf(z, 0.0f) + log1pf(expf(-fabsf(z)));
 }
 __device__ __forceinline__ float sigmoid_f(float z) { return 1.0f / (1.0f + expf(-z)); }
+
+// AO ray k (= point k / spp, sample k % spp) about the unit normal n at p: origin p + eps n, cosine-weighted
+// direction in the frame (t1, t2, n) (reading A9 / row a11).  Shared by the generator kernel and by the
+// kernels that generate the rays themselves, so both produce the same bits.
+__device__ __forceinline__ void ao_ray_from_point(const float p[3], const float n[3], uint64_t key, int64_t k, float eps,
+                                                  float o[3], float d[3]) {
+  int ax = 0;
+  if (fabsf(n[1]) < fabsf(n[ax])) ax = 1;
+  if (fabsf(n[2]) < fabsf(n[ax])) ax = 2;
+  float e[3] = { ax == 0 ? 1.0f : 0.0f, ax == 1 ? 1.0f : 0.0f, ax == 2 ? 1.0f : 0.0f };
+  float t1[3] = { e[1]*n[2] - e[2]*n[1], e[2]*n[0] - e[0]*n[2], e[0]*n[1] - e[1]*n[0] };
+  float inv = 1.0f / sqrtf(t1[0]*t1[0] + t1[1]*t1[1] + t1[2]*t1[2]);
+  t1[0] *= inv; t1[1] *= inv; t1[2] *= inv;
+  float t2[3] = { n[1]*t1[2] - n[2]*t1[1], n[2]*t1[0] - n[0]*t1[2], n[0]*t1[1] - n[1]*t1[0] };
+  float u1 = dev_uniform01(key, 2 * (uint64_t)k), u2 = dev_uniform01(key, 2 * (uint64_t)k + 1);
+  float r = sqrtf(u1), s, c;
+  sincospif(2.0f * u2, &s, &c);
+  float lx = r * c, ly = r * s, lz = sqrtf(1.0f - u1);
+  float dd[3];
+  #pragma unroll
+  for (int a = 0; a < 3; ++a) dd[a] = fmaf(lz, n[a], fmaf(ly, t2[a], lx * t1[a]));
+  inv = 1.0f / sqrtf(dd[0]*dd[0] + dd[1]*dd[1] + dd[2]*dd[2]);
+  #pragma unroll
+  for (int a = 0; a < 3; ++a) { o[a] = fmaf(eps, n[a], p[a]); d[a] = dd[a] * inv; }
+}
 
 // gamma of one ray into a bf16 row (E_pad entries, pad = 0).  sin/cos(2^k pi x) via sincospif
 // of the exactly scaled argument (ldexp), so high bands keep full fp32 accuracy.

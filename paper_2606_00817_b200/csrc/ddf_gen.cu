@@ -98,25 +98,12 @@ __global__ void gen_ao_kernel(const float* __restrict__ p, const float* __restri
   if (n_pts_dev) n_pts = *n_pts_dev;
   if (k >= n_pts * spp) return;
   int64_t i = k / spp;
-  float n[3] = { nrm[3 * i], nrm[3 * i + 1], nrm[3 * i + 2] };
-  int ax = 0;
-  if (fabsf(n[1]) < fabsf(n[ax])) ax = 1;
-  if (fabsf(n[2]) < fabsf(n[ax])) ax = 2;
-  float e[3] = { ax == 0 ? 1.0f : 0.0f, ax == 1 ? 1.0f : 0.0f, ax == 2 ? 1.0f : 0.0f };
-  float t1[3] = { e[1]*n[2] - e[2]*n[1], e[2]*n[0] - e[0]*n[2], e[0]*n[1] - e[1]*n[0] };
-  float inv = 1.0f / sqrtf(t1[0]*t1[0] + t1[1]*t1[1] + t1[2]*t1[2]);
-  t1[0] *= inv; t1[1] *= inv; t1[2] *= inv;
-  float t2[3] = { n[1]*t1[2] - n[2]*t1[1], n[2]*t1[0] - n[0]*t1[2], n[0]*t1[1] - n[1]*t1[0] };
-  float u1 = dev_uniform01(key, 2 * (uint64_t)k), u2 = dev_uniform01(key, 2 * (uint64_t)k + 1);
-  float r = sqrtf(u1), s, c;
-  sincospif(2.0f * u2, &s, &c);
-  float lx = r * c, ly = r * s, lz = sqrtf(1.0f - u1);
-  float dd[3];
+  const float n[3] = { nrm[3 * i], nrm[3 * i + 1], nrm[3 * i + 2] };
+  const float pp[3] = { p[3 * i], p[3 * i + 1], p[3 * i + 2] };
+  float oo[3], dd[3];
+  ao_ray_from_point(pp, n, key, k, eps, oo, dd);
   #pragma unroll
-  for (int a = 0; a < 3; ++a) dd[a] = fmaf(lz, n[a], fmaf(ly, t2[a], lx * t1[a]));
-  inv = 1.0f / sqrtf(dd[0]*dd[0] + dd[1]*dd[1] + dd[2]*dd[2]);
-  #pragma unroll
-  for (int a = 0; a < 3; ++a) { o[3 * k + a] = fmaf(eps, n[a], p[3 * i + a]); d[3 * k + a] = dd[a] * inv; }
+  for (int a = 0; a < 3; ++a) { o[3 * k + a] = oo[a]; d[3 * k + a] = dd[a]; }
 }
 
 __global__ void ao_reduce_kernel(const float* __restrict__ vis, const float* __restrict__ dist, int64_t n_pts, int spp,
@@ -145,6 +132,8 @@ __global__ void shadow_test_kernel(const float* __restrict__ vis, const float* _
 }
 
 static inline unsigned blocks_for(int64_t n, int t) { return (unsigned)((n + t - 1) / t); }
+
+uint64_t gen_key(uint64_t seed, uint64_t rng_stream) { return host_key(seed, rng_stream); }
 
 int gen_ao_launch(const float* p, const float* nrm, int64_t n_pts, const int64_t* n_pts_dev, int spp, uint64_t seed,
                   uint64_t rng_stream, float eps, float* o, float* d, cudaStream_t st) {

@@ -53,6 +53,9 @@ struct HgParams {
   // level features are computed once per CTA; o and d are not read
   int cam_mode, cam_w, cam_h;
   CamFrame cam;
+  // AO rays generated in the kernel (ddf_query_ao_points): ray k = sample k % spp of point k / spp; o and d are not read
+  int ao_mode; float ao_eps; uint64_t ao_key;
+  const float* ao_p; const float* ao_n;
 };
 
 struct HashPlan {
@@ -105,7 +108,9 @@ __device__ __forceinline__ uint32_t hg_level_feature(const HgLevel lv, uint32_t 
   return pack_bf16(f0, f1);
 }
 
-template <bool F16>
+// AOP: the rays are generated in the kernel from surface points (ddf_query_ao_points); a template parameter so that
+// the kernels that read rays from memory carry none of it
+template <bool F16, bool AOP = false>
 __global__ void __launch_bounds__(kHgThreads, 5) ddf_hash_kernel(const __grid_constant__ HgParams p) {
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
@@ -163,6 +168,7 @@ __global__ void __launch_bounds__(kHgThreads, 5) ddf_hash_kernel(const __grid_co
     uint32_t rw[32];                                   // the operand row, 64 bf16
     #pragma unroll
     for (int i = 0; i < 32; ++i) rw[i] = 0u;
+    float ov[3] = {0.0f, 0.0f, 0.0f};                  // the origin when the kernel generates the ray itself (ao_mode)
     if (valid) {
       // ---- gamma(d): identity, then per band 3 sines and 3 cosines (ddf.h), columns 0..26
       float g[32];
@@ -170,6 +176,12 @@ __global__ void __launch_bounds__(kHgThreads, 5) ddf_hash_kernel(const __grid_co
       for (int i = 0; i < 32; ++i) g[i] = 0.0f;
       float dv[3];
       if (p.cam_mode) pixel_dir(p.cam, p.cam_w, p.cam_h, (int)(ray % p.cam_w), (int)(ray / p.cam_w), dv);
+      else if (AOP) {
+        const int64_t pt = ray / p.spp;
+        const float pp[3] = { p.ao_p[3 * pt], p.ao_p[3 * pt + 1], p.ao_p[3 * pt + 2] };
+        const float nn[3] = { p.ao_n[3 * pt], p.ao_n[3 * pt + 1], p.ao_n[3 * pt + 2] };
+        ao_ray_from_point(pp, nn, p.ao_key, ray, p.ao_eps, ov, dv);
+      }
       else { dv[0] = p.d[3 * ray]; dv[1] = p.d[3 * ray + 1]; dv[2] = p.d[3 * ray + 2]; }
       g[0] = dv[0]; g[1] = dv[1]; g[2] = dv[2];
       #pragma unroll
@@ -191,7 +203,8 @@ __global__ void __launch_bounds__(kHgThreads, 5) ddf_hash_kernel(const __grid_co
     if (valid && !p.cam_mode) {
       #pragma unroll
       for (int a = 0; a < 3; ++a) {
-        const float v = __fdiv_rn(__fsub_rn(p.o[3 * ray + a], p.bmin[a]), p.den[a]);
+        const float oa = AOP ? ov[a] : p.o[3 * ray + a];
+        const float v = __fdiv_rn(__fsub_rn(oa, p.bmin[a]), p.den[a]);
         x01[a] = fminf(fmaxf(v, 0.0f), 1.0f);
       }
     }
@@ -369,6 +382,24 @@ int hash_forward_camera(Model* m, const ddf_camera* cam, int width, int height, 
   return DDF_OK;
 }
 
+int hash_forward_ao_points(Model* m, const float* pts, const float* nrm, int64_t n_pts, const int64_t* n_rays_dev, int spp,
+                           uint64_t key, float eps, float ao_radius, float* ao, cudaStream_t st) {
+  HashPlan* h = m->hg;
+  HgParams p = h->base;
+  const int64_t n = n_pts * spp;
+  p.o = nullptr; p.d = nullptr; p.n = n; p.n_dev = n_rays_dev; p.out0 = ao; p.out1 = nullptr;
+  p.mode_out = 2; p.spp = spp; p.ao_radius = ao_radius;
+  p.ao_mode = 1; p.ao_eps = eps; p.ao_key = key; p.ao_p = pts; p.ao_n = nrm;
+  const int64_t tiles = (n + kHgThreads - 1) / kHgThreads;
+  int64_t grid = (int64_t)m->sm_count * h->ctas_per_sm;
+  if (tiles < grid) grid = tiles;
+  if (p.table_f16) ddf_hash_kernel<true, true><<<(unsigned)grid, kHgThreads, h->smem_bytes, st>>>(p);
+  else             ddf_hash_kernel<false, true><<<(unsigned)grid, kHgThreads, h->smem_bytes, st>>>(p);
+  DDF_CUDA_TRY(cudaGetLastError());
+  m->last_launches = 1;
+  return DDF_OK;
+}
+
 int hash_forward(Model* m, const float* o, const float* d, int64_t n, const int64_t* n_dev, int mode_out,
                  float* out0, float* out1, int spp, float ao_radius, cudaStream_t st) {
   HashPlan* h = m->hg;
@@ -489,7 +520,9 @@ extern "C" int ddf_create_hashgrid(const void* table, const void* mlp, const ddf
   p.table_f16 = L.table_dtype == 2;
   h->smem_bytes = 16384 + (size_t)L.n_hidden * 8192 + (L.n_hidden + 2) * 256 + 128 + 1024;
   if ((e = cudaFuncSetAttribute(ddf_hash_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_bytes)) != cudaSuccess ||
-      (e = cudaFuncSetAttribute(ddf_hash_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_bytes)) != cudaSuccess)
+      (e = cudaFuncSetAttribute(ddf_hash_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_bytes)) != cudaSuccess ||
+      (e = cudaFuncSetAttribute(ddf_hash_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_bytes)) != cudaSuccess ||
+      (e = cudaFuncSetAttribute(ddf_hash_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_bytes)) != cudaSuccess)
     return fail(DDF_E_CUDA, e);
   // resident CTAs per SM from the kernel's own resource use (the runtime's occupancy query answers
   // for the current carve-out, which another library in the process may have left at "prefer L1")
@@ -511,7 +544,9 @@ extern "C" int ddf_create_hashgrid(const void* table, const void* mlp, const ddf
     int pct = (int)((h->ctas_per_sm * (h->smem_bytes + prop.reservedSharedMemPerBlock) * 100 + prop.sharedMemPerMultiprocessor - 1) / prop.sharedMemPerMultiprocessor);
     if (pct > 100) pct = 100;
     if ((e = cudaFuncSetAttribute(ddf_hash_kernel<false>, cudaFuncAttributePreferredSharedMemoryCarveout, pct)) != cudaSuccess ||
-        (e = cudaFuncSetAttribute(ddf_hash_kernel<true>, cudaFuncAttributePreferredSharedMemoryCarveout, pct)) != cudaSuccess)
+        (e = cudaFuncSetAttribute(ddf_hash_kernel<true>, cudaFuncAttributePreferredSharedMemoryCarveout, pct)) != cudaSuccess ||
+        (e = cudaFuncSetAttribute(ddf_hash_kernel<false, true>, cudaFuncAttributePreferredSharedMemoryCarveout, pct)) != cudaSuccess ||
+        (e = cudaFuncSetAttribute(ddf_hash_kernel<true, true>, cudaFuncAttributePreferredSharedMemoryCarveout, pct)) != cudaSuccess)
       return fail(DDF_E_CUDA, e);
   }
   if ((e = cudaDeviceSynchronize()) != cudaSuccess) return fail(DDF_E_CUDA, e);

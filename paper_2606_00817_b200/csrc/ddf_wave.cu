@@ -383,8 +383,10 @@ static int ao_wavefront_impl(ddf_model* model, const float* o, const float* d, i
   const int64_t n = (int64_t)width * height;
   if (n == 0) { if (out_count) DDF_CUDA_TRY(cudaMemsetAsync(out_count, 0, 8, st)); m->last_launches = 0; return DDF_OK; }
   if (!o || !d || !out_dist || !out_vis || !out_ao) return DDF_E_INVALID_ARG;
+  // a hash-grid field generates the AO rays inside its query kernel (ddf_query_ao_points): no ray buffer, no generator launch
+  const bool rays_in_kernel = m->hg && spp <= 32 && 32 % spp == 0;
   WaveAoWs w;
-  int rc = wave_ao_ws(m, n, spp, true, &w);
+  int rc = wave_ao_ws(m, n, rays_in_kernel ? 0 : spp, true, &w);
   if (rc != DDF_OK) return rc;
   // 1. primary rays
   int launches = 0;
@@ -394,10 +396,13 @@ static int ao_wavefront_impl(ddf_model* model, const float* o, const float* d, i
   }
   // 2. hit points, normals from the hit-point image, spp rays about each normal (compacted, size on the device)
   if ((rc = wave_ao_rays(m, w, o, d, out_dist, out_vis, width, height, spp, seed, rng_stream, eps, w.p_c, w.n_c, w.index,
-                         out_nrm, w.o2, w.d2, w.count, w.count_rays, st)) != DDF_OK) return rc;
+                         out_nrm, rays_in_kernel ? nullptr : w.o2, rays_in_kernel ? nullptr : w.d2, w.count, w.count_rays,
+                         st)) != DDF_OK) return rc;
   launches += m->last_launches;
   // 3. second query with the AO reduce fused when a pixel's rays sit in one warp; else through ddf_query_ao
-  if (has_fused_path(m) && spp <= 32 && 32 % spp == 0) {
+  if (rays_in_kernel) {
+    rc = hash_forward_ao_points(m, w.p_c, w.n_c, n, w.count_rays, spp, gen_key(seed, rng_stream), eps, ao_radius, w.ao_c, st);
+  } else if (has_fused_path(m) && spp <= 32 && 32 % spp == 0) {
     rc = fused_forward(m, w.o2, w.d2, n * spp, w.count_rays, 2, w.ao_c, nullptr, spp, ao_radius, st);
   } else {
     int64_t live = 0;

@@ -240,3 +240,33 @@ def test_shared_origin_groups_return_the_per_ray_bits(ddf, orc, table_dtype):
             ddf.ddf_ao_reduce(xi, t, npts, spp, 1.5, ao2)
             assert torch.equal(ao, ao2)
     ddf.ddf_destroy(m)
+
+
+@pytest.mark.parametrize("kind", ["hash_fp32", "hash_fp16", "dense_narrow", "dense_wide"])
+def test_query_ao_points_is_generator_plus_query_ao(ddf, kind):
+    """ddf_query_ao_points = ddf_gen_ao + ddf_query_ao bit for bit: in the hash-grid kernel the rays are generated
+    in place (never stored), every other model goes through the workspace."""
+    from ddf_inputs import layout_c0, layout_c1, make_weights
+    if kind.startswith("hash"):
+        lay = layout_hash_paper() if kind == "hash_fp32" else HashLayout(table_dtype=2)
+        _, _, m = _field(ddf, lay)
+    else:
+        lay = layout_c0() if kind == "dense_narrow" else layout_c1()
+        m = ddf.ddf_create(make_weights(lay), lay)
+    g = torch.Generator(device="cuda").manual_seed(5)
+    for npts, spp, radius in [(5000, 16, 1.5), (333, 32, float("inf")), (1, 8, 2.0), (700, 5, 1.0), (129, 4, 1.5)]:
+        p = (torch.rand((npts, 3), device="cuda", generator=g) * 2 - 1) * 1.5
+        nrm = torch.nn.functional.normalize(torch.randn((npts, 3), device="cuda", generator=g), dim=1).contiguous()
+        o = torch.empty((npts * spp, 3), device="cuda"); d = torch.empty((npts * spp, 3), device="cuda")
+        ddf.ddf_gen_ao(p, nrm, npts, spp, MASTER_SEED, STREAMS["ao_samples"], 1e-3, o, d)
+        want = torch.empty(npts, device="cuda"); got = torch.full((npts,), float("nan"), device="cuda")
+        ddf.ddf_query_ao(m, o, d, npts, spp, radius, want)
+        ddf.ddf_query_ao_points(m, p, nrm, npts, spp, MASTER_SEED, STREAMS["ao_samples"], 1e-3, radius, got)
+        torch.cuda.synchronize()
+        if kind.startswith("hash") and 32 % spp == 0: assert ddf.ddf_get_info(m, 1) == 1      # one launch, no ray buffer
+        assert torch.equal(got, want), (kind, npts, spp)
+        assert 0.0 <= float(want.min()) and float(want.max()) <= 1.0
+    ddf.ddf_query_ao_points(m, p, nrm, 0, 16, 1, 2, 1e-3, 1.0, got)
+    with pytest.raises(ddf.DdfError):
+        ddf.ddf_query_ao_points(m, p, None, 10, 16, 1, 2, 1e-3, 1.0, got)
+    ddf.ddf_destroy(m)
