@@ -232,6 +232,10 @@ def run_gpu(args):
         if world == 1:
             r, cores, sample = oracle_rate(12.0)
             out["cpu_baseline"] = {"value": r / 1e6, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
+        if world == 1:
+            # BASELINE.json configs[2], [3], [4] in the same line (the metric is quoted "at 2^20-2^24 rays"; north_star
+            # asks for the shadow / AO batches and the DDF / sphere-tracing ratio): outside the headline's timed region
+            out["config_results"] = run_config_results(ddf, torch, model, peaks, back_to_back=args.extras)
         if args.extras and world == 1:
             out["extra"] = run_extras(ddf, torch, model, peaks)
         print(json.dumps(out))
@@ -250,10 +254,10 @@ def _time_ms(torch, fn, reps=3, warm=1):
     return statistics.median(ts)
 
 
-def run_extras(ddf, torch, model, peaks):
-    """The other BASELINE.json configs, each measured the same way (median of 3 after 1 warm-up):
-    shadow (configs[2]), AO with the on-GPU reduction (configs[3]), the batch sweep and the
-    sphere-tracing comparison (configs[4])."""
+def run_config_results(ddf, torch, model, peaks, back_to_back=False):
+    """The other BASELINE.json configs, each measured the same way (CUDA events on the launching stream, median of 3
+    after 1 warm-up, inputs resident): shadow (configs[2]), AO with the on-GPU reduction (configs[3]), the batch
+    sweep 2^10 .. 2^24 and the sphere-tracing comparison on the camera rays (configs[4])."""
     from ddf_inputs import MASTER_SEED, STREAMS, layout_sdf, make_weights, random_rays
     ex = {}
     tf = lambda n, ms: n * FLOP_PER_RAY / (ms * 1e-3) / 1e12
@@ -287,7 +291,7 @@ def run_extras(ddf, torch, model, peaks):
         m = 1 << lg
         ms = _time_ms(torch, lambda: ddf.ddf_query(model, o, d, m, dist, vis), reps=3 if lg > 20 else 7)
         sweep["2^%d" % lg] = {"ms": ms, "ns_per_ray": ms * 1e6 / m, "Mrays_s": m / ms / 1e3, "frac_peak": tf(m, ms) / peaks["burst"]}
-        if lg <= 17:      # an isolated call on an idle stream above; here the per-call time of calls queued back to back
+        if back_to_back and lg <= 17:      # an isolated call on an idle stream above; here the per-call time of calls queued back to back
             nb = 50 if lg <= 14 else 16
             def burst():
                 for _ in range(nb): ddf.ddf_query(model, o, d, m, dist, vis)
@@ -311,8 +315,26 @@ def run_extras(ddf, torch, model, peaks):
         evals = int(tot.item())
         ex["sphere_trace_" + name] = {"ms": ms, "Mrays_s": n / ms / 1e3, "mlp_evals": evals, "mean_steps": float(st.float().mean()),
                                       "hit_rate": float(hit.float().mean()), "TFLOPs": evals * SDF_FLOP / (ms * 1e-3) / 1e12,
-                                      "ddf_speedup": ms / ddf_ms}
+                                      "frac_peak": evals * SDF_FLOP / (ms * 1e-3) / 1e12 / peaks["burst"], "ddf_speedup": ms / ddf_ms}
     ex["ddf_camera_2^20_ms"] = ddf_ms
+    ddf.ddf_destroy(sdf)
+    return ex
+
+
+def run_extras(ddf, torch, model, peaks):
+    """--extras: the sphere tracer's eps sweep and the SURVEY.md 8(f) rows (hash-grid field, wavefront, training, narrow networks)."""
+    from ddf_inputs import MASTER_SEED, STREAMS, layout_sdf, make_weights
+    ex = {}
+    n = 1 << 20
+    lay = layout_sdf()
+    sdf = ddf.ddf_create(make_weights(lay), lay)
+    cam = ddf.ddf_camera_from_seed(MASTER_SEED, STREAMS["camera_pos"], 2.5)
+    o = torch.empty((n, 3), device="cuda"); d = torch.empty((n, 3), device="cuda")
+    ddf.ddf_gen_camera(cam, 1024, 1024, o, d)
+    t = torch.empty(n, device="cuda"); hit = torch.empty(n, dtype=torch.uint8, device="cuda")
+    st = torch.empty(n, dtype=torch.int32, device="cuda"); tot = torch.zeros(1, dtype=torch.int64, device="cuda")
+    dist = torch.empty(n, device="cuda"); vis = torch.empty(n, device="cuda")
+    ddf_ms = _time_ms(torch, lambda: ddf.ddf_query(model, o, d, n, dist, vis))
     # "across convergence thresholds" (PAPER.md:112): the early-exit tracer at three hit thresholds
     for eps in (1e-2, 1e-4):
         prm = ddf.SdfTraceParams(64, eps, 6.0, 1.0, 0.05, 1)

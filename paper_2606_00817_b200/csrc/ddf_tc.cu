@@ -48,6 +48,7 @@ struct TcParams {
   CUtensorMap w[kMaxTcLayers];
   CUtensorMap x0, x1, g;
   CUtensorMap xs0, xs1;              // store maps (32-row boxes) on the same activation buffers
+  int hint_act, hint_w, hint_st;     // L2 eviction class of the three TMA streams (0 normal, 1 evict_last, 2 evict_first)
   const float* o; const float* d;
   int64_t n; const int64_t* n_dev;
   const float* bias; const float* head_w;
@@ -93,8 +94,8 @@ __device__ __forceinline__ void wait_bar(uint32_t bar, uint32_t parity, uint32_t
   }
 }
 
-template <int CG>
 __global__ void __launch_bounds__(kThreads, 1) ddf_tc_kernel(const __grid_constant__ TcParams p) {
+  constexpr int CG = 2;
   using Cfg = TcCfg<CG>;
   constexpr int S = Cfg::kStages;
   extern __shared__ uint8_t smem_raw[];
@@ -151,6 +152,7 @@ __global__ void __launch_bounds__(kThreads, 1) ddf_tc_kernel(const __grid_consta
     {
       uint32_t it = 0, act_phase = 0;                    // bit j of act_phase: parity for act_bar(j)
       int tile_local = 0;
+      const uint64_t pol_a = ptx::policy_of(p.hint_act), pol_w = ptx::policy_of(p.hint_w);
       for (int64_t tile = pid; tile < num_tiles; tile += num_pairs, ++tile_local) {
         const int gb = tile_local & 1;
         const int g_row = (cta_global * 2 + gb) * kTileM;
@@ -173,19 +175,11 @@ __global__ void __launch_bounds__(kThreads, 1) ddf_tc_kernel(const __grid_consta
               wait_bar<CG == 2>(empty_bar(s), ph ^ 1u, p.dbg, 0x300 + s);
               const int brow = c * kChunkN + (CG == 2 ? (int)rank * 128 : 0);
               if (ptx::elect_one()) {
-                if (CG == 2) {
-                  if (leader) ptx::mbar_arrive_expect_tx(full_bar(s), 2u * Cfg::kStageBytes);
-                  const uint32_t fb = ptx::mapa(full_bar(s), 0);
-                  if (kb < nk0) ptx::tma_load_2d_cg2(a_smem(s), amap, fb, kb * kKBlock, a_row);
-                  else          ptx::tma_load_2d_cg2(a_smem(s), &p.g, fb, (kb - nk0) * kKBlock, g_row);
-                  ptx::tma_load_2d_cg2(b_smem(s), &p.w[l], fb, kb * kKBlock, brow);
-                } else {
-                  ptx::mbar_arrive_expect_tx(full_bar(s), (uint32_t)Cfg::kStageBytes);
-                  if (kb < nk0) ptx::tma_load_2d(a_smem(s), amap, full_bar(s), kb * kKBlock, a_row);
-                  else          ptx::tma_load_2d(a_smem(s), &p.g, full_bar(s), (kb - nk0) * kKBlock, g_row);
-                  ptx::tma_load_2d(b_smem(s), &p.w[l], full_bar(s), kb * kKBlock, brow);
-                  ptx::tma_load_2d(b_smem(s) + 128 * kKBlock * 2, &p.w[l], full_bar(s), kb * kKBlock, brow + 128);
-                }
+                if (leader) ptx::mbar_arrive_expect_tx(full_bar(s), 2u * Cfg::kStageBytes);
+                const uint32_t fb = ptx::mapa(full_bar(s), 0);
+                if (kb < nk0) ptx::tma_load_2d_cg2_hint(a_smem(s), amap, fb, kb * kKBlock, a_row, pol_a);
+                else          ptx::tma_load_2d_cg2_hint(a_smem(s), &p.g, fb, (kb - nk0) * kKBlock, g_row, pol_a);
+                ptx::tma_load_2d_cg2_hint(b_smem(s), &p.w[l], fb, kb * kKBlock, brow, pol_w);
               }
               __syncwarp();
               ++it;
@@ -304,7 +298,8 @@ __global__ void __launch_bounds__(kThreads, 1) ddf_tc_kernel(const __grid_consta
               ptx::fence_proxy_async_smem();
               __syncwarp();
               if (lane == 0) {
-                ptx::tma_store_2d(smap, stage, col, cta_global * kTileM + q * 32);
+                if (p.hint_st) ptx::tma_store_2d_hint(smap, stage, col, cta_global * kTileM + q * 32, ptx::policy_of(p.hint_st));
+                else ptx::tma_store_2d(smap, stage, col, cta_global * kTileM + q * 32);
                 ptx::bulk_commit();
               }
             } else {
@@ -749,8 +744,7 @@ int tc_plan_create(Model* m) {
   if (!t) return DDF_E_NOMEM;
   memset(t, 0, sizeof(TcPlan));
   m->tc = t;
-  const char* env = getenv("DDF_TC_CTA_GROUP");
-  t->cg = (env && env[0] == '1') ? 1 : 2;
+  t->cg = 2;
   t->grid = (m->sm_count / 2) * 2;
   const size_t rows = (size_t)t->grid * kTileM;
   DDF_CUDA_TRY(cudaMalloc(&t->x0, rows * L.width * 2));
@@ -779,6 +773,8 @@ int tc_plan_create(Model* m) {
   if ((rc = make_map(&p.xs0, t->x0, L.width, rows, L.width, 32u)) != DDF_OK) return rc;
   if ((rc = make_map(&p.xs1, t->x1, L.width, rows, L.width, 32u)) != DDF_OK) return rc;
   if ((rc = make_map(&p.g, t->g, (uint64_t)m->E_pad, rows * 2, (uint64_t)m->E_pad)) != DDF_OK) return rc;
+  // L2 priorities of the persistent kernel's TMA streams: activation and weight loads evict_last, stores default
+  p.hint_act = 1; p.hint_w = 1; p.hint_st = 0;
   p.bias = m->d_b; p.head_w = m->d_head_w;
   p.x0p = t->x0; p.x1p = t->x1; p.gp = t->g;
   p.dbg = t->dbg_dev;
@@ -786,8 +782,7 @@ int tc_plan_create(Model* m) {
   p.skip_layer = L.skip_layer; p.n_out = (int)L.n_out; p.input_kind = (int)L.input_kind;
   p.Lo = (int)L.n_freq_origin; p.Ld = (int)L.n_freq_dir; p.E = m->E; p.E_pad = m->E_pad;
   p.g_last_nk16 = (m->E - (m->E_pad - kKBlock) + 15) / 16;
-  DDF_CUDA_TRY(cudaFuncSetAttribute(ddf_tc_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, TcCfg<1>::kSmemBytes));
-  DDF_CUDA_TRY(cudaFuncSetAttribute(ddf_tc_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, TcCfg<2>::kSmemBytes));
+  DDF_CUDA_TRY(cudaFuncSetAttribute(ddf_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TcCfg<2>::kSmemBytes));
   DDF_CUDA_TRY(cudaFuncSetAttribute(ddf_tc_split_layer_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TcCfg<2>::kSmemBytes));
   return DDF_OK;
 }
@@ -842,6 +837,10 @@ int tc_forward(Model* m, const float* o, const float* d, int64_t n, const int64_
   const int64_t units = t->grid / t->cg;
   const int64_t waves = (tiles + units - 1) / units;
   int grid = (int)((tiles + waves - 1) / waves) * t->cg;  // <= t->grid; n_dev can only shrink n
+#ifdef DDF_DEV
+  if (const char* e = getenv("DDF_DEV_GRID")) { int g = atoi(e); if (g >= 2 && g < grid) grid = g & ~1; }
+  if (const char* e = getenv("DDF_DEV_HINTS")) { int h = atoi(e); p.hint_act = h % 10; p.hint_w = (h / 10) % 10; p.hint_st = (h / 100) % 10; }
+#endif
   cudaLaunchConfig_t cfg;
   memset(&cfg, 0, sizeof(cfg));
   cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3(kThreads); cfg.stream = st;
@@ -849,13 +848,8 @@ int tc_forward(Model* m, const float* o, const float* d, int64_t n, const int64_
   attr[0].id = cudaLaunchAttributeClusterDimension;
   attr[0].val.clusterDim.x = (unsigned)t->cg; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
   cfg.attrs = attr; cfg.numAttrs = 1;
-  if (t->cg == 2) {
-    cfg.dynamicSmemBytes = TcCfg<2>::kSmemBytes;
-    DDF_CUDA_TRY(cudaLaunchKernelEx(&cfg, ddf_tc_kernel<2>, p));
-  } else {
-    cfg.dynamicSmemBytes = TcCfg<1>::kSmemBytes;
-    DDF_CUDA_TRY(cudaLaunchKernelEx(&cfg, ddf_tc_kernel<1>, p));
-  }
+  cfg.dynamicSmemBytes = TcCfg<2>::kSmemBytes;
+  DDF_CUDA_TRY(cudaLaunchKernelEx(&cfg, ddf_tc_kernel, p));
   m->last_launches = 1;
   return DDF_OK;
 }

@@ -79,6 +79,28 @@ __device__ __forceinline__ void tma_load_2d_cg2(uint32_t dst, const void* map, u
                :: "r"(dst), "l"(map), "r"(bar_cluster), "r"(c0), "r"(c1) : "memory");
 }
 
+// L2 eviction-priority policies for the .L2::cache_hint forms below
+__device__ __forceinline__ uint64_t policy_evict_normal() {
+  uint64_t p; asm volatile("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;" : "=l"(p)); return p;
+}
+__device__ __forceinline__ uint64_t policy_evict_last() {
+  uint64_t p; asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p)); return p;
+}
+__device__ __forceinline__ uint64_t policy_evict_first() {
+  uint64_t p; asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p)); return p;
+}
+__device__ __forceinline__ uint64_t policy_of(int cls) {
+  return cls == 1 ? policy_evict_last() : (cls == 2 ? policy_evict_first() : policy_evict_normal());
+}
+__device__ __forceinline__ void tma_load_2d_cg2_hint(uint32_t dst, const void* map, uint32_t bar_cluster, int c0, int c1, uint64_t pol) {
+  asm volatile("cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint"
+               " [%0], [%1, {%3, %4}], [%2], %5;"
+               :: "r"(dst), "l"(map), "r"(bar_cluster), "r"(c0), "r"(c1), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void tma_store_2d_hint(const void* map, uint32_t src, int c0, int c1, uint64_t pol) {
+  asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group.L2::cache_hint [%0, {%2, %3}], [%1], %4;"
+               :: "l"(map), "r"(src), "r"(c0), "r"(c1), "l"(pol) : "memory");
+}
 
 // 2-D tiled store shared::cta -> global (bulk async-group completion)
 __device__ __forceinline__ void tma_store_2d(const void* map, uint32_t src, int c0, int c1) {

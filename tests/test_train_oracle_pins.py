@@ -116,3 +116,90 @@ def test_supervision_raycast_textbook(orc):
     assert abs(rc((0, 0, -3), (0, 0, 1)) - 2.1) < 1e-12                 # slab bottom before the sphere
     s = 1 / math.sqrt(2)
     assert abs(rc((-2, 0, -2.75), (s, 0, s)) - (1.85 / s)) < 1e-9       # oblique: x is inside the slab from t = 1.1/s, z only from 1.85/s (at x = -0.15)
+
+
+# ---- orc_gen_train_batch (reading T6; "Rays that start on the surface and point in all directions ... a point
+# moved forward by s should report distance t-s", "We replace 30 percent of each batch with the ray-march
+# shifted points").  The pin shares nothing with the generator's ray casts: each ray's random draws are recomputed with
+# the numpy counter generator (ddf_inputs/rng.py), which says what SHOULD have happened to it (anchored iff u6 >= 0.5 and
+# the camera ray hit; shifted iff the emitted ray hits and u9 < 0.3), and the geometry is judged by implicit surface
+# functions and brute-force sampling along the ray, never by a ray-surface formula.
+def _unsigned_surface_distance(p, sc):
+    c = np.array(sc["sphere_c"]); r = sc["sphere_r"]
+    ds = np.abs(np.linalg.norm(p - c, axis=1) - r)
+    bmin, bmax = np.array(sc["bmin"]), np.array(sc["bmax"])
+    q = np.abs(p - 0.5 * (bmin + bmax)) - 0.5 * (bmax - bmin)              # textbook signed distance of a box
+    sd = np.linalg.norm(np.maximum(q, 0.0), axis=1) + np.minimum(q.max(axis=1), 0.0)
+    return np.minimum(ds, np.abs(sd))
+
+
+def _depth_inside(p, sc):
+    """> 0: how deep p is inside the sphere or the box (0 outside)."""
+    c = np.array(sc["sphere_c"]); r = sc["sphere_r"]
+    bmin, bmax = np.array(sc["bmin"]), np.array(sc["bmax"])
+    q = np.abs(p - 0.5 * (bmin + bmax)) - 0.5 * (bmax - bmin)
+    return np.maximum(np.maximum(r - np.linalg.norm(p - c, axis=-1), -q.max(axis=-1)), 0.0)
+
+
+def test_train_batch_generator_pins(orc):
+    from ddf_inputs.rng import MASTER_SEED, STREAMS, uniform01
+    sc = orc.TRAIN_SCENE
+    n, step, half = 1 << 18, 3, 2.0
+    o, d, t, hit = orc.gen_train_batch(MASTER_SEED, STREAMS["train_rays"], step, n, half)
+    o64, d64, t64, hit = o.astype(np.float64), d.astype(np.float64), t.astype(np.float64), hit.astype(bool)
+    base = (np.uint64(step) * np.uint64(n) + np.arange(n, dtype=np.uint64)) * np.uint64(16)
+    u = np.stack([uniform01(MASTER_SEED, STREAMS["train_rays"], base + np.uint64(j)) for j in range(11)], axis=1)
+    oo = (2.0 * u[:, 0:3] - 1.0) * half                                    # camera origin, uniform in the sampling cube
+    q = (2.0 * u[:, 3:6] - 1.0) - oo                                       # toward a point of the unit cube
+    dcam = q / np.linalg.norm(q, axis=1, keepdims=True)
+    moved = np.any(o != oo.astype(np.float32), axis=1)
+    A = u[:, 6] >= 0.5                                                     # the anchor draw
+    ok10 = u[:, 10] > 0                                                    # a zero shift moves nothing (probability 2^-24)
+
+    # every ray: unit direction; a miss has target 0; a hit's target ends ON the surface
+    assert np.abs(np.linalg.norm(d64, axis=1) - 1.0).max() < 1e-6
+    assert np.all(t[~hit] == 0.0) and np.all(t[hit] > 0.0)
+    assert _unsigned_surface_distance(o64[hit] + t64[hit, None] * d64[hit], sc).max() < 2e-5
+    assert 0.3 < hit.mean() < 0.95
+
+    # ... and it is the FIRST surface: nothing solid strictly before it, and a miss never runs deep through a solid
+    outside = _depth_inside(o64, sc) == 0.0
+    f = (np.arange(64) + 0.5) / 64
+    sel = np.nonzero(hit & outside)[0][:20000]
+    pts = o64[sel, None, :] + (f[None, :, None] * (t64[sel, None, None] - 1e-4)) * d64[sel, None, :]
+    assert _depth_inside(pts, sc).max() < 1e-5
+    sel = np.nonzero(~hit)[0][:20000]
+    s = (np.arange(512) + 0.5) / 512 * 7.5
+    pts = o64[sel, None, :] + s[None, :, None] * d64[sel, None, :]
+    assert _depth_inside(pts, sc).max() < 0.02
+
+    # camera half (u6 < 0.5): never anchored - the direction is the camera's, and the origin moves iff the ray hits and
+    # u9 < 0.3 (the shift fraction, exactly), by s = u10 * (distance before the shift) along the ray: target t - s
+    C_ = ~A
+    assert np.abs(d64[C_] - dcam[C_]).max() < 1e-6
+    assert np.array_equal(moved[C_ & ok10], (hit & (u[:, 9] < 0.3))[C_ & ok10])
+    sh = C_ & moved
+    s_ = np.linalg.norm(o64[sh] - oo[sh], axis=1)
+    assert np.abs(np.cross(o64[sh] - oo[sh], dcam[sh])).max() < 1e-5       # moved along the ray
+    assert np.abs(s_ - u[sh, 10] * (s_ + t64[sh])).max() < 5e-6           # s = u10 * t_before, target = t_before - s (fp32 outputs)
+    assert abs(moved[C_ & hit].mean() - 0.3) < 4 * math.sqrt(0.21 / (C_ & hit).sum())
+
+    # anchor half (u6 >= 0.5): anchored iff the camera ray hit, with the camera half's hit rate (two samples of one
+    # Bernoulli, 4 sigma); an anchored ray starts 1e-3 BEFORE the camera ray's surface point, pointing where the
+    # sphere sample of (u7, u8) points (reading A9)
+    p_cam = hit[C_].mean()
+    anchored = A & moved
+    sig = math.sqrt(p_cam * (1 - p_cam) * (1.0 / A.sum() + 1.0 / C_.sum()))
+    assert abs(anchored[A].mean() - p_cam) < 4 * sig, (anchored[A].mean(), p_cam, sig)
+    assert abs(anchored.mean() - 0.5 * p_cam) < 4 * sig
+    z = 2.0 * u[:, 7] - 1.0; phi = 2.0 * np.pi * u[:, 8]; rr = np.sqrt(np.maximum(0.0, 1.0 - z * z))
+    dsph = np.stack([rr * np.cos(phi), rr * np.sin(phi), z], axis=1)
+    assert np.abs(d64[anchored] - dsph[anchored]).max() < 1e-6
+    assert np.all(~moved[A & ~anchored] & ~hit[A & ~anchored])             # camera miss: emitted as it is
+    shifted = anchored & hit & (u[:, 9] < 0.3)
+    s_ = np.where(shifted, t64 * u[:, 10] / (1.0 - u[:, 10]), 0.0)         # undo the shift: s = u10 * t_before
+    o_pre = o64 - s_[:, None] * d64
+    assert np.abs(np.cross(o_pre[anchored] - oo[anchored], dcam[anchored])).max() < 2e-5   # on the camera ray
+    res = _unsigned_surface_distance(o_pre[anchored] + 1e-3 * dcam[anchored], sc)
+    assert res.max() < 5e-5, res.max()                                     # 1e-3 before the surface, not on or beyond it
+    assert (anchored & ~shifted).sum() > 10000 and shifted.sum() > 10000
