@@ -392,9 +392,20 @@ def test_sphere_trace_teacher_forcing(ddf, orc, sdf):
             tt = np.float32(tt + s)
             if tt > 6.0 or tt < 0: break
         assert (h, k + 1, tt) == (hit[i], steps[i], t[i])
-    # statistics against the CPU tracer run end to end
-    rt, rhit, rsteps = orc.sphere_trace(lay, blob, o, d, 64, 1e-3, 6.0, 1.0, 0.05)
-    assert abs(hit.mean() - rhit.mean()) < 0.06 and abs(steps.mean() - rsteps.mean()) < 3.0
+    # Statistics against the CPU tracer run end to end, on a 40 x 40 view (N = 1600 rays).  Per ray the two traces
+    # diverge (bf16 vs fp64 values of a function with Lipschitz constant >> 1 feed back into the next point), so
+    # the comparison is of two samples of one distribution.  Bound = 3 sigma of the difference of two INDEPENDENT
+    # samples of size N - sqrt(2 p (1 - p) / N) for the hit rate, sqrt((var_gpu + var_cpu) / N) for the mean step
+    # count - which over-estimates the spread of these paired samples (rays that converge quickly agree exactly).
+    o2, d2 = orc.gen_camera(cam, 40, 40)
+    t2, hit2, steps2, _, _, _ = _trace(ddf, m, o2, d2, prm1, want_trace=False)
+    rt, rhit, rsteps = orc.sphere_trace(lay, blob, o2, d2, 64, 1e-3, 6.0, 1.0, 0.05)
+    N = len(o2); ph = 0.5 * (hit2.mean() + rhit.mean())
+    b_hit = 3.0 * math.sqrt(2.0 * ph * (1.0 - ph) / N)
+    b_steps = 3.0 * math.sqrt((steps2.var() + rsteps.var()) / N)
+    print("sphere trace, %d rays: hit rate %.4f vs %.4f (bound %.4f), mean steps %.2f vs %.2f (bound %.2f)"
+          % (N, hit2.mean(), rhit.mean(), b_hit, steps2.mean(), rsteps.mean(), b_steps))
+    assert 0.2 < ph < 0.9 and abs(hit2.mean() - rhit.mean()) < b_hit and abs(steps2.mean() - rsteps.mean()) < b_steps
 
 
 def test_maximum_batch_2pow24_and_side_stream(ddf, orc, c1):

@@ -101,18 +101,22 @@ def c1(ddf):
     ddf.ddf_destroy(m)
 
 
-def _sample(n, k=1536):
-    """first and last tile, tile boundaries +-1 of the first tiles, and a stride sample."""
+def _sample(n, k=8192):
+    """the first and last tile, every tile boundary +-1 of the first 64 tiles, whole tiles from the second
+    and later waves of the persistent grid (74 CTA pairs: tiles 74 and 147 are the second tiles of the first and last pair,
+    148 opens the third wave), a tile in the middle, and a stride sample filling up to k rays in total."""
     idx = [np.arange(0, min(n, 260)), np.arange(max(0, n - 260), n)]
-    for b in range(256, min(n, 256 * 40), 256):
+    for b in range(256, min(n, 256 * 65), 256):
         idx.append(np.array([b - 1, b, b + 1]))
-    idx.append(np.arange(0, n, max(1, n // 700)))
-    idx = np.unique(np.concatenate(idx))
-    idx = idx[idx < n]
-    if len(idx) > k:
-        keep = np.random.default_rng(0).choice(len(idx), k, replace=False)
-        idx = np.sort(idx[keep])
-    return idx
+    tiles = (n + 255) // 256
+    for t in (74, 147, 148, tiles // 2):
+        if 0 < t < tiles:
+            idx.append(np.arange(t * 256, min(n, t * 256 + 256)))
+    fixed = np.unique(np.concatenate(idx)); fixed = fixed[fixed < n]
+    rest = max(0, k - len(fixed))
+    if rest == 0 or n <= k:
+        return fixed if n > k else np.arange(n)
+    return np.unique(np.concatenate([fixed, np.linspace(0, n - 1, rest + 256).astype(np.int64)]))
 
 
 def _paper_scale_parity(ddf, orc, c1, od, dd, n, what):
@@ -136,7 +140,17 @@ def _paper_scale_parity(ddf, orc, c1, od, dd, n, what):
     d2 = torch.empty(len(idx), device="cuda"); v2 = torch.empty(len(idx), device="cuda")
     ddf.ddf_query(m, od[it].contiguous(), dd[it].contiguous(), len(idx), d2, v2)
     assert torch.equal(d2, dist[it]) and torch.equal(v2, vis[it])
+    print("%s: %d rays against the exact oracle: %s" % (what, len(idx), stats))
     return stats
+
+
+def test_sample_meets_the_survey_size():
+    for n in (1 << 20, 1 << 22, 1 << 24):
+        idx = _sample(n)
+        assert len(idx) >= 8192 and len(np.unique(idx)) == len(idx) and idx.max() < n
+        for b in range(256, 256 * 65, 256):
+            assert b - 1 in idx and b in idx and b + 1 in idx
+        assert 74 * 256 + 100 in idx and 148 * 256 in idx and n - 1 in idx and 0 in idx
 
 
 def test_config1_camera_full_batch(ddf, orc, c1):
@@ -150,6 +164,33 @@ def test_config1_camera_full_batch(ddf, orc, c1):
     o_ref, d_ref = orc.gen_camera(ocam, W, H)
     assert np.allclose(od.cpu().numpy(), o_ref, atol=1e-6) and np.allclose(dd.cpu().numpy(), d_ref, atol=1e-5)
     _paper_scale_parity(ddf, orc, c1, od, dd, n, "C1 camera")
+
+
+def test_config1_tail_statistics_on_65536_rays(ddf, orc, c1):
+    """"Report max, 99.9th percentile and pass fraction, not just pass/fail" - every 16th ray of
+    the configs[1] camera batch (65,536 rays, ~30 s of oracle) answered inside the full 2^20-ray launch; the printed
+    statistics are the ones DESIGN.md 5 quotes."""
+    lay, blob, m = c1
+    W = H = 1024
+    n = W * H
+    cam = ddf.ddf_camera_from_seed(MASTER_SEED, STREAMS["camera_pos"], 2.5)
+    od = torch.empty((n, 3), device="cuda"); dd = torch.empty((n, 3), device="cuda")
+    ddf.ddf_gen_camera(cam, W, H, od, dd)
+    dist = torch.empty(n, device="cuda"); vis = torch.empty(n, device="cuda")
+    ddf.ddf_query(m, od, dd, n, dist, vis)
+    torch.cuda.synchronize()
+    idx = np.arange(5, n, 16)                                   # 65,536 rays, every tile of the launch touched
+    it = torch.from_numpy(idx).cuda()
+    z, t, xi = orc.forward(lay, blob, od[it].cpu().numpy(), dd[it].cpu().numpy(), mode=0)
+    g_d, g_v = dist[it].cpu().numpy(), vis[it].cpu().numpy()
+    ed = np.abs(g_d - t) / (1.0 + np.abs(t)); ev = np.abs(g_v - xi)
+    band = np.abs(xi - 0.5) < 1e-2
+    agree = ((g_v > 0.5) == (xi > 0.5))[~band].mean()
+    print("C1 tail, %d rays: |dd|/(1+|d|) max %.3e p99.9 %.3e rms %.3e | |dv| max %.3e p99.9 %.3e rms %.3e | "
+          "hit/miss agreement outside the band %.5f, band fraction %.4f, pass fraction %.5f"
+          % (len(idx), ed.max(), np.quantile(ed, 0.999), np.sqrt((ed ** 2).mean()), ev.max(), np.quantile(ev, 0.999),
+             np.sqrt((ev ** 2).mean()), agree, band.mean(), ((ed <= 1e-2) & (ev <= 1e-2)).mean()))
+    assert ed.max() <= 1e-2 and ev.max() <= 1e-2 and agree >= 0.999 and band.mean() < 0.2
 
 
 def test_config2_shadow_full_batch(ddf, orc, c1):
@@ -228,7 +269,7 @@ def test_config3_ao_full_batch(ddf, orc, c1):
     k = 4096
     assert np.array_equal(orc.ao_reduce(vis[:k * spp].cpu().numpy(), dist[:k * spp].cpu().numpy(), spp), ao2[:k].cpu().numpy())
     # AO image against the oracle evaluated end to end on whole pixels
-    pix = np.arange(0, npts, npts // 192)[:192]
+    pix = np.arange(0, npts, npts // 256)[:256]                # AO parity on >= 256 whole pixels
     ridx = (pix[:, None] * spp + np.arange(spp)[None, :]).reshape(-1)
     it = torch.from_numpy(ridx).cuda()
     z, t, xi = orc.forward(lay, blob, od[it].cpu().numpy(), dd[it].cpu().numpy(), mode=0)
