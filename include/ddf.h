@@ -33,9 +33,13 @@
  *    in the batch, bit-reproducible run to run (training steps accumulate gradients with atomics
  *    and are reproducible to rounding only).  Directions must be unit length (not checked).
  *  - A model (and a trainer) owns device workspaces that its calls reuse: use one model from one
- *    stream / host thread at a time; different models are independent.  A workspace is allocated
- *    (or grown: a synchronising cudaFree / cudaMalloc) the first time a call needs it for a batch
- *    that large; after that the call issues only stream-ordered work, so it can be recorded by
+ *    stream / host thread at a time; different models are independent.  ddf_query, ddf_query_logits
+ *    and ddf_query_ao never allocate (their workspace is sized at ddf_create).  The calls that need a
+ *    per-batch workspace - ddf_query_host, ddf_query_camera / ddf_query_ao_points on models that read
+ *    rays from memory, sdf_sphere_trace, the wavefront calls, and every query of a model served by the
+ *    CUDA-core path - take it from ddf_reserve; without a reservation that covers the batch they size
+ *    it themselves on first use (a synchronising cudaFree / cudaMalloc).  Once the workspace covers
+ *    the batch a call issues only stream-ordered work, so it can be recorded by
  *    stream capture and replayed as a CUDA graph (ddf_trainer_step bakes that step's learning
  *    rate into the capture; ddf_trainer_loss_grads and every query are replayable as they are).
  *  - There is no CPU fallback: without a CUDA device of compute capability 10.x the calls
@@ -106,6 +110,21 @@ int  ddf_last_cuda_error(void);                           /* cudaError_t of the 
  * path, column-split whenever the batch fits the split scratch (n <= 18,944), else persistent.
  * 3 and 4 are DDF_E_UNSUPPORTED for models the persistent kernel does not serve. */
 int  ddf_set_path(ddf_model* model, int path);
+/* Sizes the per-batch workspaces ahead of time so that no later call with at most max_rays rays allocates
+ * (SURVEY.md 8(b) "the library never allocates in ddf_query (workspace, if any, sized at create)").  `what` selects
+ * which: DDF_RESERVE_HOST - staging of ddf_query_host (32 B per ray, plus its two copy streams and events);
+ * DDF_RESERVE_RAYS - the ray buffer of ddf_query_camera / ddf_query_ao_points (24 B per ray; max_rays counts
+ * width * height or n_pts * spp); DDF_RESERVE_TRACE - sdf_sphere_trace (25 B per ray); DDF_RESERVE_WAVE - the
+ * wavefront calls on max_rays primary rays, with room for spp ambient-occlusion rays per hit (40 B per primary ray,
+ * or 32 + 24 spp if that is more; spp = 0: shadow calls only).  For a model only the CUDA-core path serves, the
+ * activation workspace of its queries (rows = max_rays) is sized too, whatever `what` is.  Synchronises the device when
+ * it (re)allocates; reservations only grow.  max_rays == 0 is a no-op; unknown bits in `what`: DDF_E_INVALID_ARG. */
+#define DDF_RESERVE_HOST  1u
+#define DDF_RESERVE_RAYS  2u
+#define DDF_RESERVE_TRACE 4u
+#define DDF_RESERVE_WAVE  8u
+#define DDF_RESERVE_ALL   15u
+int  ddf_reserve(ddf_model* model, uint32_t what, int64_t max_rays, int spp);
 /* which = 0: 1 if the tcgen05 path serves this model, else 0; 1: kernels launched by the
  * last query call on this model; 2: E (encoded input width); 3: rays per tile of the path. */
 int64_t ddf_get_info(const ddf_model* model, int which);

@@ -13,7 +13,7 @@ from .binding import (  # noqa: F401
     ddf_gen_shadow_from_hits, ddf_query_shadowed, ddf_query_shadowed_lights, ddf_gen_ao_from_hits, ddf_query_ao_wavefront, ddf_query_shaded, ddf_query_ao_points,
     DdfTrainParams, make_train_params, Trainer, ddf_trainer_create, ddf_trainer_destroy, ddf_trainer_step,
     ddf_trainer_loss_grads, ddf_trainer_export, ddf_trainer_steps, ddf_scene_raycast, ddf_gen_train_batch,
-    ddf_query_camera,
+    ddf_query_camera, ddf_reserve, RESERVE_HOST, RESERVE_RAYS, RESERVE_TRACE, RESERVE_WAVE, RESERVE_ALL,
     EXPORTED_SYMBOLS,
 )
 from .build import build  # noqa: F401

@@ -13,7 +13,7 @@ _LIB_PATH = os.path.join(_HERE, "libddf.so")
 
 EXPORTED_SYMBOLS = [
     "ddf_create", "ddf_destroy", "ddf_status_string", "ddf_last_cuda_error", "ddf_set_path",
-    "ddf_get_info", "ddf_query", "ddf_query_host", "ddf_query_logits", "ddf_camera_from_seed",
+    "ddf_get_info", "ddf_reserve", "ddf_query", "ddf_query_host", "ddf_query_logits", "ddf_camera_from_seed",
     "ddf_gen_camera", "ddf_gen_sphere_points", "ddf_gen_shadow", "ddf_gen_gbuffer", "ddf_gen_ao",
     "ddf_ao_reduce", "ddf_query_ao", "ddf_shadow_test", "sdf_sphere_trace",
     "ddf_hashgrid_table_entries", "ddf_create_hashgrid", "ddf_gen_shadow_from_hits", "ddf_query_shadowed", "ddf_query_shadowed_lights",
@@ -195,6 +195,13 @@ def ddf_destroy(model):
         rc = lib().ddf_destroy(model.handle)
         model.handle = None
         _check(rc, "ddf_destroy")
+
+
+RESERVE_HOST, RESERVE_RAYS, RESERVE_TRACE, RESERVE_WAVE, RESERVE_ALL = 1, 2, 4, 8, 15
+
+
+def ddf_reserve(model, what, max_rays, spp=0):
+    _check(lib().ddf_reserve(model.handle, C.c_uint32(what), C.c_int64(max_rays), C.c_int(spp)), "ddf_reserve")
 
 
 def ddf_set_path(model, path):

@@ -222,8 +222,62 @@ static int create_impl(const void* weights, const ddf_layout* layout, ddf_model*
     rc = narrow_plan_create(m, hw.data(), hb.data());
     if (rc != DDF_OK) { free_model(m); return rc; }
   }
-  DDF_CUDA_TRY(cudaDeviceSynchronize());
+  {
+    cudaError_t es = cudaDeviceSynchronize();
+    if (es != cudaSuccess) { g_last_cuda_error = (int)es; (void)cudaGetLastError(); free_model(m); return DDF_E_CUDA; }
+  }
   *out = reinterpret_cast<ddf_model*>(m);
+  return DDF_OK;
+}
+
+namespace ddf {
+// staging of ddf_query_host (32 B per ray) and the ray workspace of ddf_query_camera / ddf_query_ao_points on models
+// that read their rays from memory (24 B per ray): grown on first use, or ahead of time by ddf_reserve
+static int host_reserve(Model* m, int64_t n) {
+  if (n <= m->host_rows) return DDF_OK;
+  cudaFree(m->h2d_o); cudaFree(m->h2d_d); cudaFree(m->d2h_dist); cudaFree(m->d2h_vis);
+  m->h2d_o = m->h2d_d = m->d2h_dist = m->d2h_vis = nullptr; m->host_rows = 0;
+  DDF_CUDA_TRY(cudaMalloc(&m->h2d_o, (size_t)n * 12));
+  DDF_CUDA_TRY(cudaMalloc(&m->h2d_d, (size_t)n * 12));
+  DDF_CUDA_TRY(cudaMalloc(&m->d2h_dist, (size_t)n * 4));
+  DDF_CUDA_TRY(cudaMalloc(&m->d2h_vis, (size_t)n * 4));
+  m->host_rows = n;
+  if (!m->host_s_in) {
+    DDF_CUDA_TRY(cudaStreamCreateWithFlags(&m->host_s_in, cudaStreamNonBlocking));
+    DDF_CUDA_TRY(cudaStreamCreateWithFlags(&m->host_s_out, cudaStreamNonBlocking));
+    for (int i = 0; i < 16; ++i) DDF_CUDA_TRY(cudaEventCreateWithFlags(&m->host_ev[i], cudaEventDisableTiming));
+  }
+  return DDF_OK;
+}
+static int rays_reserve(Model* m, int64_t n) {
+  if (n <= m->cam_rows) return DDF_OK;
+  cudaFree(m->cam_o); cudaFree(m->cam_d); m->cam_o = m->cam_d = nullptr; m->cam_rows = 0;
+  DDF_CUDA_TRY(cudaMalloc(&m->cam_o, (size_t)n * 12));
+  DDF_CUDA_TRY(cudaMalloc(&m->cam_d, (size_t)n * 12));
+  m->cam_rows = n;
+  return DDF_OK;
+}
+static int ao_out_reserve(Model* m, int64_t n) {
+  if (n <= m->ws_out_rows) return DDF_OK;
+  cudaFree(m->ws_dist); cudaFree(m->ws_vis); m->ws_dist = m->ws_vis = nullptr; m->ws_out_rows = 0;
+  DDF_CUDA_TRY(cudaMalloc(&m->ws_dist, (size_t)n * 4));
+  DDF_CUDA_TRY(cudaMalloc(&m->ws_vis, (size_t)n * 4));
+  m->ws_out_rows = n;
+  return DDF_OK;
+}
+}  // namespace ddf
+
+extern "C" int ddf_reserve(ddf_model* model, uint32_t what, int64_t max_rays, int spp) {
+  if (!model || max_rays < 0 || spp < 0 || (what & ~(uint32_t)DDF_RESERVE_ALL)) return DDF_E_INVALID_ARG;
+  Model* m = reinterpret_cast<Model*>(model);
+  int rc = DDF_OK;
+  if (max_rays == 0) return DDF_OK;
+  if ((what & DDF_RESERVE_HOST) && (rc = host_reserve(m, max_rays)) != DDF_OK) return rc;
+  if ((what & DDF_RESERVE_RAYS) && (rc = rays_reserve(m, max_rays)) != DDF_OK) return rc;
+  if ((what & DDF_RESERVE_RAYS) && !has_fused_path(m) && (rc = ao_out_reserve(m, max_rays)) != DDF_OK) return rc;
+  if ((what & DDF_RESERVE_TRACE) && (rc = trace_reserve(m, max_rays, 4096)) != DDF_OK) return rc;
+  if ((what & DDF_RESERVE_WAVE) && (rc = wave_reserve(m, max_rays, spp)) != DDF_OK) return rc;
+  if (!has_fused_path(m) && (rc = ensure_workspace(m, max_rays)) != DDF_OK) return rc;
   return DDF_OK;
 }
 
@@ -285,26 +339,13 @@ extern "C" int ddf_query_host(ddf_model* model, const float* origins, const floa
   Model* m = reinterpret_cast<Model*>(model);
   const bool ray = m->lay.input_kind == 0, two = m->lay.n_out == 2;
   if (!origins || !out_dist || (ray && !dirs)) return DDF_E_INVALID_ARG;
-  if (n > m->host_rows) {
-    cudaFree(m->h2d_o); cudaFree(m->h2d_d); cudaFree(m->d2h_dist); cudaFree(m->d2h_vis);
-    m->h2d_o = m->h2d_d = m->d2h_dist = m->d2h_vis = nullptr; m->host_rows = 0;
-    DDF_CUDA_TRY(cudaMalloc(&m->h2d_o, (size_t)n * 12));
-    DDF_CUDA_TRY(cudaMalloc(&m->h2d_d, (size_t)n * 12));
-    DDF_CUDA_TRY(cudaMalloc(&m->d2h_dist, (size_t)n * 4));
-    DDF_CUDA_TRY(cudaMalloc(&m->d2h_vis, (size_t)n * 4));
-    m->host_rows = n;
-  }
+  { int rc = host_reserve(m, n); if (rc != DDF_OK) return rc; }        // a no-op after ddf_reserve(DDF_RESERVE_HOST, >= n)
   cudaStream_t st = (cudaStream_t)stream;
   // Large batches are cut into up to 8 tile-aligned chunks: the uploads run ahead on their own
   // stream, chunk i is answered on `stream` as soon as it has landed, and its results go back
   // on a third stream while chunk i+1 is being answered (results do not depend on the batching).
   int chunks = 1;
   if (n >= (1 << 18)) chunks = n >= (1 << 21) ? 8 : 4;
-  if (chunks > 1 && !m->host_s_in) {
-    DDF_CUDA_TRY(cudaStreamCreateWithFlags(&m->host_s_in, cudaStreamNonBlocking));
-    DDF_CUDA_TRY(cudaStreamCreateWithFlags(&m->host_s_out, cudaStreamNonBlocking));
-    for (int i = 0; i < 16; ++i) DDF_CUDA_TRY(cudaEventCreateWithFlags(&m->host_ev[i], cudaEventDisableTiming));
-  }
   if (chunks == 1) {
     DDF_CUDA_TRY(cudaMemcpyAsync(m->h2d_o, origins, (size_t)n * 12, cudaMemcpyHostToDevice, st));
     if (ray) DDF_CUDA_TRY(cudaMemcpyAsync(m->h2d_d, dirs, (size_t)n * 12, cudaMemcpyHostToDevice, st));
@@ -317,27 +358,33 @@ extern "C" int ddf_query_host(ddf_model* model, const float* origins, const floa
   }
   const int64_t per = ((n + chunks - 1) / chunks + 255) / 256 * 256;
   int launches = 0;
-  for (int c = 0; c < chunks; ++c) {
-    const int64_t b = (int64_t)c * per, e = b + per < n ? b + per : n;
-    if (b >= e) { chunks = c; break; }
-    DDF_CUDA_TRY(cudaMemcpyAsync(m->h2d_o + 3 * b, origins + 3 * b, (size_t)(e - b) * 12, cudaMemcpyHostToDevice, m->host_s_in));
-    if (ray) DDF_CUDA_TRY(cudaMemcpyAsync(m->h2d_d + 3 * b, dirs + 3 * b, (size_t)(e - b) * 12, cudaMemcpyHostToDevice, m->host_s_in));
-    DDF_CUDA_TRY(cudaEventRecord(m->host_ev[c], m->host_s_in));
-  }
-  for (int c = 0; c < chunks; ++c) {
-    const int64_t b = (int64_t)c * per, e = b + per < n ? b + per : n;
-    DDF_CUDA_TRY(cudaStreamWaitEvent(st, m->host_ev[c], 0));
-    int rc = run_query(m, m->h2d_o + 3 * b, ray ? m->h2d_d + 3 * b : nullptr, e - b, 0, m->d2h_dist + b, two ? m->d2h_vis + b : nullptr, stream);
-    if (rc != DDF_OK) return rc;
-    launches += m->last_launches;
-    DDF_CUDA_TRY(cudaEventRecord(m->host_ev[8 + c], st));
-    DDF_CUDA_TRY(cudaStreamWaitEvent(m->host_s_out, m->host_ev[8 + c], 0));
-    DDF_CUDA_TRY(cudaMemcpyAsync(out_dist + b, m->d2h_dist + b, (size_t)(e - b) * 4, cudaMemcpyDeviceToHost, m->host_s_out));
-    if (two && out_vis) DDF_CUDA_TRY(cudaMemcpyAsync(out_vis + b, m->d2h_vis + b, (size_t)(e - b) * 4, cudaMemcpyDeviceToHost, m->host_s_out));
-  }
+  // the chunk pipeline; whatever it returns, no copy from or into the caller's host buffers may still be in flight
+  auto pipeline = [&]() -> int {
+    for (int c = 0; c < chunks; ++c) {
+      const int64_t b = (int64_t)c * per, e = b + per < n ? b + per : n;
+      if (b >= e) { chunks = c; break; }
+      DDF_CUDA_TRY(cudaMemcpyAsync(m->h2d_o + 3 * b, origins + 3 * b, (size_t)(e - b) * 12, cudaMemcpyHostToDevice, m->host_s_in));
+      if (ray) DDF_CUDA_TRY(cudaMemcpyAsync(m->h2d_d + 3 * b, dirs + 3 * b, (size_t)(e - b) * 12, cudaMemcpyHostToDevice, m->host_s_in));
+      DDF_CUDA_TRY(cudaEventRecord(m->host_ev[c], m->host_s_in));
+    }
+    for (int c = 0; c < chunks; ++c) {
+      const int64_t b = (int64_t)c * per, e = b + per < n ? b + per : n;
+      DDF_CUDA_TRY(cudaStreamWaitEvent(st, m->host_ev[c], 0));
+      int rc = run_query(m, m->h2d_o + 3 * b, ray ? m->h2d_d + 3 * b : nullptr, e - b, 0, m->d2h_dist + b, two ? m->d2h_vis + b : nullptr, stream);
+      if (rc != DDF_OK) return rc;
+      launches += m->last_launches;
+      DDF_CUDA_TRY(cudaEventRecord(m->host_ev[8 + c], st));
+      DDF_CUDA_TRY(cudaStreamWaitEvent(m->host_s_out, m->host_ev[8 + c], 0));
+      DDF_CUDA_TRY(cudaMemcpyAsync(out_dist + b, m->d2h_dist + b, (size_t)(e - b) * 4, cudaMemcpyDeviceToHost, m->host_s_out));
+      if (two && out_vis) DDF_CUDA_TRY(cudaMemcpyAsync(out_vis + b, m->d2h_vis + b, (size_t)(e - b) * 4, cudaMemcpyDeviceToHost, m->host_s_out));
+    }
+    return DDF_OK;
+  };
+  const int rc = pipeline();
   m->last_launches = launches;
-  DDF_CUDA_TRY(cudaStreamSynchronize(st));
-  DDF_CUDA_TRY(cudaStreamSynchronize(m->host_s_out));
+  const cudaError_t e0 = cudaStreamSynchronize(m->host_s_in), e1 = cudaStreamSynchronize(st), e2 = cudaStreamSynchronize(m->host_s_out);
+  if (rc != DDF_OK) { (void)cudaGetLastError(); return rc; }
+  DDF_CUDA_TRY(e0); DDF_CUDA_TRY(e1); DDF_CUDA_TRY(e2);
   return DDF_OK;
 }
 
@@ -351,13 +398,9 @@ extern "C" int ddf_query_camera(ddf_model* model, const ddf_camera* cam, int wid
   if (!out_dist) return DDF_E_INVALID_ARG;
   cudaStream_t st = (cudaStream_t)stream;
   if (m->hg) return hash_forward_camera(m, cam, width, height, out_dist, out_vis, st);
-  if (n > m->cam_rows) {
-    cudaFree(m->cam_o); cudaFree(m->cam_d); m->cam_o = m->cam_d = nullptr; m->cam_rows = 0;
-    DDF_CUDA_TRY(cudaMalloc(&m->cam_o, (size_t)n * 12));
-    DDF_CUDA_TRY(cudaMalloc(&m->cam_d, (size_t)n * 12));
-    m->cam_rows = n;
-  }
-  int rc = ddf_gen_camera(cam, width, height, m->cam_o, m->cam_d, stream);
+  int rc = rays_reserve(m, n);                                // a no-op after ddf_reserve(DDF_RESERVE_RAYS, >= n)
+  if (rc != DDF_OK) return rc;
+  rc = ddf_gen_camera(cam, width, height, m->cam_o, m->cam_d, stream);
   if (rc != DDF_OK) return rc;
   rc = run_query(m, m->cam_o, m->cam_d, n, 0, out_dist, out_vis, stream);
   if (rc == DDF_OK) m->last_launches += 1;
@@ -376,13 +419,9 @@ extern "C" int ddf_query_ao_points(ddf_model* model, const float* p, const float
   if (m->hg && spp <= 32 && 32 % spp == 0)                    // the rays never exist in memory
     return hash_forward_ao_points(m, p, nrm, n_pts, nullptr, spp, gen_key(seed, rng_stream), eps, ao_radius, ao, st);
   const int64_t n = n_pts * spp;
-  if (n > m->cam_rows) {
-    cudaFree(m->cam_o); cudaFree(m->cam_d); m->cam_o = m->cam_d = nullptr; m->cam_rows = 0;
-    DDF_CUDA_TRY(cudaMalloc(&m->cam_o, (size_t)n * 12));
-    DDF_CUDA_TRY(cudaMalloc(&m->cam_d, (size_t)n * 12));
-    m->cam_rows = n;
-  }
-  int rc = ddf_gen_ao(p, nrm, n_pts, spp, seed, rng_stream, eps, m->cam_o, m->cam_d, stream);
+  int rc = rays_reserve(m, n);
+  if (rc != DDF_OK) return rc;
+  rc = ddf_gen_ao(p, nrm, n_pts, spp, seed, rng_stream, eps, m->cam_o, m->cam_d, stream);
   if (rc != DDF_OK) return rc;
   rc = ddf_query_ao(model, m->cam_o, m->cam_d, n_pts, spp, ao_radius, ao, stream);
   if (rc == DDF_OK) m->last_launches += 1;
@@ -391,7 +430,7 @@ extern "C" int ddf_query_ao_points(ddf_model* model, const float* p, const float
 
 extern "C" int ddf_query_ao(ddf_model* model, const float* o, const float* d, int64_t n_pts, int spp,
                             float ao_radius, float* ao, void* stream) {
-  if (!model || n_pts < 0 || spp <= 0) return DDF_E_INVALID_ARG;
+  if (!model || n_pts < 0 || spp <= 0 || n_pts > (int64_t)0x7fffffff / spp) return DDF_E_INVALID_ARG;
   if (n_pts == 0) return DDF_OK;
   Model* m = reinterpret_cast<Model*>(model);
   if (!o || !d || !ao || m->lay.n_out != 2 || m->lay.input_kind != 0) return DDF_E_INVALID_ARG;
@@ -399,13 +438,9 @@ extern "C" int ddf_query_ao(ddf_model* model, const float* o, const float* d, in
   cudaStream_t st = (cudaStream_t)stream;
   if (has_fused_path(m) && spp <= 32 && 32 % spp == 0)          // a pixel's rays sit in one warp of a tile
     return fused_forward(m, o, d, n, nullptr, 2, ao, nullptr, spp, ao_radius, st);
-  if (n > m->ws_out_rows) {
-    cudaFree(m->ws_dist); cudaFree(m->ws_vis); m->ws_dist = m->ws_vis = nullptr; m->ws_out_rows = 0;
-    DDF_CUDA_TRY(cudaMalloc(&m->ws_dist, (size_t)n * 4));
-    DDF_CUDA_TRY(cudaMalloc(&m->ws_vis, (size_t)n * 4));
-    m->ws_out_rows = n;
-  }
-  int rc = run_query(m, o, d, n, 0, m->ws_dist, m->ws_vis, stream);
+  int rc = ao_out_reserve(m, n);
+  if (rc != DDF_OK) return rc;
+  rc = run_query(m, o, d, n, 0, m->ws_dist, m->ws_vis, stream);
   if (rc != DDF_OK) return rc;
   int launches = m->last_launches;
   rc = ddf_ao_reduce(m->ws_vis, m->ws_dist, n_pts, spp, ao_radius, ao, stream);

@@ -88,6 +88,11 @@ void tc_plan_destroy(Model* m);
 int tc_forward(Model* m, const float* o, const float* d, int64_t n, const int64_t* n_dev,
                int mode_out, float* out0, float* out1, int spp, float ao_radius, cudaStream_t st);
 
+// ---- workspaces sized ahead of time (ddf_reserve) or on first use
+int trace_reserve(Model* m, int64_t n, int max_steps);          // ddf_trace.cu
+int wave_reserve_bytes(Model* m, size_t need);                  // ddf_wave.cu
+int wave_reserve(Model* m, int64_t n, int spp);
+
 // ---- hash-grid field (ddf_hash.cu)
 void hash_plan_destroy(Model* m);
 int hash_forward(Model* m, const float* o, const float* d, int64_t n, const int64_t* n_dev, int mode_out,
@@ -145,20 +150,26 @@ __device__ __forceinline__ void ao_ray_from_point(const float p[3], const float 
   if (fabsf(n[1]) < fabsf(n[ax])) ax = 1;
   if (fabsf(n[2]) < fabsf(n[ax])) ax = 2;
   float e[3] = { ax == 0 ? 1.0f : 0.0f, ax == 1 ? 1.0f : 0.0f, ax == 2 ? 1.0f : 0.0f };
-  float t1[3] = { e[1]*n[2] - e[2]*n[1], e[2]*n[0] - e[0]*n[2], e[0]*n[1] - e[1]*n[0] };
-  float inv = 1.0f / sqrtf(t1[0]*t1[0] + t1[1]*t1[1] + t1[2]*t1[2]);
-  t1[0] *= inv; t1[1] *= inv; t1[2] *= inv;
-  float t2[3] = { n[1]*t1[2] - n[2]*t1[1], n[2]*t1[0] - n[0]*t1[2], n[0]*t1[1] - n[1]*t1[0] };
+  // every product and sum below is an explicit round-to-nearest operation: the kernels that inline this helper must
+  // produce the same bits whatever FMA contraction the optimiser would choose in each of them
+  #define DDF_CROSS(a, b, c, d) __fsub_rn(__fmul_rn(a, b), __fmul_rn(c, d))
+  #define DDF_SUMSQ(v) __fadd_rn(__fadd_rn(__fmul_rn(v[0], v[0]), __fmul_rn(v[1], v[1])), __fmul_rn(v[2], v[2]))
+  float t1[3] = { DDF_CROSS(e[1], n[2], e[2], n[1]), DDF_CROSS(e[2], n[0], e[0], n[2]), DDF_CROSS(e[0], n[1], e[1], n[0]) };
+  float inv = __frcp_rn(__fsqrt_rn(DDF_SUMSQ(t1)));
+  t1[0] = __fmul_rn(t1[0], inv); t1[1] = __fmul_rn(t1[1], inv); t1[2] = __fmul_rn(t1[2], inv);
+  float t2[3] = { DDF_CROSS(n[1], t1[2], n[2], t1[1]), DDF_CROSS(n[2], t1[0], n[0], t1[2]), DDF_CROSS(n[0], t1[1], n[1], t1[0]) };
   float u1 = dev_uniform01(key, 2 * (uint64_t)k), u2 = dev_uniform01(key, 2 * (uint64_t)k + 1);
-  float r = sqrtf(u1), s, c;
-  sincospif(2.0f * u2, &s, &c);
-  float lx = r * c, ly = r * s, lz = sqrtf(1.0f - u1);
+  float r = __fsqrt_rn(u1), s, c;
+  sincospif(__fmul_rn(2.0f, u2), &s, &c);
+  float lx = __fmul_rn(r, c), ly = __fmul_rn(r, s), lz = __fsqrt_rn(__fsub_rn(1.0f, u1));
   float dd[3];
   #pragma unroll
-  for (int a = 0; a < 3; ++a) dd[a] = fmaf(lz, n[a], fmaf(ly, t2[a], lx * t1[a]));
-  inv = 1.0f / sqrtf(dd[0]*dd[0] + dd[1]*dd[1] + dd[2]*dd[2]);
+  for (int a = 0; a < 3; ++a) dd[a] = __fmaf_rn(lz, n[a], __fmaf_rn(ly, t2[a], __fmul_rn(lx, t1[a])));
+  inv = __frcp_rn(__fsqrt_rn(DDF_SUMSQ(dd)));
   #pragma unroll
-  for (int a = 0; a < 3; ++a) { o[a] = fmaf(eps, n[a], p[a]); d[a] = dd[a] * inv; }
+  for (int a = 0; a < 3; ++a) { o[a] = __fmaf_rn(eps, n[a], p[a]); d[a] = __fmul_rn(dd[a], inv); }
+  #undef DDF_CROSS
+  #undef DDF_SUMSQ
 }
 
 // gamma of one ray into a bf16 row (E_pad entries, pad = 0).  sin/cos(2^k pi x) via sincospif

@@ -262,7 +262,7 @@ __global__ void __launch_bounds__(kHgThreads, 5) ddf_hash_kernel(const __grid_co
         }
         __syncwarp();
       }
-      while (!ptx::mbar_try_wait(bar, phase)) { }
+      ptx::mbar_wait_bounded(bar, phase);
       phase ^= 1u;
       ptx::tc_fence_after();
       uint32_t r[64];
@@ -519,10 +519,14 @@ extern "C" int ddf_create_hashgrid(const void* table, const void* mlp, const ddf
   p.n_levels = (int)L.n_levels; p.Ld = (int)L.n_freq_dir; p.n_hidden = (int)L.n_hidden; p.n_out = (int)L.n_out;
   p.table_f16 = L.table_dtype == 2;
   h->smem_bytes = 16384 + (size_t)L.n_hidden * 8192 + (L.n_hidden + 2) * 256 + 128 + 1024;
-  if ((e = cudaFuncSetAttribute(ddf_hash_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_bytes)) != cudaSuccess ||
-      (e = cudaFuncSetAttribute(ddf_hash_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_bytes)) != cudaSuccess ||
-      (e = cudaFuncSetAttribute(ddf_hash_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_bytes)) != cudaSuccess ||
-      (e = cudaFuncSetAttribute(ddf_hash_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_bytes)) != cudaSuccess)
+  // function attributes are process-wide: the limit is the device's, the carve-out (below) the largest any model asked for,
+  // so creating a smaller field never lowers what an existing larger one launches with
+  const int optin = (int)prop.sharedMemPerBlockOptin;
+  if ((size_t)optin < h->smem_bytes) return fail(DDF_E_UNSUPPORTED, cudaSuccess);
+  if ((e = cudaFuncSetAttribute(ddf_hash_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, optin)) != cudaSuccess ||
+      (e = cudaFuncSetAttribute(ddf_hash_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, optin)) != cudaSuccess ||
+      (e = cudaFuncSetAttribute(ddf_hash_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, optin)) != cudaSuccess ||
+      (e = cudaFuncSetAttribute(ddf_hash_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, optin)) != cudaSuccess)
     return fail(DDF_E_CUDA, e);
   // resident CTAs per SM from the kernel's own resource use (the runtime's occupancy query answers
   // for the current carve-out, which another library in the process may have left at "prefer L1")
@@ -543,6 +547,9 @@ extern "C" int ddf_create_hashgrid(const void* table, const void* mlp, const ddf
   {
     int pct = (int)((h->ctas_per_sm * (h->smem_bytes + prop.reservedSharedMemPerBlock) * 100 + prop.sharedMemPerMultiprocessor - 1) / prop.sharedMemPerMultiprocessor);
     if (pct > 100) pct = 100;
+    static int s_carveout = 0;
+    if (pct > s_carveout) s_carveout = pct;
+    pct = s_carveout;
     if ((e = cudaFuncSetAttribute(ddf_hash_kernel<false>, cudaFuncAttributePreferredSharedMemoryCarveout, pct)) != cudaSuccess ||
         (e = cudaFuncSetAttribute(ddf_hash_kernel<true>, cudaFuncAttributePreferredSharedMemoryCarveout, pct)) != cudaSuccess ||
         (e = cudaFuncSetAttribute(ddf_hash_kernel<false, true>, cudaFuncAttributePreferredSharedMemoryCarveout, pct)) != cudaSuccess ||

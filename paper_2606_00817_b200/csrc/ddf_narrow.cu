@@ -138,7 +138,7 @@ __global__ void __launch_bounds__(kNwThreads) ddf_narrow_kernel(const __grid_con
         }
         __syncwarp();
       }
-      while (!ptx::mbar_try_wait(bar, phase)) { }
+      ptx::mbar_wait_bounded(bar, phase);
       phase ^= 1u;
       ptx::tc_fence_after();
       const float* bl = fsm + l * W;
@@ -249,7 +249,9 @@ int narrow_plan_create(Model* m, const uint16_t* hw, const float* hb) {
   for (int l = 0; l < (int)L.n_hidden; ++l) p.w_blk_off[l] = blk_off[l];
   p.total_blocks = total;
   t->smem_bytes = smem;
-  DDF_CUDA_TRY(cudaFuncSetAttribute(ddf_narrow_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  // function attributes are process-wide: the limit is the device's, the carve-out the largest any live or past model asked
+  // for, so creating a smaller network never lowers what an existing larger one launches with
+  DDF_CUDA_TRY(cudaFuncSetAttribute(ddf_narrow_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)prop.sharedMemPerBlockOptin));
   cudaFuncAttributes fa;
   DDF_CUDA_TRY(cudaFuncGetAttributes(&fa, ddf_narrow_kernel));
   const int regs_cta = ((fa.numRegs * 32 + 255) / 256 * 256) * (kNwThreads / 32);
@@ -261,7 +263,9 @@ int narrow_plan_create(Model* m, const uint16_t* hw, const float* hb) {
   t->ctas_per_sm = occ;
   int pct = (int)((occ * (smem + prop.reservedSharedMemPerBlock) * 100 + prop.sharedMemPerMultiprocessor - 1) / prop.sharedMemPerMultiprocessor);
   if (pct > 100) pct = 100;
-  DDF_CUDA_TRY(cudaFuncSetAttribute(ddf_narrow_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, pct));
+  static int s_carveout = 0;
+  if (pct > s_carveout) s_carveout = pct;
+  DDF_CUDA_TRY(cudaFuncSetAttribute(ddf_narrow_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, s_carveout));
   return DDF_OK;
 }
 

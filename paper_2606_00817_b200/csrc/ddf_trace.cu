@@ -74,6 +74,23 @@ __global__ void trace_update_kernel(const int32_t* __restrict__ idx_in, const in
 
 using namespace ddf;
 
+namespace ddf {
+// workspace of sdf_sphere_trace for n rays and S steps: pts 12n, z 4n, idx 2*4n, done n, counts
+static size_t trace_need(int64_t n, int S, size_t* rows) {
+  const size_t a = (size_t)((n + 63) / 64 * 64);
+  if (rows) *rows = a;
+  return a * 12 + a * 4 + a * 8 + a + (size_t)(S + 2) * 8;
+}
+int trace_reserve(Model* m, int64_t n, int S) {
+  const size_t need = trace_need(n, S, nullptr);
+  if (need <= m->trace_ws_bytes) return DDF_OK;
+  cudaFree(m->trace_ws); m->trace_ws = nullptr; m->trace_ws_bytes = 0;
+  DDF_CUDA_TRY(cudaMalloc(&m->trace_ws, need));
+  m->trace_ws_bytes = need;
+  return DDF_OK;
+}
+}  // namespace ddf
+
 extern "C" int sdf_sphere_trace(ddf_model* model, const float* o, const float* d, int64_t n,
                                 const sdf_trace_params* prm, float* out_t, uint8_t* out_hit,
                                 int32_t* out_steps, float* trace_p, float* trace_s, int64_t* total_evals,
@@ -86,14 +103,9 @@ extern "C" int sdf_sphere_trace(ddf_model* model, const float* o, const float* d
   if (!o || !d || !out_t || !out_hit || !out_steps) return DDF_E_INVALID_ARG;
   cudaStream_t st = (cudaStream_t)stream;
   const int S = prm->max_steps;
-  // workspace: pts 12n, z 4n, idx 2*4n, done n, counts
-  const size_t a = (size_t)((n + 63) / 64 * 64);
-  const size_t need = a * 12 + a * 4 + a * 8 + a + (size_t)(S + 2) * 8;
-  if (need > m->trace_ws_bytes) {
-    cudaFree(m->trace_ws); m->trace_ws = nullptr; m->trace_ws_bytes = 0;
-    DDF_CUDA_TRY(cudaMalloc(&m->trace_ws, need));
-    m->trace_ws_bytes = need;
-  }
+  size_t a;
+  (void)trace_need(n, S, &a);
+  { int rc = trace_reserve(m, n, S); if (rc != DDF_OK) return rc; }    // a no-op after ddf_reserve(DDF_RESERVE_TRACE)
   uint8_t* base = (uint8_t*)m->trace_ws;
   TraceWs w;
   w.pts = (float*)base;                 base += a * 12;

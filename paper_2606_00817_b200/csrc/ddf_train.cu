@@ -213,6 +213,7 @@ __device__ __forceinline__ void adam_slice(float* __restrict__ prm, float* __res
   for (int64_t i = first; i < n4; i += stride) {
     float4 gi = reinterpret_cast<float4*>(g)[i], mi = __ldcs(reinterpret_cast<float4*>(m) + i), vi = __ldcs(reinterpret_cast<float4*>(v) + i),
            pi = reinterpret_cast<float4*>(prm)[i];
+    const bool g_nonzero = gi.x != 0.0f || gi.y != 0.0f || gi.z != 0.0f || gi.w != 0.0f;
     if (i < rep4) {
       #pragma unroll
       for (int k = 0; k < kTrRep; ++k) {
@@ -226,7 +227,8 @@ __device__ __forceinline__ void adam_slice(float* __restrict__ prm, float* __res
     ADAM1(x) ADAM1(y) ADAM1(z) ADAM1(w)
     #undef ADAM1
     __stcs(reinterpret_cast<float4*>(m) + i, mi); __stcs(reinterpret_cast<float4*>(v) + i, vi); reinterpret_cast<float4*>(prm)[i] = pi;
-    if (gi.x != 0.0f || gi.y != 0.0f || gi.z != 0.0f || gi.w != 0.0f) reinterpret_cast<float4*>(g)[i] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+    // clear what was LOADED from g (gi now also holds the folded private copies, which may cancel it exactly)
+    if (g_nonzero) reinterpret_cast<float4*>(g)[i] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
   }
   for (int64_t i = (n4 << 2) + first; i < n; i += stride) {
     const float gi = g[i];
@@ -466,7 +468,8 @@ extern "C" int ddf_trainer_create(const float* table, const float* mlp, const dd
   p.tmask = (1u << L.log2_table_size) - 1u;
   p.n_levels = (int)L.n_levels; p.Ld = (int)L.n_freq_dir; p.n_hidden = H; p.E = E; p.NF = NF;
   T->smem_bytes = (size_t)((E + (H - 1) * kTrW) * kTrW + H * kTrW + 2 * kTrW + (H + 3) * kTrW * kTrPitch) * 4;
-  if ((e = cudaFuncSetAttribute(train_fwd_bwd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T->smem_bytes)) != cudaSuccess) return fail(e);
+  // process-wide attribute: the device's limit, so a second, smaller trainer never lowers it for a live larger one
+  if ((e = cudaFuncSetAttribute(train_fwd_bwd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)prop.sharedMemPerBlockOptin)) != cudaSuccess) return fail(e);
   if ((e = train_tc_prepare()) != cudaSuccess) return fail(e);
   T->sms = prop.multiProcessorCount;
   if (params->arithmetic == DDF_TRAIN_BF16X3 &&

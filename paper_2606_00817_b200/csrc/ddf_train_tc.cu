@@ -313,7 +313,7 @@ __global__ void __launch_bounds__(kTrThreads, 1) tc_mlp_kernel(const __grid_cons
                              sm_u32 + kOffWh + l * kWTile, sm_u32 + kOffWl + l * kWTile, 4, 0u, 0u, idF);
         ptx::umma_commit<1>(bar);
       }
-      while (!ptx::mbar_try_wait(bar, phase)) { }
+      ptx::mbar_wait_bounded(bar, phase);
       phase ^= 1u;
       ptx::tc_fence_after();
       uint32_t v[32];
@@ -394,7 +394,7 @@ __global__ void __launch_bounds__(kTrThreads, 1) tc_mlp_kernel(const __grid_cons
         for (int q = 0; q < kTrRays; ++q) s += get(Gh, Gl, q, u);
         atomicAdd(p.g_mlp + p.b_off[l] + u, s);
       }
-      while (!ptx::mbar_try_wait(bar, phase)) { }
+      ptx::mbar_wait_bounded(bar, phase);
       phase ^= 1u;
       ptx::tc_fence_after();
       if (l > 0) {                                             // delta of the layer below: ReLU mask of its output

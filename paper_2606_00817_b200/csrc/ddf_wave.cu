@@ -173,6 +173,23 @@ __global__ void wave_ao_scatter_kernel(const float* __restrict__ vis, int64_t n,
   if (k < *count) out_ao[index[k]] = ao_c[k];
 }
 
+int wave_reserve_bytes(Model* m, size_t need) {
+  if (need <= m->wave_ws_bytes) return DDF_OK;
+  cudaFree(m->wave_ws); m->wave_ws = nullptr; m->wave_ws_bytes = 0;
+  DDF_CUDA_TRY(cudaMalloc(&m->wave_ws, need));
+  m->wave_ws_bytes = need;
+  return DDF_OK;
+}
+// the largest workspace any wavefront call needs for n primary rays (spp AO rays per hit; 0: shadows only)
+int wave_reserve(Model* m, int64_t n, int spp) {
+  const size_t nb = (size_t)((n + kWaveBlock - 1) / kWaveBlock);
+  const size_t a = (size_t)((n + 63) / 64 * 64);
+  const size_t head = ((nb * 4 + 255) / 256) * 256 + 256;
+  size_t need = head + a * (12 + 12 + 4 + 4 + 4 + 4);
+  if (spp > 0) { const size_t ao = head + a * (12 + 12 + 4 + 4) + a * (size_t)spp * 24; if (ao > need) need = ao; }
+  return wave_reserve_bytes(m, need);
+}
+
 struct WaveWs { int32_t* block_counts; float *o2, *d2, *tmax, *dist2, *vis2; int32_t* index; int64_t* count; };
 
 // workspace: block counts always; the ray buffers only for ddf_query_shadowed (full = true)
@@ -181,11 +198,7 @@ static int wave_ws(Model* m, int64_t n, bool full, WaveWs* w) {
   const size_t a = (size_t)((n + 63) / 64 * 64);
   size_t need = ((nb * 4 + 255) / 256) * 256 + 256;
   if (full) need += a * (12 + 12 + 4 + 4 + 4 + 4);
-  if (need > m->wave_ws_bytes) {
-    cudaFree(m->wave_ws); m->wave_ws = nullptr; m->wave_ws_bytes = 0;
-    DDF_CUDA_TRY(cudaMalloc(&m->wave_ws, need));
-    m->wave_ws_bytes = need;
-  }
+  { int rc = wave_reserve_bytes(m, need); if (rc != DDF_OK) return rc; }
   uint8_t* b = (uint8_t*)m->wave_ws;
   w->count = (int64_t*)b;                 b += 256;
   w->block_counts = (int32_t*)b;          b += ((nb * 4 + 255) / 256) * 256;
@@ -313,11 +326,7 @@ static int wave_ao_ws(Model* m, int64_t n, int spp, bool full, WaveAoWs* w) {
   const size_t a = (size_t)((n + 63) / 64 * 64);
   size_t need = ((nb * 4 + 255) / 256) * 256 + 256;
   if (full) need += a * (12 + 12 + 4 + 4) + a * (size_t)spp * 24;
-  if (need > m->wave_ws_bytes) {
-    cudaFree(m->wave_ws); m->wave_ws = nullptr; m->wave_ws_bytes = 0;
-    DDF_CUDA_TRY(cudaMalloc(&m->wave_ws, need));
-    m->wave_ws_bytes = need;
-  }
+  { int rc = wave_reserve_bytes(m, need); if (rc != DDF_OK) return rc; }
   uint8_t* b = (uint8_t*)m->wave_ws;
   w->count = (int64_t*)b; w->count_rays = (int64_t*)(b + 8);  b += 256;
   w->block_counts = (int32_t*)b;                              b += ((nb * 4 + 255) / 256) * 256;

@@ -74,6 +74,8 @@ def test_argument_errors_without_gpu(libddf):
     assert libddf.ddf_gen_sphere_points(C.c_uint64(1), C.c_uint64(1), C.c_int64(-1), C.c_float(1), None, None, None) == -1
     assert libddf.ddf_ao_reduce(None, None, C.c_int64(0), 16, C.c_float(1), None, None) == 0
     assert libddf.ddf_ao_reduce(None, None, C.c_int64(4), 0, C.c_float(1), None, None) == -1
+    assert libddf.ddf_reserve(None, C.c_uint32(1), C.c_int64(16), 0) == -1
+    assert libddf.ddf_query_ao(None, None, None, C.c_int64(1 << 30), 16, C.c_float(1), None, None) == -1
 
 
 def test_camera_from_seed_matches_oracle_twin(libddf, orc):

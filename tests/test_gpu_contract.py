@@ -434,3 +434,36 @@ def test_maximum_batch_2pow24_and_side_stream(ddf, orc, c1):
     z, t, xi = orc.forward(lay, make_weights(lay), o[idx], d[idx], mode=0)
     g = dist[-(1 << 16):].cpu().numpy()[idx]
     assert (np.abs(g - t) / (1 + np.abs(t))).max() <= 1e-2
+
+
+def test_reserved_calls_do_not_allocate(ddf, c1, sdf):
+    """ddf_reserve sizes the per-batch workspaces; afterwards ddf_query_host, ddf_query_camera and sdf_sphere_trace
+    leave the device's free memory where it was (no allocation in the query calls), also for a
+    batch larger than any seen before."""
+    lay, m = c1
+    n = 300_000
+    o, d = random_rays(n)
+    oh, dh = torch.from_numpy(o).pin_memory(), torch.from_numpy(d).pin_memory()
+    dist_h, vis_h = torch.empty(n).pin_memory(), torch.empty(n).pin_memory()
+    dist = torch.empty(n, device="cuda"); vis = torch.empty(n, device="cuda")
+    ddf.ddf_reserve(m, ddf.RESERVE_HOST | ddf.RESERVE_RAYS, n)
+    torch.cuda.synchronize()
+    free0 = torch.cuda.mem_get_info()[0]
+    ddf.ddf_query_host(m, oh, dh, n, dist_h, vis_h)
+    cam = ddf.ddf_camera_from_seed(MASTER_SEED, STREAMS["camera_pos"], 2.5)
+    ddf.ddf_query_camera(m, cam, 500, 600, dist, vis)
+    torch.cuda.synchronize()
+    assert torch.cuda.mem_get_info()[0] == free0
+    ddf.ddf_query(m, _cuda(o), _cuda(d), n, dist, vis)
+    torch.cuda.synchronize()
+    assert torch.equal(dist.cpu(), dist_h) and torch.equal(vis.cpu(), vis_h)
+    slay, sblob, sm = sdf
+    k = 50_000
+    ddf.ddf_reserve(sm, ddf.RESERVE_TRACE, k)
+    t = torch.empty(k, device="cuda"); hit = torch.empty(k, dtype=torch.uint8, device="cuda"); steps = torch.empty(k, dtype=torch.int32, device="cuda")
+    oc, dc = _cuda(o[:k] * 2.0), _cuda(d[:k])
+    torch.cuda.synchronize()
+    free1 = torch.cuda.mem_get_info()[0]
+    ddf.sdf_sphere_trace(sm, oc, dc, k, ddf.SdfTraceParams(8, 1e-3, 6.0, 1.0, 0.05, 1), t, hit, steps, None, None, None)
+    torch.cuda.synchronize()
+    assert torch.cuda.mem_get_info()[0] == free1

@@ -270,3 +270,48 @@ def test_query_ao_points_is_generator_plus_query_ao(ddf, kind):
     with pytest.raises(ddf.DdfError):
         ddf.ddf_query_ao_points(m, p, None, 10, 16, 1, 2, 1e-3, 1.0, got)
     ddf.ddf_destroy(m)
+
+
+def test_a_smaller_model_created_later_does_not_break_a_larger_one(ddf):
+    """Function attributes (dynamic shared-memory limit, carve-out) are per process, not per model: a large hash-grid
+    field, a large narrow network and a large trainer must still launch - with the same bits - after a smaller object of
+    the same kind was created (ddf.h: "different models are independent")."""
+    from ddf_inputs import Layout, make_weights
+    o, d = random_rays(3000)
+    od, dd = _cuda(o), _cuda(d)
+
+    def ask(m):
+        dist = torch.empty(3000, device="cuda"); vis = torch.empty(3000, device="cuda")
+        ddf.ddf_query(m, od, dd, 3000, dist, vis)
+        torch.cuda.synchronize()
+        return dist.clone(), vis.clone()
+
+    big_h = HashLayout(n_levels=4, log2_table=12, n_hidden=4)              # 51.8 KB of dynamic shared memory
+    small_h = HashLayout(n_levels=4, log2_table=12, n_hidden=1)
+    big_n = Layout(0, 10, 4, 4, 128, -1, 2, 0)                             # ~200 KB (weights resident)
+    small_n = Layout(0, 4, 4, 3, 64, -1, 2, 0)
+    _, _, mh = _field(ddf, big_h)
+    mn = ddf.ddf_create(make_weights(big_n), big_n)
+    before = ask(mh), ask(mn)
+    _, _, sh = _field(ddf, small_h)
+    sn = ddf.ddf_create(make_weights(small_n), small_n)
+    ask(sh); ask(sn)
+    after = ask(mh), ask(mn)
+    for (a, b), (c, e) in zip(before, after):
+        assert torch.equal(a, c) and torch.equal(b, e)
+    for m in (mh, mn, sh, sn):
+        ddf.ddf_destroy(m)
+    # trainers: a 4-hidden-layer field, then a 1-hidden-layer one, then a step of the first (CUDA-core arithmetic uses
+    # the dynamic shared-memory limit)
+    lay_b, lay_s = HashLayout(n_levels=4, log2_table=12, n_hidden=4), HashLayout(n_levels=4, log2_table=12, n_hidden=1)
+    trs = []
+    for lay in (lay_b, lay_s):
+        nt = ddf.ddf_hashgrid_table_entries(lay)
+        trs.append(ddf.ddf_trainer_create(make_hash_table(lay, nt), make_hash_mlp(lay), lay, ddf.make_train_params(total_steps=10, arithmetic=1)))
+    t = torch.full((3000,), 1.0, device="cuda"); hit = torch.ones(3000, dtype=torch.uint8, device="cuda")
+    loss = torch.zeros(1, device="cuda")
+    ddf.ddf_trainer_step(trs[0], od, dd, t, hit, 3000, loss)
+    torch.cuda.synchronize()
+    assert np.isfinite(float(loss.item()))
+    for tr in trs:
+        ddf.ddf_trainer_destroy(tr)
