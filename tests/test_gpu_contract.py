@@ -398,7 +398,7 @@ def test_sphere_trace_teacher_forcing(ddf, orc, sdf):
     # samples of size N - sqrt(2 p (1 - p) / N) for the hit rate, sqrt((var_gpu + var_cpu) / N) for the mean step
     # count - which over-estimates the spread of these paired samples (rays that converge quickly agree exactly).
     o2, d2 = orc.gen_camera(cam, 40, 40)
-    t2, hit2, steps2, _, _, _ = _trace(ddf, m, o2, d2, prm1, want_trace=False)
+    t2, hit2, steps2, _ = _trace(ddf, m, o2, d2, prm1, want_trace=False)
     rt, rhit, rsteps = orc.sphere_trace(lay, blob, o2, d2, 64, 1e-3, 6.0, 1.0, 0.05)
     N = len(o2); ph = 0.5 * (hit2.mean() + rhit.mean())
     b_hit = 3.0 * math.sqrt(2.0 * ph * (1.0 - ph) / N)

@@ -301,9 +301,9 @@ def test_a_smaller_model_created_later_does_not_break_a_larger_one(ddf):
         assert torch.equal(a, c) and torch.equal(b, e)
     for m in (mh, mn, sh, sn):
         ddf.ddf_destroy(m)
-    # trainers: a 4-hidden-layer field, then a 1-hidden-layer one, then a step of the first (CUDA-core arithmetic uses
-    # the dynamic shared-memory limit)
-    lay_b, lay_s = HashLayout(n_levels=4, log2_table=12, n_hidden=4), HashLayout(n_levels=4, log2_table=12, n_hidden=1)
+    # trainers: the paper's 16-level, 2-hidden-layer field, then a 2-level, 1-hidden-layer one, then a step of the first
+    # (the CUDA-core arithmetic launches with the first one's dynamic shared-memory size)
+    lay_b, lay_s = HashLayout(log2_table=12), HashLayout(n_levels=2, log2_table=12, n_hidden=1, n_freq_dir=0)
     trs = []
     for lay in (lay_b, lay_s):
         nt = ddf.ddf_hashgrid_table_entries(lay)
