@@ -289,7 +289,7 @@ extern "C" int ddf_destroy(ddf_model* model) {
 }
 
 extern "C" int ddf_set_path(ddf_model* model, int path) {
-  if (!model || path < 0 || path > 4) return DDF_E_INVALID_ARG;
+  if (!model || path < 0 || path > 5) return DDF_E_INVALID_ARG;
   Model* m = reinterpret_cast<Model*>(model);
   if (m->hg) return path == 0 ? DDF_OK : DDF_E_UNSUPPORTED;
   if (path == 2 && !m->tc && !m->nw) return DDF_E_UNSUPPORTED;

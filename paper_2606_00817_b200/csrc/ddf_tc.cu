@@ -49,6 +49,7 @@ struct TcParams {
   CUtensorMap x0, x1, g;
   CUtensorMap xs0, xs1;              // store maps (32-row boxes) on the same activation buffers
   int hint_act, hint_w, hint_st;     // L2 eviction class of the three TMA streams (0 normal, 1 evict_last, 2 evict_first)
+  int res_stages, res_e16;           // activation-resident kernel: weight stages that fit, gamma rows (E rounded up to 16)
   const float* o; const float* d;
   int64_t n; const int64_t* n_dev;
   const float* bias; const float* head_w;
@@ -65,6 +66,8 @@ struct TcParams {
 struct TcPlan {
   int cg;
   int grid;
+  bool res_ok;                       // the activation-resident kernel serves this layout
+  size_t res_smem;
   __nv_bfloat16 *x0, *x1, *g;
   float2* zpart;                     // column-split path: head partials [rows][n_chunks][2 halves]
   uint32_t* dbg_host; uint32_t* dbg_dev;
@@ -395,6 +398,10 @@ __global__ void __launch_bounds__(kThreads, 1) ddf_tc_kernel(const __grid_consta
   if (CG == 2) ptx::cluster_sync(); else __syncthreads();
   if (warp == 2) ptx::tmem_dealloc<CG>(tmem_base, 512);
 }
+
+}  // namespace ddf
+#include "ddf_tc_res.cuh"
+namespace ddf {
 
 // ------------------------------------------------------------------------------------------
 // Column-split path for small batches.  With fewer ray tiles than CTA pairs the persistent kernel
@@ -784,6 +791,16 @@ int tc_plan_create(Model* m) {
   p.g_last_nk16 = (m->E - (m->E_pad - kKBlock) + 15) / 16;
   DDF_CUDA_TRY(cudaFuncSetAttribute(ddf_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TcCfg<2>::kSmemBytes));
   DDF_CUDA_TRY(cudaFuncSetAttribute(ddf_tc_split_layer_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TcCfg<2>::kSmemBytes));
+  // activation-resident kernel: 64 rays x width bf16 resident per CTA, parked chunks in 256 TMEM columns (<= 5 chunks)
+  p.res_e16 = (m->E + 15) / 16 * 16;
+  p.res_stages = 0;
+  for (int s = kResMaxStages; s >= 2; --s)
+    if (res_smem_bytes((int)L.width, p.res_e16, s) <= (size_t)TcCfg<2>::kSmemBytes) { p.res_stages = s; break; }
+  t->res_ok = p.res_stages >= 2 && L.width / kChunkN <= 5 && m->E_pad <= 128;
+  if (t->res_ok) {
+    t->res_smem = res_smem_bytes((int)L.width, p.res_e16, p.res_stages);
+    DDF_CUDA_TRY(cudaFuncSetAttribute(ddf_tc_res_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TcCfg<2>::kSmemBytes));
+  }
   return DDF_OK;
 }
 
@@ -830,8 +847,25 @@ int tc_forward(Model* m, const float* o, const float* d, int64_t n, const int64_
   const int64_t tile_rays = (int64_t)kTileM * t->cg;
   int64_t tiles = (n + tile_rays - 1) / tile_rays;
   // small batches: split the output columns of a layer over the CTA pairs (ddf_set_path 3 / 4 pin the choice)
-  const int64_t split_max = (t->cg != 2 || m->path == 3) ? 0 : (m->path == 4 ? t->grid / 2 : kSplitAutoTiles);
+  const int64_t split_max = (m->path == 3 || m->path == 5) ? 0 : (m->path == 4 ? t->grid / 2 : kSplitAutoTiles);
   if (tiles <= split_max) return tc_forward_split(m, p, tiles, st);
+  if (m->path == 5 && t->res_ok) {
+    // activation-resident kernel: tiles of 128 rays per CTA pair, same equal-tiles grid rule
+    const int64_t rtiles = (n + 2 * kResRays - 1) / (2 * kResRays);
+    const int64_t units = t->grid / 2, waves = (rtiles + units - 1) / units;
+    const int rgrid = (int)((rtiles + waves - 1) / waves) * 2;
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof(cfg));
+    cfg.gridDim = dim3((unsigned)rgrid); cfg.blockDim = dim3(kThreads); cfg.stream = st;
+    cfg.dynamicSmemBytes = t->res_smem;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = 2; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    DDF_CUDA_TRY(cudaLaunchKernelEx(&cfg, ddf_tc_res_kernel, p));
+    m->last_launches = 1;
+    return DDF_OK;
+  }
   // as many CTAs (pairs) as give every one the same number of tiles (+-1): the last wave of a persistent grid is
   // otherwise part empty, and the CTAs that would idle through it only add L2 contention and power in the others
   const int64_t units = t->grid / t->cg;
