@@ -108,7 +108,12 @@ int  ddf_last_cuda_error(void);                           /* cudaError_t of the 
  * CTA pairs, heads - which keeps the whole chip busy on a small batch (2.5x faster at n <= 2,048).
  * Both return the same bits.  3 = tcgen05 path, always the single persistent launch; 4 = tcgen05
  * path, column-split whenever the batch fits the split scratch (n <= 18,944), else persistent.
- * 3 and 4 are DDF_E_UNSUPPORTED for models the persistent kernel does not serve. */
+ * 5 = tcgen05 path, activation-resident kernel for every batch size: the same forward pass with the layer hand-off kept
+ * in shared and tensor memory (64 rays per CTA resident as the MMA's B operand; no activation is written to global
+ * memory - BASELINE.json north_star (b) "Activations stay on-chip between layers"), for widths that are a multiple of
+ * 256 up to 1280 with an encoding of at most 128 values; other layouts fall back to the persistent kernel.  Its results
+ * agree with the persistent kernel's up to the order in which the same products are added (not bit for bit).
+ * 3, 4 and 5 are DDF_E_UNSUPPORTED for models the persistent kernel does not serve. */
 int  ddf_set_path(ddf_model* model, int path);
 /* Sizes the per-batch workspaces ahead of time so that no later call with at most max_rays rays allocates
  * (SURVEY.md 8(b) "the library never allocates in ddf_query (workspace, if any, sized at create)").  `what` selects

@@ -849,6 +849,9 @@ int tc_forward(Model* m, const float* o, const float* d, int64_t n, const int64_
   // small batches: split the output columns of a layer over the CTA pairs (ddf_set_path 3 / 4 pin the choice)
   const int64_t split_max = (m->path == 3 || m->path == 5) ? 0 : (m->path == 4 ? t->grid / 2 : kSplitAutoTiles);
   if (tiles <= split_max) return tc_forward_split(m, p, tiles, st);
+#ifdef DDF_DEV
+  if (const char* e = getenv("DDF_DEV_RES")) p.hint_st = atoi(e);
+#endif
   if (m->path == 5 && t->res_ok) {
     // activation-resident kernel: tiles of 128 rays per CTA pair, same equal-tiles grid rule
     const int64_t rtiles = (n + 2 * kResRays - 1) / (2 * kResRays);

@@ -210,6 +210,12 @@ __device__ __forceinline__ void tmem_st_wait() { asm volatile("tcgen05.wait::st.
 __device__ __forceinline__ void st_cluster_v4(uint32_t addr_cluster, uint4 v) {
   asm volatile("st.shared::cluster.v4.b32 [%0], {%1, %2, %3, %4};" :: "r"(addr_cluster), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
 }
+// asynchronous 16-byte store into another CTA's shared memory; its completion is counted (16 bytes of transaction) on an
+// mbarrier of that CTA, so the writer neither fences nor waits
+__device__ __forceinline__ void st_async_v4(uint32_t addr_cluster, uint4 v, uint32_t bar_cluster) {
+  asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v4.b32 [%0], {%1, %2, %3, %4}, [%5];"
+               :: "r"(addr_cluster), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w), "r"(bar_cluster) : "memory");
+}
 // arrive that publishes this thread's earlier writes (to any CTA of the cluster) to whoever waits on the barrier
 __device__ __forceinline__ void mbar_arrive_release_cluster(uint32_t bar_cluster_addr) {
   asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" :: "r"(bar_cluster_addr) : "memory");

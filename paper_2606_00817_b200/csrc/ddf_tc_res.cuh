@@ -43,15 +43,18 @@ __device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
   return *reinterpret_cast<uint32_t*>(&t);
 }
 
-// one K row (128 bytes = 64 rays) of the resident operand in CTA `dest`: 8 x 16 bytes, 128-byte swizzle
-__device__ __forceinline__ void res_store_row(uint32_t h_base, int row, const uint32_t (&w)[32], bool local, uint32_t dest) {
+// one K row (128 bytes = 64 rays) of the resident operand: 8 x 16 bytes, 128-byte swizzle.  Into this CTA's own rows:
+// plain stores (the caller fences and arrives).  Into the peer's: asynchronous stores that count their bytes on the
+// peer's barrier `bar_peer` (a shared::cluster address) - nothing to fence, nothing to wait for.
+__device__ __forceinline__ void res_store_row(uint32_t h_base, int row, const uint32_t (&w)[32], bool local, uint32_t peer, uint32_t bar_peer) {
   const uint32_t a = h_base + (uint32_t)row * 128u;
+  const uint32_t ar = local ? 0u : ptx::mapa(a, peer);
   #pragma unroll
   for (int i = 0; i < 8; ++i) {
     const uint4 v = make_uint4(w[4 * i], w[4 * i + 1], w[4 * i + 2], w[4 * i + 3]);
-    const uint32_t addr = a + (uint32_t)((i ^ (row & 7)) << 4);
-    if (local) ptx::st_shared_v4(addr, v);
-    else ptx::st_cluster_v4(ptx::mapa(addr, dest), v);
+    const uint32_t off = (uint32_t)((i ^ (row & 7)) << 4);
+    if (local) ptx::st_shared_v4(a + off, v);
+    else ptx::st_async_v4(ar + off, v, bar_peer);
   }
 }
 
@@ -67,7 +70,10 @@ __global__ void __launch_bounds__(kThreads, 1) ddf_tc_res_kernel(const __grid_co
   auto empty_bar  = [&](int s) { return bar + 8u * (8 + s); };
   auto tfull_bar  = [&](int b) { return bar + 8u * (16 + b); };
   auto tempty_bar = [&](int b) { return bar + 8u * (18 + b); };
-  auto hready_bar = [&](int j) { return bar + 8u * (20 + j); };        // chunk j of the next layer's input is in place (both CTAs)
+  // chunk j of the next layer's input is in place in THIS CTA: 4 arrivals of the local epilogue warps (one of them
+  // announcing the 16 KB the peer's warps send asynchronously) + those bytes
+  auto hready_bar = [&](int j) { return bar + 8u * (20 + j); };
+  auto pready_bar = [&](int j) { return bar + 8u * (33 + j); };        // leader only: chunk j is in place in the peer CTA too
   const uint32_t gready_bar = bar + 8u * 28, gfree_bar = bar + 8u * 29, zready_bar = bar + 8u * 30;
   const uint32_t tmem_slot = bar + 8u * 32;
 
@@ -84,7 +90,7 @@ __global__ void __launch_bounds__(kThreads, 1) ddf_tc_res_kernel(const __grid_co
   if (threadIdx.x == 0) {
     for (int s = 0; s < S; ++s) { ptx::mbar_init(full_bar(s), 1); ptx::mbar_init(empty_bar(s), 1); }
     for (int b = 0; b < 2; ++b) { ptx::mbar_init(tfull_bar(b), 1); ptx::mbar_init(tempty_bar(b), 16); }
-    for (int j = 0; j < kMaxChunks; ++j) ptx::mbar_init(hready_bar(j), 16);
+    for (int j = 0; j < kMaxChunks; ++j) { ptx::mbar_init(hready_bar(j), 4); ptx::mbar_init(pready_bar(j), 1); }
     ptx::mbar_init(gready_bar, 4); ptx::mbar_init(gfree_bar, 1); ptx::mbar_init(zready_bar, 8);
     ptx::fence_mbar_init();
   }
@@ -186,9 +192,14 @@ __global__ void __launch_bounds__(kThreads, 1) ddf_tc_res_kernel(const __grid_co
             } else {
               int chunk = nc - 1;
               for (int cj = 0; cj < nc; ++cj) {
+#ifdef DDF_DEV
+                if (c == 0 && (p.hint_st & 8)) { hphase ^= (1u << chunk); } else       // timing experiment: ignore the hand-over
+#endif
                 if (c == 0) {
                   wait_bar<true>(hready_bar(chunk), (hphase >> chunk) & 1u, p.dbg, 0x2200 + chunk);
+                  wait_bar<true>(pready_bar(chunk), (hphase >> chunk) & 1u, p.dbg, 0x2900 + chunk);
                   hphase ^= (1u << chunk);
+                  ptx::fence_proxy_async_smem();                 // the peer's asynchronous stores -> the tensor core's reads
                   ptx::tc_fence_after();
                 }
                 const uint64_t hd = hdesc0 + (uint64_t)((uint32_t)chunk * (4u * kKBlock * 128u >> 4));
@@ -202,6 +213,22 @@ __global__ void __launch_bounds__(kThreads, 1) ddf_tc_res_kernel(const __grid_co
           }
         }
       }
+    } else {
+      // the peer CTA's warp 1 relays "chunk in place here" to the leader, whose MMAs read both CTAs' operands
+      uint32_t hphase = 0;
+      for (int64_t tile = pid; tile < num_tiles; tile += num_pairs) {
+        for (int l = 1; l < p.n_hidden; ++l) {
+          int chunk = nc - 1;
+          for (int cj = 0; cj < nc; ++cj) {
+            wait_bar<true>(hready_bar(chunk), (hphase >> chunk) & 1u, p.dbg, 0x2a00 + chunk);
+            hphase ^= (1u << chunk);
+            ptx::fence_proxy_async_smem();
+            __syncwarp();
+            if (lane == 0) ptx::mbar_arrive_cluster(ptx::mapa(pready_bar(chunk), 0));
+            if (++chunk == nc) chunk = 0;
+          }
+        }
+      }
     }
   } else if (warp >= 4) {
     // ================================================================ epilogue (8 warps)
@@ -212,6 +239,16 @@ __global__ void __launch_bounds__(kThreads, 1) ddf_tc_res_kernel(const __grid_co
     const uint32_t lane_sel = (uint32_t)(q * 32) << 16;
     const uint32_t tempty_remote = ptx::mapa(tempty_bar(0), 0);
     const uint32_t stash = tmem_base + lane_sel + 4u * kResRays + (uint32_t)h * 32u;    // + 64 columns per parked chunk
+    const uint32_t hready_peer = ptx::mapa(hready_bar(0), (uint32_t)h);
+    // rows of chunk j written: the local warps publish them to the async proxy and arrive on this CTA's barrier (lane
+    // quarter 0 also announces the peer's 16 KB); the warps that sent to the peer have nothing left to do
+    auto hand_over = [&](int j) {
+      if (local) {
+        ptx::fence_proxy_async_smem();
+        __syncwarp();
+        if (lane == 0) { if (q == 0) ptx::mbar_arrive_expect_tx(hready_bar(j), 128u * 128u); else ptx::mbar_arrive(hready_bar(j)); }
+      }
+    };
     uint32_t cc = 0;
     int tile_local = 0;
     for (int64_t tile = pid; tile < num_tiles; tile += num_pairs, ++tile_local) {
@@ -242,17 +279,13 @@ __global__ void __launch_bounds__(kThreads, 1) ddf_tc_res_kernel(const __grid_co
               ptx::tmem_st_wait();
             } else {
               // every MMA of the layer has completed: the input rows are dead in both CTAs
-              res_store_row(Hs, fg, w, local, (uint32_t)h);
-              if (local) ptx::fence_proxy_async_smem(); else ptx::fence_proxy_async_cluster();
-              __syncwarp();
-              if (lane == 0) ptx::mbar_arrive_cluster(ptx::mapa(hready_bar(c), 0));
+              res_store_row(Hs, fg, w, local, (uint32_t)h, hready_peer + 8u * c);
+              hand_over(c);
               for (int j = 0; j < nc - 1; ++j) {
                 ptx::tmem_ld32(stash + (uint32_t)j * kResRays, w);
                 ptx::tmem_ld_wait();
-                res_store_row(Hs, j * kChunkN + (int)rank * 128 + fl, w, local, (uint32_t)h);
-                if (local) ptx::fence_proxy_async_smem(); else ptx::fence_proxy_async_cluster();
-                __syncwarp();
-                if (lane == 0) ptx::mbar_arrive_cluster(ptx::mapa(hready_bar(j), 0));
+                res_store_row(Hs, j * kChunkN + (int)rank * 128 + fl, w, local, (uint32_t)h, hready_peer + 8u * j);
+                hand_over(j);
               }
               ptx::tc_fence_before();
             }
