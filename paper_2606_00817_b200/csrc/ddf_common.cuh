@@ -172,6 +172,30 @@ __device__ __forceinline__ void ao_ray_from_point(const float p[3], const float 
   #undef DDF_SUMSQ
 }
 
+// The 3-vectors of 32 consecutive rays (first ray `first`, AoS float[n][3]) into registers, lane j <- ray first + j:
+// the warp reads its 384 contiguous bytes as 24 coalesced 16-byte loads and regroups them by shuffles (SURVEY.md row a1
+// "flat float4 over the n*3 array, regroup in shuffles").  Falls back to per-ray scalar loads for a 4-byte-aligned
+// buffer or a ragged last warp.  All 32 lanes must call it; lanes whose ray is >= n get zeros.
+__device__ __forceinline__ void load_ray_vec3(const float* __restrict__ base, int64_t first, int64_t n, int lane, float v[3]) {
+  const float* w = base + 3 * first;
+  const bool fast = first + 32 <= n && (reinterpret_cast<uintptr_t>(w) & 15) == 0;       // warp-uniform
+  if (fast) {
+    float4 q = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+    if (lane < 24) q = __ldg(reinterpret_cast<const float4*>(w) + lane);
+    #pragma unroll
+    for (int i = 0; i < 3; ++i) {
+      const int f = 3 * lane + i, src = f >> 2, comp = f & 3;
+      const float s0 = __shfl_sync(0xffffffffu, q.x, src), s1 = __shfl_sync(0xffffffffu, q.y, src);
+      const float s2 = __shfl_sync(0xffffffffu, q.z, src), s3 = __shfl_sync(0xffffffffu, q.w, src);
+      v[i] = comp == 0 ? s0 : (comp == 1 ? s1 : (comp == 2 ? s2 : s3));
+    }
+  } else {
+    const int64_t g = first + lane;
+    const bool ok = g < n;
+    v[0] = ok ? base[3 * g] : 0.0f; v[1] = ok ? base[3 * g + 1] : 0.0f; v[2] = ok ? base[3 * g + 2] : 0.0f;
+  }
+}
+
 // gamma of one ray into a bf16 row (E_pad entries, pad = 0).  sin/cos(2^k pi x) via sincospif
 // of the exactly scaled argument (ldexp), so high bands keep full fp32 accuracy.
 __device__ __forceinline__ void encode_vec_bf16(const float v[3], int nfreq, __nv_bfloat16* row) {

@@ -97,6 +97,92 @@ __device__ __forceinline__ void wait_bar(uint32_t bar, uint32_t parity, uint32_t
   }
 }
 
+// ---- pieces shared by the persistent and the column-split kernel (one instruction sequence, so both return the same bits)
+// the MMAs of one 64-K stage into accumulator d_tmem: 4 steps of K = 16 (fewer for gamma's last block)
+__device__ __forceinline__ void tc_issue_stage(uint32_t d_tmem, uint32_t a_addr, uint32_t b_addr, int nk16, int kb, uint32_t idesc) {
+  const uint64_t adesc = ptx::smem_desc_k_sw128(a_addr);
+  const uint64_t bdesc = ptx::smem_desc_k_sw128(b_addr);
+  if (nk16 == 4) {
+    ptx::umma_bf16<2>(d_tmem, adesc, bdesc, idesc, (uint32_t)(kb != 0));
+    ptx::umma_bf16<2>(d_tmem, adesc + 2u, bdesc + 2u, idesc, 1u);
+    ptx::umma_bf16<2>(d_tmem, adesc + 4u, bdesc + 4u, idesc, 1u);
+    ptx::umma_bf16<2>(d_tmem, adesc + 6u, bdesc + 6u, idesc, 1u);
+  } else {
+    for (int k = 0; k < nk16; ++k)
+      ptx::umma_bf16<2>(d_tmem, adesc + 2u * k, bdesc + 2u * k, idesc, (uint32_t)((kb | k) != 0));
+  }
+}
+
+// An epilogue warp's 32 rows x 128 columns of a finished accumulator chunk: tcgen05.ld, + bias, ReLU, then either
+// bf16 -> swizzled 32 x 64 staging box -> TMA store at (col0 + 64 box, out_row) (hidden layers), or this chunk's share
+// of the head dot products from the un-rounded values (last layer).  The accumulator is handed back to the MMA warp
+// (arrival on tempty_addr, the leader CTA's barrier) as soon as its last column has been read.
+__device__ __forceinline__ void tc_epilogue_chunk(const TcParams& p, uint32_t taddr, uint32_t tempty_addr, int lane, const float* bias,
+                                                  int col0, bool hidden, const CUtensorMap* smap, int out_row, uint32_t stage, int hint_st,
+                                                  float& pc0, float& pc1) {
+  #pragma unroll 1
+  for (int box = 0; box < 2; ++box) {
+    uint32_t r[64];
+    ptx::tmem_ld32(taddr + box * 64, *reinterpret_cast<uint32_t(*)[32]>(&r[0]));
+    ptx::tmem_ld32(taddr + box * 64 + 32, *reinterpret_cast<uint32_t(*)[32]>(&r[32]));
+    ptx::tmem_ld_wait();
+    if (box == 1) {
+      ptx::tc_fence_before();
+      __syncwarp();
+      if (lane == 0) ptx::mbar_arrive_cluster(tempty_addr);
+    }
+    const int col = col0 + box * 64;
+    const float4* b4 = reinterpret_cast<const float4*>(bias + col);
+    #pragma unroll
+    for (int i = 0; i < 16; ++i) {
+      float4 bb = __ldg(b4 + i);
+      r[4 * i + 0] = __float_as_uint(fmaxf(__uint_as_float(r[4 * i + 0]) + bb.x, 0.0f));
+      r[4 * i + 1] = __float_as_uint(fmaxf(__uint_as_float(r[4 * i + 1]) + bb.y, 0.0f));
+      r[4 * i + 2] = __float_as_uint(fmaxf(__uint_as_float(r[4 * i + 2]) + bb.z, 0.0f));
+      r[4 * i + 3] = __float_as_uint(fmaxf(__uint_as_float(r[4 * i + 3]) + bb.w, 0.0f));
+    }
+    if (hidden) {
+      if (lane == 0) ptx::bulk_wait_read<0>();          // staging box free again
+      __syncwarp();
+      #pragma unroll
+      for (int j = 0; j < 8; ++j) {
+        uint4 pk;
+        __nv_bfloat162 t0 = __floats2bfloat162_rn(__uint_as_float(r[8 * j + 0]), __uint_as_float(r[8 * j + 1]));
+        __nv_bfloat162 t1 = __floats2bfloat162_rn(__uint_as_float(r[8 * j + 2]), __uint_as_float(r[8 * j + 3]));
+        __nv_bfloat162 t2 = __floats2bfloat162_rn(__uint_as_float(r[8 * j + 4]), __uint_as_float(r[8 * j + 5]));
+        __nv_bfloat162 t3 = __floats2bfloat162_rn(__uint_as_float(r[8 * j + 6]), __uint_as_float(r[8 * j + 7]));
+        pk.x = *reinterpret_cast<uint32_t*>(&t0); pk.y = *reinterpret_cast<uint32_t*>(&t1);
+        pk.z = *reinterpret_cast<uint32_t*>(&t2); pk.w = *reinterpret_cast<uint32_t*>(&t3);
+        ptx::st_shared_v4(stage + (uint32_t)lane * 128u + (uint32_t)((j ^ (lane & 7)) << 4), pk);
+      }
+      ptx::fence_proxy_async_smem();
+      __syncwarp();
+      if (lane == 0) {
+        if (hint_st) ptx::tma_store_2d_hint(smap, stage, col, out_row, ptx::policy_of(hint_st));
+        else ptx::tma_store_2d(smap, stage, col, out_row);
+        ptx::bulk_commit();
+      }
+    } else {
+      const float4* w0 = reinterpret_cast<const float4*>(p.head_w + col);
+      #pragma unroll
+      for (int i = 0; i < 16; ++i) {
+        float4 ww = __ldg(w0 + i);
+        pc0 = fmaf(__uint_as_float(r[4 * i + 0]), ww.x, pc0); pc0 = fmaf(__uint_as_float(r[4 * i + 1]), ww.y, pc0);
+        pc0 = fmaf(__uint_as_float(r[4 * i + 2]), ww.z, pc0); pc0 = fmaf(__uint_as_float(r[4 * i + 3]), ww.w, pc0);
+      }
+      if (p.n_out == 2) {
+        const float4* w1 = reinterpret_cast<const float4*>(p.head_w + p.width + col);
+        #pragma unroll
+        for (int i = 0; i < 16; ++i) {
+          float4 ww = __ldg(w1 + i);
+          pc1 = fmaf(__uint_as_float(r[4 * i + 0]), ww.x, pc1); pc1 = fmaf(__uint_as_float(r[4 * i + 1]), ww.y, pc1);
+          pc1 = fmaf(__uint_as_float(r[4 * i + 2]), ww.z, pc1); pc1 = fmaf(__uint_as_float(r[4 * i + 3]), ww.w, pc1);
+        }
+      }
+    }
+  }
+}
+
 __global__ void __launch_bounds__(kThreads, 1) ddf_tc_kernel(const __grid_constant__ TcParams p) {
   constexpr int CG = 2;
   using Cfg = TcCfg<CG>;
@@ -214,19 +300,9 @@ __global__ void __launch_bounds__(kThreads, 1) ddf_tc_kernel(const __grid_consta
               ptx::tc_fence_after();
               const bool g_last = (l == 0) ? (kb == nk0 - 1) : (kb == nk - 1 && nk1 > 0);
               const int nk16 = g_last ? p.g_last_nk16 : 4;
-              const uint64_t adesc = ptx::smem_desc_k_sw128(a_smem(s));
-              const uint64_t bdesc = ptx::smem_desc_k_sw128(b_smem(s));
               const bool free_gamma = (l == gamma_layer && c == p.n_chunks - 1 && kb == nk - 1);
               if (ptx::elect_one()) {
-                if (nk16 == 4) {
-                  ptx::umma_bf16<CG>(d_tmem, adesc, bdesc, idesc, (uint32_t)(kb != 0));
-                  ptx::umma_bf16<CG>(d_tmem, adesc + 2u, bdesc + 2u, idesc, 1u);
-                  ptx::umma_bf16<CG>(d_tmem, adesc + 4u, bdesc + 4u, idesc, 1u);
-                  ptx::umma_bf16<CG>(d_tmem, adesc + 6u, bdesc + 6u, idesc, 1u);
-                } else {
-                  for (int k = 0; k < nk16; ++k)
-                    ptx::umma_bf16<CG>(d_tmem, adesc + 2u * k, bdesc + 2u * k, idesc, (uint32_t)((kb | k) != 0));
-                }
+                tc_issue_stage(d_tmem, a_smem(s), b_smem(s), nk16, kb, idesc);
                 ptx::umma_commit<CG>(empty_bar(s));
                 if (free_gamma) ptx::umma_commit<CG>(gfree_bar(gb));
                 if (kb == nk - 1) ptx::umma_commit<CG>(tfull_bar(buf));
@@ -260,70 +336,8 @@ __global__ void __launch_bounds__(kThreads, 1) ddf_tc_kernel(const __grid_consta
           ptx::tc_fence_after();
           const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + buf * kChunkN + h * 128;
           float pc0 = 0.0f, pc1 = 0.0f;           // this chunk's share of the head dot products
-          #pragma unroll 1
-          for (int box = 0; box < 2; ++box) {
-            uint32_t r[64];
-            ptx::tmem_ld32(taddr + box * 64, *reinterpret_cast<uint32_t(*)[32]>(&r[0]));
-            ptx::tmem_ld32(taddr + box * 64 + 32, *reinterpret_cast<uint32_t(*)[32]>(&r[32]));
-            ptx::tmem_ld_wait();
-            if (box == 1) {                       // accumulator fully read: hand it back to the MMA warp
-              ptx::tc_fence_before();
-              __syncwarp();
-              if (lane == 0) {
-                if (CG == 2) ptx::mbar_arrive_cluster(tempty_remote + 8u * buf);
-                else ptx::mbar_arrive(tempty_bar(buf));
-              }
-            }
-            const int col = c * kChunkN + h * 128 + box * 64;
-            const float4* b4 = reinterpret_cast<const float4*>(bias + col);
-            #pragma unroll
-            for (int i = 0; i < 16; ++i) {
-              float4 bb = __ldg(b4 + i);
-              r[4 * i + 0] = __float_as_uint(fmaxf(__uint_as_float(r[4 * i + 0]) + bb.x, 0.0f));
-              r[4 * i + 1] = __float_as_uint(fmaxf(__uint_as_float(r[4 * i + 1]) + bb.y, 0.0f));
-              r[4 * i + 2] = __float_as_uint(fmaxf(__uint_as_float(r[4 * i + 2]) + bb.z, 0.0f));
-              r[4 * i + 3] = __float_as_uint(fmaxf(__uint_as_float(r[4 * i + 3]) + bb.w, 0.0f));
-            }
-            if (l < last_layer) {
-              if (lane == 0) ptx::bulk_wait_read<0>();          // staging box free again
-              __syncwarp();
-              #pragma unroll
-              for (int j = 0; j < 8; ++j) {
-                uint4 pk;
-                __nv_bfloat162 t0 = __floats2bfloat162_rn(__uint_as_float(r[8 * j + 0]), __uint_as_float(r[8 * j + 1]));
-                __nv_bfloat162 t1 = __floats2bfloat162_rn(__uint_as_float(r[8 * j + 2]), __uint_as_float(r[8 * j + 3]));
-                __nv_bfloat162 t2 = __floats2bfloat162_rn(__uint_as_float(r[8 * j + 4]), __uint_as_float(r[8 * j + 5]));
-                __nv_bfloat162 t3 = __floats2bfloat162_rn(__uint_as_float(r[8 * j + 6]), __uint_as_float(r[8 * j + 7]));
-                pk.x = *reinterpret_cast<uint32_t*>(&t0); pk.y = *reinterpret_cast<uint32_t*>(&t1);
-                pk.z = *reinterpret_cast<uint32_t*>(&t2); pk.w = *reinterpret_cast<uint32_t*>(&t3);
-                ptx::st_shared_v4(stage + (uint32_t)lane * 128u + (uint32_t)((j ^ (lane & 7)) << 4), pk);
-              }
-              ptx::fence_proxy_async_smem();
-              __syncwarp();
-              if (lane == 0) {
-                if (p.hint_st) ptx::tma_store_2d_hint(smap, stage, col, cta_global * kTileM + q * 32, ptx::policy_of(p.hint_st));
-                else ptx::tma_store_2d(smap, stage, col, cta_global * kTileM + q * 32);
-                ptx::bulk_commit();
-              }
-            } else {
-              const float4* w0 = reinterpret_cast<const float4*>(p.head_w + col);
-              #pragma unroll
-              for (int i = 0; i < 16; ++i) {
-                float4 ww = __ldg(w0 + i);
-                pc0 = fmaf(__uint_as_float(r[4 * i + 0]), ww.x, pc0); pc0 = fmaf(__uint_as_float(r[4 * i + 1]), ww.y, pc0);
-                pc0 = fmaf(__uint_as_float(r[4 * i + 2]), ww.z, pc0); pc0 = fmaf(__uint_as_float(r[4 * i + 3]), ww.w, pc0);
-              }
-              if (p.n_out == 2) {
-                const float4* w1 = reinterpret_cast<const float4*>(p.head_w + p.width + col);
-                #pragma unroll
-                for (int i = 0; i < 16; ++i) {
-                  float4 ww = __ldg(w1 + i);
-                  pc1 = fmaf(__uint_as_float(r[4 * i + 0]), ww.x, pc1); pc1 = fmaf(__uint_as_float(r[4 * i + 1]), ww.y, pc1);
-                  pc1 = fmaf(__uint_as_float(r[4 * i + 2]), ww.z, pc1); pc1 = fmaf(__uint_as_float(r[4 * i + 3]), ww.w, pc1);
-                }
-              }
-            }
-          }
+          tc_epilogue_chunk(p, taddr, tempty_remote + 8u * buf, lane, bias, c * kChunkN + h * 128, l < last_layer, smap,
+                            cta_global * kTileM + q * 32, stage, p.hint_st, pc0, pc1);
           // chunk partials are summed in chunk order: the column-split path (below) adds the same
           // partials in the same order, so both give the same bits
           if (l == last_layer) { z0 += pc0; z1 += pc1; }
@@ -375,13 +389,12 @@ __global__ void __launch_bounds__(kThreads, 1) ddf_tc_kernel(const __grid_consta
         __align__(16) __nv_bfloat16 enc[256];
         #pragma unroll 1
         for (int k = 0; k < p.E_pad; ++k) enc[k] = __float2bfloat16_rn(0.0f);
+        float v[3], w[3];
+        load_ray_vec3(p.o, grow - lane, n, lane, v);                     // coalesced 16-byte loads, regrouped by shuffles
+        if (p.input_kind == 0) load_ray_vec3(p.d, grow - lane, n, lane, w);
         if (grow < n) {
-          float v[3] = { p.o[3 * grow], p.o[3 * grow + 1], p.o[3 * grow + 2] };
           encode_vec_bf16(v, p.Lo, enc);
-          if (p.input_kind == 0) {
-            float w[3] = { p.d[3 * grow], p.d[3 * grow + 1], p.d[3 * grow + 2] };
-            encode_vec_bf16(w, p.Ld, enc + 3 + 6 * p.Lo);
-          }
+          if (p.input_kind == 0) encode_vec_bf16(w, p.Ld, enc + 3 + 6 * p.Lo);
         }
         uint4* dst = reinterpret_cast<uint4*>(p.gp + ((size_t)(cta_global * 2 + gb) * kTileM + row) * p.E_pad);
         const uint4* src = reinterpret_cast<const uint4*>(enc);
@@ -559,18 +572,8 @@ __global__ void __launch_bounds__(kThreads, 1) ddf_tc_split_layer_kernel(const _
           ptx::tc_fence_after();
           const bool g_last = (l == 0) ? (kb == nk0 - 1) : (kb == nk - 1 && nk1 > 0);
           const int nk16 = g_last ? p.g_last_nk16 : 4;
-          const uint64_t adesc = ptx::smem_desc_k_sw128(a_smem(s));
-          const uint64_t bdesc = ptx::smem_desc_k_sw128(b_smem(s));
           if (ptx::elect_one()) {
-            if (nk16 == 4) {
-              ptx::umma_bf16<CG>(d_tmem, adesc, bdesc, idesc, (uint32_t)(kb != 0));
-              ptx::umma_bf16<CG>(d_tmem, adesc + 2u, bdesc + 2u, idesc, 1u);
-              ptx::umma_bf16<CG>(d_tmem, adesc + 4u, bdesc + 4u, idesc, 1u);
-              ptx::umma_bf16<CG>(d_tmem, adesc + 6u, bdesc + 6u, idesc, 1u);
-            } else {
-              for (int k = 0; k < nk16; ++k)
-                ptx::umma_bf16<CG>(d_tmem, adesc + 2u * k, bdesc + 2u * k, idesc, (uint32_t)((kb | k) != 0));
-            }
+            tc_issue_stage(d_tmem, a_smem(s), b_smem(s), nk16, kb, idesc);
             ptx::umma_commit<CG>(empty_bar(s));
             if (kb == nk - 1) ptx::umma_commit<CG>(tfull_bar(buf));
           }
@@ -596,66 +599,8 @@ __global__ void __launch_bounds__(kThreads, 1) ddf_tc_split_layer_kernel(const _
       ptx::tc_fence_after();
       const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + buf * kChunkN + h * 128;
       float pc0 = 0.0f, pc1 = 0.0f;
-      #pragma unroll 1
-      for (int box = 0; box < 2; ++box) {
-        uint32_t r[64];
-        ptx::tmem_ld32(taddr + box * 64, *reinterpret_cast<uint32_t(*)[32]>(&r[0]));
-        ptx::tmem_ld32(taddr + box * 64 + 32, *reinterpret_cast<uint32_t(*)[32]>(&r[32]));
-        ptx::tmem_ld_wait();
-        if (box == 1) {
-          ptx::tc_fence_before();
-          __syncwarp();
-          if (lane == 0) ptx::mbar_arrive_cluster(tempty_remote + 8u * buf);
-        }
-        const int col = c * kChunkN + h * 128 + box * 64;
-        const float4* b4 = reinterpret_cast<const float4*>(bias + col);
-        #pragma unroll
-        for (int i = 0; i < 16; ++i) {
-          float4 bb = __ldg(b4 + i);
-          r[4 * i + 0] = __float_as_uint(fmaxf(__uint_as_float(r[4 * i + 0]) + bb.x, 0.0f));
-          r[4 * i + 1] = __float_as_uint(fmaxf(__uint_as_float(r[4 * i + 1]) + bb.y, 0.0f));
-          r[4 * i + 2] = __float_as_uint(fmaxf(__uint_as_float(r[4 * i + 2]) + bb.z, 0.0f));
-          r[4 * i + 3] = __float_as_uint(fmaxf(__uint_as_float(r[4 * i + 3]) + bb.w, 0.0f));
-        }
-        if (l < last_layer) {
-          if (lane == 0) ptx::bulk_wait_read<0>();
-          __syncwarp();
-          #pragma unroll
-          for (int j = 0; j < 8; ++j) {
-            uint4 pk;
-            __nv_bfloat162 t0 = __floats2bfloat162_rn(__uint_as_float(r[8 * j + 0]), __uint_as_float(r[8 * j + 1]));
-            __nv_bfloat162 t1 = __floats2bfloat162_rn(__uint_as_float(r[8 * j + 2]), __uint_as_float(r[8 * j + 3]));
-            __nv_bfloat162 t2 = __floats2bfloat162_rn(__uint_as_float(r[8 * j + 4]), __uint_as_float(r[8 * j + 5]));
-            __nv_bfloat162 t3 = __floats2bfloat162_rn(__uint_as_float(r[8 * j + 6]), __uint_as_float(r[8 * j + 7]));
-            pk.x = *reinterpret_cast<uint32_t*>(&t0); pk.y = *reinterpret_cast<uint32_t*>(&t1);
-            pk.z = *reinterpret_cast<uint32_t*>(&t2); pk.w = *reinterpret_cast<uint32_t*>(&t3);
-            ptx::st_shared_v4(stage + (uint32_t)lane * 128u + (uint32_t)((j ^ (lane & 7)) << 4), pk);
-          }
-          ptx::fence_proxy_async_smem();
-          __syncwarp();
-          if (lane == 0) {
-            ptx::tma_store_2d(smap, stage, col, t_row + q * 32);
-            ptx::bulk_commit();
-          }
-        } else {
-          const float4* w0 = reinterpret_cast<const float4*>(p.head_w + col);
-          #pragma unroll
-          for (int i = 0; i < 16; ++i) {
-            float4 ww = __ldg(w0 + i);
-            pc0 = fmaf(__uint_as_float(r[4 * i + 0]), ww.x, pc0); pc0 = fmaf(__uint_as_float(r[4 * i + 1]), ww.y, pc0);
-            pc0 = fmaf(__uint_as_float(r[4 * i + 2]), ww.z, pc0); pc0 = fmaf(__uint_as_float(r[4 * i + 3]), ww.w, pc0);
-          }
-          if (p.n_out == 2) {
-            const float4* w1 = reinterpret_cast<const float4*>(p.head_w + p.width + col);
-            #pragma unroll
-            for (int i = 0; i < 16; ++i) {
-              float4 ww = __ldg(w1 + i);
-              pc1 = fmaf(__uint_as_float(r[4 * i + 0]), ww.x, pc1); pc1 = fmaf(__uint_as_float(r[4 * i + 1]), ww.y, pc1);
-              pc1 = fmaf(__uint_as_float(r[4 * i + 2]), ww.z, pc1); pc1 = fmaf(__uint_as_float(r[4 * i + 3]), ww.w, pc1);
-            }
-          }
-        }
-      }
+      tc_epilogue_chunk(p, taddr, tempty_remote + 8u * buf, lane, bias, c * kChunkN + h * 128, l < last_layer, smap, t_row + q * 32,
+                        stage, 0, pc0, pc1);
       if (l == last_layer) zpart[((size_t)(t_row + row) * p.n_chunks + c) * 2 + h] = make_float2(pc0, pc1);
     }
     if (lane == 0) ptx::bulk_wait_read<0>();     // the staging boxes must outlive the bulk stores that read them

@@ -216,6 +216,9 @@ __global__ void __launch_bounds__(kThreads, 1) ddf_tc_res_kernel(const __grid_co
     } else {
       // the peer CTA's warp 1 relays "chunk in place here" to the leader, whose MMAs read both CTAs' operands
       uint32_t hphase = 0;
+#ifdef DDF_DEV
+      if (!(p.hint_st & 8))
+#endif
       for (int64_t tile = pid; tile < num_tiles; tile += num_pairs) {
         for (int l = 1; l < p.n_hidden; ++l) {
           int chunk = nc - 1;
@@ -269,6 +272,9 @@ __global__ void __launch_bounds__(kThreads, 1) ddf_tc_res_kernel(const __grid_co
           ptx::tc_fence_before();
           __syncwarp();
           if (lane == 0) ptx::mbar_arrive_cluster(tempty_remote + 8u * buf);       // accumulator read: back to the MMA warp
+#ifdef DDF_DEV
+          if (p.hint_st & 16) continue;                                    // timing experiment: no epilogue work at all
+#endif
           if (l < last_layer) {
             uint32_t w[32];
             #pragma unroll
@@ -360,13 +366,12 @@ __global__ void __launch_bounds__(kThreads, 1) ddf_tc_res_kernel(const __grid_co
       __align__(16) __nv_bfloat16 enc[128];
       #pragma unroll 1
       for (int k = 0; k < p.res_e16; ++k) enc[k] = __float2bfloat16_rn(0.0f);
+      float v[3], w[3];
+      load_ray_vec3(p.o, grow - lane, n, lane, v);                         // coalesced 16-byte loads, regrouped by shuffles
+      if (p.input_kind == 0) load_ray_vec3(p.d, grow - lane, n, lane, w);
       if (grow < n) {
-        float v[3] = { p.o[3 * grow], p.o[3 * grow + 1], p.o[3 * grow + 2] };
         encode_vec_bf16(v, p.Lo, enc);
-        if (p.input_kind == 0) {
-          float w[3] = { p.d[3 * grow], p.d[3 * grow + 1], p.d[3 * grow + 2] };
-          encode_vec_bf16(w, p.Ld, enc + 3 + 6 * p.Lo);
-        }
+        if (p.input_kind == 0) encode_vec_bf16(w, p.Ld, enc + 3 + 6 * p.Lo);
       }
       // gamma of the tile before is read until the skip layer's last chunk: one buffer, freed by that MMA's commit
       wait_bar<true>(gfree_bar, (uint32_t)((tile_local & 1) ^ 1), p.dbg, 0x2800);
