@@ -28,9 +28,13 @@ FLOP_PER_RAY = 23_403_520            # 2*(90*1280 + 6*1280^2 + 1370*1280 + 1280*
 METRIC = "DDF ray queries/s"
 UNIT = "Mrays/s"
 WORKLOAD = "configs[1]: paper-scale DDF (90-dim enc, 8x1280, skip@4, bf16), 2^20 camera rays 1024x1024"
-# dram__bytes_read.sum + dram__bytes_write.sum of ddf_tc_kernel<2> for one 2^20-ray launch, from
-# the ncu --set full capture summarised in profiles/r01_ncu_summary.md (None until captured)
-NCU_DRAM_TRAFFIC_BYTES = 18.22e9
+# dram__bytes_read.sum + dram__bytes_write.sum of ddf_tc_kernel for one 2^20-ray launch, from the ncu --set full capture
+# summarised in profiles/r02_ncu_summary.md (2.549 GB read + 13.746 GB written; captured on the tree of commit 0b630ce,
+# the last change to csrc/ddf_tc.cu - re-capture after every change to that file)
+NCU_DRAM_TRAFFIC_BYTES = 16.295e9
+# the same two counters for ddf_tc_res_kernel (activation-resident kernel, ddf_set_path 5): 48.98 MB read + 1.78 MB written,
+# profiles/r02_res_ncu_summary.md, same tree
+NCU_RES_DRAM_TRAFFIC_BYTES = 50.77e6
 
 
 def _peaks():
@@ -223,7 +227,7 @@ def run_gpu(args):
         "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 24 * n, "d2h_bytes_per_step": 8 * n},
         "gpu_launches": launches,
-        "roofline": {"bound": "tensor", "kernel": "ddf_tc_kernel<2>", "achieved": achieved, "peak": peaks["burst"],
+        "roofline": {"bound": "tensor", "kernel": "ddf_tc_kernel", "achieved": achieved, "peak": peaks["burst"],
                      "unit": "TFLOP/s", "frac": achieved / peaks["burst"], "traffic": NCU_DRAM_TRAFFIC_BYTES,
                      "frac_of_sustained_peak": achieved / peaks["sustained"], "peak_source": peaks["source"],
                      "kernel_ms": kern_avg, "kernel_share_of_step": kern_avg / statistics.mean(step_ms),
@@ -319,6 +323,13 @@ def run_config_results(ddf, torch, model, peaks, back_to_back=False):
                                       "frac_peak": evals * SDF_FLOP / (ms * 1e-3) / 1e12 / peaks["burst"], "ddf_speedup": ms / ddf_ms}
     ex["ddf_camera_2^20_ms"] = ddf_ms
     ddf.ddf_destroy(sdf)
+    # ---- the same camera batch on the activation-resident kernel (ddf_set_path 5): no activation leaves the SM pair
+    ddf.ddf_set_path(model, 5)
+    res_ms = _time_ms(torch, lambda: ddf.ddf_query(model, o, d, n, dist, vis), reps=5)
+    ddf.ddf_set_path(model, 0)
+    ex["resident_kernel_camera_2^20"] = {"ms": res_ms, "Mrays_s": n / res_ms / 1e3, "TFLOPs": tf(n, res_ms), "frac_peak": tf(n, res_ms) / peaks["burst"],
+                                         "vs_persistent_kernel": ddf_ms / res_ms, "dram_traffic_bytes_ncu": NCU_RES_DRAM_TRAFFIC_BYTES,
+                                         "persistent_kernel_dram_traffic_bytes_ncu": NCU_DRAM_TRAFFIC_BYTES}
     return ex
 
 
