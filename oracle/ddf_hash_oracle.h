@@ -108,7 +108,10 @@ void orc_adam_step(float* p, const double* g, double* m, double* v, int64_t n, i
 double orc_solid_scene_raycast(const double o[3], const double d[3], const double sphere_c[3],
                                double sphere_r, const double bmin[3], const double bmax[3]);
 
-/* one training batch, reading T6 (ddf.h ddf_gen_train_batch): counters (step n + k) 16 + j */
+/* one training batch, reading T6 (ddf.h ddf_gen_train_batch): counters (step n + k) 16 + j.
+ * Pinned by tests/test_train_oracle_pins.py::test_train_batch_generator_pins: the draws recomputed
+ * with the numpy counter generator say which rays must be anchored / shifted; geometry judged by implicit surface
+ * functions and brute-force sampling along the ray. */
 void orc_gen_train_batch(const double sphere_c[3], double sphere_r, const double bmin[3], const double bmax[3],
                          uint64_t seed, uint64_t stream, int64_t step, int64_t n, double sample_half,
                          float* o, float* d, float* t, uint8_t* hit);
