@@ -121,10 +121,18 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * per, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": WORKLOAD, "note": "CPU oracle (oracle/ddf_oracle.c), each step a bounded sample"},
-        "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "config": config_dict(int(os.environ.get("WORLD_SIZE", "1"))),
+        "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
+                         "sample": sample + " per step (CPU oracle, oracle/ddf_oracle.c, as it stands)"},
         "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0}))
+
+
+def config_dict(world):
+    """The workload both arms of the bench are quoted on (the reference arm times a bounded sample of it per step)."""
+    return {"workload": WORKLOAD, "rays_per_gpu": 1 << 20, "parallelism": "replicas x%d, rays sharded" % world,
+            "flop_per_ray": FLOP_PER_RAY, "l2": "512 MB memset between timed steps (L2 flush)",
+            "step": "ddf_gen_camera + ddf_query"}
 
 
 def shard_plan(world, rank, rays_per_gpu):
@@ -221,9 +229,7 @@ def run_gpu(args):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": t_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "bf16", "data": "synthetic",
-        "config": {"workload": WORKLOAD, "rays_per_gpu": n, "parallelism": "replicas x%d, rays sharded" % world,
-                   "flop_per_ray": FLOP_PER_RAY, "l2": "512 MB memset between timed steps (L2 flush)",
-                   "step": "ddf_gen_camera + ddf_query"},
+        "config": config_dict(world),
         "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 24 * n, "d2h_bytes_per_step": 8 * n},
         "gpu_launches": launches,
