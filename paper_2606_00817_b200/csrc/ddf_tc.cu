@@ -794,9 +794,6 @@ int tc_forward(Model* m, const float* o, const float* d, int64_t n, const int64_
   // small batches: split the output columns of a layer over the CTA pairs (ddf_set_path 3 / 4 pin the choice)
   const int64_t split_max = (m->path == 3 || m->path == 5) ? 0 : (m->path == 4 ? t->grid / 2 : kSplitAutoTiles);
   if (tiles <= split_max) return tc_forward_split(m, p, tiles, st);
-#ifdef DDF_DEV
-  if (const char* e = getenv("DDF_DEV_RES")) p.hint_st = atoi(e);
-#endif
   if (m->path == 5 && t->res_ok) {
     // activation-resident kernel: tiles of 128 rays per CTA pair, same equal-tiles grid rule
     const int64_t rtiles = (n + 2 * kResRays - 1) / (2 * kResRays);
@@ -819,10 +816,6 @@ int tc_forward(Model* m, const float* o, const float* d, int64_t n, const int64_
   const int64_t units = t->grid / t->cg;
   const int64_t waves = (tiles + units - 1) / units;
   int grid = (int)((tiles + waves - 1) / waves) * t->cg;  // <= t->grid; n_dev can only shrink n
-#ifdef DDF_DEV
-  if (const char* e = getenv("DDF_DEV_GRID")) { int g = atoi(e); if (g >= 2 && g < grid) grid = g & ~1; }
-  if (const char* e = getenv("DDF_DEV_HINTS")) { int h = atoi(e); p.hint_act = h % 10; p.hint_w = (h / 10) % 10; p.hint_st = (h / 100) % 10; }
-#endif
   cudaLaunchConfig_t cfg;
   memset(&cfg, 0, sizeof(cfg));
   cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3(kThreads); cfg.stream = st;

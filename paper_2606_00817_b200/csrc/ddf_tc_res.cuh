@@ -192,9 +192,6 @@ __global__ void __launch_bounds__(kThreads, 1) ddf_tc_res_kernel(const __grid_co
             } else {
               int chunk = nc - 1;
               for (int cj = 0; cj < nc; ++cj) {
-#ifdef DDF_DEV
-                if (c == 0 && (p.hint_st & 8)) { hphase ^= (1u << chunk); } else       // timing experiment: ignore the hand-over
-#endif
                 if (c == 0) {
                   wait_bar<true>(hready_bar(chunk), (hphase >> chunk) & 1u, p.dbg, 0x2200 + chunk);
                   wait_bar<true>(pready_bar(chunk), (hphase >> chunk) & 1u, p.dbg, 0x2900 + chunk);
@@ -216,9 +213,6 @@ __global__ void __launch_bounds__(kThreads, 1) ddf_tc_res_kernel(const __grid_co
     } else {
       // the peer CTA's warp 1 relays "chunk in place here" to the leader, whose MMAs read both CTAs' operands
       uint32_t hphase = 0;
-#ifdef DDF_DEV
-      if (!(p.hint_st & 8))
-#endif
       for (int64_t tile = pid; tile < num_tiles; tile += num_pairs) {
         for (int l = 1; l < p.n_hidden; ++l) {
           int chunk = nc - 1;
@@ -272,9 +266,6 @@ __global__ void __launch_bounds__(kThreads, 1) ddf_tc_res_kernel(const __grid_co
           ptx::tc_fence_before();
           __syncwarp();
           if (lane == 0) ptx::mbar_arrive_cluster(tempty_remote + 8u * buf);       // accumulator read: back to the MMA warp
-#ifdef DDF_DEV
-          if (p.hint_st & 16) continue;                                    // timing experiment: no epilogue work at all
-#endif
           if (l < last_layer) {
             uint32_t w[32];
             #pragma unroll
