@@ -302,11 +302,13 @@ def run_config_results(ddf, torch, model, peaks, back_to_back=False):
         m = 1 << lg
         ms = _time_ms(torch, lambda: ddf.ddf_query(model, o, d, m, dist, vis), reps=3 if lg > 20 else 7)
         sweep["2^%d" % lg] = {"ms": ms, "ns_per_ray": ms * 1e6 / m, "Mrays_s": m / ms / 1e3, "frac_peak": tf(m, ms) / peaks["burst"]}
-        if back_to_back and lg <= 17:      # an isolated call on an idle stream above; here the per-call time of calls queued back to back
-            nb = 50 if lg <= 14 else 16
+        if lg <= 17:      # an isolated call on an idle stream above (latency); here the per-call time of calls queued back to back (throughput)
+            nb = (50 if lg <= 14 else 16) if back_to_back else (20 if lg <= 14 else 8)
             def burst():
                 for _ in range(nb): ddf.ddf_query(model, o, d, m, dist, vis)
-            sweep["2^%d" % lg]["ms_back_to_back"] = _time_ms(torch, burst, reps=3) / nb
+            bb = _time_ms(torch, burst, reps=3) / nb
+            sweep["2^%d" % lg]["ms_back_to_back"] = bb
+            sweep["2^%d" % lg]["frac_peak_back_to_back"] = tf(m, bb) / peaks["burst"]
     ex["sweep"] = sweep
     del o, d, dist, vis, ao
     # ---- configs[4]: sphere tracing an SDF MLP of the same width and depth on the camera rays
