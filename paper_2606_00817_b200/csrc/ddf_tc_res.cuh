@@ -75,6 +75,9 @@ __global__ void __launch_bounds__(kThreads, 1) ddf_tc_res_kernel(const __grid_co
   auto hready_bar = [&](int j) { return bar + 8u * (20 + j); };
   auto pready_bar = [&](int j) { return bar + 8u * (33 + j); };        // leader only: chunk j is in place in the peer CTA too
   const uint32_t gready_bar = bar + 8u * 28, gfree_bar = bar + 8u * 29, zready_bar = bar + 8u * 30;
+  // rows of input chunk j are dead: the layer's LAST output chunk (every other one finished before it started) has
+  // completed its MMAs over them (tcgen05.commit, both CTAs)
+  auto hdead_bar = [&](int j) { return bar + 8u * (41 + j); };
   const uint32_t tmem_slot = bar + 8u * 32;
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -90,7 +93,7 @@ __global__ void __launch_bounds__(kThreads, 1) ddf_tc_res_kernel(const __grid_co
   if (threadIdx.x == 0) {
     for (int s = 0; s < S; ++s) { ptx::mbar_init(full_bar(s), 1); ptx::mbar_init(empty_bar(s), 1); }
     for (int b = 0; b < 2; ++b) { ptx::mbar_init(tfull_bar(b), 1); ptx::mbar_init(tempty_bar(b), 16); }
-    for (int j = 0; j < kMaxChunks; ++j) { ptx::mbar_init(hready_bar(j), 4); ptx::mbar_init(pready_bar(j), 1); }
+    for (int j = 0; j < kMaxChunks; ++j) { ptx::mbar_init(hready_bar(j), 4); ptx::mbar_init(pready_bar(j), 1); ptx::mbar_init(hdead_bar(j), 1); }
     ptx::mbar_init(gready_bar, 4); ptx::mbar_init(gfree_bar, 1); ptx::mbar_init(zready_bar, 8);
     ptx::fence_mbar_init();
   }
@@ -128,13 +131,8 @@ __global__ void __launch_bounds__(kThreads, 1) ddf_tc_res_kernel(const __grid_co
         for (int c = 0; c < nc; ++c) {
           const int wrow = c * kChunkN + (int)rank * 128;
           for (int g = 0; g < ng; ++g) load(&p.w[l], gcol0 + g * kKBlock, wrow);
-          if (l > 0) {
-            int chunk = nc - 1;
-            for (int cj = 0; cj < nc; ++cj) {
-              for (int b = 0; b < 4; ++b) load(&p.w[l], (chunk * 4 + b) * kKBlock, wrow);
-              if (++chunk == nc) chunk = 0;
-            }
-          }
+          if (l > 0)
+            for (int kb = 0; kb < 4 * nc; ++kb) load(&p.w[l], kb * kKBlock, wrow);
         }
       }
     }
@@ -190,8 +188,10 @@ __global__ void __launch_bounds__(kThreads, 1) ddf_tc_res_kernel(const __grid_co
               if (gamma_layer == 0 && last_c && ptx::elect_one()) ptx::umma_commit<2>(gfree_bar);
               __syncwarp();
             } else {
-              int chunk = nc - 1;
-              for (int cj = 0; cj < nc; ++cj) {
+              // the layer's last output chunk frees the input rows chunk by chunk as it walks K: the parked output
+              // chunks are copied over them while it is still running (no hand-over at the layer's end to wait for)
+              const bool frees = last_c && l < last_layer;
+              for (int chunk = 0; chunk < nc; ++chunk) {
                 if (c == 0) {
                   wait_bar<true>(hready_bar(chunk), (hphase >> chunk) & 1u, p.dbg, 0x2200 + chunk);
                   wait_bar<true>(pready_bar(chunk), (hphase >> chunk) & 1u, p.dbg, 0x2900 + chunk);
@@ -202,9 +202,8 @@ __global__ void __launch_bounds__(kThreads, 1) ddf_tc_res_kernel(const __grid_co
                 const uint64_t hd = hdesc0 + (uint64_t)((uint32_t)chunk * (4u * kKBlock * 128u >> 4));
                 #pragma unroll
                 for (int b = 0; b < 4; ++b)
-                  issue(d_tmem, hd + (uint64_t)((uint32_t)b * (kKBlock * 128u >> 4)), 4, ng == 0 && cj == 0 && b == 0,
-                        (cj == nc - 1 && b == 3) ? tfull_bar(buf) : 0u);
-                if (++chunk == nc) chunk = 0;
+                  issue(d_tmem, hd + (uint64_t)((uint32_t)b * (kKBlock * 128u >> 4)), 4, ng == 0 && chunk == 0 && b == 0,
+                        b < 3 ? 0u : (chunk == nc - 1 ? tfull_bar(buf) : (frees ? hdead_bar(chunk) : 0u)));
               }
             }
           }
@@ -215,14 +214,12 @@ __global__ void __launch_bounds__(kThreads, 1) ddf_tc_res_kernel(const __grid_co
       uint32_t hphase = 0;
       for (int64_t tile = pid; tile < num_tiles; tile += num_pairs) {
         for (int l = 1; l < p.n_hidden; ++l) {
-          int chunk = nc - 1;
-          for (int cj = 0; cj < nc; ++cj) {
+          for (int chunk = 0; chunk < nc; ++chunk) {
             wait_bar<true>(hready_bar(chunk), (hphase >> chunk) & 1u, p.dbg, 0x2a00 + chunk);
             hphase ^= (1u << chunk);
             ptx::fence_proxy_async_smem();
             __syncwarp();
             if (lane == 0) ptx::mbar_arrive_cluster(ptx::mapa(pready_bar(chunk), 0));
-            if (++chunk == nc) chunk = 0;
           }
         }
       }
@@ -246,7 +243,7 @@ __global__ void __launch_bounds__(kThreads, 1) ddf_tc_res_kernel(const __grid_co
         if (lane == 0) { if (q == 0) ptx::mbar_arrive_expect_tx(hready_bar(j), 128u * 128u); else ptx::mbar_arrive(hready_bar(j)); }
       }
     };
-    uint32_t cc = 0;
+    uint32_t cc = 0, dphase = 0;
     int tile_local = 0;
     for (int64_t tile = pid; tile < num_tiles; tile += num_pairs, ++tile_local) {
       float za[4] = { 0.0f, 0.0f, 0.0f, 0.0f };                           // (z0, z1) of rays 2 lane, 2 lane + 1 of half h (last layer)
@@ -271,20 +268,27 @@ __global__ void __launch_bounds__(kThreads, 1) ddf_tc_res_kernel(const __grid_co
             #pragma unroll
             for (int i = 0; i < 32; ++i)
               w[i] = pack_bf16x2(fmaxf(__uint_as_float(r[2 * i]) + bf, 0.0f), fmaxf(__uint_as_float(r[2 * i + 1]) + bf, 0.0f));
-            if (c < nc - 1) {
-              ptx::tmem_st32(stash + (uint32_t)c * kResRays, w);          // park: the layer's input is still being read
-              ptx::tmem_st_wait();
-            } else {
-              // every MMA of the layer has completed: the input rows are dead in both CTAs
+            if (l == 0 || c == nc - 1) {
+              // layer 0 reads gamma, not H (whose rows the tile before has finished with); a last chunk's accumulator
+              // completes only when every MMA of the layer has: either way the rows are dead in both CTAs
               res_store_row(Hs, fg, w, local, (uint32_t)h, hready_peer + 8u * c);
               hand_over(c);
-              for (int j = 0; j < nc - 1; ++j) {
-                ptx::tmem_ld32(stash + (uint32_t)j * kResRays, w);
-                ptx::tmem_ld_wait();
-                res_store_row(Hs, j * kChunkN + (int)rank * 128 + fl, w, local, (uint32_t)h, hready_peer + 8u * j);
-                hand_over(j);
+            } else {
+              ptx::tmem_st32(stash + (uint32_t)c * kResRays, w);          // park: the layer's input is still being read
+              ptx::tmem_st_wait();
+              if (c == nc - 2) {
+                // the last chunk is now walking K and frees the input chunk by chunk: copy the parked chunks over it
+                for (int j = 0; j < nc - 1; ++j) {
+                  wait_bar<true>(hdead_bar(j), (dphase >> j) & 1u, p.dbg, 0x2b00 + j);
+                  dphase ^= (1u << j);
+                  ptx::tc_fence_after();
+                  ptx::tmem_ld32(stash + (uint32_t)j * kResRays, w);
+                  ptx::tmem_ld_wait();
+                  res_store_row(Hs, j * kChunkN + (int)rank * 128 + fl, w, local, (uint32_t)h, hready_peer + 8u * j);
+                  hand_over(j);
+                }
+                ptx::tc_fence_before();
               }
-              ptx::tc_fence_before();
             }
           } else {
             // heads: this warp's 32 features x 64 rays -> per-ray partial sums, lane L ends with rays 2L, 2L+1
