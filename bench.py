@@ -32,9 +32,9 @@ WORKLOAD = "configs[1]: paper-scale DDF (90-dim enc, 8x1280, skip@4, bf16), 2^20
 # summarised in profiles/r02_ncu_summary.md (2.549 GB read + 13.746 GB written; captured on the tree of commit 0b630ce,
 # the last change to csrc/ddf_tc.cu - re-capture after every change to that file)
 NCU_DRAM_TRAFFIC_BYTES = 16.295e9
-# the same two counters for ddf_tc_res_kernel (activation-resident kernel, ddf_set_path 5): 48.98 MB read + 1.78 MB written,
-# profiles/r02_res_ncu_summary.md, same tree
-NCU_RES_DRAM_TRAFFIC_BYTES = 50.77e6
+# the same two counters for ddf_tc_res_kernel (activation-resident kernel, ddf_set_path 5): 48.97 MB read + 1.70 MB written,
+# profiles/r02_res_ncu_summary.md (captured after the last change to csrc/ddf_tc_res.cuh)
+NCU_RES_DRAM_TRAFFIC_BYTES = 50.67e6
 
 
 def _peaks():
