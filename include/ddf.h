@@ -59,7 +59,8 @@ typedef enum ddf_status {
   DDF_E_BAD_LAYOUT  = -2,   /* ddf_layout fields inconsistent or struct_size/version wrong  */
   DDF_E_UNSUPPORTED = -3,   /* shape or device not supported by any kernel                  */
   DDF_E_CUDA        = -4,   /* a CUDA call failed; see ddf_last_cuda_error()                */
-  DDF_E_NOMEM       = -5    /* host or device allocation failed                             */
+  DDF_E_NOMEM       = -5,   /* host or device allocation failed                             */
+  DDF_E_TOO_LARGE   = -6    /* batch larger than the fixed capacity of a *_static entry point */
 } ddf_status;
 
 #define DDF_LAYOUT_VERSION 1u
@@ -248,6 +249,30 @@ int  ddf_gen_shadow_from_hits(ddf_model* model, const float* o, const float* d, 
                               const float* vis, int64_t n, const float light[3], float eps,
                               float* o2, float* d2, float* tmax, int32_t* index, int64_t* count,
                               void* stream);
+/* ddf_gen_shadow_from_hits for callers that must not allocate device memory.  Same inputs, same outputs, same
+ * bits as ddf_gen_shadow_from_hits (it launches the same three kernels), but it takes no model: the few numbers
+ * the compaction keeps between its launches (one int32 per 256 primary rays) sit in a fixed 256 KB array inside
+ * the library image instead of a cudaMalloc'ed workspace.  It is meant for hosts that gave all device memory to
+ * their own pool when they started (a renderer with a fixed budget, a training framework's caching allocator), so
+ * that a cudaMalloc made on the library's behalf would fail, and for frame loops that cannot take the device-wide
+ * stall of a cudaMalloc / cudaFree.  What to know before using it:
+ *  - n may be at most DDF_STATIC_MAX_RAYS (2^24 = 16,777,216); a larger n returns DDF_E_TOO_LARGE and nothing is
+ *    launched.  Split a larger batch and add the offsets yourself, or use ddf_gen_shadow_from_hits.
+ *  - The call itself never calls cudaMalloc, cudaFree or any library routine that allocates.  The array costs its
+ *    256 KB on every GPU on which the process loads libddf.so, from load until exit, used or not.
+ *  - The first call on each device looks the array's device address up (cudaGetSymbolAddress, with the caller's
+ *    current device; a failure comes back as DDF_E_CUDA) and keeps it.  Make that first call during start-up, on
+ *    the device you will use, before any stream capture is begun; later calls on that device only launch kernels.
+ *  - There is one array per device and every call on that device uses it.  Two calls whose kernels can be on the
+ *    GPU at the same time (different streams, or different host threads on different streams) overwrite each
+ *    other's numbers and return garbage: issue them on one stream, or order the streams with events.  Calls that
+ *    follow one another on a stream need no clearing in between - each call rewrites every entry it reads, so a
+ *    larger earlier batch leaves nothing behind that a smaller later one could pick up.
+ * All pointers [device] except light [host]; sizes and meaning as for ddf_gen_shadow_from_hits. */
+#define DDF_STATIC_MAX_RAYS 16777216
+int  ddf_gen_shadow_from_hits_static(const float* o, const float* d, const float* dist, const float* vis,
+                                     int64_t n, const float light[3], float eps, float* o2, float* d2,
+                                     float* tmax, int32_t* index, int64_t* count, void* stream);
 /* The whole loop in one call: primary query -> hit compaction -> shadow rays -> second query on
  * the compacted batch (its size never leaves the device on the tcgen05 and hash-grid paths) ->
  * lit[i] = 1 if ray i hit (vis > 0.5) and its shadow ray is NOT occluded (not (vis2 > 0.5 and

@@ -10,7 +10,7 @@ from .binding import (  # noqa: F401
     ddf_get_info, ddf_camera_from_seed, ddf_gen_camera, ddf_gen_sphere_points, ddf_gen_shadow,
     ddf_gen_gbuffer, ddf_gen_ao, ddf_ao_reduce, ddf_shadow_test, sdf_sphere_trace, ddf_status_string,
     DdfHashgridLayout, make_hashgrid_layout, ddf_hashgrid_table_entries, ddf_create_hashgrid,
-    ddf_gen_shadow_from_hits, ddf_query_shadowed, ddf_query_shadowed_lights, ddf_gen_ao_from_hits, ddf_query_ao_wavefront, ddf_query_shaded, ddf_query_ao_points,
+    ddf_gen_shadow_from_hits, ddf_gen_shadow_from_hits_static, STATIC_MAX_RAYS, ddf_query_shadowed, ddf_query_shadowed_lights, ddf_gen_ao_from_hits, ddf_query_ao_wavefront, ddf_query_shaded, ddf_query_ao_points,
     DdfTrainParams, make_train_params, Trainer, ddf_trainer_create, ddf_trainer_destroy, ddf_trainer_step,
     ddf_trainer_loss_grads, ddf_trainer_export, ddf_trainer_steps, ddf_scene_raycast, ddf_gen_train_batch,
     ddf_query_camera, ddf_reserve, RESERVE_HOST, RESERVE_RAYS, RESERVE_TRACE, RESERVE_WAVE, RESERVE_ALL,

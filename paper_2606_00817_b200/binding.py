@@ -20,6 +20,7 @@ EXPORTED_SYMBOLS = [
     "ddf_gen_ao_from_hits", "ddf_query_ao_wavefront", "ddf_query_shaded", "ddf_query_ao_points",
     "ddf_trainer_create", "ddf_trainer_destroy", "ddf_trainer_step", "ddf_trainer_loss_grads", "ddf_trainer_export",
     "ddf_trainer_steps", "ddf_scene_raycast", "ddf_gen_train_batch", "ddf_query_camera",
+    "ddf_gen_shadow_from_hits_static",
 ]
 
 
@@ -288,6 +289,21 @@ def ddf_gen_shadow_from_hits(model, o, d, dist, vis, n, light, eps, o2, d2, tmax
     _check(lib().ddf_gen_shadow_from_hits(model.handle, _dev(o), _dev(d), _dev(dist), _dev(vis), C.c_int64(n), li,
                                           C.c_float(eps), _dev(o2), _dev(d2), _dev(tmax), _dev(index, torch.int32),
                                           _dev(count, torch.int64), _stream(stream)), "ddf_gen_shadow_from_hits")
+
+
+STATIC_MAX_RAYS = 1 << 24
+
+
+def ddf_gen_shadow_from_hits_static(o, d, dist, vis, n, light, eps, o2, d2, tmax, index, count, stream=None):
+    """ddf_gen_shadow_from_hits without a model and without any device allocation: for programs whose own pool
+    already holds all device memory, or that cannot afford the stall of a cudaMalloc inside a frame.  The
+    compaction's scratch is a fixed array inside libddf.so, so n is limited to STATIC_MAX_RAYS (DdfError beyond it),
+    the first call on a device should be made at start-up, and calls must not overlap on the GPU (one stream, or
+    streams ordered by events).  Same results, bit for bit, as ddf_gen_shadow_from_hits."""
+    li = (C.c_float * 3)(*[float(x) for x in light])
+    _check(lib().ddf_gen_shadow_from_hits_static(_dev(o), _dev(d), _dev(dist), _dev(vis), C.c_int64(n), li,
+                                                 C.c_float(eps), _dev(o2), _dev(d2), _dev(tmax), _dev(index, torch.int32),
+                                                 _dev(count, torch.int64), _stream(stream)), "ddf_gen_shadow_from_hits_static")
 
 
 def ddf_query_shadowed(model, o, d, n, light, eps, out_dist, out_vis, out_lit, out_count=None, stream=None):

@@ -54,6 +54,7 @@ extern "C" const char* ddf_status_string(int s) {
     case DDF_E_UNSUPPORTED: return "unsupported layout or device";
     case DDF_E_CUDA: return "CUDA error";
     case DDF_E_NOMEM: return "out of memory";
+    case DDF_E_TOO_LARGE: return "batch exceeds the fixed capacity of this entry point";
     default: return "unknown status";
   }
 }

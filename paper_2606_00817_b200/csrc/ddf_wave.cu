@@ -4,6 +4,7 @@
 // batch is in increasing primary-ray order and reproducible; its size stays on the device and is
 // read by the query kernels themselves (n_dev), so the loop needs no host round trip.
 #include "ddf_common.cuh"
+#include <mutex>
 
 namespace ddf {
 
@@ -467,4 +468,63 @@ extern "C" int ddf_query_shaded(ddf_model* model, const float* o, const float* d
   }
   m->last_launches = launches;
   return DDF_OK;
+}
+
+// ---- ddf_gen_shadow_from_hits for hosts that cannot allocate device memory ---------------------
+// The compaction above needs one int32 per 256 primary rays between its three launches (how many hits each block
+// saw, then where each block's hits start).  Every other entry point keeps those numbers in a workspace that belongs
+// to a model and is obtained with cudaMalloc.  Some hosts cannot do that: a renderer or a training framework that
+// took the whole device for its own pool at start-up and has nothing left for the driver to hand out, or a frame
+// loop that cannot accept the device-wide stall a cudaMalloc / cudaFree brings.  For them the numbers live in the
+// array below, which is part of the library image: every GPU that loads libddf.so carries its 256 KB until the
+// process ends, whether or not this entry point is ever called.  65,536 entries cover DDF_STATIC_MAX_RAYS = 2^24
+// primary rays (configs[3]'s 1024 x 1024 x 16 batch).
+namespace ddf {
+
+constexpr int64_t kStaticMaxRays = DDF_STATIC_MAX_RAYS;
+constexpr int64_t kStaticBlocks = kStaticMaxRays / kWaveBlock;
+static_assert(kStaticBlocks * kWaveBlock == kStaticMaxRays, "the ray limit is a whole number of count blocks");
+
+static __device__ __align__(256) int32_t g_static_block_counts[kStaticBlocks];
+
+// In host code `g_static_block_counts` is only a handle the runtime knows the array by - handing it to a kernel as a
+// pointer would make the kernel read host memory or fault.  The address the kernels need is asked from the runtime,
+// once per device and with that device current, and remembered here.
+constexpr int kStaticMaxDevices = 64;
+static std::mutex g_static_mu;
+static int32_t* g_static_dev_ptr[kStaticMaxDevices];
+
+static int static_block_counts(int32_t** out) {
+  int dev = -1;
+  DDF_CUDA_TRY(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= kStaticMaxDevices) return DDF_E_UNSUPPORTED;
+  std::lock_guard<std::mutex> lock(g_static_mu);
+  if (!g_static_dev_ptr[dev]) {
+    void* p = nullptr;
+    DDF_CUDA_TRY(cudaGetSymbolAddress(&p, g_static_block_counts));
+    if (!p) return DDF_E_CUDA;
+    g_static_dev_ptr[dev] = static_cast<int32_t*>(p);
+  }
+  *out = g_static_dev_ptr[dev];
+  return DDF_OK;
+}
+
+}  // namespace ddf
+
+extern "C" int ddf_gen_shadow_from_hits_static(const float* o, const float* d, const float* dist, const float* vis,
+                                               int64_t n, const float light[3], float eps, float* o2, float* d2,
+                                               float* tmax, int32_t* index, int64_t* count, void* stream) {
+  if (!light || !count || n < 0) return DDF_E_INVALID_ARG;
+  if (n > kStaticMaxRays) return DDF_E_TOO_LARGE;
+  cudaStream_t st = (cudaStream_t)stream;
+  if (n == 0) { DDF_CUDA_TRY(cudaMemsetAsync(count, 0, 8, st)); return DDF_OK; }
+  if (!o || !d || !dist || !vis || !o2 || !d2 || !tmax || !index) return DDF_E_INVALID_ARG;
+  WaveWs w = {};
+  int rc = static_block_counts(&w.block_counts);
+  if (rc != DDF_OK) return rc;
+  // Nothing in the array has to be cleared between calls: the count launch writes every one of the ceil(n / 256)
+  // entries the scan and the scatter go on to read, and no launch reads past them, so whatever an earlier
+  // (possibly larger) batch left behind is never seen.
+  if ((rc = wave_count(w, vis, n, count, st)) != DDF_OK) return rc;
+  return wave_scatter(w, o, d, dist, vis, n, light, eps, o2, d2, tmax, index, st);
 }
