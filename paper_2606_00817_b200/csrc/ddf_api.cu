@@ -275,10 +275,14 @@ extern "C" int ddf_reserve(ddf_model* model, uint32_t what, int64_t max_rays, in
   if (max_rays == 0) return DDF_OK;
   if ((what & DDF_RESERVE_HOST) && (rc = host_reserve(m, max_rays)) != DDF_OK) return rc;
   if ((what & DDF_RESERVE_RAYS) && (rc = rays_reserve(m, max_rays)) != DDF_OK) return rc;
-  if ((what & DDF_RESERVE_RAYS) && !has_fused_path(m) && (rc = ao_out_reserve(m, max_rays)) != DDF_OK) return rc;
+  // ddf_query_ao keeps per-ray results (8 B per ray) whenever the reduce cannot be fused: no fused path, or an spp whose
+  // rays do not fill whole warp fractions
+  const bool ao_unfused = !has_fused_path(m) || (spp > 0 && (spp > 32 || 32 % spp != 0));
+  if ((what & DDF_RESERVE_RAYS) && ao_unfused && (rc = ao_out_reserve(m, max_rays)) != DDF_OK) return rc;
   if ((what & DDF_RESERVE_TRACE) && (rc = trace_reserve(m, max_rays, 4096)) != DDF_OK) return rc;
   if ((what & DDF_RESERVE_WAVE) && (rc = wave_reserve(m, max_rays, spp)) != DDF_OK) return rc;
-  if (!has_fused_path(m) && (rc = ensure_workspace(m, max_rays)) != DDF_OK) return rc;
+  // the CUDA-core path walks a batch in passes of kSimtChunkRows rays: that is all its workspace ever holds
+  if (!has_fused_path(m) && (rc = ensure_workspace(m, max_rays < kSimtChunkRows ? max_rays : kSimtChunkRows)) != DDF_OK) return rc;
   return DDF_OK;
 }
 

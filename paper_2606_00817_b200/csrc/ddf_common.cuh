@@ -77,6 +77,7 @@ struct Model {
 };
 
 // ---- SIMT path (ddf_simt.cu)
+constexpr int64_t kSimtChunkRows = 16384;   // rays per pass of simt_forward: the most rows its activation workspace ever holds
 int simt_forward(Model* m, const float* o, const float* d, int64_t n, int mode_out,
                  float* out0, float* out1, cudaStream_t st);
 int ensure_workspace(Model* m, int64_t rows);

@@ -130,7 +130,7 @@ int ensure_workspace(Model* m, int64_t rows) {
 
 int simt_forward(Model* m, const float* o, const float* d, int64_t n, int mode_out,
                  float* out0, float* out1, cudaStream_t st) {
-  const int64_t kChunk = 16384;
+  const int64_t kChunk = kSimtChunkRows;
   int rc = ensure_workspace(m, n < kChunk ? n : kChunk);
   if (rc != DDF_OK) return rc;
   const ddf_layout& L = m->lay;

@@ -467,3 +467,47 @@ def test_reserved_calls_do_not_allocate(ddf, c1, sdf):
     ddf.sdf_sphere_trace(sm, oc, dc, k, ddf.SdfTraceParams(8, 1e-3, 6.0, 1.0, 0.05, 1), t, hit, steps, None, None, None)
     torch.cuda.synchronize()
     assert torch.cuda.mem_get_info()[0] == free1
+
+
+def test_reserve_on_the_cuda_core_path_is_bounded_and_covers_queries_and_wavefront_calls(ddf):
+    """A model forced to the CUDA-core path answers a batch in passes of 16,384 rays, so ddf_reserve for 2^22 rays must
+    size its activation workspace for 16,384 rows (about 172 MB at width 1280), not for 2^22 (44 GB); after the
+    reservation a query larger than one pass and a wavefront call leave the free memory where it was.  ddf_query_ao
+    with an spp that does not divide 32 keeps per-ray results: RESERVE_RAYS with that spp covers them on a fused model."""
+    lay = layout_c1()
+    m = ddf.ddf_create(make_weights(lay), lay)
+    ddf.ddf_set_path(m, 1)
+    n = 40_000                                                   # three passes, the last one ragged
+    o, d = random_rays(n)
+    oc, dc = _cuda(o), _cuda(d)
+    dist = torch.empty(n, device="cuda"); vis = torch.empty(n, device="cuda")
+    lit = torch.empty(n, dtype=torch.uint8, device="cuda"); cnt = torch.zeros(1, dtype=torch.int64, device="cuda")
+    torch.cuda.synchronize()
+    free0 = torch.cuda.mem_get_info()[0]
+    ddf.ddf_reserve(m, ddf.RESERVE_WAVE, 1 << 22, 0)
+    torch.cuda.synchronize()
+    free1 = torch.cuda.mem_get_info()[0]
+    wave_bytes = 40 * (1 << 22)
+    assert free0 - free1 < wave_bytes + 256 * 1024 * 1024, (free0 - free1)      # 168 MB wavefront + ~172 MB activations
+    ddf.ddf_query(m, oc, dc, n, dist, vis)
+    ddf.ddf_query_shadowed(m, oc, dc, n, (3.0, 3.0, 3.0), 1e-3, dist, vis, lit, cnt)
+    torch.cuda.synchronize()
+    assert torch.cuda.mem_get_info()[0] == free1
+    assert 0 < int(cnt.item()) < n
+    # same bits as the fused kernel's batch-size-independent answer on the first pass boundary
+    ddf.ddf_set_path(m, 0)
+    d0 = torch.empty(n, device="cuda"); v0 = torch.empty(n, device="cuda")
+    ddf.ddf_query(m, oc, dc, n, d0, v0)
+    torch.cuda.synchronize()
+    assert float((d0 - dist).abs().max()) <= 1e-2 * (1 + float(d0.abs().max())) and float((v0 - vis).abs().max()) <= 1e-2
+    # fused model, spp = 12: the unfused reduce's per-ray results come from the reservation
+    n_pts, spp = 2_000, 12
+    ao = torch.empty(n_pts, device="cuda")
+    ddf.ddf_reserve(m, ddf.RESERVE_RAYS, n_pts * spp, spp)
+    torch.cuda.synchronize()
+    free2 = torch.cuda.mem_get_info()[0]
+    ddf.ddf_query_ao(m, oc[:n_pts * spp], dc[:n_pts * spp], n_pts, spp, 2.0, ao)
+    torch.cuda.synchronize()
+    assert torch.cuda.mem_get_info()[0] == free2
+    assert bool(((ao >= 0) & (ao <= 1)).all())
+    ddf.ddf_destroy(m)
