@@ -33,15 +33,20 @@
  *    in the batch, bit-reproducible run to run (training steps accumulate gradients with atomics
  *    and are reproducible to rounding only).  Directions must be unit length (not checked).
  *  - A model (and a trainer) owns device workspaces that its calls reuse: use one model from one
- *    stream / host thread at a time; different models are independent.  ddf_query, ddf_query_logits
- *    and ddf_query_ao never allocate (their workspace is sized at ddf_create).  The calls that need a
- *    per-batch workspace - ddf_query_host, ddf_query_camera / ddf_query_ao_points on models that read
- *    rays from memory, sdf_sphere_trace, the wavefront calls, and every query of a model served by the
- *    CUDA-core path - take it from ddf_reserve; without a reservation that covers the batch they size
+ *    stream / host thread at a time; different models are independent.  On a fused path ddf_query,
+ *    ddf_query_logits and ddf_query_ao with an spp that divides 32 never allocate (their workspace is sized
+ *    at ddf_create).  The calls that need a per-batch workspace - ddf_query_host, ddf_query_camera /
+ *    ddf_query_ao_points on models that read rays from memory, ddf_query_ao with any other spp,
+ *    sdf_sphere_trace, the wavefront calls, and every query of a model served by the CUDA-core path
+ *    (also one forced there by ddf_set_path(model, 1): reserve after that call) - take it from ddf_reserve; without a reservation that covers the batch they size
  *    it themselves on first use (a synchronising cudaFree / cudaMalloc).  Once the workspace covers
  *    the batch a call issues only stream-ordered work, so it can be recorded by
  *    stream capture and replayed as a CUDA graph (ddf_trainer_step bakes that step's learning
  *    rate into the capture; ddf_trainer_loss_grads and every query are replayable as they are).
+ *  - Every wait inside the tensor-core kernels is bounded: if a barrier is not reached within one minute of wall-clock
+ *    time (only a bug in the library, or a context frozen from outside for that long, can cause it) the kernel traps
+ *    instead of hanging the device.  A trap is a sticky CUDA error - the context is unusable afterwards and every call
+ *    returns DDF_E_CUDA; the process has to reset the device or exit.
  *  - There is no CPU fallback: without a CUDA device of compute capability 10.x the calls
  *    return DDF_E_UNSUPPORTED / DDF_E_CUDA.
  */
@@ -120,10 +125,12 @@ int  ddf_set_path(ddf_model* model, int path);
  * (SURVEY.md 8(b) "the library never allocates in ddf_query (workspace, if any, sized at create)").  `what` selects
  * which: DDF_RESERVE_HOST - staging of ddf_query_host (32 B per ray, plus its two copy streams and events);
  * DDF_RESERVE_RAYS - the ray buffer of ddf_query_camera / ddf_query_ao_points (24 B per ray; max_rays counts
- * width * height or n_pts * spp); DDF_RESERVE_TRACE - sdf_sphere_trace (25 B per ray); DDF_RESERVE_WAVE - the
+ * width * height or n_pts * spp), and, when the reduce of ddf_query_ao cannot be fused into the query (spp does not
+ * divide 32, or only the CUDA-core path serves the model), its per-ray results (8 B per ray); DDF_RESERVE_TRACE - sdf_sphere_trace (25 B per ray); DDF_RESERVE_WAVE - the
  * wavefront calls on max_rays primary rays, with room for spp ambient-occlusion rays per hit (40 B per primary ray,
  * or 32 + 24 spp if that is more; spp = 0: shadow calls only).  For a model only the CUDA-core path serves, the
- * activation workspace of its queries (rows = max_rays) is sized too, whatever `what` is.  Synchronises the device when
+ * activation workspace of its queries is sized too, whatever `what` is: that path answers a batch in passes of 16,384
+ * rays, so the workspace holds min(max_rays, 16,384) rows (about 2 E_pad + 8 width bytes each) however large the batch.  Synchronises the device when
  * it (re)allocates; reservations only grow.  max_rays == 0 is a no-op; unknown bits in `what`: DDF_E_INVALID_ARG. */
 #define DDF_RESERVE_HOST  1u
 #define DDF_RESERVE_RAYS  2u

@@ -89,7 +89,7 @@ __device__ __forceinline__ void wait_bar(uint32_t bar, uint32_t parity, uint32_t
     if ((++spins & 1023u) == 0) {
       uint64_t now = globaltimer_ns();
       if (t0 == 0) t0 = now;
-      else if (now - t0 > 4000000000ull) {
+      else if (now - t0 > ptx::kWaitTrapNs) {
         if (dbg && atomicCAS(dbg, 0u, code) == 0u) { dbg[1] = blockIdx.x; dbg[2] = parity; dbg[3] = threadIdx.x; __threadfence_system(); }
         __trap();
       }
@@ -741,7 +741,8 @@ int tc_plan_create(Model* m) {
   p.res_stages = 0;
   for (int s = kResMaxStages; s >= 2; --s)
     if (res_smem_bytes((int)L.width, p.res_e16, s) <= (size_t)TcCfg<2>::kSmemBytes) { p.res_stages = s; break; }
-  t->res_ok = p.res_stages >= 2 && L.width / kChunkN <= 5 && m->E_pad <= 128;
+  // two hidden layers at least: with one, nothing orders a tile's head partials (zbuf) before the next tile's writes
+  t->res_ok = p.res_stages >= 2 && L.width / kChunkN <= 5 && m->E_pad <= 128 && L.n_hidden >= 2;
   if (t->res_ok) {
     t->res_smem = res_smem_bytes((int)L.width, p.res_e16, p.res_stages);
     DDF_CUDA_TRY(cudaFuncSetAttribute(ddf_tc_res_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TcCfg<2>::kSmemBytes));

@@ -59,15 +59,21 @@ __device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
 // tcgen05.commit need no generic-proxy acquire beyond the default.
 __device__ __forceinline__ bool mbar_try_wait_cluster(uint32_t bar, uint32_t parity) { return mbar_try_wait(bar, parity); }
 
+// How long one mbarrier wait may last before the kernel traps.  %globaltimer is wall-clock time, so the bound has to
+// cover a correct kernel that is paused from outside - single-stepped in a debugger, replayed under a profiler or a
+// sanitizer, time-sliced with another context - and still turn a protocol slip into an error rather than a hung
+// device: one minute.  A trap is a sticky CUDA error: the context is lost and every later call returns DDF_E_CUDA.
+constexpr uint64_t kWaitTrapNs = 60ull * 1000000000ull;
+
 // Bounded wait for kernels without a debug word: a protocol slip becomes a trap (the next call returns DDF_E_CUDA)
-// after 4 s on %globaltimer instead of a hung device.
+// after kWaitTrapNs on %globaltimer instead of a hung device.
 __device__ __forceinline__ void mbar_wait_bounded(uint32_t bar, uint32_t parity) {
   uint32_t spins = 0; uint64_t t0 = 0;
   while (!mbar_try_wait(bar, parity)) {
     if ((++spins & 4095u) == 0) {
       uint64_t now; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(now));
       if (t0 == 0) t0 = now;
-      else if (now - t0 > 4000000000ull) asm volatile("trap;");
+      else if (now - t0 > kWaitTrapNs) asm volatile("trap;");
     }
   }
 }

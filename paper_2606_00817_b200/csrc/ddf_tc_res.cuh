@@ -10,12 +10,16 @@
 //   D          = fp32 in TMEM, 128 lanes (features) x 128 columns (rays of the pair), double buffered (256 columns)
 //
 // An output chunk (256 features of the pair) cannot overwrite the layer's input while later chunks still read it, so
-// the epilogue parks chunks 0 .. nc-2 as packed bf16 in the other 256 TMEM columns (tcgen05.st); the last chunk's
-// accumulator completes only when every MMA of the layer has, i.e. when the input is dead, and is written straight
-// into the input's rows; then the parked chunks are copied back (tcgen05.ld -> st.shared).  Each CTA computes half of
-// the features for ALL 128 rays but needs, as its next B operand, all features for ITS 64 rays: the other half of
-// every chunk crosses to the peer CTA through distributed shared memory.  The next layer walks K in the order the
-// rows become ready (last chunk, then 0 .. nc-2), gated per 256-row chunk by mbarriers.
+// the epilogue parks chunks 0 .. nc-2 as packed bf16 in the other 256 TMEM columns (tcgen05.st).  Every chunk walks K
+// in natural order (gamma blocks, then input chunks 0 .. nc-1); the layer's LAST output chunk commits to a per-chunk
+// "dead" barrier as it leaves each 256-row input chunk behind, and the epilogue copies parked chunk j back over input
+// chunk j (tcgen05.ld -> st.shared) as soon as that barrier fires - while the last chunk is still running.  The last
+// chunk's own accumulator completes only when every MMA of the layer has, and is written straight into its rows.
+// Layer 0 reads gamma, not H, so it writes every chunk directly.  Each CTA computes half of the features for ALL 128
+// rays but needs, as its next B operand, all features for ITS 64 rays: the other half of every chunk crosses to the
+// peer CTA through distributed shared memory.  The next layer's first output chunk waits per 256-row input chunk
+// (mbarriers) for both halves to be in place.  Needs at least two hidden layers: the layer-0 hand-over barriers are
+// what keeps a tile's head partials from being overwritten by the next tile (tc_plan_create checks).
 //
 //   warp 0      TMA producer (weights only)        warps 2-3   encoder: gamma of the next tile, registers -> smem
 //   warp 1      MMA issuer (leader CTA)            warps 4-11  epilogue: +bias, ReLU, bf16, park / hand over; heads
@@ -106,10 +110,10 @@ __global__ void __launch_bounds__(kThreads, 1) ddf_tc_res_kernel(const __grid_co
   uint32_t tmem_base;
   asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
 
-  // K-block order of a layer: the gamma blocks first (always in place), then the hidden blocks in the order their rows are
-  // handed over - the last output chunk of the layer before is written directly, chunks 0 .. nc-2 are copied back after
-  // it.  Producer and issuer walk it with counters only (no division: the issuer's loop must stay well under the
-  // 256 clocks its four MMAs of a stage take).
+  // K-block order of a layer: the gamma blocks first (always in place), then the hidden blocks in natural order, chunk 0
+  // .. nc-1; the first output chunk of a layer waits for each input chunk's hand-over as it reaches it.  Producer and
+  // issuer walk it with counters only (no division: the issuer's loop must stay well under the 256 clocks its four
+  // MMAs of a stage take).
   if (warp == 0) {
     // ================================================================ TMA producer: this CTA's 128 feature rows of each weight tile
     const uint64_t pol_w = ptx::policy_evict_last();
