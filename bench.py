@@ -28,13 +28,43 @@ FLOP_PER_RAY = 23_403_520            # 2*(90*1280 + 6*1280^2 + 1370*1280 + 1280*
 METRIC = "DDF ray queries/s"
 UNIT = "Mrays/s"
 WORKLOAD = "configs[1]: paper-scale DDF (90-dim enc, 8x1280, skip@4, bf16), 2^20 camera rays 1024x1024"
-# dram__bytes_read.sum + dram__bytes_write.sum of ddf_tc_kernel for one 2^20-ray launch, from the ncu --set full capture
-# summarised in profiles/r02_ncu_summary.md (2.549 GB read + 13.746 GB written; captured on the tree of commit 0b630ce,
-# the last change to csrc/ddf_tc.cu - re-capture after every change to that file)
-NCU_DRAM_TRAFFIC_BYTES = 16.295e9
-# the same two counters for ddf_tc_res_kernel (activation-resident kernel, ddf_set_path 5): 48.97 MB read + 1.70 MB written,
-# profiles/r02_res_ncu_summary.md (captured after the last change to csrc/ddf_tc_res.cuh)
-NCU_RES_DRAM_TRAFFIC_BYTES = 50.67e6
+# dram__bytes_read.sum / dram__bytes_write.sum of one 2^20-ray launch of each dense kernel, from an `ncu --set full` capture:
+# kept in a small text file that names its capture command and is rewritten by `bench.py --write-traffic` (below), so
+# the `traffic` figures of the bench line always come from a committed artifact, never from a number typed in here.
+TRAFFIC_FILE = os.path.join(ROOT, "profiles", "r03_dram_bytes.txt")
+
+
+def ncu_traffic():
+    """kernel name -> DRAM bytes (read + written) per launch; a kernel the file does not list reports null."""
+    out = {}
+    if os.path.exists(TRAFFIC_FILE):
+        for line in open(TRAFFIC_FILE):
+            f = line.split()
+            if len(f) >= 3 and not line.startswith("#"):
+                out[f[0]] = float(f[1]) + float(f[2])
+    return out
+
+
+def write_traffic(csv_paths, head):
+    """`ncu -i X.ncu-rep --page raw --csv --print-units base > X.csv` of the capture(s) -> profiles/r03_dram_bytes.txt."""
+    import csv
+    scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
+    rows = {}
+    for path in csv_paths:
+        table = [r for r in csv.reader(open(path)) if r]
+        hdr = next(i for i, r in enumerate(table) if "Kernel Name" in r)
+        names, units = table[hdr], table[hdr + 1]
+        ik, ir, iw = names.index("Kernel Name"), names.index("dram__bytes_read.sum"), names.index("dram__bytes_write.sum")
+        for r in table[hdr + 2:]:
+            kernel = r[ik].split("(")[0].split("::")[-1]
+            rows[kernel] = (float(r[ir].replace(",", "")) * scale[units[ir]], float(r[iw].replace(",", "")) * scale[units[iw]])
+    with open(TRAFFIC_FILE, "w") as f:
+        f.write("# DRAM bytes of ONE launch on 2^20 configs[1] camera rays: kernel, dram__bytes_read.sum, dram__bytes_write.sum\n")
+        f.write("# tree: %s; capture commands and the rest of the counters: profiles/r03_ncu_summary.md; written by\n" % head)
+        f.write("# python bench.py --write-traffic %s\n" % " ".join(csv_paths))
+        for k in sorted(rows):
+            f.write("%s %.0f %.0f\n" % (k, rows[k][0], rows[k][1]))
+    print(open(TRAFFIC_FILE).read())
 
 
 def _peaks():
@@ -188,23 +218,25 @@ def run_gpu(args):
         ddf.ddf_query(model, o, d, n, dist_o, vis_o)
         if ev: ev[2].record()
 
-    for _ in range(W):
-        flush.zero_(); step()
-    torch.cuda.synchronize()
-    if world > 1: dist.barrier()
-    torch.cuda.synchronize()
-    sampler = ClockSampler(local); sampler.start(); t_wall0 = time.time()
-    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(K)]
-    for k in range(K):
-        flush.zero_()                       # L2 flush between timed iterations (outside the event pairs)
-        step(evs[k])
-    torch.cuda.synchronize()
-    if world > 1: dist.barrier()
-    torch.cuda.synchronize()
-    t_wall1 = time.time()
-    clocks = sampler.stop(t_wall0, t_wall1)
-    step_ms = [e[0].elapsed_time(e[2]) for e in evs]
-    kern_ms = [e[1].elapsed_time(e[2]) for e in evs]
+    def timed_region():
+        """W warm-up steps, then K timed steps with an L2 flush between them, clocks sampled alongside"""
+        for _ in range(W):
+            flush.zero_(); step()
+        torch.cuda.synchronize()
+        if world > 1: dist.barrier()
+        torch.cuda.synchronize()
+        sampler = ClockSampler(local); sampler.start(); t_wall0 = time.time()
+        evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(K)]
+        for k in range(K):
+            flush.zero_()                       # L2 flush between timed iterations (outside the event pairs)
+            step(evs[k])
+        torch.cuda.synchronize()
+        if world > 1: dist.barrier()
+        torch.cuda.synchronize()
+        t_wall1 = time.time()
+        return ([e[0].elapsed_time(e[2]) for e in evs], [e[1].elapsed_time(e[2]) for e in evs], sampler.stop(t_wall0, t_wall1))
+
+    step_ms, kern_ms, clocks = timed_region()
     value, t_max = aggregate(sum(step_ms), n * K, dist, world)
     launches = K * 2                        # gen_camera_kernel + ddf_tc_kernel per step
 
@@ -222,9 +254,17 @@ def run_gpu(args):
     e2e_value, _ = aggregate(e2e_ms, n * K, dist, world)
     assert torch.equal(dist_h, dist_o.cpu())
 
+    # ---- the activation-resident kernel (ddf_set_path 5) under the SAME protocol: K flushed steps, sustained clocks
+    ddf.ddf_set_path(model, 5)
+    _, res_kern_ms, res_clocks = timed_region()
+    ddf.ddf_set_path(model, 0)
+
     peaks = _peaks()
+    traffic = ncu_traffic()
     kern_avg = statistics.mean(kern_ms)
     achieved = n * FLOP_PER_RAY / (kern_avg * 1e-3) / 1e12
+    res_avg = statistics.mean(res_kern_ms)
+    res_achieved = n * FLOP_PER_RAY / (res_avg * 1e-3) / 1e12
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": t_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -234,10 +274,14 @@ def run_gpu(args):
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 24 * n, "d2h_bytes_per_step": 8 * n},
         "gpu_launches": launches,
         "roofline": {"bound": "tensor", "kernel": "ddf_tc_kernel", "achieved": achieved, "peak": peaks["burst"],
-                     "unit": "TFLOP/s", "frac": achieved / peaks["burst"], "traffic": NCU_DRAM_TRAFFIC_BYTES,
+                     "unit": "TFLOP/s", "frac": achieved / peaks["burst"], "traffic": traffic.get("ddf_tc_kernel"),
                      "frac_of_sustained_peak": achieved / peaks["sustained"], "peak_source": peaks["source"],
                      "kernel_ms": kern_avg, "kernel_share_of_step": kern_avg / statistics.mean(step_ms),
-                     "ray_io_GBps": 32 * n / (kern_avg * 1e-3) / 1e9},
+                     "ray_io_GBps": 32 * n / (kern_avg * 1e-3) / 1e9,
+                     # the kernel that keeps every activation on chip, same steps, same flush, same peak
+                     "resident": {"kernel": "ddf_tc_res_kernel", "kernel_ms": res_avg, "achieved": res_achieved,
+                                  "frac": res_achieved / peaks["burst"], "traffic": traffic.get("ddf_tc_res_kernel"),
+                                  "vs_persistent": kern_avg / res_avg, "sm_mhz": res_clocks.get("sm_mhz")}},
     }
     if rank == 0:
         if world == 1:
@@ -246,12 +290,43 @@ def run_gpu(args):
         if world == 1:
             # BASELINE.json configs[2], [3], [4] in the same line (the metric is quoted "at 2^20-2^24 rays"; north_star
             # asks for the shadow / AO batches and the DDF / sphere-tracing ratio): outside the headline's timed region
-            out["config_results"] = run_config_results(ddf, torch, model, peaks, back_to_back=args.extras)
+            full = run_config_results(ddf, torch, model, peaks, back_to_back=args.extras)
+            out["config_results"] = full if args.extras else compact_config_results(full)
         if args.extras and world == 1:
             out["extra"] = run_extras(ddf, torch, model, peaks)
-        print(json.dumps(out))
+        print(json.dumps(out if args.extras else sig(out)))
     if world > 1:
         dist.destroy_process_group()
+
+
+def sig(x, digits=5):
+    """every float of a nested result rounded to `digits` significant digits: the default line has to stay short enough
+    for the driver's record to keep all of it"""
+    if isinstance(x, float):
+        return float("%.*g" % (digits, x)) if x == x and abs(x) != float("inf") else x
+    if isinstance(x, dict):
+        return {k: sig(v, digits) for k, v in x.items()}
+    if isinstance(x, (list, tuple)):
+        return [sig(v, digits) for v in x]
+    return x
+
+
+def compact_config_results(ex):
+    """The default line's copy of run_config_results: what north_star asks to be reported (camera, shadow and AO batches,
+    the 2^10 .. 2^24 sweep, sphere tracing in both modes and across thresholds) without the derived fields, which follow
+    from ms, the ray count and FLOP_PER_RAY.  --extras prints the long form."""
+    sw = ex["sweep"]
+    lgs = range(10, 25)
+    st = {k[len("sphere_trace_"):]: v for k, v in ex.items() if k.startswith("sphere_trace_")}
+    return sig({
+        "Mrays_s": {"camera_2^20": (1 << 20) / ex["ddf_camera_2^20_ms"] / 1e3, "shadow_2^22": ex["shadow_2^22"]["Mrays_s"],
+                    "ao_16.7M": ex["ao_16.7M"]["Mrays_s"]},
+        "gen_ms": {"shadow_2^22": ex["shadow_2^22"]["gen_ms"], "ao_16.7M": ex["ao_16.7M"]["gen_ms"]},
+        "sweep_ms_2^10..2^24": [sw["2^%d" % lg]["ms"] for lg in lgs],
+        "sweep_ms_back_to_back_2^10..2^17": [sw["2^%d" % lg]["ms_back_to_back"] for lg in range(10, 18)],
+        # [ms, MLP evaluations, DDF speed-up] per tracer mode / hit threshold
+        "sphere_trace_ms_evals_ddfx": {k: [v["ms"], v["mlp_evals"], v["ddf_speedup"]] for k, v in st.items()},
+    }, 4)
 
 
 def _time_ms(torch, fn, reps=3, warm=1):
@@ -329,6 +404,12 @@ def run_config_results(ddf, torch, model, peaks, back_to_back=False):
         ex["sphere_trace_" + name] = {"ms": ms, "Mrays_s": n / ms / 1e3, "mlp_evals": evals, "mean_steps": float(st.float().mean()),
                                       "hit_rate": float(hit.float().mean()), "TFLOPs": evals * SDF_FLOP / (ms * 1e-3) / 1e12,
                                       "frac_peak": evals * SDF_FLOP / (ms * 1e-3) / 1e12 / peaks["burst"], "ddf_speedup": ms / ddf_ms}
+    # "across convergence thresholds": the early-exit tracer at two more hit thresholds
+    for eps in (1e-2, 1e-4):
+        prm = ddf.SdfTraceParams(64, eps, 6.0, 1.0, 0.05, 1)
+        ms = _time_ms(torch, lambda: ddf.sdf_sphere_trace(sdf, o, d, n, prm, t, hit, st, None, None, tot), reps=2)
+        ex["sphere_trace_early_exit_eps%g" % eps] = {"ms": ms, "mlp_evals": int(tot.item()), "mean_steps": float(st.float().mean()),
+                                                     "hit_rate": float(hit.float().mean()), "ddf_speedup": ms / ddf_ms}
     ex["ddf_camera_2^20_ms"] = ddf_ms
     ddf.ddf_destroy(sdf)
     # ---- the same camera batch on the activation-resident kernel (ddf_set_path 5): no activation leaves the SM pair
@@ -336,33 +417,15 @@ def run_config_results(ddf, torch, model, peaks, back_to_back=False):
     res_ms = _time_ms(torch, lambda: ddf.ddf_query(model, o, d, n, dist, vis), reps=5)
     ddf.ddf_set_path(model, 0)
     ex["resident_kernel_camera_2^20"] = {"ms": res_ms, "Mrays_s": n / res_ms / 1e3, "TFLOPs": tf(n, res_ms), "frac_peak": tf(n, res_ms) / peaks["burst"],
-                                         "vs_persistent_kernel": ddf_ms / res_ms, "dram_traffic_bytes_ncu": NCU_RES_DRAM_TRAFFIC_BYTES,
-                                         "persistent_kernel_dram_traffic_bytes_ncu": NCU_DRAM_TRAFFIC_BYTES}
+                                         "vs_persistent_kernel": ddf_ms / res_ms, "dram_traffic_bytes_ncu": ncu_traffic().get("ddf_tc_res_kernel"),
+                                         "persistent_kernel_dram_traffic_bytes_ncu": ncu_traffic().get("ddf_tc_kernel")}
     return ex
 
 
 def run_extras(ddf, torch, model, peaks):
-    """--extras: the sphere tracer's eps sweep and the SURVEY.md 8(f) rows (hash-grid field, wavefront, training, narrow networks)."""
+    """--extras: the SURVEY.md 8(f) rows (hash-grid field, wavefront, training, narrow networks)."""
     from ddf_inputs import MASTER_SEED, STREAMS, layout_sdf, make_weights
     ex = {}
-    n = 1 << 20
-    lay = layout_sdf()
-    sdf = ddf.ddf_create(make_weights(lay), lay)
-    cam = ddf.ddf_camera_from_seed(MASTER_SEED, STREAMS["camera_pos"], 2.5)
-    o = torch.empty((n, 3), device="cuda"); d = torch.empty((n, 3), device="cuda")
-    ddf.ddf_gen_camera(cam, 1024, 1024, o, d)
-    t = torch.empty(n, device="cuda"); hit = torch.empty(n, dtype=torch.uint8, device="cuda")
-    st = torch.empty(n, dtype=torch.int32, device="cuda"); tot = torch.zeros(1, dtype=torch.int64, device="cuda")
-    dist = torch.empty(n, device="cuda"); vis = torch.empty(n, device="cuda")
-    ddf_ms = _time_ms(torch, lambda: ddf.ddf_query(model, o, d, n, dist, vis))
-    # "across convergence thresholds" (PAPER.md:112): the early-exit tracer at three hit thresholds
-    for eps in (1e-2, 1e-4):
-        prm = ddf.SdfTraceParams(64, eps, 6.0, 1.0, 0.05, 1)
-        ms = _time_ms(torch, lambda: ddf.sdf_sphere_trace(sdf, o, d, n, prm, t, hit, st, None, None, tot), reps=2)
-        ex["sphere_trace_early_exit_eps%g" % eps] = {"ms": ms, "mlp_evals": int(tot.item()), "mean_steps": float(st.float().mean()),
-                                                     "hit_rate": float(hit.float().mean()), "ddf_speedup": ms / ddf_ms}
-    ddf.ddf_destroy(sdf)
-    del o, d, t, hit, st, dist, vis
     ex["hashgrid_field"] = run_hashgrid(ddf, torch, peaks)
     ex["wavefront_shadowed_camera_2^20"] = run_wavefront(ddf, torch)
     ex["training_hashgrid"] = run_training(ddf, torch)
@@ -631,8 +694,13 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--extras", action="store_true", help="also measure shadow / AO / sweep / sphere tracing")
+    ap.add_argument("--write-traffic", nargs="+", metavar="NCU_RAW_CSV",
+                    help="no benchmark: rewrite profiles/r03_dram_bytes.txt from `ncu --page raw --csv --print-units base` files")
     args = ap.parse_args()
-    if args.impl == "reference":
+    if args.write_traffic:
+        head = subprocess.run(["git", "-C", ROOT, "rev-parse", "--short", "HEAD"], capture_output=True, text=True).stdout.strip()
+        write_traffic(args.write_traffic, "commit " + head if head else "unknown commit")
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_gpu(args)
