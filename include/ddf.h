@@ -126,7 +126,7 @@ int  ddf_set_path(ddf_model* model, int path);
  * which: DDF_RESERVE_HOST - staging of ddf_query_host (32 B per ray, plus its two copy streams and events);
  * DDF_RESERVE_RAYS - the ray buffer of ddf_query_camera / ddf_query_ao_points (24 B per ray; max_rays counts
  * width * height or n_pts * spp), and, when the reduce of ddf_query_ao cannot be fused into the query (spp does not
- * divide 32, or only the CUDA-core path serves the model), its per-ray results (8 B per ray); DDF_RESERVE_TRACE - sdf_sphere_trace (25 B per ray); DDF_RESERVE_WAVE - the
+ * divide 32, or only the CUDA-core path serves the model), its per-ray results (8 B per ray); DDF_RESERVE_TRACE - sdf_sphere_trace (37 B per ray); DDF_RESERVE_WAVE - the
  * wavefront calls on max_rays primary rays, with room for spp ambient-occlusion rays per hit (40 B per primary ray,
  * or 32 + 24 spp if that is more; spp = 0: shadow calls only).  For a model only the CUDA-core path serves, the
  * activation workspace of its queries is sized too, whatever `what` is: that path answers a batch in passes of 16,384
@@ -406,12 +406,16 @@ int  ddf_gen_train_batch(const ddf_scene* scene, uint64_t seed, uint64_t rng_str
  *   t = 0; for step < max_steps: p = o + t d; s = s(p); if |s| < eps: hit, stop;
  *          t += s; if t > t_max or t < 0: miss, stop.   Unconverged: miss.
  * early_exit 0: every ray is evaluated max_steps times (finished rays keep their state);
- * early_exit 1: finished rays are compacted away between steps.
+ * early_exit 1: finished rays are compacted away between steps (stable: the live list keeps ray order).
+ * omega in (1, 2): over-relaxed steps, t += omega * s; when the spheres at the previous and at the current point do
+ * not touch (|s| + |s_prev| < t - t_prev) the step may have jumped a surface: the ray goes back to t_prev + s_prev
+ * (that evaluation counted) and takes plain steps from then on.  omega <= 1 (0 included): the plain rule above,
+ * bit for bit; omega >= 2, negative or NaN: DDF_E_INVALID_ARG.
  * out_t [n], out_hit [n] (0/1), out_steps [n] (SDF evaluations that counted for the ray).
  * trace_p / trace_s (may be NULL): [n][max_steps][3] / [n][max_steps] visited points and values
  * (unvisited entries are NaN).  total_evals [device] int64 (may be NULL): MLP evaluations made. */
 typedef struct sdf_trace_params {
-  int32_t max_steps; float eps; float t_max; float base_radius; float alpha; int32_t early_exit;
+  int32_t max_steps; float eps; float t_max; float base_radius; float alpha; int32_t early_exit; float omega;
 } sdf_trace_params;
 int  sdf_sphere_trace(ddf_model* model, const float* o, const float* d, int64_t n,
                       const sdf_trace_params* params, float* out_t, uint8_t* out_hit,

@@ -60,7 +60,7 @@ class DdfScene(C.Structure):
 
 class SdfTraceParams(C.Structure):
     _fields_ = [("max_steps", C.c_int32), ("eps", C.c_float), ("t_max", C.c_float),
-                ("base_radius", C.c_float), ("alpha", C.c_float), ("early_exit", C.c_int32)]
+                ("base_radius", C.c_float), ("alpha", C.c_float), ("early_exit", C.c_int32), ("omega", C.c_float)]
 
 
 _lib = None

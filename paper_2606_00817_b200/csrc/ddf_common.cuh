@@ -93,6 +93,9 @@ int tc_forward(Model* m, const float* o, const float* d, int64_t n, const int64_
 int trace_reserve(Model* m, int64_t n, int max_steps);          // ddf_trace.cu
 int wave_reserve_bytes(Model* m, size_t need);                  // ddf_wave.cu
 int wave_reserve(Model* m, int64_t n, int spp);
+// exclusive scan of n_blocks int32 block counts in place (one block), the total to *count (device): the middle step of
+// every stable compaction in the library
+int scan_block_counts(int32_t* block_counts, int64_t n_blocks, int64_t* count, cudaStream_t st);
 
 // ---- hash-grid field (ddf_hash.cu)
 void hash_plan_destroy(Model* m);

@@ -174,6 +174,12 @@ __global__ void wave_ao_scatter_kernel(const float* __restrict__ vis, int64_t n,
   if (k < *count) out_ao[index[k]] = ao_c[k];
 }
 
+int scan_block_counts(int32_t* block_counts, int64_t n_blocks, int64_t* count, cudaStream_t st) {
+  wave_scan_kernel<<<1, 1024, 0, st>>>(block_counts, n_blocks, count, nullptr, 1);
+  DDF_CUDA_TRY(cudaGetLastError());
+  return DDF_OK;
+}
+
 int wave_reserve_bytes(Model* m, size_t need) {
   if (need <= m->wave_ws_bytes) return DDF_OK;
   cudaFree(m->wave_ws); m->wave_ws = nullptr; m->wave_ws_bytes = 0;

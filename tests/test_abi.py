@@ -52,7 +52,7 @@ def test_status_strings(libddf):
 def test_layout_struct_matches_header():
     from paper_2606_00817_b200 import DdfLayout, DdfCamera, DdfScene, SdfTraceParams
     assert C.sizeof(DdfLayout) == 44 and C.sizeof(DdfCamera) == 28 and C.sizeof(DdfScene) == 40
-    assert C.sizeof(SdfTraceParams) == 24
+    assert C.sizeof(SdfTraceParams) == 28
 
 
 def test_argument_errors_without_gpu(libddf):

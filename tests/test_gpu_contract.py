@@ -363,6 +363,70 @@ def test_sphere_trace_alpha0_is_bit_identical_to_the_cpu_tracer(ddf, orc, sdf):
     assert h.sum() > 1000 and np.all(want[h] > 0) and np.all(np.abs(want[h] - t[h]) < 1e-3 / 0.05)
 
 
+def _replay_step_rule(s_row, omega, eps, t_max, max_steps=64):
+    """the (over-relaxed) step rule of include/ddf.h in fp32, fed with the values the kernel itself saw"""
+    f = np.float32
+    tt = f(0.0); tp = f(0.0); sp = f(np.nan); om = f(max(omega, 1.0)); h = 0; k = 0
+    for k in range(max_steps):
+        s = f(s_row[k])
+        if om > 1 and f(abs(s) + abs(sp)) < f(tt - tp):
+            tt = f(tp + sp); om = f(1.0); sp = f(np.nan)
+            if tt > t_max or tt < 0: break
+            continue
+        if abs(s) < eps: h = 1; break
+        tp, sp = tt, s
+        tt = f(np.float64(om) * np.float64(s) + np.float64(tt))      # one rounding, like fmaf (the product is exact in fp64)
+        if tt > t_max or tt < 0: break
+    return h, k + 1, tt
+
+
+@pytest.mark.parametrize("eps", [1e-2, 1e-3, 1e-4])
+@pytest.mark.parametrize("omega", [0.0, 1.0, 1.1, 1.5, 1.9])
+def test_over_relaxed_sphere_trace_and_thresholds_alpha0_bit_identical_to_the_cpu_tracer(ddf, orc, sdf, omega, eps):
+    """SURVEY.md 8(f) f4, PAPER.md:112 ("across convergence thresholds"): with the MLP term off, the CUDA tracer with
+    over-relaxed steps (fall-back included) and at every hit threshold returns the CPU tracer's t, hit and steps
+    exactly, in both modes; omega 0 and 1 are the plain rule; large omega does fall back on this view."""
+    lay, blob, m = sdf
+    cam = orc.camera_from_seed(MASTER_SEED, STREAMS["camera_pos"], 2.5)
+    o, d = orc.gen_camera(cam, 48, 48)
+    rt, rhit, rsteps, _, rs = orc.sphere_trace(lay, blob, o, d, 64, eps, 6.0, 1.0, 0.0, want_trace=True, omega=max(omega, 1.0))
+    for early in (0, 1):
+        prm = ddf.SdfTraceParams(64, eps, 6.0, 1.0, 0.0, early, omega)
+        t, hit, steps, tot = _trace(ddf, m, o, d, prm)
+        assert np.array_equal(hit, rhit) and np.array_equal(steps, rsteps) and np.array_equal(t, rt)
+        assert tot == (64 * len(o) if not early else int(steps.sum()))
+    assert 500 < rhit.sum() < len(o)
+    if omega <= 1.0:
+        pt, phit, psteps = orc.sphere_trace(lay, blob, o, d, 64, eps, 6.0, 1.0, 0.0)
+        assert np.array_equal(pt, rt) and np.array_equal(psteps, rsteps)
+    if omega >= 1.5:
+        # a fall-back shows as a step whose t went backwards: the point after it is closer to the origin of the ray
+        assert (rsteps[rhit == 1] >= 3).any()
+
+
+@pytest.mark.parametrize("omega,eps", [(1.3, 1e-3), (1.0, 1e-2), (1.0, 1e-4), (1.6, 1e-2)])
+def test_over_relaxed_sphere_trace_teacher_forcing_with_the_mlp_on(ddf, orc, sdf, omega, eps):
+    """MLP on (alpha 0.05): both modes agree bit for bit, the values at the visited points match the oracle's SDF, and the
+    rule of ddf.h replayed on the kernel's own values reproduces every decision, at other thresholds and with omega > 1."""
+    lay, blob, m = sdf
+    cam = orc.camera_from_seed(MASTER_SEED, STREAMS["camera_pos"], 2.5)
+    o, d = orc.gen_camera(cam, 24, 24)
+    t, hit, steps, tot, tp, ts = _trace(ddf, m, o, d, ddf.SdfTraceParams(64, eps, 6.0, 1.0, 0.05, 0, omega), want_trace=True)
+    t1, hit1, steps1, tot1, tp1, ts1 = _trace(ddf, m, o, d, ddf.SdfTraceParams(64, eps, 6.0, 1.0, 0.05, 1, omega), want_trace=True)
+    assert np.array_equal(t, t1) and np.array_equal(hit, hit1) and np.array_equal(steps, steps1)
+    assert np.array_equal(np.nan_to_num(ts, nan=-9.0), np.nan_to_num(ts1, nan=-9.0))
+    assert tot == 64 * len(o) and tot1 == int(steps.sum())
+    visited = ~np.isnan(ts)
+    assert np.array_equal(visited.sum(1), steps)
+    rows, cols = np.nonzero(visited)
+    pick = np.random.default_rng(0).choice(len(rows), 600, replace=False)
+    s_ref = orc.sdf_eval(lay, blob, tp[rows[pick], cols[pick]], 1.0, 0.05, mode=0)
+    assert np.abs(ts[rows[pick], cols[pick]] - s_ref).max() < 0.05 * 4e-2 + 1e-6
+    for i in range(len(o)):
+        assert _replay_step_rule(ts[i], omega, eps, 6.0) == (hit[i], steps[i], t[i]), i
+    assert 0.1 < hit.mean() < 0.95
+
+
 def test_sphere_trace_teacher_forcing(ddf, orc, sdf):
     """MLP on: trajectories are chaotic under bf16, so the oracle re-evaluates s at the kernel's
     own visited points (same tolerance per step); end results are compared statistically."""

@@ -65,6 +65,7 @@ def check_parity(dist, vis, t_ref, xi_ref, what=""):
 
 def check_quantised(z_gpu, z_q, what=""):
     e = np.abs(z_gpu - z_q)
+    print("QUANT %-40s n=%6d max %.3e mean %.3e" % (what, e.shape[0], float(e.max()), float(e.mean())))
     assert e.max() <= 4e-2 and e.mean() <= 3e-3, (what, float(e.max()), float(e.mean()))
 
 
