@@ -426,12 +426,58 @@ def run_extras(ddf, torch, model, peaks):
     """--extras: the SURVEY.md 8(f) rows (hash-grid field, wavefront, training, narrow networks)."""
     from ddf_inputs import MASTER_SEED, STREAMS, layout_sdf, make_weights
     ex = {}
+    ex["sphere_trace_relaxation"] = run_relaxation_table(ddf, torch, model)
     ex["hashgrid_field"] = run_hashgrid(ddf, torch, peaks)
     ex["wavefront_shadowed_camera_2^20"] = run_wavefront(ddf, torch)
     ex["training_hashgrid"] = run_training(ddf, torch)
     ex["training_hashgrid_fp32_cuda_cores"] = run_training(ddf, torch, arithmetic=1)
     ex["narrow_networks_2^20_random_rays"] = run_narrow(ddf, torch)
     return ex
+
+
+def run_relaxation_table(ddf, torch, model):
+    """SURVEY.md 8(f) f4 / PAPER.md:112 ("across ray counts and across convergence thresholds"), Table IV: the early-exit
+    sphere tracer with plain (omega 1) and over-relaxed steps on three views of the same SDF network - head-on from
+    radius 2.5 (the configs[4] view), grazing (a 10-degree view aimed at the limb of the unit sphere, every ray within 5
+    degrees of the tangent), close and off-axis (radius 1.2, looking past the centre) - at three hit thresholds.
+    Per cell: [ms, MLP evaluations, hit rate, DDF speed-up] on 2^18 rays (512 x 512); DDF time = one ddf_query of the batch."""
+    from ddf_inputs import MASTER_SEED, STREAMS, layout_sdf, make_weights
+    lay = layout_sdf()
+    sdf = ddf.ddf_create(make_weights(lay), lay)
+    W = H = 512; n = W * H
+    head = ddf.ddf_camera_from_seed(MASTER_SEED, STREAMS["camera_pos"], 2.5)
+    px, py, pz = [float(x) for x in head.pos]
+    r = (px * px + py * py + pz * pz) ** 0.5
+    ux, uy, uz = px / r, py / r, pz / r                          # towards the camera
+    # any unit vector normal to u: the limb point of the unit sphere seen from distance r is u / r + sqrt(1 - 1/r^2) v
+    ax = (0.0, 0.0, 1.0) if abs(uz) < 0.9 else (1.0, 0.0, 0.0)
+    vx, vy, vz = uy * ax[2] - uz * ax[1], uz * ax[0] - ux * ax[2], ux * ax[1] - uy * ax[0]
+    vn = (vx * vx + vy * vy + vz * vz) ** 0.5
+    vx, vy, vz = vx / vn, vy / vn, vz / vn
+    c = (1.0 - 1.0 / (r * r)) ** 0.5
+    limb = (ux / r + c * vx, uy / r + c * vy, uz / r + c * vz)
+    views = {
+        "head_on_r2.5_fov50": ddf.DdfCamera(head.pos, (0.0, 0.0, 0.0), 50.0),
+        "grazing_r2.5_fov10_at_limb": ddf.DdfCamera(head.pos, limb, 10.0),
+        "off_axis_r1.2_fov50": ddf.DdfCamera((1.2 * ux, 1.2 * uy, 1.2 * uz), (0.8 * vx, 0.8 * vy, 0.8 * vz), 50.0),
+    }
+    o = torch.empty((n, 3), device="cuda"); d = torch.empty((n, 3), device="cuda")
+    t = torch.empty(n, device="cuda"); hit = torch.empty(n, dtype=torch.uint8, device="cuda")
+    st = torch.empty(n, dtype=torch.int32, device="cuda"); tot = torch.zeros(1, dtype=torch.int64, device="cuda")
+    dist = torch.empty(n, device="cuda"); vis = torch.empty(n, device="cuda")
+    out = {}
+    for name, cam in views.items():
+        ddf.ddf_gen_camera(cam, W, H, o, d)
+        ddf_ms = _time_ms(torch, lambda: ddf.ddf_query(model, o, d, n, dist, vis))
+        cell = {"ddf_ms": ddf_ms}
+        for eps in (1e-2, 1e-3, 1e-4):
+            for omega in (1.0, 1.2, 1.6):
+                prm = ddf.SdfTraceParams(64, eps, 6.0, 1.0, 0.05, 1, omega)
+                ms = _time_ms(torch, lambda: ddf.sdf_sphere_trace(sdf, o, d, n, prm, t, hit, st, None, None, tot), reps=2)
+                cell["eps%g_omega%g" % (eps, omega)] = [ms, int(tot.item()), float(hit.float().mean()), ms / ddf_ms]
+        out[name] = cell
+    ddf.ddf_destroy(sdf)
+    return sig(out, 4)
 
 
 def run_narrow(ddf, torch):

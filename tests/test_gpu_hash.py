@@ -1,7 +1,7 @@
 """GPU parity of the paper's own field (hash grid + direction bands + 2x64 MLP)
 against oracle/ddf_hash_oracle.c, through the C ABI.  Tolerances as for the dense network
 (BASELINE.json north_star): |dd| <= 1e-2 (1+|d|), |dv| <= 1e-2, >= 99.9 % hit/miss agreement outside
-|xi - 0.5| < 1e-2, against the EXACT fp64 oracle; logits within 2e-2 (mean 2e-3) of the oracle's
+|xi - 0.5| < 1e-2, against the EXACT fp64 oracle; logits within 8e-3 (mean 5e-6) of the oracle's
 quantised mode.  The integer decisions (cell, index) are taken in fp32 on both sides (reading H2/H3)."""
 import numpy as np
 import pytest
@@ -64,7 +64,9 @@ def _parity(ddf, orc, field, od, dd, n, what, k=6000):
     ddf.ddf_query_logits(m, od[it].contiguous(), dd[it].contiguous(), len(idx), zg)
     zq, _, _ = orc.hash_forward(lay, table, mlp, o, d, mode=1)
     e = np.abs(zg.cpu().numpy() - zq)
-    assert e.max() <= 2e-2 and e.mean() <= 2e-3, (what, e.max(), e.mean())
+    print("QUANT %-40s n=%6d max %.3e mean %.3e" % ("hash " + what, e.shape[0], float(e.max()), float(e.mean())))
+    # ~2x what the committed kernel measures over every case of this file (max 3.2e-3, mean 8.8e-7)
+    assert e.max() <= 8e-3 and e.mean() <= 5e-6, (what, e.max(), e.mean())
     # batch independence, bit exact
     d2 = torch.empty(len(idx), device="cuda"); v2 = torch.empty(len(idx), device="cuda")
     ddf.ddf_query(m, od[it].contiguous(), dd[it].contiguous(), len(idx), d2, v2)

@@ -63,10 +63,17 @@ def check_parity(dist, vis, t_ref, xi_ref, what=""):
     return stats
 
 
-def check_quantised(z_gpu, z_q, what=""):
+def check_quantised(z_gpu, z_q, what="", max_tol=4.5e-2, mean_tol=2e-3):
+    """Second gate: logits against the oracle's quantised mode (same bf16 rounding points, fp64 sums).  Most logits agree
+    to ~1e-6; the tail comes from hidden activations that sit on a bf16 rounding boundary and round the other way under
+    the kernel's fp32 summation order - one flip moves one activation by 2^-8 of its value and the remaining layers
+    carry it to the logit.  Bounds are ~2x what the committed kernels measure (printed below on every run):
+    the defaults are for the 8 x 1280 network on >= 8,192 rays (measured max 2.1e-2, mean 9.6e-4), shallower or narrower
+    networks pass their own."""
     e = np.abs(z_gpu - z_q)
-    print("QUANT %-40s n=%6d max %.3e mean %.3e" % (what, e.shape[0], float(e.max()), float(e.mean())))
-    assert e.max() <= 4e-2 and e.mean() <= 3e-3, (what, float(e.max()), float(e.mean()))
+    print("QUANT %-40s n=%6d max %.3e mean %.3e rays above 1e-3: %d" % (what, e.shape[0], float(e.max()), float(e.mean()),
+                                                                        int((e.reshape(e.shape[0], -1).max(1) > 1e-3).sum())))
+    assert e.max() <= max_tol and e.mean() <= mean_tol, (what, float(e.max()), float(e.mean()), max_tol, mean_tol)
 
 
 # ------------------------------------------------------------------ configs[0]: all 4096 rays
@@ -87,7 +94,7 @@ def test_config0_all_rays(ddf, orc, c0):
     z, t, xi = orc.forward(lay, blob, o, d, mode=0)
     check_parity(dist, vis, t, xi, "C0")
     zq, _, _ = orc.forward(lay, blob, o, d, mode=1)
-    check_quantised(_query(ddf, m, o, d, logits=True), zq, "C0 quantised")
+    check_quantised(_query(ddf, m, o, d, logits=True), zq, "C0 quantised", max_tol=5e-3, mean_tol=2e-6)   # measured 2.2e-3 / 4.5e-7
 
 
 # ------------------------------------------------------------------ paper-scale network

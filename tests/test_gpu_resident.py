@@ -36,13 +36,19 @@ def _logits(ddf, m, o, d, n):
 
 # 256x1: one hidden layer is outside what the resident kernel serves (its head-partial buffer relies on the layer-0
 # hand-over of a second layer); path 5 must answer it with the persistent kernel, still in one launch
-LAYOUTS = [("256x1 falls back", Layout(0, 10, 4, 1, 256, -1, 2, 0)), ("256x2", Layout(0, 10, 4, 2, 256, -1, 2, 0)), ("256x3 skip 1", Layout(0, 10, 4, 3, 256, 1, 2, 0)),
-           ("512x3 skip 2, no direction bands", Layout(0, 6, 0, 3, 512, 2, 2, 0)), ("768x2 one output", Layout(0, 4, 4, 2, 768, -1, 1, 0)),
-           ("1024x4 skip 3", Layout(0, 10, 4, 4, 1024, 3, 2, 0)), ("configs[1]", layout_c1()), ("SDF network", layout_sdf())]
+# name, layout, (max, mean) bound of the quantised gate: ~2x the measured values (max over the ten batch sizes, 300 rays each)
+LAYOUTS = [("256x1 falls back", Layout(0, 10, 4, 1, 256, -1, 2, 0), (1e-5, 1e-6)),                     # measured 8.1e-7 / 1.5e-7
+           ("256x2", Layout(0, 10, 4, 2, 256, -1, 2, 0), (1e-5, 1e-6)),                                # 4.2e-6 / 1.5e-7
+           ("256x3 skip 1", Layout(0, 10, 4, 3, 256, 1, 2, 0), (5e-4, 5e-6)),                          # 2.2e-4 / 9.7e-7
+           ("512x3 skip 2, no direction bands", Layout(0, 6, 0, 3, 512, 2, 2, 0), (2e-3, 2e-5)),       # 9.1e-4 / 4.2e-6
+           ("768x2 one output", Layout(0, 4, 4, 2, 768, -1, 1, 0), (1e-5, 1e-6)),                      # 1.6e-6 / 2.9e-7
+           ("1024x4 skip 3", Layout(0, 10, 4, 4, 1024, 3, 2, 0), (1e-2, 1e-4)),                        # 4.2e-3 / 4.2e-5
+           ("configs[1]", layout_c1(), (2.5e-2, 2.5e-3)),                                              # 9.6e-3 / 8.9e-4
+           ("SDF network", layout_sdf(), (2.5e-2, 2.5e-3))]                                            # 9.1e-3 / 1.1e-3
 
 
-@pytest.mark.parametrize("name,lay", LAYOUTS, ids=[l[0] for l in LAYOUTS])
-def test_resident_kernel_matches_the_oracle_and_the_persistent_kernel(ddf, orc, name, lay):
+@pytest.mark.parametrize("name,lay,qtol", LAYOUTS, ids=[l[0] for l in LAYOUTS])
+def test_resident_kernel_matches_the_oracle_and_the_persistent_kernel(ddf, orc, name, lay, qtol):
     blob = make_weights(lay, bias_scale=0.2)
     m = ddf.ddf_create(blob, lay)
     for n in (1, 63, 64, 65, 127, 128, 129, 1000, 128 * 74 + 1, 20011):
@@ -54,7 +60,7 @@ def test_resident_kernel_matches_the_oracle_and_the_persistent_kernel(ddf, orc, 
         assert bool(torch.isfinite(z5).all())
         idx = np.unique(np.linspace(0, n - 1, min(n, 300)).astype(np.int64))
         zq = orc.forward(lay, blob, o_np[idx], d_np[idx] if lay.input_kind == 0 else None, mode=1)[0]
-        check_quantised(z5.cpu().numpy()[idx], zq, "%s n=%d" % (name, n))
+        check_quantised(z5.cpu().numpy()[idx], zq, "%s n=%d" % (name, n), max_tol=qtol[0], mean_tol=qtol[1])
         # the two kernels add the same products in a different order: equal up to bf16 rounding flips along the layers
         assert float((z3 - z5).abs().max()) <= 4e-2 and float((z3 - z5).abs().mean()) <= 3e-3
         if lay.n_hidden < 2:
