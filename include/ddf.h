@@ -32,6 +32,12 @@
  *  - Results are a pure function of (weights, ray): independent of n and of the ray's position
  *    in the batch, bit-reproducible run to run (training steps accumulate gradients with atomics
  *    and are reproducible to rounding only).  Directions must be unit length (not checked).
+ *  - A model (and a trainer) lives on the CUDA device that was current when it was created: its weights, workspaces,
+ *    tensor maps and kernel attributes exist there only.  Every call that takes one (ddf_destroy included; not
+ *    ddf_set_path / ddf_get_info / ddf_trainer_steps, which touch host state only) must be made with that device
+ *    current (cudaSetDevice) and with pointers and a stream of that device; with another device current it returns
+ *    DDF_E_INVALID_ARG and launches nothing.  Multi-GPU use is one model per device (bench.py --gpus N: one process per
+ *    GPU); ddf_get_info(model, 4) tells which device a model belongs to.
  *  - A model (and a trainer) owns device workspaces that its calls reuse: use one model from one
  *    stream / host thread at a time; different models are independent.  On a fused path ddf_query,
  *    ddf_query_logits and ddf_query_ao with an spp that divides 32 never allocate (their workspace is sized
@@ -139,7 +145,8 @@ int  ddf_set_path(ddf_model* model, int path);
 #define DDF_RESERVE_ALL   15u
 int  ddf_reserve(ddf_model* model, uint32_t what, int64_t max_rays, int spp);
 /* which = 0: 1 if the tcgen05 path serves this model, else 0; 1: kernels launched by the
- * last query call on this model; 2: E (encoded input width); 3: rays per tile of the path. */
+ * last query call on this model; 2: E (encoded input width); 3: rays per tile of the path;
+ * 4: ordinal of the CUDA device the model was created on. */
 int64_t ddf_get_info(const ddf_model* model, int which);
 
 /* ---------------------------------------------------------------- the paper's own field

@@ -149,6 +149,7 @@ static int create_impl(const void* weights, const ddf_layout* layout, ddf_model*
   if (!m) return DDF_E_NOMEM;
   memset(m, 0, sizeof(Model));
   m->lay = *layout;
+  m->device = dev;
   m->sm_count = prop.multiProcessorCount;
   const ddf_layout& L = m->lay;
   m->E = 3 + 6 * (int)L.n_freq_origin + (L.input_kind == 0 ? 3 + 6 * (int)L.n_freq_dir : 0);
@@ -271,6 +272,7 @@ static int ao_out_reserve(Model* m, int64_t n) {
 extern "C" int ddf_reserve(ddf_model* model, uint32_t what, int64_t max_rays, int spp) {
   if (!model || max_rays < 0 || spp < 0 || (what & ~(uint32_t)DDF_RESERVE_ALL)) return DDF_E_INVALID_ARG;
   Model* m = reinterpret_cast<Model*>(model);
+  { const int rc_dev = check_device(m->device); if (rc_dev != DDF_OK) return rc_dev; }
   int rc = DDF_OK;
   if (max_rays == 0) return DDF_OK;
   if ((what & DDF_RESERVE_HOST) && (rc = host_reserve(m, max_rays)) != DDF_OK) return rc;
@@ -288,6 +290,7 @@ extern "C" int ddf_reserve(ddf_model* model, uint32_t what, int64_t max_rays, in
 
 extern "C" int ddf_destroy(ddf_model* model) {
   if (!model) return DDF_OK;
+  { const int rc_dev = check_device(reinterpret_cast<Model*>(model)->device); if (rc_dev != DDF_OK) return rc_dev; }
   cudaDeviceSynchronize();
   free_model(reinterpret_cast<Model*>(model));
   return DDF_OK;
@@ -310,6 +313,7 @@ extern "C" int64_t ddf_get_info(const ddf_model* model, int which) {
     case 0: return has_fused_path(m) ? 1 : 0;
     case 1: return m->last_launches;
     case 2: return m->E;
+    case 4: return m->device;
     case 3: return m->hg ? 128 : ((m->tc && m->path != 1) ? 256 : ((m->nw && m->path != 1) ? 128 : 64));
     default: return DDF_E_INVALID_ARG;
   }
@@ -318,6 +322,7 @@ extern "C" int64_t ddf_get_info(const ddf_model* model, int which) {
 static int run_query(Model* m, const float* o, const float* d, int64_t n, int mode_out,
                      float* out0, float* out1, void* stream) {
   if (n < 0) return DDF_E_INVALID_ARG;
+  { const int rc_dev = check_device(m->device); if (rc_dev != DDF_OK) return rc_dev; }
   if (n == 0) { m->last_launches = 0; return DDF_OK; }
   if (!o || !out0 || (m->lay.input_kind == 0 && !d)) return DDF_E_INVALID_ARG;
   cudaStream_t st = (cudaStream_t)stream;
@@ -342,6 +347,7 @@ extern "C" int ddf_query_host(ddf_model* model, const float* origins, const floa
   if (!model || n < 0) return DDF_E_INVALID_ARG;
   if (n == 0) return DDF_OK;
   Model* m = reinterpret_cast<Model*>(model);
+  { const int rc_dev = check_device(m->device); if (rc_dev != DDF_OK) return rc_dev; }
   const bool ray = m->lay.input_kind == 0, two = m->lay.n_out == 2;
   if (!origins || !out_dist || (ray && !dirs)) return DDF_E_INVALID_ARG;
   { int rc = host_reserve(m, n); if (rc != DDF_OK) return rc; }        // a no-op after ddf_reserve(DDF_RESERVE_HOST, >= n)
@@ -397,6 +403,7 @@ extern "C" int ddf_query_camera(ddf_model* model, const ddf_camera* cam, int wid
                                 float* out_dist, float* out_vis, void* stream) {
   if (!model || !cam || width < 0 || height < 0) return DDF_E_INVALID_ARG;
   Model* m = reinterpret_cast<Model*>(model);
+  { const int rc_dev = check_device(m->device); if (rc_dev != DDF_OK) return rc_dev; }
   if (m->lay.input_kind != 0) return DDF_E_INVALID_ARG;
   const int64_t n = (int64_t)width * height;
   if (n == 0) { m->last_launches = 0; return DDF_OK; }
@@ -417,6 +424,7 @@ extern "C" int ddf_query_ao_points(ddf_model* model, const float* p, const float
                                    void* stream) {
   if (!model || n_pts < 0 || spp <= 0 || n_pts * spp > 0x7fffffff) return DDF_E_INVALID_ARG;
   Model* m = reinterpret_cast<Model*>(model);
+  { const int rc_dev = check_device(m->device); if (rc_dev != DDF_OK) return rc_dev; }
   if (m->lay.n_out != 2 || m->lay.input_kind != 0) return DDF_E_INVALID_ARG;
   if (n_pts == 0) { m->last_launches = 0; return DDF_OK; }
   if (!p || !nrm || !ao) return DDF_E_INVALID_ARG;
@@ -438,6 +446,7 @@ extern "C" int ddf_query_ao(ddf_model* model, const float* o, const float* d, in
   if (!model || n_pts < 0 || spp <= 0 || n_pts > (int64_t)0x7fffffff / spp) return DDF_E_INVALID_ARG;
   if (n_pts == 0) return DDF_OK;
   Model* m = reinterpret_cast<Model*>(model);
+  { const int rc_dev = check_device(m->device); if (rc_dev != DDF_OK) return rc_dev; }
   if (!o || !d || !ao || m->lay.n_out != 2 || m->lay.input_kind != 0) return DDF_E_INVALID_ARG;
   const int64_t n = n_pts * spp;
   cudaStream_t st = (cudaStream_t)stream;

@@ -74,7 +74,16 @@ struct Model {
   HashPlan* hg;                    // non-null: this model is a hash-grid field (ddf_create_hashgrid)
   int sm_count;
   int last_launches;
+  int device;                      // CUDA device ordinal the model was created on: every call must find it current
 };
+
+// A model's (and a trainer's) pointers, tensor maps and per-context function attributes belong to the device it was
+// created on; a call made with another device current would launch there on foreign addresses.  Refuse it instead.
+inline int check_device(int owner) {
+  int cur = -1;
+  if (cudaGetDevice(&cur) != cudaSuccess) { (void)cudaGetLastError(); return DDF_E_CUDA; }
+  return cur == owner ? DDF_OK : DDF_E_INVALID_ARG;
+}
 
 // ---- SIMT path (ddf_simt.cu)
 constexpr int64_t kSimtChunkRows = 16384;   // rays per pass of simt_forward: the most rows its activation workspace ever holds

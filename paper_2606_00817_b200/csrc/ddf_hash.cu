@@ -463,6 +463,7 @@ extern "C" int ddf_create_hashgrid(const void* table, const void* mlp, const ddf
   if (!h) { delete m; return DDF_E_NOMEM; }
   memset(h, 0, sizeof(HashPlan));
   m->hg = h;
+  m->device = dev;
   m->sm_count = prop.multiProcessorCount;
   m->E = n_feat + n_dir;
   m->lay.struct_size = sizeof(ddf_layout); m->lay.version = DDF_LAYOUT_VERSION;

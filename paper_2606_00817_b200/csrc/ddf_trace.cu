@@ -152,6 +152,7 @@ extern "C" int sdf_sphere_trace(ddf_model* model, const float* o, const float* d
                                 void* stream) {
   if (!model || !prm || n < 0 || n > 0x7fffffff) return DDF_E_INVALID_ARG;
   Model* m = reinterpret_cast<Model*>(model);
+  { const int rc_dev = check_device(m->device); if (rc_dev != DDF_OK) return rc_dev; }
   if (m->lay.input_kind != 1 || m->lay.n_out != 1) return DDF_E_INVALID_ARG;
   if (prm->max_steps < 1 || prm->max_steps > 4096) return DDF_E_INVALID_ARG;
   if (!(prm->omega >= 0.0f && prm->omega < 2.0f)) return DDF_E_INVALID_ARG;     // also refuses NaN

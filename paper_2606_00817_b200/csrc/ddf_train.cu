@@ -417,6 +417,7 @@ extern "C" int ddf_trainer_create(const float* table, const float* mlp, const dd
   if (!T) return DDF_E_NOMEM;
   memset(T, 0, sizeof(Trainer));
   T->lay = *layout; T->prm = *params; T->entries = entries; T->n_table = entries * 2;
+  T->device = dev;
   const ddf_hashgrid_layout& L = T->lay;
   const int NF = (int)L.n_levels * 2, E = NF + 3 + 6 * (int)L.n_freq_dir, H = (int)L.n_hidden;
   TrParams& p = T->base;
@@ -481,6 +482,7 @@ extern "C" int ddf_trainer_create(const float* table, const float* mlp, const dd
 
 extern "C" int ddf_trainer_destroy(ddf_trainer* trainer) {
   if (!trainer) return DDF_OK;
+  { const int rc_dev = check_device(reinterpret_cast<Trainer*>(trainer)->device); if (rc_dev != DDF_OK) return rc_dev; }
   cudaDeviceSynchronize();
   tr_free(reinterpret_cast<Trainer*>(trainer));
   return DDF_OK;
@@ -521,6 +523,7 @@ extern "C" int ddf_trainer_loss_grads(ddf_trainer* trainer, const float* o, cons
                                       float* grad_mlp, void* stream) {
   if (!trainer || n <= 0 || !o || !d || !t || !hit) return DDF_E_INVALID_ARG;
   Trainer* T = reinterpret_cast<Trainer*>(trainer);
+  { const int rc_dev = check_device(T->device); if (rc_dev != DDF_OK) return rc_dev; }
   cudaStream_t st = (cudaStream_t)stream;
   const size_t total = (size_t)(T->n_table + T->n_mlp);
   int rc = tr_launch_grads(T, o, d, t, hit, n, loss, st);
@@ -540,6 +543,7 @@ extern "C" int ddf_trainer_step(ddf_trainer* trainer, const float* o, const floa
                                 const uint8_t* hit, int64_t n, float* loss, void* stream) {
   if (!trainer || n <= 0 || !o || !d || !t || !hit) return DDF_E_INVALID_ARG;
   Trainer* T = reinterpret_cast<Trainer*>(trainer);
+  { const int rc_dev = check_device(T->device); if (rc_dev != DDF_OK) return rc_dev; }
   cudaStream_t st = (cudaStream_t)stream;
   int rc = tr_launch_grads(T, o, d, t, hit, n, loss, st);
   if (rc != DDF_OK) return rc;
@@ -561,6 +565,7 @@ extern "C" int ddf_trainer_step(ddf_trainer* trainer, const float* o, const floa
 extern "C" int ddf_trainer_export(ddf_trainer* trainer, float* table, float* mlp) {
   if (!trainer || !table || !mlp) return DDF_E_INVALID_ARG;
   Trainer* T = reinterpret_cast<Trainer*>(trainer);
+  { const int rc_dev = check_device(T->device); if (rc_dev != DDF_OK) return rc_dev; }
   DDF_CUDA_TRY(cudaDeviceSynchronize());
   DDF_CUDA_TRY(cudaMemcpy(table, T->p_table, (size_t)T->n_table * 4, cudaMemcpyDeviceToHost));
   DDF_CUDA_TRY(cudaMemcpy(mlp, T->p_mlp, (size_t)T->n_mlp * 4, cudaMemcpyDeviceToHost));

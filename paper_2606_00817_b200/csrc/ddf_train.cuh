@@ -42,6 +42,7 @@ struct Trainer {
   float *ws_feat, *ws_dfeat, *ws_slab, *ws_rep;  // tensor-core path workspace; ws_feat / ws_dfeat hold ws_rays rays
   int64_t ws_rays;
   int sms;
+  int device;                                    // CUDA device ordinal of every pointer below (check_device)
 };
 
 // corner indices (into the table, in float2 units) and weights of one level

@@ -252,6 +252,7 @@ extern "C" int ddf_gen_shadow_from_hits(ddf_model* model, const float* o, const 
   if (n == 0) { DDF_CUDA_TRY(cudaMemsetAsync(count, 0, 8, st)); return DDF_OK; }
   if (!o || !d || !dist || !vis || !o2 || !d2 || !tmax || !index) return DDF_E_INVALID_ARG;
   Model* m = reinterpret_cast<Model*>(model);
+  { const int rc_dev = check_device(m->device); if (rc_dev != DDF_OK) return rc_dev; }
   WaveWs w;
   int rc = wave_ws(m, n, false, &w);
   if (rc != DDF_OK) return rc;
@@ -267,6 +268,7 @@ static int shadowed_lights_impl(ddf_model* model, const float* o, const float* d
                                 float* out_vis, uint8_t* out_lit_mask, int64_t* out_count, void* stream, bool do_primary) {
   if (!model || !lights || n < 0 || n > 0x7fffffff || n_lights < 1 || n_lights > 8) return DDF_E_INVALID_ARG;
   Model* m = reinterpret_cast<Model*>(model);
+  { const int rc_dev = check_device(m->device); if (rc_dev != DDF_OK) return rc_dev; }
   if (m->lay.input_kind != 0 || m->lay.n_out != 2) return DDF_E_INVALID_ARG;
   cudaStream_t st = (cudaStream_t)stream;
   if (n == 0) { if (out_count) DDF_CUDA_TRY(cudaMemsetAsync(out_count, 0, 8, st)); m->last_launches = 0; return DDF_OK; }
@@ -378,6 +380,7 @@ extern "C" int ddf_gen_ao_from_hits(ddf_model* model, const float* o, const floa
   if ((o2 == nullptr) != (d2 == nullptr)) return DDF_E_INVALID_ARG;
   cudaStream_t st = (cudaStream_t)stream;
   Model* m = reinterpret_cast<Model*>(model);
+  { const int rc_dev = check_device(m->device); if (rc_dev != DDF_OK) return rc_dev; }
   const int64_t n = (int64_t)width * height;
   if (n == 0) { DDF_CUDA_TRY(cudaMemsetAsync(count, 0, 8, st)); m->last_launches = 0; return DDF_OK; }
   if (!o || !d || !dist || !vis || !p_c || !nrm_c || !index) return DDF_E_INVALID_ARG;
@@ -394,6 +397,7 @@ static int ao_wavefront_impl(ddf_model* model, const float* o, const float* d, i
                              int64_t* out_count, void* stream, bool do_primary) {
   if (!model || width < 0 || height < 0 || spp <= 0 || (int64_t)width * height * spp > 0x7fffffff) return DDF_E_INVALID_ARG;
   Model* m = reinterpret_cast<Model*>(model);
+  { const int rc_dev = check_device(m->device); if (rc_dev != DDF_OK) return rc_dev; }
   if (m->lay.input_kind != 0 || m->lay.n_out != 2) return DDF_E_INVALID_ARG;
   cudaStream_t st = (cudaStream_t)stream;
   const int64_t n = (int64_t)width * height;
@@ -454,6 +458,7 @@ extern "C" int ddf_query_shaded(ddf_model* model, const float* o, const float* d
     return DDF_E_INVALID_ARG;
   if ((n_lights > 0 && (!lights || !out_lit_mask)) || (spp > 0 && !out_ao)) return DDF_E_INVALID_ARG;
   Model* m = reinterpret_cast<Model*>(model);
+  { const int rc_dev = check_device(m->device); if (rc_dev != DDF_OK) return rc_dev; }
   if (m->lay.input_kind != 0 || m->lay.n_out != 2) return DDF_E_INVALID_ARG;
   cudaStream_t st = (cudaStream_t)stream;
   const int64_t n = (int64_t)width * height;

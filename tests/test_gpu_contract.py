@@ -575,3 +575,27 @@ def test_reserve_on_the_cuda_core_path_is_bounded_and_covers_queries_and_wavefro
     assert torch.cuda.mem_get_info()[0] == free2
     assert bool(((ao >= 0) & (ao <= 1)).all())
     ddf.ddf_destroy(m)
+
+
+def test_a_model_belongs_to_the_device_it_was_created_on(ddf, c1):
+    """ddf_get_info(model, 4) is the creating device; with another device current every call is refused (needs two GPUs
+    for the refusal itself; on a one-GPU box only the ownership record and the pass-through are checked)."""
+    lay, m = c1
+    assert ddf.ddf_get_info(m, 4) == torch.cuda.current_device()
+    if torch.cuda.device_count() < 2:
+        return
+    home = torch.cuda.current_device()
+    o, d = random_rays(64)
+    oc, dc = _cuda(o), _cuda(d)
+    dist = torch.empty(64, device="cuda"); vis = torch.empty(64, device="cuda")
+    try:
+        torch.cuda.set_device((home + 1) % torch.cuda.device_count())
+        with pytest.raises(ddf.DdfError, match="invalid argument"):
+            ddf.ddf_query(m, oc, dc, 64, dist, vis)
+        with pytest.raises(ddf.DdfError, match="invalid argument"):
+            ddf.ddf_reserve(m, ddf.RESERVE_HOST, 64)
+    finally:
+        torch.cuda.set_device(home)
+    ddf.ddf_query(m, oc, dc, 64, dist, vis)
+    torch.cuda.synchronize()
+    assert bool(torch.isfinite(dist).all())
