@@ -259,6 +259,14 @@ def test_bad_arguments(ddf, c1):
     t = torch.zeros(4, device="cuda"); h = torch.zeros(4, dtype=torch.uint8, device="cuda"); s = torch.zeros(4, dtype=torch.int32, device="cuda")
     with pytest.raises(ddf.DdfError):
         ddf.sdf_sphere_trace(m, x, x, 4, prm, t, h, s)         # a DDF model is not an SDF model
+    slay = layout_sdf()
+    sm = ddf.ddf_create(make_weights(slay), slay)
+    for omega in (2.0, 2.5, -0.5, float("nan")):               # the relaxation factor must lie in [0, 2)
+        with pytest.raises(ddf.DdfError, match="invalid argument"):
+            ddf.sdf_sphere_trace(sm, x, x, 4, ddf.SdfTraceParams(64, 1e-3, 6.0, 1.0, 0.05, 0, omega), t, h, s)
+    ddf.sdf_sphere_trace(sm, x, x, 4, ddf.SdfTraceParams(64, 1e-3, 6.0, 1.0, 0.05, 0, 1.999), t, h, s)
+    torch.cuda.synchronize()
+    ddf.ddf_destroy(sm)
 
 
 @pytest.mark.parametrize("lay", [Layout(0, 6, 3, 4, 512, 2, 2, 1), Layout(0, 6, 3, 4, 128, 2, 2, 0), Layout(0, 4, 4, 3, 64, -1, 2, 1),
